@@ -1,0 +1,1161 @@
+// plk_api.cu -- the C ABI of include/plk.h: instance, arena sub-allocation, validation, level scheduling and kernel
+// launches.  No device memory is allocated here (the arena is the caller's); no arithmetic of the method runs on
+// the host.  Citations as in plk.h (P: PAPER.md line, S8x: SURVEY.md section 8(x)).
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include "../../include/plk.h"
+#include "plk_common.cuh"
+#include "plk_gen.cuh"
+#include "plk_misc.cuh"
+#include "plk_nuc.cuh"
+#include "plk_schedule.h"
+#ifdef PLK_WITH_TENSOR
+#include "plk_tc.cuh"
+#endif
+
+using namespace plk;
+
+namespace {
+
+constexpr size_t ALIGN = 1024;
+constexpr size_t RING_BYTES = 8u << 20;  // parameter staging ring (pinned host + device mirror)
+inline size_t round_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
+
+struct Layout {
+  int S, SP, C, P;
+  size_t w;                 // bytes per real
+  size_t W;                 // one partials slot
+  size_t mx_bytes;          // per-slot maxima (SP = 64, deferred rescaling), else 0
+  int post_slots, compact_slots, pre_slots;
+  size_t compact_bytes, matrix_bytes, eigen_bytes, scale_bytes;
+  int n_tiles, max_grad;
+  size_t off_post, off_compact, off_pre, off_pre_mx, off_matrix, off_eigen, off_scale, off_weights, off_pi,
+      off_rates, off_catw, off_site, off_block_partial, off_grad_partial, off_grad_out, off_logl, off_site_deriv,
+      off_stage, off_ring, total;
+  size_t stage_bytes;
+};
+
+bool compute_layout(const plk_config& c, Layout& L) {
+  if (c.tip_count < 2 || c.pattern_count < 1 || c.category_count < 1 || c.category_count > 16) return false;
+  if (c.state_count < 2 || c.state_count > 64) return false;
+  if (c.state_count == 4 && c.category_count > 8) return false;
+  if (c.partials_buffer_count < c.tip_count || c.compact_buffer_count < 0 ||
+      c.compact_buffer_count > c.tip_count || c.partials_slot_count < 0 || c.preorder_buffer_count < 0 ||
+      c.preorder_slot_count < 0 || c.matrix_buffer_count < 1 || c.eigen_buffer_count < 1 ||
+      c.scale_buffer_count < 0)
+    return false;
+  if (c.precision != PLK_FP64 && c.precision != PLK_FP32) return false;
+  L.S = c.state_count;
+  L.SP = c.state_count == 4 ? 4 : 64;
+  L.C = c.category_count;
+  L.P = c.pattern_count;
+  L.w = c.precision == PLK_FP64 ? 8 : 4;
+  L.W = round_up((size_t)L.C * L.P * L.SP * L.w, ALIGN);
+  L.mx_bytes = L.SP == 4 ? 0 : round_up((size_t)L.C * L.P * L.w, ALIGN);
+  L.post_slots = c.partials_slot_count > 0 ? c.partials_slot_count : c.partials_buffer_count - c.compact_buffer_count;
+  L.compact_slots = c.compact_buffer_count;
+  L.pre_slots = c.preorder_slot_count > 0 ? c.preorder_slot_count : c.preorder_buffer_count;
+  L.compact_bytes = round_up((size_t)L.P, ALIGN);
+  L.matrix_bytes = round_up((size_t)L.C * L.SP * L.SP * L.w, ALIGN);
+  // eigen buffer: U, Uinv (S*S fp64), lambda (S fp64), Q64 (S*S fp64), QT (SP*SP reals)
+  L.eigen_bytes = round_up((size_t)(3 * L.S * L.S + L.S) * 8, ALIGN) + round_up((size_t)L.SP * L.SP * L.w, ALIGN);
+  L.scale_bytes = L.SP == 4 ? round_up((size_t)L.P * 2, ALIGN) : L.mx_bytes;
+  L.n_tiles = L.SP == 4 ? (L.P + NUC_THREADS - 1) / NUC_THREADS : (L.P + GEN_TP - 1) / GEN_TP;
+  L.max_grad = c.partials_buffer_count;
+  size_t o = 0;
+  auto take = [&](size_t bytes) { size_t at = o; o += round_up(bytes, ALIGN); return at; };
+  L.off_post = take((size_t)L.post_slots * L.W);
+  L.off_compact = take((size_t)L.compact_slots * L.compact_bytes);
+  L.off_pre = take((size_t)L.pre_slots * L.W);
+  L.off_pre_mx = take((size_t)L.pre_slots * L.mx_bytes);
+  L.off_matrix = take((size_t)c.matrix_buffer_count * L.matrix_bytes);
+  L.off_eigen = take((size_t)c.eigen_buffer_count * L.eigen_bytes);
+  L.off_scale = take((size_t)c.scale_buffer_count * L.scale_bytes);
+  L.off_weights = take((size_t)L.P * 8);
+  L.off_pi = take((size_t)L.SP * 8);
+  L.off_rates = take((size_t)L.C * 8);
+  L.off_catw = take((size_t)L.C * 8);
+  L.off_site = take((size_t)L.P * 8);
+  L.off_block_partial = take((size_t)(L.P / 32 + 2) * 8);
+  L.off_grad_partial = take((size_t)L.max_grad * L.n_tiles * 8);
+  L.off_grad_out = take((size_t)L.max_grad * 8);
+  L.off_logl = take(64);
+  L.off_site_deriv = take((c.flags & PLK_FLAG_SITE_DERIVATIVES) ? (size_t)L.max_grad * L.P * 8 : 0);
+  L.stage_bytes = round_up((size_t)L.C * L.P * L.S * 8, ALIGN);
+  L.off_stage = take(L.stage_bytes);
+  L.off_ring = take(RING_BYTES);
+  L.total = o;
+  return true;
+}
+
+}  // namespace
+
+struct plk_instance {
+  plk_config cfg;
+  Layout L;
+  cudaStream_t stream;
+  char* arena;
+  bool f32;
+  bool deferred;  // SP = 64: rescaling deferred to the consumer
+  // buffer tables (host bookkeeping only)
+  std::vector<int> post_slot, post_kind, post_pending_scale;
+  std::vector<char> post_written;
+  std::vector<int> pre_slot;
+  std::vector<char> pre_written, pre_has_mx;
+  std::vector<char> matrix_written, scale_written, eigen_written, q_written;
+  int next_post_slot = 0, next_compact_slot = 0, next_pre_slot = 0;
+  bool have_weights = false, have_pi = false, have_rates = false, have_catw = false;
+  int root_pre_filled = -1;
+  // parameter ring
+  char* h_ring = nullptr;
+  size_t ring_pos = 0;
+  int64_t launches = 0;
+
+  template <typename X> X* at(size_t off) const { return reinterpret_cast<X*>(arena + off); }
+  void* post_ptr(int idx) const {
+    if (post_kind[idx] == KIND_STATES) return arena + L.off_compact + (size_t)post_slot[idx] * L.compact_bytes;
+    return arena + L.off_post + (size_t)post_slot[idx] * L.W;
+  }
+  void* pre_ptr(int idx) const { return arena + L.off_pre + (size_t)pre_slot[idx] * L.W; }
+  void* pre_mx_ptr(int idx) const { return arena + L.off_pre_mx + (size_t)pre_slot[idx] * L.mx_bytes; }
+  void* matrix_ptr(int idx) const { return arena + L.off_matrix + (size_t)idx * L.matrix_bytes; }
+  void* scale_ptr(int idx) const { return arena + L.off_scale + (size_t)idx * L.scale_bytes; }
+  char* eigen_base(int idx) const { return arena + L.off_eigen + (size_t)idx * L.eigen_bytes; }
+  double* eig_U(int idx) const { return reinterpret_cast<double*>(eigen_base(idx)); }
+  double* eig_Uinv(int idx) const { return eig_U(idx) + L.S * L.S; }
+  double* eig_Q64(int idx) const { return eig_U(idx) + 2 * L.S * L.S; }
+  double* eig_lam(int idx) const { return eig_U(idx) + 3 * L.S * L.S; }
+  void* eig_QT(int idx) const { return eigen_base(idx) + round_up((size_t)(3 * L.S * L.S + L.S) * 8, ALIGN); }
+};
+
+namespace {
+
+#define CU(call)                                  \
+  do {                                            \
+    cudaError_t e_ = (call);                      \
+    if (e_ != cudaSuccess) return PLK_ERR_CUDA;   \
+  } while (0)
+#define CHECK_LAUNCH(inst)                        \
+  do {                                            \
+    ++(inst)->launches;                           \
+    if (cudaGetLastError() != cudaSuccess) return PLK_ERR_CUDA; \
+  } while (0)
+
+// Reserve `bytes` in the parameter ring; returns the host pointer and the matching device pointer.  The host
+// region is copied to the device with copy_ring() after it was filled.  Wrapping synchronises the stream so that
+// earlier asynchronous copies have left the pinned buffer.
+int ring_alloc(plk_instance* in, size_t bytes, char** h, char** d) {
+  bytes = round_up(bytes, 256);
+  if (bytes > RING_BYTES) return PLK_ERR_OUT_OF_MEMORY;
+  if (in->ring_pos + bytes > RING_BYTES) {
+    CU(cudaStreamSynchronize(in->stream));
+    in->ring_pos = 0;
+  }
+  *h = in->h_ring + in->ring_pos;
+  *d = in->arena + in->L.off_ring + in->ring_pos;
+  in->ring_pos += bytes;
+  return PLK_SUCCESS;
+}
+int copy_ring(plk_instance* in, const char* h, char* d, size_t bytes) {
+  CU(cudaMemcpyAsync(d, h, bytes, cudaMemcpyHostToDevice, in->stream));
+  return PLK_SUCCESS;
+}
+
+int bind_post_full(plk_instance* in, int idx, int kind) {
+  if (in->post_slot[idx] >= 0 && in->post_kind[idx] != KIND_STATES) {
+    in->post_kind[idx] = kind;
+    return PLK_SUCCESS;
+  }
+  if (in->next_post_slot >= in->L.post_slots) return PLK_ERR_OUT_OF_MEMORY;
+  in->post_slot[idx] = in->next_post_slot++;
+  in->post_kind[idx] = kind;
+  return PLK_SUCCESS;
+}
+int bind_pre(plk_instance* in, int idx) {
+  if (in->pre_slot[idx] >= 0) return PLK_SUCCESS;
+  if (in->next_pre_slot >= in->L.pre_slots) return PLK_ERR_OUT_OF_MEMORY;
+  in->pre_slot[idx] = in->next_pre_slot++;
+  return PLK_SUCCESS;
+}
+
+template <typename F>
+int by_precision(const plk_instance* in, F&& f) {
+  return in->f32 ? f(float()) : f(double());
+}
+
+inline unsigned blocks_for(size_t n, int threads) { return (unsigned)((n + threads - 1) / threads); }
+
+// host fp64 -> device staging -> padded T rows at dst
+int upload_rows(plk_instance* in, const double* src, void* dst, size_t rows) {
+  const Layout& L = in->L;
+  const size_t bytes = rows * L.S * 8;
+  if (bytes > L.stage_bytes) return PLK_ERR_OUT_OF_MEMORY;
+  double* stage = in->at<double>(L.off_stage);
+  CU(cudaMemcpyAsync(stage, src, bytes, cudaMemcpyHostToDevice, in->stream));
+  int rc = by_precision(in, [&](auto tag) -> int {
+    using T = decltype(tag);
+    k_pad_rows<T><<<blocks_for(rows * L.SP, 256), 256, 0, in->stream>>>(stage, static_cast<T*>(dst), rows, L.S, L.SP);
+    return PLK_SUCCESS;
+  });
+  CHECK_LAUNCH(in);
+  CU(cudaStreamSynchronize(in->stream));  // the staging area is reused by the next setter
+  return rc;
+}
+
+int upload_small(plk_instance* in, const double* src, size_t n, size_t off, size_t n_padded) {
+  std::vector<double> tmp(n_padded, 0.0);
+  for (size_t i = 0; i < n; ++i) {
+    if (!std::isfinite(src[i])) return PLK_ERR_OUT_OF_RANGE;
+    tmp[i] = src[i];
+  }
+  CU(cudaMemcpyAsync(in->arena + off, tmp.data(), n_padded * 8, cudaMemcpyHostToDevice, in->stream));
+  CU(cudaStreamSynchronize(in->stream));
+  return PLK_SUCCESS;
+}
+
+int download(plk_instance* in, double* host, const double* dev, size_t n) {
+  CU(cudaMemcpyAsync(host, dev, n * 8, cudaMemcpyDeviceToHost, in->stream));
+  CU(cudaStreamSynchronize(in->stream));
+  return PLK_SUCCESS;
+}
+
+// ---- kernel dispatch helpers ---------------------------------------------------------------------------------
+template <typename T>
+int launch_post4(plk_instance* in, const DevOp* d_ops, int n_ops) {
+  const Layout& L = in->L;
+  dim3 grid(blocks_for(L.P, NUC_THREADS), n_ops);
+  switch (L.C) {
+#define CASE(CC) case CC: k_post4<T, CC><<<grid, NUC_THREADS, 0, in->stream>>>(d_ops, L.P); break;
+    CASE(1) CASE(2) CASE(3) CASE(4) CASE(5) CASE(6) CASE(7) CASE(8)
+#undef CASE
+    default: return PLK_ERR_UNSUPPORTED;
+  }
+  CHECK_LAUNCH(in);
+  return PLK_SUCCESS;
+}
+
+template <typename T>
+int launch_pre4(plk_instance* in, const DevPreItem* d_items, int n, const T* Q, double* site) {
+  const Layout& L = in->L;
+  dim3 grid(blocks_for(L.P, NUC_THREADS), n);
+  const double* cw = in->at<double>(L.off_catw);
+  const double* cr = in->at<double>(L.off_rates);
+  const double* wt = in->at<double>(L.off_weights);
+  double* gp = in->at<double>(L.off_grad_partial);
+  switch (L.C) {
+#define CASE(CC) case CC: k_pre4<T, CC><<<grid, NUC_THREADS, 0, in->stream>>>(d_items, L.P, Q, cw, cr, wt, gp, L.n_tiles, site); break;
+    CASE(1) CASE(2) CASE(3) CASE(4) CASE(5) CASE(6) CASE(7) CASE(8)
+#undef CASE
+    default: return PLK_ERR_UNSUPPORTED;
+  }
+  CHECK_LAUNCH(in);
+  return PLK_SUCCESS;
+}
+
+template <typename T>
+int launch_deriv4(plk_instance* in, const DevBranch* d_br, int n, const T* Q, double* site) {
+  const Layout& L = in->L;
+  dim3 grid(blocks_for(L.P, NUC_THREADS), n);
+  const double* cw = in->at<double>(L.off_catw);
+  const double* cr = in->at<double>(L.off_rates);
+  const double* wt = in->at<double>(L.off_weights);
+  double* gp = in->at<double>(L.off_grad_partial);
+  switch (L.C) {
+#define CASE(CC) case CC: k_deriv4<T, CC><<<grid, NUC_THREADS, 0, in->stream>>>(d_br, L.P, Q, cw, cr, wt, gp, L.n_tiles, site); break;
+    CASE(1) CASE(2) CASE(3) CASE(4) CASE(5) CASE(6) CASE(7) CASE(8)
+#undef CASE
+    default: return PLK_ERR_UNSUPPORTED;
+  }
+  CHECK_LAUNCH(in);
+  return PLK_SUCCESS;
+}
+
+template <typename K>
+int opt_in_smem(K kernel, size_t bytes) {
+  if (bytes > 48 * 1024) CU(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes));
+  return PLK_SUCCESS;
+}
+
+template <typename T>
+int launch_post64(plk_instance* in, const DevOp* d_ops, int n_ops) {
+  const Layout& L = in->L;
+#ifdef PLK_WITH_TENSOR
+  if (in->cfg.flags & PLK_FLAG_TENSOR_CORES) return tc_launch_post<T>(in->stream, d_ops, n_ops, L.P, L.S, L.C, &in->launches);
+#endif
+  int rc = opt_in_smem(k_post64<T>, post64_smem<T>());
+  if (rc) return rc;
+  dim3 grid(L.n_tiles, L.C, n_ops);
+  k_post64<T><<<grid, GEN_THREADS, post64_smem<T>(), in->stream>>>(d_ops, L.P, L.S, L.C);
+  CHECK_LAUNCH(in);
+  return PLK_SUCCESS;
+}
+
+template <typename T>
+int launch_pre64(plk_instance* in, const DevPreItem* d_items, int n, const T* Q, double* site) {
+  const Layout& L = in->L;
+  const double* cw = in->at<double>(L.off_catw);
+  const double* cr = in->at<double>(L.off_rates);
+  const double* wt = in->at<double>(L.off_weights);
+  double* gp = in->at<double>(L.off_grad_partial);
+#ifdef PLK_WITH_TENSOR
+  if (in->cfg.flags & PLK_FLAG_TENSOR_CORES)
+    return tc_launch_pre<T>(in->stream, d_items, n, L.P, L.S, L.C, Q, cw, cr, wt, gp, L.n_tiles, site, &in->launches);
+#endif
+  int rc = opt_in_smem(k_pre64<T>, pre64_smem<T>());
+  if (rc) return rc;
+  dim3 grid(L.n_tiles, n);
+  k_pre64<T><<<grid, GEN_THREADS, pre64_smem<T>(), in->stream>>>(d_items, L.P, L.S, L.C, Q, cw, cr, wt, gp, L.n_tiles, site);
+  CHECK_LAUNCH(in);
+  return PLK_SUCCESS;
+}
+
+template <typename T>
+int launch_deriv64(plk_instance* in, const DevBranch* d_br, int n, const T* Q, double* site) {
+  const Layout& L = in->L;
+  int rc = opt_in_smem(k_deriv64<T>, deriv64_smem<T>());
+  if (rc) return rc;
+  dim3 grid(L.n_tiles, n);
+  k_deriv64<T><<<grid, GEN_THREADS, deriv64_smem<T>(), in->stream>>>(
+      d_br, L.P, L.S, L.C, Q, in->at<double>(L.off_catw), in->at<double>(L.off_rates), in->at<double>(L.off_weights),
+      in->at<double>(L.off_grad_partial), L.n_tiles, site);
+  CHECK_LAUNCH(in);
+  return PLK_SUCCESS;
+}
+
+int check_model_ready(const plk_instance* in, bool need_rates) {
+  if (!in->have_catw || !in->have_pi || !in->have_weights) return PLK_ERR_UNINITIALIZED;
+  if (need_rates && !in->have_rates) return PLK_ERR_UNINITIALIZED;
+  return PLK_SUCCESS;
+}
+
+// operand description of a post-order buffer used as input
+int operand_of(const plk_instance* in, int idx, const void** ptr, int* kind, const void** pending) {
+  if (idx < 0 || idx >= in->cfg.partials_buffer_count) return PLK_ERR_OUT_OF_RANGE;
+  if (in->post_slot[idx] < 0 || !in->post_written[idx]) return PLK_ERR_UNINITIALIZED;
+  *ptr = in->post_ptr(idx);
+  *kind = in->post_kind[idx];
+  *pending = (in->deferred && in->post_pending_scale[idx] >= 0) ? in->scale_ptr(in->post_pending_scale[idx]) : nullptr;
+  return PLK_SUCCESS;
+}
+
+}  // namespace
+
+// =================================================================================================================
+extern "C" {
+
+size_t plk_arena_bytes(const plk_config* cfg) {
+  Layout L;
+  if (cfg == nullptr || !compute_layout(*cfg, L)) return 0;
+  return L.total;
+}
+
+int plk_create(const plk_config* cfg, void* d_arena, size_t arena_bytes, void* cuda_stream, plk_instance** out) {
+  if (out == nullptr) return PLK_ERR_OUT_OF_RANGE;
+  *out = nullptr;
+  if (cfg == nullptr || d_arena == nullptr) return PLK_ERR_OUT_OF_RANGE;
+  Layout L;
+  if (!compute_layout(*cfg, L)) {
+    if (cfg->state_count < 2 || cfg->state_count > 64) return PLK_ERR_UNSUPPORTED;
+    if (cfg->state_count == 4 && cfg->category_count > 8) return PLK_ERR_UNSUPPORTED;
+    return PLK_ERR_OUT_OF_RANGE;
+  }
+  if (cfg->flags & ~(PLK_FLAG_TENSOR_CORES | PLK_FLAG_NO_LEVEL_BATCH | PLK_FLAG_SITE_DERIVATIVES)) return PLK_ERR_UNSUPPORTED;
+#ifndef PLK_WITH_TENSOR
+  if ((cfg->flags & PLK_FLAG_TENSOR_CORES) && L.SP == 64) return PLK_ERR_UNSUPPORTED;
+#endif
+  if (arena_bytes < L.total) return PLK_ERR_OUT_OF_MEMORY;
+  if (reinterpret_cast<uintptr_t>(d_arena) % ALIGN != 0) return PLK_ERR_OUT_OF_RANGE;
+  int n_dev = 0;
+  if (cudaGetDeviceCount(&n_dev) != cudaSuccess || n_dev == 0) return PLK_ERR_CUDA;
+  plk_instance* in = new (std::nothrow) plk_instance();
+  if (in == nullptr) return PLK_ERR_OUT_OF_MEMORY;
+  in->cfg = *cfg;
+  in->L = L;
+  in->stream = static_cast<cudaStream_t>(cuda_stream);
+  in->arena = static_cast<char*>(d_arena);
+  in->f32 = cfg->precision == PLK_FP32;
+  in->deferred = L.SP != 4;
+  in->post_slot.assign(cfg->partials_buffer_count, -1);
+  in->post_kind.assign(cfg->partials_buffer_count, KIND_PARTIALS);
+  in->post_pending_scale.assign(cfg->partials_buffer_count, -1);
+  in->post_written.assign(cfg->partials_buffer_count, 0);
+  in->pre_slot.assign(cfg->preorder_buffer_count, -1);
+  in->pre_written.assign(cfg->preorder_buffer_count, 0);
+  in->pre_has_mx.assign(cfg->preorder_buffer_count, 0);
+  in->matrix_written.assign(cfg->matrix_buffer_count, 0);
+  in->scale_written.assign(cfg->scale_buffer_count, 0);
+  in->eigen_written.assign(cfg->eigen_buffer_count, 0);
+  in->q_written.assign(cfg->eigen_buffer_count, 0);
+  if (cudaHostAlloc(reinterpret_cast<void**>(&in->h_ring), RING_BYTES, cudaHostAllocDefault) != cudaSuccess) {
+    delete in;
+    return PLK_ERR_CUDA;
+  }
+  // zero everything outside the big partials regions once: padding of matrices / frequencies must be zero
+  const size_t small_from = L.off_matrix;
+  if (cudaMemsetAsync(in->arena + small_from, 0, L.total - small_from, in->stream) != cudaSuccess ||
+      cudaStreamSynchronize(in->stream) != cudaSuccess) {
+    cudaFreeHost(in->h_ring);
+    delete in;
+    return PLK_ERR_CUDA;
+  }
+  *out = in;
+  return PLK_SUCCESS;
+}
+
+int plk_destroy(plk_instance* in) {
+  if (in == nullptr) return PLK_SUCCESS;
+  cudaStreamSynchronize(in->stream);
+  if (in->h_ring) cudaFreeHost(in->h_ring);
+  delete in;
+  return PLK_SUCCESS;
+}
+
+const char* plk_error_string(int status) {
+  switch (status) {
+    case PLK_SUCCESS: return "success";
+    case PLK_ERR_GENERAL: return "general error";
+    case PLK_ERR_OUT_OF_MEMORY: return "arena too small or no free buffer slot";
+    case PLK_ERR_OUT_OF_RANGE: return "index, count, shape or value out of range";
+    case PLK_ERR_UNINITIALIZED: return "buffer or model component read before it was written";
+    case PLK_ERR_UNSUPPORTED: return "unsupported configuration";
+    case PLK_ERR_FLOATING_POINT: return "log-likelihood or derivative is not finite";
+    case PLK_ERR_CUDA: return "CUDA error (no device or a runtime call failed)";
+    case PLK_ERR_STOP_CODON: return "stop codon in a codon alignment";
+    default: return "unknown status";
+  }
+}
+
+// ---- setters ----------------------------------------------------------------------------------------------------
+
+int plk_set_tip_states(plk_instance* in, int tip, const int32_t* states) {
+  if (in == nullptr || states == nullptr) return PLK_ERR_OUT_OF_RANGE;
+  if (tip < 0 || tip >= in->cfg.tip_count) return PLK_ERR_OUT_OF_RANGE;
+  const Layout& L = in->L;
+  if (!(in->post_slot[tip] >= 0 && in->post_kind[tip] == KIND_STATES)) {
+    if (in->post_slot[tip] >= 0) return PLK_ERR_OUT_OF_RANGE;  // already bound as partials
+    if (in->next_compact_slot >= L.compact_slots) return PLK_ERR_OUT_OF_MEMORY;
+    in->post_slot[tip] = in->next_compact_slot++;
+    in->post_kind[tip] = KIND_STATES;
+  }
+  if ((size_t)L.P * 4 > L.stage_bytes) return PLK_ERR_OUT_OF_MEMORY;
+  int32_t* stage = in->at<int32_t>(L.off_stage);
+  CU(cudaMemcpyAsync(stage, states, (size_t)L.P * 4, cudaMemcpyHostToDevice, in->stream));
+  k_pack_states<<<blocks_for(L.P, 256), 256, 0, in->stream>>>(stage, static_cast<uint8_t*>(in->post_ptr(tip)), L.P, L.S);
+  CHECK_LAUNCH(in);
+  CU(cudaStreamSynchronize(in->stream));
+  in->post_written[tip] = 1;
+  in->post_pending_scale[tip] = -1;
+  return PLK_SUCCESS;
+}
+
+int plk_set_tip_partials(plk_instance* in, int tip, const double* partials) {
+  if (in == nullptr || partials == nullptr) return PLK_ERR_OUT_OF_RANGE;
+  if (tip < 0 || tip >= in->cfg.tip_count) return PLK_ERR_OUT_OF_RANGE;
+  if (in->post_slot[tip] >= 0 && in->post_kind[tip] == KIND_STATES) return PLK_ERR_OUT_OF_RANGE;
+  int rc = bind_post_full(in, tip, KIND_BCAST);
+  if (rc) return rc;
+  rc = upload_rows(in, partials, in->post_ptr(tip), (size_t)in->L.P);
+  if (rc) return rc;
+  in->post_written[tip] = 1;
+  in->post_pending_scale[tip] = -1;
+  return PLK_SUCCESS;
+}
+
+int plk_set_partials(plk_instance* in, int buffer, const double* partials) {
+  if (in == nullptr || partials == nullptr) return PLK_ERR_OUT_OF_RANGE;
+  if (buffer < 0 || buffer >= in->cfg.partials_buffer_count) return PLK_ERR_OUT_OF_RANGE;
+  if (in->post_slot[buffer] >= 0 && in->post_kind[buffer] == KIND_STATES) return PLK_ERR_OUT_OF_RANGE;
+  int rc = bind_post_full(in, buffer, KIND_PARTIALS);
+  if (rc) return rc;
+  rc = upload_rows(in, partials, in->post_ptr(buffer), (size_t)in->L.C * in->L.P);
+  if (rc) return rc;
+  in->post_written[buffer] = 1;
+  in->post_pending_scale[buffer] = -1;
+  return PLK_SUCCESS;
+}
+
+int plk_set_pattern_weights(plk_instance* in, const double* w) {
+  if (in == nullptr || w == nullptr) return PLK_ERR_OUT_OF_RANGE;
+  int rc = upload_small(in, w, in->L.P, in->L.off_weights, in->L.P);
+  if (rc == PLK_SUCCESS) in->have_weights = true;
+  return rc;
+}
+int plk_set_state_frequencies(plk_instance* in, const double* pi) {
+  if (in == nullptr || pi == nullptr) return PLK_ERR_OUT_OF_RANGE;
+  int rc = upload_small(in, pi, in->L.S, in->L.off_pi, in->L.SP);
+  if (rc == PLK_SUCCESS) {
+    in->have_pi = true;
+    in->root_pre_filled = -1;
+  }
+  return rc;
+}
+int plk_set_category_rates(plk_instance* in, const double* r) {
+  if (in == nullptr || r == nullptr) return PLK_ERR_OUT_OF_RANGE;
+  int rc = upload_small(in, r, in->L.C, in->L.off_rates, in->L.C);
+  if (rc == PLK_SUCCESS) in->have_rates = true;
+  return rc;
+}
+int plk_set_category_weights(plk_instance* in, const double* w) {
+  if (in == nullptr || w == nullptr) return PLK_ERR_OUT_OF_RANGE;
+  int rc = upload_small(in, w, in->L.C, in->L.off_catw, in->L.C);
+  if (rc == PLK_SUCCESS) in->have_catw = true;
+  return rc;
+}
+
+static int rebuild_rate_matrix(plk_instance* in, int eigen) {
+  const Layout& L = in->L;
+  char *h, *d;
+  int rc = ring_alloc(in, sizeof(void*), &h, &d);
+  if (rc) return rc;
+  void* qt = in->eig_QT(eigen);
+  std::memcpy(h, &qt, sizeof(void*));
+  rc = copy_ring(in, h, d, sizeof(void*));
+  if (rc) return rc;
+  const size_t smem = (size_t)(2 * L.S * L.S + L.S) * 8;
+  rc = by_precision(in, [&](auto tag) -> int {
+    using T = decltype(tag);
+    int r2 = opt_in_smem(k_transition<T>, smem);
+    if (r2) return r2;
+    k_transition<T><<<1, 256, smem, in->stream>>>(in->eig_U(eigen), in->eig_Uinv(eigen), in->eig_lam(eigen), nullptr,
+                                                 nullptr, reinterpret_cast<void* const*>(d), in->eig_Q64(eigen), L.S,
+                                                 L.SP, 1, 1);
+    return PLK_SUCCESS;
+  });
+  if (rc) return rc;
+  CHECK_LAUNCH(in);
+  return PLK_SUCCESS;
+}
+
+int plk_set_eigen_decomposition(plk_instance* in, int eigen, const double* U, const double* Uinv, const double* lam) {
+  if (in == nullptr || U == nullptr || Uinv == nullptr || lam == nullptr) return PLK_ERR_OUT_OF_RANGE;
+  if (eigen < 0 || eigen >= in->cfg.eigen_buffer_count) return PLK_ERR_OUT_OF_RANGE;
+  const int S = in->L.S;
+  for (int i = 0; i < S * S; ++i)
+    if (!std::isfinite(U[i]) || !std::isfinite(Uinv[i])) return PLK_ERR_OUT_OF_RANGE;
+  for (int i = 0; i < S; ++i)
+    if (!std::isfinite(lam[i])) return PLK_ERR_OUT_OF_RANGE;
+  CU(cudaMemcpyAsync(in->eig_U(eigen), U, (size_t)S * S * 8, cudaMemcpyHostToDevice, in->stream));
+  CU(cudaMemcpyAsync(in->eig_Uinv(eigen), Uinv, (size_t)S * S * 8, cudaMemcpyHostToDevice, in->stream));
+  CU(cudaMemcpyAsync(in->eig_lam(eigen), lam, (size_t)S * 8, cudaMemcpyHostToDevice, in->stream));
+  int rc = rebuild_rate_matrix(in, eigen);
+  if (rc) return rc;
+  CU(cudaStreamSynchronize(in->stream));
+  in->eigen_written[eigen] = 1;
+  in->q_written[eigen] = 1;
+  return PLK_SUCCESS;
+}
+
+int plk_set_rate_matrix(plk_instance* in, int eigen, const double* Q) {
+  if (in == nullptr || Q == nullptr) return PLK_ERR_OUT_OF_RANGE;
+  if (eigen < 0 || eigen >= in->cfg.eigen_buffer_count) return PLK_ERR_OUT_OF_RANGE;
+  const Layout& L = in->L;
+  for (int i = 0; i < L.S * L.S; ++i)
+    if (!std::isfinite(Q[i])) return PLK_ERR_OUT_OF_RANGE;
+  CU(cudaMemcpyAsync(in->eig_Q64(eigen), Q, (size_t)L.S * L.S * 8, cudaMemcpyHostToDevice, in->stream));
+  by_precision(in, [&](auto tag) -> int {
+    using T = decltype(tag);
+    k_pad_matrices<T><<<blocks_for((size_t)L.SP * L.SP, 256), 256, 0, in->stream>>>(
+        in->eig_Q64(eigen), static_cast<T*>(in->eig_QT(eigen)), 1, L.S, L.SP);
+    return PLK_SUCCESS;
+  });
+  CHECK_LAUNCH(in);
+  CU(cudaStreamSynchronize(in->stream));
+  in->q_written[eigen] = 1;
+  return PLK_SUCCESS;
+}
+
+int plk_set_transition_matrix(plk_instance* in, int matrix, const double* m) {
+  if (in == nullptr || m == nullptr) return PLK_ERR_OUT_OF_RANGE;
+  if (matrix < 0 || matrix >= in->cfg.matrix_buffer_count) return PLK_ERR_OUT_OF_RANGE;
+  const Layout& L = in->L;
+  const size_t bytes = (size_t)L.C * L.S * L.S * 8;
+  if (bytes > L.stage_bytes) return PLK_ERR_OUT_OF_MEMORY;
+  double* stage = in->at<double>(L.off_stage);
+  CU(cudaMemcpyAsync(stage, m, bytes, cudaMemcpyHostToDevice, in->stream));
+  by_precision(in, [&](auto tag) -> int {
+    using T = decltype(tag);
+    k_pad_matrices<T><<<blocks_for((size_t)L.C * L.SP * L.SP, 256), 256, 0, in->stream>>>(
+        stage, static_cast<T*>(in->matrix_ptr(matrix)), L.C, L.S, L.SP);
+    return PLK_SUCCESS;
+  });
+  CHECK_LAUNCH(in);
+  CU(cudaStreamSynchronize(in->stream));
+  in->matrix_written[matrix] = 1;
+  return PLK_SUCCESS;
+}
+
+// ---- step 1: transition matrices ------------------------------------------------------------------------------
+
+static int update_matrices_impl(plk_instance* in, int eigen, const int32_t* matrix_idx, const double* h_t,
+                                const double* d_t, int count) {
+  if (in == nullptr || count < 0) return PLK_ERR_OUT_OF_RANGE;
+  if (count == 0) return PLK_SUCCESS;
+  if (matrix_idx == nullptr) return PLK_ERR_OUT_OF_RANGE;
+  if (eigen < 0 || eigen >= in->cfg.eigen_buffer_count) return PLK_ERR_OUT_OF_RANGE;
+  if (!in->eigen_written[eigen] || !in->have_rates) return PLK_ERR_UNINITIALIZED;
+  const Layout& L = in->L;
+  for (int i = 0; i < count; ++i) {
+    if (matrix_idx[i] < 0 || matrix_idx[i] >= in->cfg.matrix_buffer_count) return PLK_ERR_OUT_OF_RANGE;
+    if (h_t != nullptr && !(h_t[i] >= 0.0 && std::isfinite(h_t[i]))) return PLK_ERR_OUT_OF_RANGE;
+  }
+  char *h, *d;
+  const size_t ptr_bytes = round_up((size_t)count * sizeof(void*), 256);
+  int rc = ring_alloc(in, ptr_bytes + (size_t)count * 8, &h, &d);
+  if (rc) return rc;
+  void** hp = reinterpret_cast<void**>(h);
+  for (int i = 0; i < count; ++i) hp[i] = in->matrix_ptr(matrix_idx[i]);
+  size_t bytes = ptr_bytes;
+  if (h_t != nullptr) {
+    std::memcpy(h + ptr_bytes, h_t, (size_t)count * 8);
+    bytes += (size_t)count * 8;
+    d_t = reinterpret_cast<const double*>(d + ptr_bytes);
+  }
+  rc = copy_ring(in, h, d, bytes);
+  if (rc) return rc;
+  const size_t smem = (size_t)(2 * L.S * L.S + L.C * L.S) * 8;
+  rc = by_precision(in, [&](auto tag) -> int {
+    using T = decltype(tag);
+    int r2 = opt_in_smem(k_transition<T>, smem);
+    if (r2) return r2;
+    k_transition<T><<<count, 256, smem, in->stream>>>(in->eig_U(eigen), in->eig_Uinv(eigen), in->eig_lam(eigen),
+                                                     in->at<double>(L.off_rates), d_t,
+                                                     reinterpret_cast<void* const*>(d), nullptr, L.S, L.SP, L.C, 0);
+    return PLK_SUCCESS;
+  });
+  if (rc) return rc;
+  CHECK_LAUNCH(in);
+  for (int i = 0; i < count; ++i) in->matrix_written[matrix_idx[i]] = 1;
+  return PLK_SUCCESS;
+}
+
+int plk_update_transition_matrices(plk_instance* in, int eigen, const int32_t* matrix_idx, const double* t, int count) {
+  if (count > 0 && t == nullptr) return PLK_ERR_OUT_OF_RANGE;
+  return update_matrices_impl(in, eigen, matrix_idx, t, nullptr, count);
+}
+int plk_update_transition_matrices_device(plk_instance* in, int eigen, const int32_t* matrix_idx, const double* d_t,
+                                          int count) {
+  if (count > 0 && d_t == nullptr) return PLK_ERR_OUT_OF_RANGE;
+  return update_matrices_impl(in, eigen, matrix_idx, nullptr, d_t, count);
+}
+
+// ---- steps 2-3: post-order ---------------------------------------------------------------------------------------
+
+int plk_update_partials(plk_instance* in, const plk_op* ops, int count) {
+  if (in == nullptr || count < 0) return PLK_ERR_OUT_OF_RANGE;
+  if (count == 0) return PLK_SUCCESS;
+  std::vector<int> level;
+  const int n_levels = schedule_post(ops, count, level);
+  if (n_levels < 0) return n_levels;
+  const plk_config& cfg = in->cfg;
+  // validate everything before touching any state
+  for (int i = 0; i < count; ++i) {
+    const plk_op& o = ops[i];
+    if (o.dest >= cfg.partials_buffer_count || o.child1 >= cfg.partials_buffer_count ||
+        o.child2 >= cfg.partials_buffer_count || o.child1_matrix >= cfg.matrix_buffer_count ||
+        o.child2_matrix >= cfg.matrix_buffer_count || o.dest_scale >= cfg.scale_buffer_count || o.dest_scale < -1)
+      return PLK_ERR_OUT_OF_RANGE;
+    if (!in->matrix_written[o.child1_matrix] || !in->matrix_written[o.child2_matrix]) return PLK_ERR_UNINITIALIZED;
+    if (in->post_slot[o.dest] >= 0 && in->post_kind[o.dest] == KIND_STATES) return PLK_ERR_OUT_OF_RANGE;
+  }
+  {  // children must be written already or produced earlier in this list
+    std::vector<char> will(cfg.partials_buffer_count, 0);
+    int fresh = 0;
+    for (int i = 0; i < count; ++i) {
+      const plk_op& o = ops[i];
+      if (!(in->post_written[o.child1] || will[o.child1]) || !(in->post_written[o.child2] || will[o.child2]))
+        return PLK_ERR_UNINITIALIZED;
+      if (in->post_slot[o.dest] < 0 && !will[o.dest]) ++fresh;
+      will[o.dest] = 1;
+    }
+    if (in->next_post_slot + fresh > in->L.post_slots) return PLK_ERR_OUT_OF_MEMORY;
+  }
+  // host bookkeeping in list order, launch items sorted by level
+  std::vector<DevOp> items(count);
+  for (int i = 0; i < count; ++i) {
+    const plk_op& o = ops[i];
+    int rc = bind_post_full(in, o.dest, KIND_PARTIALS);
+    if (rc) return rc;
+    DevOp& d = items[i];
+    d.dest = in->post_ptr(o.dest);
+    const int ch[2] = {o.child1, o.child2};
+    const int mt[2] = {o.child1_matrix, o.child2_matrix};
+    for (int k = 0; k < 2; ++k) {
+      rc = operand_of(in, ch[k], &d.child[k], &d.kind[k], &d.cscale[k]);
+      if (rc) return rc;
+      d.mat[k] = in->matrix_ptr(mt[k]);
+    }
+    d.scale = o.dest_scale >= 0 ? in->scale_ptr(o.dest_scale) : nullptr;
+    in->post_written[o.dest] = 1;
+    in->post_pending_scale[o.dest] = in->deferred ? o.dest_scale : -1;
+    if (o.dest_scale >= 0) in->scale_written[o.dest_scale] = 1;
+  }
+  std::vector<int> order(count);
+  std::vector<int> level_start(n_levels + 1, 0);
+  if (cfg.flags & PLK_FLAG_NO_LEVEL_BATCH) {
+    for (int i = 0; i < count; ++i) order[i] = i;
+  } else {
+    for (int i = 0; i < count; ++i) ++level_start[level[i] + 1];
+    for (int l = 0; l < n_levels; ++l) level_start[l + 1] += level_start[l];
+    std::vector<int> fill(level_start.begin(), level_start.end() - 1);
+    for (int i = 0; i < count; ++i) order[fill[level[i]]++] = i;
+  }
+  char *h, *d;
+  int rc = ring_alloc(in, (size_t)count * sizeof(DevOp), &h, &d);
+  if (rc) return rc;
+  DevOp* hops = reinterpret_cast<DevOp*>(h);
+  for (int i = 0; i < count; ++i) hops[i] = items[order[i]];
+  rc = copy_ring(in, h, d, (size_t)count * sizeof(DevOp));
+  if (rc) return rc;
+  const DevOp* dops = reinterpret_cast<const DevOp*>(d);
+  auto launch = [&](int first, int n) {
+    return by_precision(in, [&](auto tag) -> int {
+      using T = decltype(tag);
+      return in->L.SP == 4 ? launch_post4<T>(in, dops + first, n) : launch_post64<T>(in, dops + first, n);
+    });
+  };
+  if (cfg.flags & PLK_FLAG_NO_LEVEL_BATCH) {
+    for (int i = 0; i < count; ++i) {
+      rc = launch(i, 1);
+      if (rc) return rc;
+    }
+  } else {
+    for (int l = 0; l < n_levels; ++l) {
+      const int n = level_start[l + 1] - level_start[l];
+      for (int first = 0; first < n; first += 32768) {  // grid.y / grid.z limit
+        rc = launch(level_start[l] + first, n - first < 32768 ? n - first : 32768);
+        if (rc) return rc;
+      }
+    }
+  }
+  return PLK_SUCCESS;
+}
+
+// ---- step 4: root ---------------------------------------------------------------------------------------------------
+
+static int root_impl(plk_instance* in, int root, const int32_t* scale_idx, int scale_count, double* d_sum,
+                     double* d_site) {
+  const Layout& L = in->L;
+  const plk_config& cfg = in->cfg;
+  if (scale_count < 0 || (scale_count > 0 && scale_idx == nullptr)) return PLK_ERR_OUT_OF_RANGE;
+  int rc = check_model_ready(in, false);
+  if (rc) return rc;
+  const void* rptr;
+  const void* pending;
+  int kind;
+  rc = operand_of(in, root, &rptr, &kind, &pending);
+  if (rc) return rc;
+  if (kind == KIND_STATES) return PLK_ERR_OUT_OF_RANGE;
+  for (int i = 0; i < scale_count; ++i) {
+    if (scale_idx[i] < 0 || scale_idx[i] >= cfg.scale_buffer_count) return PLK_ERR_OUT_OF_RANGE;
+    if (!in->scale_written[scale_idx[i]]) return PLK_ERR_UNINITIALIZED;
+  }
+  // deferred rescaling: the root's own pending factor is not applied to the stored values, so it must not be
+  // counted: drop it from the list
+  std::vector<const void*> list;
+  const int own = in->deferred ? in->post_pending_scale[root] : -1;
+  bool own_listed = false;
+  for (int i = 0; i < scale_count; ++i) {
+    if (scale_idx[i] == own && !own_listed) {
+      own_listed = true;
+      continue;
+    }
+    list.push_back(in->scale_ptr(scale_idx[i]));
+  }
+  if (own >= 0 && !own_listed) return PLK_ERR_UNSUPPORTED;  // would need the factor applied with negative sign
+  char *h = nullptr, *d = nullptr;
+  if (!list.empty()) {
+    rc = ring_alloc(in, list.size() * sizeof(void*), &h, &d);
+    if (rc) return rc;
+    std::memcpy(h, list.data(), list.size() * sizeof(void*));
+    rc = copy_ring(in, h, d, list.size() * sizeof(void*));
+    if (rc) return rc;
+  }
+  double* bp = in->at<double>(L.off_block_partial);
+  const int G = L.SP == 4 ? 1 : 16;
+  const int n_blocks = (int)blocks_for((size_t)L.P * G, 128);
+  by_precision(in, [&](auto tag) -> int {
+    using T = decltype(tag);
+    const T* r = static_cast<const T*>(rptr);
+    if (L.SP == 4)
+      k_root<T, 4, 1><<<n_blocks, 128, 0, in->stream>>>(r, kind, L.P, L.C, in->at<double>(L.off_pi),
+                                                        in->at<double>(L.off_catw),
+                                                        reinterpret_cast<const void* const*>(d), (int)list.size(),
+                                                        in->at<double>(L.off_weights), d_site, bp);
+    else
+      k_root<T, 64, 16><<<n_blocks, 128, 0, in->stream>>>(r, kind, L.P, L.C, in->at<double>(L.off_pi),
+                                                          in->at<double>(L.off_catw),
+                                                          reinterpret_cast<const void* const*>(d), (int)list.size(),
+                                                          in->at<double>(L.off_weights), d_site, bp);
+    return PLK_SUCCESS;
+  });
+  CHECK_LAUNCH(in);
+  k_sum_rows<<<1, 128, 0, in->stream>>>(bp, n_blocks, n_blocks, d_sum);
+  CHECK_LAUNCH(in);
+  return PLK_SUCCESS;
+}
+
+int plk_root_log_likelihoods_device(plk_instance* in, int root, const int32_t* scale_idx, int scale_count,
+                                    double* d_out_sum, double* d_out_site) {
+  if (in == nullptr || d_out_sum == nullptr) return PLK_ERR_OUT_OF_RANGE;
+  return root_impl(in, root, scale_idx, scale_count, d_out_sum, d_out_site);
+}
+
+int plk_root_log_likelihoods(plk_instance* in, int root, const int32_t* scale_idx, int scale_count, double* out_sum,
+                             double* out_site) {
+  if (in == nullptr || out_sum == nullptr) return PLK_ERR_OUT_OF_RANGE;
+  const Layout& L = in->L;
+  double* d_sum = in->at<double>(L.off_logl);
+  double* d_site = in->at<double>(L.off_site);
+  int rc = root_impl(in, root, scale_idx, scale_count, d_sum, d_site);
+  if (rc) return rc;
+  if (out_site != nullptr) CU(cudaMemcpyAsync(out_site, d_site, (size_t)L.P * 8, cudaMemcpyDeviceToHost, in->stream));
+  rc = download(in, out_sum, d_sum, 1);
+  if (rc) return rc;
+  return std::isfinite(*out_sum) ? PLK_SUCCESS : PLK_ERR_FLOATING_POINT;
+}
+
+// ---- steps 5-6: pre-order and derivatives --------------------------------------------------------------------------
+
+static int fill_root_pre(plk_instance* in, int root_pre) {
+  const Layout& L = in->L;
+  if (root_pre < 0 || root_pre >= in->cfg.preorder_buffer_count) return PLK_ERR_OUT_OF_RANGE;
+  if (!in->have_pi) return PLK_ERR_UNINITIALIZED;
+  int rc = bind_pre(in, root_pre);
+  if (rc) return rc;
+  if (in->root_pre_filled != root_pre || !in->pre_written[root_pre]) {
+    const size_t n = (size_t)L.C * L.P * L.SP;
+    by_precision(in, [&](auto tag) -> int {
+      using T = decltype(tag);
+      k_fill_root_pre<T><<<blocks_for(n, 256), 256, 0, in->stream>>>(static_cast<T*>(in->pre_ptr(root_pre)),
+                                                                     in->at<double>(L.off_pi), n, L.SP);
+      return PLK_SUCCESS;
+    });
+    CHECK_LAUNCH(in);
+    in->root_pre_filled = root_pre;
+  }
+  in->pre_written[root_pre] = 1;
+  in->pre_has_mx[root_pre] = 0;
+  return PLK_SUCCESS;
+}
+
+// Shared by plk_update_pre_partials (want_grad = false) and plk_pre_order_gradient.
+static int pre_impl(plk_instance* in, int eigen, int root_pre, const plk_pre_op* ops, int count, bool want_grad,
+                    double* d_grad, double* d_site) {
+  const Layout& L = in->L;
+  const plk_config& cfg = in->cfg;
+  if (count < 0) return PLK_ERR_OUT_OF_RANGE;
+  if (cfg.preorder_buffer_count == 0) return PLK_ERR_UNSUPPORTED;
+  if (want_grad) {
+    if (eigen < 0 || eigen >= cfg.eigen_buffer_count) return PLK_ERR_OUT_OF_RANGE;
+    if (!in->q_written[eigen]) return PLK_ERR_UNINITIALIZED;
+    int rc = check_model_ready(in, true);
+    if (rc) return rc;
+    if (count > L.max_grad) return PLK_ERR_OUT_OF_RANGE;
+  }
+  std::vector<int> level, partner;
+  const int n_levels = schedule_pre(ops, count, level, partner);
+  if (n_levels < 0) return n_levels;
+  for (int i = 0; i < count; ++i) {
+    const plk_pre_op& o = ops[i];
+    if (o.dest_pre >= cfg.preorder_buffer_count || o.parent_pre >= cfg.preorder_buffer_count ||
+        o.matrix >= cfg.matrix_buffer_count || o.sibling_matrix >= cfg.matrix_buffer_count ||
+        o.sibling_post >= cfg.partials_buffer_count || o.node_post >= cfg.partials_buffer_count || o.node_post < -1)
+      return PLK_ERR_OUT_OF_RANGE;
+    if (want_grad && o.node_post < 0) return PLK_ERR_OUT_OF_RANGE;
+    if (!want_grad && o.dest_pre < 0) return PLK_ERR_OUT_OF_RANGE;
+    if (!in->matrix_written[o.matrix] || !in->matrix_written[o.sibling_matrix]) return PLK_ERR_UNINITIALIZED;
+  }
+  int rc = fill_root_pre(in, root_pre);
+  if (rc) return rc;
+  {  // parents must be written already or produced earlier in this list; count fresh slots
+    std::vector<char> will(cfg.preorder_buffer_count, 0);
+    int fresh = 0;
+    for (int i = 0; i < count; ++i) {
+      const plk_pre_op& o = ops[i];
+      if (!(in->pre_written[o.parent_pre] || will[o.parent_pre])) return PLK_ERR_UNINITIALIZED;
+      if (o.dest_pre >= 0) {
+        if (in->pre_slot[o.dest_pre] < 0 && !will[o.dest_pre]) ++fresh;
+        will[o.dest_pre] = 1;
+      }
+    }
+    if (in->next_pre_slot + fresh > L.pre_slots) return PLK_ERR_OUT_OF_MEMORY;
+  }
+  // build items in list order (bookkeeping), one per pair / unpaired op
+  struct HostItem { DevPreItem it; int level; };
+  std::vector<HostItem> items;
+  items.reserve(count);
+  for (int i = 0; i < count; ++i) {
+    if (partner[i] >= 0 && partner[i] < i) continue;  // emitted with its partner
+    const plk_pre_op& a = ops[i];
+    DevPreItem it;
+    std::memset(&it, 0, sizeof(it));
+    it.qm = in->pre_ptr(a.parent_pre);
+    it.qm_scale = (in->deferred && in->pre_has_mx[a.parent_pre]) ? in->pre_mx_ptr(a.parent_pre) : nullptr;
+    const plk_pre_op* pair[2] = {&a, partner[i] >= 0 ? &ops[partner[i]] : nullptr};
+    const int op_index[2] = {i, partner[i]};
+    // operands: child 0 = a's node, child 1 = a's sibling (= partner's node)
+    int post_idx[2] = {a.node_post, a.sibling_post};
+    if (pair[1] != nullptr) {
+      if (post_idx[0] < 0) post_idx[0] = pair[1]->sibling_post;
+      if (pair[1]->node_post >= 0 && pair[1]->node_post != a.sibling_post) return PLK_ERR_OUT_OF_RANGE;
+      if (a.node_post >= 0 && pair[1]->sibling_post != a.node_post) return PLK_ERR_OUT_OF_RANGE;
+    }
+    const int mats[2] = {a.matrix, a.sibling_matrix};
+    for (int k = 0; k < 2; ++k) {
+      it.mat[k] = in->matrix_ptr(mats[k]);
+      if (post_idx[k] >= 0) {
+        rc = operand_of(in, post_idx[k], &it.p[k], &it.kind[k], &it.p_scale[k]);
+        if (rc) return rc;
+      } else {
+        it.p[k] = nullptr;
+        it.kind[k] = KIND_NONE;
+        it.p_scale[k] = nullptr;
+      }
+      it.slot[k] = -1;
+      it.q[k] = nullptr;
+      it.q_scale[k] = nullptr;
+      if (pair[k] != nullptr) {
+        if (want_grad) it.slot[k] = op_index[k];
+        if (pair[k]->dest_pre >= 0) {
+          rc = bind_pre(in, pair[k]->dest_pre);
+          if (rc) return rc;
+          it.q[k] = in->pre_ptr(pair[k]->dest_pre);
+          it.q_scale[k] = in->deferred ? in->pre_mx_ptr(pair[k]->dest_pre) : nullptr;
+        }
+      }
+    }
+    items.push_back({it, level[i]});
+    // bookkeeping after the item's inputs were resolved
+    for (int k = 0; k < 2; ++k)
+      if (pair[k] != nullptr && pair[k]->dest_pre >= 0) {
+        in->pre_written[pair[k]->dest_pre] = 1;
+        in->pre_has_mx[pair[k]->dest_pre] = in->deferred ? 1 : 0;
+        if (in->root_pre_filled == pair[k]->dest_pre) in->root_pre_filled = -1;
+      }
+  }
+  const int n_items = (int)items.size();
+  if (n_items > 0) {
+    std::vector<int> level_start(n_levels + 1, 0);
+    for (const HostItem& hi : items) ++level_start[hi.level + 1];
+    for (int l = 0; l < n_levels; ++l) level_start[l + 1] += level_start[l];
+    std::vector<int> fill(level_start.begin(), level_start.end() - 1);
+    char *h, *d;
+    rc = ring_alloc(in, (size_t)n_items * sizeof(DevPreItem), &h, &d);
+    if (rc) return rc;
+    DevPreItem* hit = reinterpret_cast<DevPreItem*>(h);
+    for (const HostItem& hi : items) hit[fill[hi.level]++] = hi.it;
+    rc = copy_ring(in, h, d, (size_t)n_items * sizeof(DevPreItem));
+    if (rc) return rc;
+    const DevPreItem* dit = reinterpret_cast<const DevPreItem*>(d);
+    const void* Q = want_grad ? in->eig_QT(eigen) : in->eig_QT(0);
+    for (int l = 0; l < n_levels; ++l) {
+      const int n = level_start[l + 1] - level_start[l];
+      for (int first = 0; first < n; first += 32768) {
+        const int m = n - first < 32768 ? n - first : 32768;
+        rc = by_precision(in, [&](auto tag) -> int {
+          using T = decltype(tag);
+          const DevPreItem* p0 = dit + level_start[l] + first;
+          return L.SP == 4 ? launch_pre4<T>(in, p0, m, static_cast<const T*>(Q), d_site)
+                           : launch_pre64<T>(in, p0, m, static_cast<const T*>(Q), d_site);
+        });
+        if (rc) return rc;
+      }
+    }
+  }
+  if (want_grad && count > 0) {
+    k_sum_rows<<<count, 128, 0, in->stream>>>(in->at<double>(L.off_grad_partial), L.n_tiles, L.n_tiles, d_grad);
+    CHECK_LAUNCH(in);
+  }
+  return PLK_SUCCESS;
+}
+
+int plk_update_pre_partials(plk_instance* in, int root_pre, const plk_pre_op* ops, int count) {
+  if (in == nullptr) return PLK_ERR_OUT_OF_RANGE;
+  return pre_impl(in, 0, root_pre, ops, count, false, nullptr, nullptr);
+}
+
+int plk_pre_order_gradient_device(plk_instance* in, int eigen, int root_pre, const plk_pre_op* ops, int count,
+                                  double* d_out_gradient, double* d_out_site) {
+  if (in == nullptr || (count > 0 && d_out_gradient == nullptr)) return PLK_ERR_OUT_OF_RANGE;
+  return pre_impl(in, eigen, root_pre, ops, count, true, d_out_gradient, d_out_site);
+}
+
+static int finish_gradient(plk_instance* in, int count, double* out_gradient, double* out_site, double* d_site) {
+  const Layout& L = in->L;
+  if (count == 0) return PLK_SUCCESS;
+  if (out_site != nullptr)
+    CU(cudaMemcpyAsync(out_site, d_site, (size_t)count * L.P * 8, cudaMemcpyDeviceToHost, in->stream));
+  int rc = download(in, out_gradient, in->at<double>(L.off_grad_out), count);
+  if (rc) return rc;
+  for (int i = 0; i < count; ++i)
+    if (!std::isfinite(out_gradient[i])) return PLK_ERR_FLOATING_POINT;
+  return PLK_SUCCESS;
+}
+
+int plk_pre_order_gradient(plk_instance* in, int eigen, int root_pre, const plk_pre_op* ops, int count,
+                           double* out_gradient, double* out_site) {
+  if (in == nullptr || (count > 0 && out_gradient == nullptr)) return PLK_ERR_OUT_OF_RANGE;
+  const Layout& L = in->L;
+  if (out_site != nullptr && !(in->cfg.flags & PLK_FLAG_SITE_DERIVATIVES)) return PLK_ERR_UNSUPPORTED;
+  double* d_site = out_site != nullptr ? in->at<double>(L.off_site_deriv) : nullptr;
+  int rc = pre_impl(in, eigen, root_pre, ops, count, true, in->at<double>(L.off_grad_out), d_site);
+  if (rc) return rc;
+  return finish_gradient(in, count, out_gradient, out_site, d_site);
+}
+
+int plk_branch_derivatives(plk_instance* in, int eigen, const int32_t* post_idx, const int32_t* pre_idx, int count,
+                           double* out_gradient, double* out_site) {
+  if (in == nullptr || count < 0) return PLK_ERR_OUT_OF_RANGE;
+  if (count == 0) return PLK_SUCCESS;
+  if (post_idx == nullptr || pre_idx == nullptr || out_gradient == nullptr) return PLK_ERR_OUT_OF_RANGE;
+  const Layout& L = in->L;
+  const plk_config& cfg = in->cfg;
+  if (cfg.preorder_buffer_count == 0) return PLK_ERR_UNSUPPORTED;
+  if (out_site != nullptr && !(cfg.flags & PLK_FLAG_SITE_DERIVATIVES)) return PLK_ERR_UNSUPPORTED;
+  if (eigen < 0 || eigen >= cfg.eigen_buffer_count || count > L.max_grad) return PLK_ERR_OUT_OF_RANGE;
+  if (!in->q_written[eigen]) return PLK_ERR_UNINITIALIZED;
+  int rc = check_model_ready(in, true);
+  if (rc) return rc;
+  char *h, *d;
+  rc = ring_alloc(in, (size_t)count * sizeof(DevBranch), &h, &d);
+  if (rc) return rc;
+  DevBranch* hb = reinterpret_cast<DevBranch*>(h);
+  for (int i = 0; i < count; ++i) {
+    if (pre_idx[i] < 0 || pre_idx[i] >= cfg.preorder_buffer_count) return PLK_ERR_OUT_OF_RANGE;
+    if (in->pre_slot[pre_idx[i]] < 0 || !in->pre_written[pre_idx[i]]) return PLK_ERR_UNINITIALIZED;
+    const void* pending;
+    rc = operand_of(in, post_idx[i], &hb[i].p, &hb[i].kind, &pending);
+    if (rc) return rc;
+    hb[i].q = in->pre_ptr(pre_idx[i]);
+    hb[i].slot = i;
+  }
+  rc = copy_ring(in, h, d, (size_t)count * sizeof(DevBranch));
+  if (rc) return rc;
+  double* d_site = out_site != nullptr ? in->at<double>(L.off_site_deriv) : nullptr;
+  const DevBranch* db = reinterpret_cast<const DevBranch*>(d);
+  for (int first = 0; first < count; first += 32768) {
+    const int m = count - first < 32768 ? count - first : 32768;
+    rc = by_precision(in, [&](auto tag) -> int {
+      using T = decltype(tag);
+      const T* Q = static_cast<const T*>(in->eig_QT(eigen));
+      return L.SP == 4 ? launch_deriv4<T>(in, db + first, m, Q, d_site) : launch_deriv64<T>(in, db + first, m, Q, d_site);
+    });
+    if (rc) return rc;
+  }
+  k_sum_rows<<<count, 128, 0, in->stream>>>(in->at<double>(L.off_grad_partial), L.n_tiles, L.n_tiles,
+                                            in->at<double>(L.off_grad_out));
+  CHECK_LAUNCH(in);
+  return finish_gradient(in, count, out_gradient, out_site, d_site);
+}
+
+// ---- read-back -------------------------------------------------------------------------------------------------------
+
+int plk_get_partials(plk_instance* in, int buffer, int pre, double* out) {
+  if (in == nullptr || out == nullptr) return PLK_ERR_OUT_OF_RANGE;
+  const Layout& L = in->L;
+  const size_t rows = (size_t)L.C * L.P;
+  double* stage = in->at<double>(L.off_stage);
+  const void* src;
+  int kind = KIND_PARTIALS;
+  if (pre) {
+    if (buffer < 0 || buffer >= in->cfg.preorder_buffer_count) return PLK_ERR_OUT_OF_RANGE;
+    if (in->pre_slot[buffer] < 0 || !in->pre_written[buffer]) return PLK_ERR_UNINITIALIZED;
+    src = in->pre_ptr(buffer);
+  } else {
+    const void* pending;
+    int rc = operand_of(in, buffer, &src, &kind, &pending);
+    if (rc) return rc;
+  }
+  if (kind == KIND_STATES) {
+    k_expand_states<<<blocks_for(rows * L.S, 256), 256, 0, in->stream>>>(static_cast<const uint8_t*>(src), stage, L.C,
+                                                                        L.P, L.S);
+    CHECK_LAUNCH(in);
+  } else {
+    const int reps = kind == KIND_BCAST ? L.C : 1;
+    const size_t n_rows = kind == KIND_BCAST ? (size_t)L.P : rows;
+    for (int r = 0; r < reps; ++r) {
+      by_precision(in, [&](auto tag) -> int {
+        using T = decltype(tag);
+        k_unpad_rows<T><<<blocks_for(n_rows * L.S, 256), 256, 0, in->stream>>>(
+            static_cast<const T*>(src), stage + (size_t)r * L.P * L.S, n_rows, L.S, L.SP);
+        return PLK_SUCCESS;
+      });
+      CHECK_LAUNCH(in);
+    }
+  }
+  return download(in, out, stage, rows * L.S);
+}
+
+int plk_get_scale_factors(plk_instance* in, int scale, double* out) {
+  if (in == nullptr || out == nullptr) return PLK_ERR_OUT_OF_RANGE;
+  if (scale < 0 || scale >= in->cfg.scale_buffer_count) return PLK_ERR_OUT_OF_RANGE;
+  if (!in->scale_written[scale]) return PLK_ERR_UNINITIALIZED;
+  const Layout& L = in->L;
+  double* stage = in->at<double>(L.off_stage);
+  by_precision(in, [&](auto tag) -> int {
+    using T = decltype(tag);
+    k_scale_logs<T><<<blocks_for(L.P, 256), 256, 0, in->stream>>>(in->scale_ptr(scale), stage, L.P, L.C,
+                                                                  in->deferred ? 1 : 0);
+    return PLK_SUCCESS;
+  });
+  CHECK_LAUNCH(in);
+  return download(in, out, stage, L.P);
+}
+
+int plk_get_transition_matrix(plk_instance* in, int matrix, double* out) {
+  if (in == nullptr || out == nullptr) return PLK_ERR_OUT_OF_RANGE;
+  if (matrix < 0 || matrix >= in->cfg.matrix_buffer_count) return PLK_ERR_OUT_OF_RANGE;
+  if (!in->matrix_written[matrix]) return PLK_ERR_UNINITIALIZED;
+  const Layout& L = in->L;
+  double* stage = in->at<double>(L.off_stage);
+  by_precision(in, [&](auto tag) -> int {
+    using T = decltype(tag);
+    k_unpad_matrices<T><<<blocks_for((size_t)L.C * L.S * L.S, 256), 256, 0, in->stream>>>(
+        static_cast<const T*>(in->matrix_ptr(matrix)), stage, L.C, L.S, L.SP);
+    return PLK_SUCCESS;
+  });
+  CHECK_LAUNCH(in);
+  return download(in, out, stage, (size_t)L.C * L.S * L.S);
+}
+
+int plk_get_rate_matrix(plk_instance* in, int eigen, double* out) {
+  if (in == nullptr || out == nullptr) return PLK_ERR_OUT_OF_RANGE;
+  if (eigen < 0 || eigen >= in->cfg.eigen_buffer_count) return PLK_ERR_OUT_OF_RANGE;
+  if (!in->q_written[eigen]) return PLK_ERR_UNINITIALIZED;
+  return download(in, out, in->eig_Q64(eigen), (size_t)in->L.S * in->L.S);
+}
+
+int plk_synchronize(plk_instance* in) {
+  if (in == nullptr) return PLK_ERR_OUT_OF_RANGE;
+  CU(cudaStreamSynchronize(in->stream));
+  return PLK_SUCCESS;
+}
+
+int64_t plk_kernel_launch_count(const plk_instance* in) { return in == nullptr ? 0 : in->launches; }
+
+// ---- host-only helpers -------------------------------------------------------------------------------------------------
+
+int plk_schedule_levels(const plk_op* ops, int count, int32_t* out_level) {
+  std::vector<int> level;
+  const int n = schedule_post(ops, count, level);
+  if (n >= 0 && out_level != nullptr)
+    for (int i = 0; i < count; ++i) out_level[i] = level[i];
+  return n;
+}
+
+int plk_schedule_pre_levels(const plk_pre_op* ops, int count, int32_t* out_level, int32_t* out_partner) {
+  std::vector<int> level, partner;
+  const int n = schedule_pre(ops, count, level, partner);
+  if (n >= 0)
+    for (int i = 0; i < count; ++i) {
+      if (out_level != nullptr) out_level[i] = level[i];
+      if (out_partner != nullptr) out_partner[i] = partner[i];
+    }
+  return n;
+}
+
+}  // extern "C"

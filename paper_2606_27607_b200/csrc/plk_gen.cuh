@@ -1,0 +1,420 @@
+// plk_gen.cuh -- CUDA-core kernels for state counts padded to SP = 64 (61-state codon models): the comparison arm
+// BASELINE.json configs[2] asks for ("CUDA-core vs tensor-core partials update") and the path used when the
+// instance was created without PLK_FLAG_TENSOR_CORES.
+//
+// A block of 256 threads handles one (operation, category, tile of 32 patterns).  Thread (pp = tid / 8, sb = tid % 8)
+// owns 8 output states of pattern pp: chunks of VEC = 16 / sizeof(T) consecutive states, interleaved over sb so that
+// the 8 lanes of one pattern read 128 contiguous bytes of a matrix row from shared memory (conflict-free 128-bit
+// loads) while the operand value is a broadcast.  Matrices are staged in shared memory as A[x][s] (i.e. transposed
+// on load for M.x, natural for M^T.x).
+//
+// Rescaling is DEFERRED: a node stores its partials unscaled together with
+// mx[c][p] = max_s p[c][p][s]; whoever reads the node multiplies M.x by 2^-e, e = exponent of max_c mx[c][p].
+// This keeps the (operation, category, tile) work items independent of one another.
+#pragma once
+#include "plk_common.cuh"
+
+namespace plk {
+
+constexpr int SP64 = 64;
+constexpr int GEN_TP = 32;        // patterns per tile
+constexpr int GEN_THREADS = 256;  // 32 patterns x 8 state-lanes
+
+template <typename T>
+struct Gen {
+  static constexpr int VEC = 16 / sizeof(T);  // 4 (fp32) or 2 (fp64)
+  static constexpr int NCH = 8 / VEC;         // chunks per thread
+  static constexpr int TS = SP64 + VEC;       // padded tile row stride
+};
+template <typename T>
+struct VecOf;
+template <>
+struct VecOf<float> {
+  using type = float4;
+};
+template <>
+struct VecOf<double> {
+  using type = double2;
+};
+
+__device__ __forceinline__ void unpack(const float4& v, float* o) { o[0] = v.x; o[1] = v.y; o[2] = v.z; o[3] = v.w; }
+__device__ __forceinline__ void unpack(const double2& v, double* o) { o[0] = v.x; o[1] = v.y; }
+__device__ __forceinline__ float4 pack(const float* o, float4) { return make_float4(o[0], o[1], o[2], o[3]); }
+__device__ __forceinline__ double2 pack(const double* o, double2) { return make_double2(o[0], o[1]); }
+
+// state owned by (sb, chunk i, element j)
+template <typename T>
+__device__ __forceinline__ int state_of(int sb, int i, int j) {
+  return (Gen<T>::VEC * 8) * i + Gen<T>::VEC * sb + j;
+}
+
+// A[x][s] <- transpose ? M[s][x] : M[x][s]    (M row-major [64][64] in global memory)
+template <typename T>
+__device__ __forceinline__ void fill_matrix(T* __restrict__ A, const T* __restrict__ M, bool transpose) {
+  for (int idx = threadIdx.x; idx < SP64 * SP64; idx += GEN_THREADS) {
+    const T v = M[idx];
+    const int r = idx >> 6, col = idx & 63;
+    if (transpose) A[col * SP64 + r] = v; else A[idx] = v;
+  }
+}
+
+// tile[pp][x] for patterns p0..p0+31 of one operand; rows beyond P are zero
+template <typename T>
+__device__ __forceinline__ void load_tile(T* __restrict__ tile, int kind, const void* ptr, int c, int p0, int P, int S) {
+  constexpr int VEC = Gen<T>::VEC, TS = Gen<T>::TS, CPR = SP64 / VEC;  // chunks per row
+  using V = typename VecOf<T>::type;
+  if (kind == KIND_NONE) {
+    for (int idx = threadIdx.x; idx < GEN_TP * TS; idx += GEN_THREADS) tile[idx] = T(0);
+  } else if (kind == KIND_STATES) {
+    const uint8_t* st = static_cast<const uint8_t*>(ptr);
+    for (int idx = threadIdx.x; idx < GEN_TP * SP64; idx += GEN_THREADS) {
+      const int row = idx >> 6, x = idx & 63;
+      T v = T(0);
+      if (p0 + row < P) {
+        const int z = st[p0 + row];
+        v = (z >= S) ? (x < S ? T(1) : T(0)) : (x == z ? T(1) : T(0));
+      }
+      tile[row * TS + x] = v;
+    }
+  } else {
+    const T* base = static_cast<const T*>(ptr) + (kind == KIND_BCAST ? (size_t)0 : (size_t)c * P * SP64);
+    for (int idx = threadIdx.x; idx < GEN_TP * CPR; idx += GEN_THREADS) {
+      const int row = idx / CPR, ch = idx % CPR;
+      T tmp[VEC];
+      if (p0 + row < P) {
+        unpack(*reinterpret_cast<const V*>(base + (size_t)(p0 + row) * SP64 + ch * VEC), tmp);
+      } else {
+#pragma unroll
+        for (int j = 0; j < VEC; ++j) tmp[j] = T(0);
+      }
+#pragma unroll
+      for (int j = 0; j < VEC; ++j) tile[row * TS + ch * VEC + j] = tmp[j];
+    }
+  }
+}
+
+// pending per-pattern exponent of an operand (deferred rescaling); 0 when it carries none
+template <typename T>
+__device__ __forceinline__ int pending_exp(const void* mx, int p, int P, int C) {
+  if (mx == nullptr || p >= P) return 0;
+  const T* m = static_cast<const T*>(mx);
+  T v = T(0);
+  for (int c = 0; c < C; ++c) v = fmax(v, m[(size_t)c * P + p]);
+  return exp_of(v);
+}
+
+// acc[i*VEC+j] = sum_x A[x][state_of(sb,i,j)] * vrow[x]
+template <typename T>
+__device__ __forceinline__ void mv64(const T* __restrict__ A, const T* __restrict__ vrow, int sb, T acc[8]) {
+  constexpr int VEC = Gen<T>::VEC, NCH = Gen<T>::NCH;
+  using V = typename VecOf<T>::type;
+#pragma unroll
+  for (int k = 0; k < 8; ++k) acc[k] = T(0);
+#pragma unroll 4
+  for (int x = 0; x < SP64; ++x) {
+    const T v = vrow[x];
+#pragma unroll
+    for (int i = 0; i < NCH; ++i) {
+      T a[VEC];
+      unpack(*reinterpret_cast<const V*>(A + x * SP64 + (VEC * 8) * i + VEC * sb), a);
+#pragma unroll
+      for (int j = 0; j < VEC; ++j) acc[i * VEC + j] = fma(a[j], v, acc[i * VEC + j]);
+    }
+  }
+}
+
+// acc = column z of the matrix (row z of A[x][s]); a missing state gives `missing` for real states, 0 for padding
+template <typename T>
+__device__ __forceinline__ void gather64(const T* __restrict__ A, int z, int S, T missing, int sb, T acc[8]) {
+  constexpr int VEC = Gen<T>::VEC, NCH = Gen<T>::NCH;
+#pragma unroll
+  for (int i = 0; i < NCH; ++i)
+#pragma unroll
+    for (int j = 0; j < VEC; ++j) {
+      const int s = state_of<T>(sb, i, j);
+      acc[i * VEC + j] = z < S ? A[z * SP64 + s] : (s < S ? missing : T(0));
+    }
+}
+
+// store 8 owned states of pattern p to dst[p][.] (row stride SP64)
+template <typename T>
+__device__ __forceinline__ void store_states(T* __restrict__ dst_row, int sb, const T acc[8]) {
+  constexpr int VEC = Gen<T>::VEC, NCH = Gen<T>::NCH;
+  using V = typename VecOf<T>::type;
+#pragma unroll
+  for (int i = 0; i < NCH; ++i)
+    *reinterpret_cast<V*>(dst_row + (VEC * 8) * i + VEC * sb) = pack(acc + i * VEC, V());
+}
+
+template <typename T>
+__device__ __forceinline__ T lane8_max(T v) {
+  v = fmax(v, __shfl_xor_sync(0xffffffffu, v, 1));
+  v = fmax(v, __shfl_xor_sync(0xffffffffu, v, 2));
+  v = fmax(v, __shfl_xor_sync(0xffffffffu, v, 4));
+  return v;
+}
+template <typename T>
+__device__ __forceinline__ T lane8_sum(T v) {
+  v += __shfl_xor_sync(0xffffffffu, v, 1);
+  v += __shfl_xor_sync(0xffffffffu, v, 2);
+  v += __shfl_xor_sync(0xffffffffu, v, 4);
+  return v;
+}
+
+template <typename T>
+constexpr size_t post64_smem() {
+  return (2 * SP64 * SP64 + 2 * GEN_TP * Gen<T>::TS) * sizeof(T) + 2 * GEN_TP * sizeof(int);
+}
+template <typename T>
+constexpr size_t pre64_smem() {
+  return (3 * SP64 * SP64 + 5 * GEN_TP * Gen<T>::TS) * sizeof(T) + 3 * GEN_TP * sizeof(int) +
+         4 * GEN_TP * sizeof(double);
+}
+template <typename T>
+constexpr size_t deriv64_smem() {
+  return (SP64 * SP64 + 2 * GEN_TP * Gen<T>::TS) * sizeof(T) + 2 * GEN_TP * sizeof(double);
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// post-order update, one (tile, category, operation) per block (maxima for step 3)
+// ---------------------------------------------------------------------------------------------------------------
+template <typename T>
+__global__ void __launch_bounds__(GEN_THREADS) k_post64(const DevOp* __restrict__ ops, int P, int S, int C) {
+  constexpr int TS = Gen<T>::TS;
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  T* A0 = reinterpret_cast<T*>(smem_raw);
+  T* A1 = A0 + SP64 * SP64;
+  T* V0 = A1 + SP64 * SP64;
+  T* V1 = V0 + GEN_TP * TS;
+  int* sE = reinterpret_cast<int*>(V1 + GEN_TP * TS);
+
+  const DevOp op = ops[blockIdx.z];
+  const int c = blockIdx.y, p0 = blockIdx.x * GEN_TP;
+  const int pp = threadIdx.x >> 3, sb = threadIdx.x & 7, p = p0 + pp;
+
+  fill_matrix<T>(A0, static_cast<const T*>(op.mat[0]) + (size_t)c * SP64 * SP64, true);
+  fill_matrix<T>(A1, static_cast<const T*>(op.mat[1]) + (size_t)c * SP64 * SP64, true);
+  if (op.kind[0] != KIND_STATES) load_tile<T>(V0, op.kind[0], op.child[0], c, p0, P, S);
+  if (op.kind[1] != KIND_STATES) load_tile<T>(V1, op.kind[1], op.child[1], c, p0, P, S);
+  if (threadIdx.x < 2 * GEN_TP) {
+    const int k = threadIdx.x / GEN_TP, r = threadIdx.x % GEN_TP;
+    sE[threadIdx.x] = pending_exp<T>(op.cscale[k], p0 + r, P, C);
+  }
+  __syncthreads();
+
+  T a[8], b[8];
+  if (op.kind[0] == KIND_STATES) {
+    const int z = p < P ? static_cast<const uint8_t*>(op.child[0])[p] : 0;
+    gather64<T>(A0, z, S, T(1), sb, a);
+  } else {
+    mv64<T>(A0, V0 + pp * TS, sb, a);
+  }
+  if (op.kind[1] == KIND_STATES) {
+    const int z = p < P ? static_cast<const uint8_t*>(op.child[1])[p] : 0;
+    gather64<T>(A1, z, S, T(1), sb, b);
+  } else {
+    mv64<T>(A1, V1 + pp * TS, sb, b);
+  }
+  const Pow2Pair<T> f0 = pow2_pair(-sE[pp], T(0)), f1 = pow2_pair(-sE[GEN_TP + pp], T(0));
+  T mx = T(0);
+#pragma unroll
+  for (int k = 0; k < 8; ++k) {
+    a[k] = ((a[k] * f0.f1) * f0.f2) * ((b[k] * f1.f1) * f1.f2);
+    mx = fmax(mx, a[k]);
+  }
+  mx = lane8_max(mx);
+  if (p < P) {
+    store_states<T>(static_cast<T*>(op.dest) + ((size_t)c * P + p) * SP64, sb, a);
+    if (sb == 0 && op.scale != nullptr) static_cast<T*>(op.scale)[(size_t)c * P + p] = mx;
+  }
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// pre-order update of both children of one parent + both branch derivatives
+// one (tile, item) per block, categories looped inside so that num_p and den_p are summed over c in the block
+// ---------------------------------------------------------------------------------------------------------------
+template <typename T>
+__global__ void __launch_bounds__(GEN_THREADS) k_pre64(const DevPreItem* __restrict__ items, int P, int S, int C,
+                                                       const T* __restrict__ Qg, const double* __restrict__ catw,
+                                                       const double* __restrict__ catr,
+                                                       const double* __restrict__ weights,
+                                                       double* __restrict__ grad_partial, int n_tiles,
+                                                       double* __restrict__ site_out) {
+  constexpr int TS = Gen<T>::TS;
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  T* B0 = reinterpret_cast<T*>(smem_raw);
+  T* B1 = B0 + SP64 * SP64;
+  T* BQ = B1 + SP64 * SP64;
+  T* tQM = BQ + SP64 * SP64;
+  T* tX[2] = {tQM + GEN_TP * TS, tQM + 2 * GEN_TP * TS};
+  T* tU[2] = {tQM + 3 * GEN_TP * TS, tQM + 4 * GEN_TP * TS};
+  int* sE = reinterpret_cast<int*>(tQM + 5 * GEN_TP * TS);              // [3][32]: child0, child1, parent q
+  double* sNum = reinterpret_cast<double*>(sE + 3 * GEN_TP + (GEN_TP & 1));  // [2][32]
+  double* sDen = sNum + 2 * GEN_TP;
+
+  const DevPreItem it = items[blockIdx.y];
+  const int p0 = blockIdx.x * GEN_TP;
+  const int pp = threadIdx.x >> 3, sb = threadIdx.x & 7, p = p0 + pp;
+  const bool want_grad = it.slot[0] >= 0 || it.slot[1] >= 0;
+  T* B[2] = {B0, B1};
+
+  if (want_grad) fill_matrix<T>(BQ, Qg, true);
+  if (threadIdx.x < 3 * GEN_TP) {
+    const int k = threadIdx.x / GEN_TP, r = threadIdx.x % GEN_TP;
+    sE[threadIdx.x] = pending_exp<T>(k == 2 ? it.qm_scale : it.p_scale[k], p0 + r, P, C);
+  }
+  if (threadIdx.x < 4 * GEN_TP) sNum[threadIdx.x] = 0.0;  // sNum and sDen are contiguous
+
+  int z[2] = {0, 0};
+#pragma unroll
+  for (int k = 0; k < 2; ++k)
+    if (it.kind[k] == KIND_STATES && p < P) z[k] = static_cast<const uint8_t*>(it.p[k])[p];
+
+  for (int c = 0; c < C; ++c) {
+    __syncthreads();
+    fill_matrix<T>(B0, static_cast<const T*>(it.mat[0]) + (size_t)c * SP64 * SP64, true);
+    fill_matrix<T>(B1, static_cast<const T*>(it.mat[1]) + (size_t)c * SP64 * SP64, true);
+    load_tile<T>(tQM, KIND_PARTIALS, it.qm, c, p0, P, S);
+    load_tile<T>(tX[0], it.kind[0], it.p[0], c, p0, P, S);
+    load_tile<T>(tX[1], it.kind[1], it.p[1], c, p0, P, S);
+    __syncthreads();
+
+    T a[2][8], qx[2][8];
+#pragma unroll
+    for (int k = 0; k < 2; ++k) {
+      if (it.kind[k] == KIND_STATES) {
+        gather64<T>(B[k], z[k], S, T(1), sb, a[k]);
+        if (want_grad) gather64<T>(BQ, z[k], S, T(0), sb, qx[k]);
+      } else {
+        mv64<T>(B[k], tX[k] + pp * TS, sb, a[k]);
+        if (want_grad) mv64<T>(BQ, tX[k] + pp * TS, sb, qx[k]);
+      }
+      const Pow2Pair<T> f = pow2_pair(-sE[k * GEN_TP + pp], T(0));
+#pragma unroll
+      for (int i = 0; i < 8; ++i) a[k][i] = (a[k][i] * f.f1) * f.f2;
+    }
+    {
+      const Pow2Pair<T> f = pow2_pair(-sE[2 * GEN_TP + pp], T(0));
+#pragma unroll
+      for (int i = 0; i < Gen<T>::NCH; ++i)
+#pragma unroll
+        for (int j = 0; j < Gen<T>::VEC; ++j) {
+          const int s = state_of<T>(sb, i, j);
+          const T qm = (tQM[pp * TS + s] * f.f1) * f.f2;
+          tU[0][pp * TS + s] = qm * a[1][i * Gen<T>::VEC + j];
+          tU[1][pp * TS + s] = qm * a[0][i * Gen<T>::VEC + j];
+        }
+    }
+    __syncthreads();
+    fill_matrix<T>(B0, static_cast<const T*>(it.mat[0]) + (size_t)c * SP64 * SP64, false);
+    fill_matrix<T>(B1, static_cast<const T*>(it.mat[1]) + (size_t)c * SP64 * SP64, false);
+    __syncthreads();
+
+#pragma unroll
+    for (int k = 0; k < 2; ++k) {
+      T q[8];
+      mv64<T>(B[k], tU[k] + pp * TS, sb, q);
+      T mx = T(0);
+#pragma unroll
+      for (int i = 0; i < 8; ++i) mx = fmax(mx, q[i]);
+      mx = lane8_max(mx);
+      if (it.q[k] != nullptr && p < P) {
+        store_states<T>(static_cast<T*>(it.q[k]) + ((size_t)c * P + p) * SP64, sb, q);
+        if (sb == 0) static_cast<T*>(it.q_scale[k])[(size_t)c * P + p] = mx;
+      }
+      if (it.slot[k] >= 0) {
+        T n = T(0), d = T(0);
+#pragma unroll
+        for (int i = 0; i < Gen<T>::NCH; ++i)
+#pragma unroll
+          for (int j = 0; j < Gen<T>::VEC; ++j) {
+            const int s = state_of<T>(sb, i, j);
+            n = fma(q[i * Gen<T>::VEC + j], qx[k][i * Gen<T>::VEC + j], n);
+            d = fma(q[i * Gen<T>::VEC + j], tX[k][pp * TS + s], d);
+          }
+        n = lane8_sum(n);
+        d = lane8_sum(d);
+        if (sb == 0) {  // one writer per (k, pp): no race
+          sNum[k * GEN_TP + pp] += catw[c] * catr[c] * (double)n;
+          sDen[k * GEN_TP + pp] += catw[c] * (double)d;
+        }
+      }
+    }
+  }
+  __syncthreads();
+  if (want_grad && threadIdx.x < 2 * GEN_TP) {  // warp 0 -> child 0, warp 1 -> child 1
+    const int k = threadIdx.x / GEN_TP, r = threadIdx.x % GEN_TP;
+    double v = 0.0;
+    if (it.slot[k] >= 0 && p0 + r < P) {
+      const double ratio = sNum[k * GEN_TP + r] / sDen[k * GEN_TP + r];
+      if (site_out != nullptr) site_out[(size_t)it.slot[k] * P + p0 + r] = ratio;
+      v = weights[p0 + r] * ratio;
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
+    if (r == 0 && it.slot[k] >= 0) grad_partial[(size_t)it.slot[k] * n_tiles + blockIdx.x] = v;
+  }
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// unfused branch derivatives from stored pre- and post-order partials
+// ---------------------------------------------------------------------------------------------------------------
+template <typename T>
+__global__ void __launch_bounds__(GEN_THREADS) k_deriv64(const DevBranch* __restrict__ br, int P, int S, int C,
+                                                         const T* __restrict__ Qg, const double* __restrict__ catw,
+                                                         const double* __restrict__ catr,
+                                                         const double* __restrict__ weights,
+                                                         double* __restrict__ grad_partial, int n_tiles,
+                                                         double* __restrict__ site_out) {
+  constexpr int TS = Gen<T>::TS;
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  T* BQ = reinterpret_cast<T*>(smem_raw);
+  T* tQ = BQ + SP64 * SP64;
+  T* tX = tQ + GEN_TP * TS;
+  double* sNum = reinterpret_cast<double*>(tX + GEN_TP * TS);
+  double* sDen = sNum + GEN_TP;
+
+  const DevBranch b = br[blockIdx.y];
+  const int p0 = blockIdx.x * GEN_TP;
+  const int pp = threadIdx.x >> 3, sb = threadIdx.x & 7;
+  fill_matrix<T>(BQ, Qg, true);
+  if (threadIdx.x < 2 * GEN_TP) sNum[threadIdx.x] = 0.0;
+  for (int c = 0; c < C; ++c) {
+    __syncthreads();
+    load_tile<T>(tQ, KIND_PARTIALS, b.q, c, p0, P, S);
+    load_tile<T>(tX, b.kind, b.p, c, p0, P, S);
+    __syncthreads();
+    T qx[8];
+    mv64<T>(BQ, tX + pp * TS, sb, qx);
+    T n = T(0), d = T(0);
+#pragma unroll
+    for (int i = 0; i < Gen<T>::NCH; ++i)
+#pragma unroll
+      for (int j = 0; j < Gen<T>::VEC; ++j) {
+        const int s = state_of<T>(sb, i, j);
+        n = fma(tQ[pp * TS + s], qx[i * Gen<T>::VEC + j], n);
+        d = fma(tQ[pp * TS + s], tX[pp * TS + s], d);
+      }
+    n = lane8_sum(n);
+    d = lane8_sum(d);
+    if (sb == 0) {
+      sNum[pp] += catw[c] * catr[c] * (double)n;
+      sDen[pp] += catw[c] * (double)d;
+    }
+  }
+  __syncthreads();
+  if (threadIdx.x < GEN_TP) {
+    const int r = threadIdx.x;
+    double v = 0.0;
+    if (p0 + r < P) {
+      const double ratio = sNum[r] / sDen[r];
+      if (site_out != nullptr) site_out[(size_t)b.slot * P + p0 + r] = ratio;
+      v = weights[p0 + r] * ratio;
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
+    if (r == 0) grad_partial[(size_t)b.slot * n_tiles + blockIdx.x] = v;
+  }
+}
+
+}  // namespace plk
