@@ -1,0 +1,103 @@
+"""GPU parity (-m gpu): libplk.so through its C ABI (via the thin binding) against the CPU oracle, element by
+element on the same seeded inputs.  Tolerances (BASELINE.json north_star):
+  fp64          site log-likelihoods, logL and every branch gradient within 1e-10 relative (strict, element-wise);
+  fp32 / tensor site log-likelihoods and logL within 1e-4 relative; gradients |dg_k| <= 1e-4 A_k for every branch and
+                ||dg|| <= 1e-4 ||g||; at perturbed branch lengths (away from the truth) strict 1e-4 on |g_k| > 1e-3 A_k.
+Sizes are reduced so that the oracle finishes in seconds but still span several pattern tiles and a ragged tail
+(tile = 128 patterns for 4 states, 32 for 61 states)."""
+import numpy as np
+import pytest
+
+import oracle_runner as orc
+from paper_2606_27607_b200 import plk, workloads
+from paper_2606_27607_b200.client import Evaluator
+
+pytestmark = pytest.mark.gpu
+
+FP64_TOL = 1e-10
+FP32_TOL = 1e-4
+
+
+def _check_logl(site_gpu, logl_gpu, ref, tol):
+    rel = np.max(np.abs(site_gpu - ref["site_logl"]) / np.abs(ref["site_logl"]))
+    assert rel <= tol, f"site logL rel err {rel:.3e} > {tol}"
+    assert abs(logl_gpu - ref["logL"]) <= tol * abs(ref["logL"])
+
+
+def _check_grad(g_gpu, ref, precision, root):
+    strict, rel_cond, norm = orc.gradient_errors(g_gpu, ref)
+    assert g_gpu[root] == 0.0
+    if precision == plk.FP64:
+        assert strict <= FP64_TOL, f"fp64 gradient strict rel err {strict:.3e}"
+    else:
+        assert rel_cond <= FP32_TOL, f"fp32 gradient err / A_k = {rel_cond:.3e}"
+        assert norm <= FP32_TOL, f"fp32 gradient 2-norm rel err {norm:.3e}"
+        # every branch beyond strict tolerance must be a heavy-cancellation branch (ratio > 100)
+        g = ref["grad"]
+        bad = np.abs(g_gpu - g) > FP32_TOL * np.abs(g)
+        assert np.all(ref["cond"][bad] > 100.0 * np.abs(g[bad]))
+
+
+def _run_case(wl, precision, flags=0, tips_as_partials=False, t=None):
+    ev = Evaluator(wl, precision=precision, flags=flags | plk.FLAG_SITE_DERIVATIVES, tips_as_partials=tips_as_partials)
+    try:
+        logl, site = ev.log_likelihood(t)
+        grad, site_d = ev.gradient(want_site=True)
+        launches = ev.inst.kernel_launch_count()
+    finally:
+        ev.close()
+    assert launches > 0
+    ref = orc.evaluate(wl, t, keep_site_derivatives=True)
+    tol = FP64_TOL if precision == plk.FP64 else FP32_TOL
+    _check_logl(site, logl, ref, tol)
+    _check_grad(grad, ref, precision, wl.tree.root)
+    # per-pattern derivatives, norm-wise per branch (last sentence)
+    for k in range(wl.tree.n_nodes):
+        if k == wl.tree.root:
+            continue
+        scale = np.max(np.abs(ref["site_derivs"][k]))
+        if scale > 0:
+            assert np.max(np.abs(site_d[k] - ref["site_derivs"][k])) <= (1e-9 if precision == plk.FP64 else 2e-4) * scale
+    return ref, grad
+
+
+PREC = [pytest.param(plk.FP64, id="fp64"), pytest.param(plk.FP32, id="fp32")]
+
+
+def test_config0_full():
+    """BASELINE configs[0] at full size: HKY, 8 taxa, 1000 distinct patterns, 4 gamma categories, fp64."""
+    _run_case(workloads.config(0), plk.FP64)
+
+
+@pytest.mark.parametrize("precision", PREC)
+@pytest.mark.parametrize("as_partials", [False, True], ids=["compact", "tip-partials"])
+def test_config1_reduced(precision, as_partials):
+    """configs[1] shape (GTR, 128 taxa, Yule, 5% ambiguity) at 3000 patterns = 23 tiles of 128 + a tail of 56."""
+    _run_case(workloads.config(1, n_patterns=3000), precision, tips_as_partials=as_partials)
+
+
+@pytest.mark.parametrize("precision", PREC)
+def test_config1_perturbed_branch_lengths(precision):
+    wl = workloads.config(1, n_patterns=2000)
+    ref, grad = _run_case(wl, precision, t=wl.perturbed_branch_lengths())
+    if precision == plk.FP32:  # away from the truth strict 1e-4 holds on all well-conditioned branches
+        g = ref["grad"]
+        ok = np.abs(g) > 1e-3 * ref["cond"]
+        assert np.max(np.abs(grad[ok] - g[ok]) / np.abs(g[ok])) <= FP32_TOL
+
+
+@pytest.mark.parametrize("precision", PREC)
+def test_config2_reduced_cuda_cores(precision):
+    """configs[2] shape (GY94, 61 states, 32 taxa) at 500 patterns = 15 tiles of 32 + a tail of 20; CUDA-core path."""
+    _run_case(workloads.config(2, n_patterns=500), precision)
+
+
+def test_config3_reduced_cuda_cores():
+    """configs[3] shape (GY94, 256 taxa, 510 branches, level-batched) at 150 patterns, fp32."""
+    _run_case(workloads.config(3, n_patterns=150), plk.FP32)
+
+
+@pytest.mark.parametrize("n_tips,n_patterns", [(8, 100), (32, 1000), (128, 777), (512, 300)])
+def test_config4_sweep_points(n_tips, n_patterns):
+    """configs[4]: HKY fp32 sweep, small points + a deep 512-taxon tree (rescaling is necessary in fp32 there)."""
+    _run_case(workloads.config(4, n_tips=n_tips, n_patterns=n_patterns), plk.FP32)
