@@ -58,6 +58,11 @@ enum {                                                /* plk_config.flags (bit s
                                   fp32 -> split-TF32 tcgen05; without it they run on the CUDA cores     */
   PLK_FLAG_NO_LEVEL_BATCH = 2, /* launch one kernel per operation instead of one per dependency level
                                   (reference behaviour for tests; slower)                               */
+  PLK_FLAG_LEVEL_BATCH_ONLY = 8,  /* 4-state kernels: always one launch per dependency level                */
+  PLK_FLAG_PATTERN_WALK_ONLY = 16, /* 4-state kernels: always ONE launch per call in which every warp keeps its
+                                  patterns and walks the whole operation list in the order given (patterns are
+                                  independent, so list order is the only dependency).  Without either flag the
+                                  library picks the cheaper shape from P, C, the list length and its level count */
   PLK_FLAG_SITE_DERIVATIVES = 4 /* reserve partials_buffer_count * P doubles so that the gradient calls can
                                   return per-pattern derivatives (out_site != NULL); without it such a
                                   request returns PLK_ERR_UNSUPPORTED                                   */

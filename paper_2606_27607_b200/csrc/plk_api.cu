@@ -24,6 +24,8 @@ namespace {
 constexpr size_t ALIGN = 1024;
 constexpr size_t RING_BYTES = 8u << 20;  // parameter staging ring (pinned host + device mirror)
 inline size_t round_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
+constexpr int NUC_MAX_WALK_WARPS = 16384;  // walk-shape grid cap (256 SMs x 64 warps); sizes the partial-sum rows
+inline int nuc_lanes_per_pattern(int C) { return C % 4 == 0 ? 4 : (C % 2 == 0 ? 2 : 1); }  // NucMap<C>::LP
 
 struct Layout {
   int S, SP, C, P;
@@ -64,7 +66,16 @@ bool compute_layout(const plk_config& c, Layout& L) {
   // eigen buffer: U, Uinv (S*S fp64), lambda (S fp64), Q64 (S*S fp64), QT (SP*SP reals)
   L.eigen_bytes = round_up((size_t)(3 * L.S * L.S + L.S) * 8, ALIGN) + round_up((size_t)L.SP * L.SP * L.w, ALIGN);
   L.scale_bytes = L.SP == 4 ? round_up((size_t)L.P * 2, ALIGN) : L.mx_bytes;
-  L.n_tiles = L.SP == 4 ? (L.P + NUC_THREADS - 1) / NUC_THREADS : (L.P + GEN_TP - 1) / GEN_TP;
+  if (L.SP == 4) {
+    // rows of gradient partial sums: one per block (level shape, k_deriv4) or one per warp (walk shape, capped)
+    const int ppw = 32 / nuc_lanes_per_pattern(L.C);
+    const int n_chunks = (L.P + ppw - 1) / ppw;
+    const int level_blocks = (n_chunks + NUC_WARPS - 1) / NUC_WARPS;
+    const int walk_warps = n_chunks < NUC_MAX_WALK_WARPS ? n_chunks : NUC_MAX_WALK_WARPS;
+    L.n_tiles = level_blocks > walk_warps ? level_blocks : walk_warps;
+  } else {
+    L.n_tiles = (L.P + GEN_TP - 1) / GEN_TP;
+  }
   L.max_grad = c.partials_buffer_count;
   size_t o = 0;
   auto take = [&](size_t bytes) { size_t at = o; o += round_up(bytes, ALIGN); return at; };
@@ -114,6 +125,8 @@ struct plk_instance {
   char* h_ring = nullptr;
   size_t ring_pos = 0;
   int64_t launches = 0;
+  int sm_count = 148;
+  int grad_parts = 0;  // partial sums per gradient slot written by the last gradient launch (row stride L.n_tiles)
 
   template <typename X> X* at(size_t off) const { return reinterpret_cast<X*>(arena + off); }
   void* post_ptr(int idx) const {
@@ -224,10 +237,47 @@ int download(plk_instance* in, double* host, const double* dev, size_t n) {
 }
 
 // ---- kernel dispatch helpers ---------------------------------------------------------------------------------
+// geometry of the 4-state kernels (plk_nuc.cuh): chunks of 32 / LP patterns, one warp each
+struct NucGeom {
+  int ppw, n_chunks, level_blocks;
+};
+inline NucGeom nuc_geom(const Layout& L) {
+  NucGeom g;
+  g.ppw = 32 / nuc_lanes_per_pattern(L.C);
+  g.n_chunks = (L.P + g.ppw - 1) / g.ppw;
+  g.level_blocks = (g.n_chunks + NUC_WARPS - 1) / NUC_WARPS;
+  return g;
+}
+// walk shape: one resident wave in which every warp owns the same number of chunks (no tail wave)
+template <typename K>
+int nuc_walk_warps(const plk_instance* in, K kernel, int n_chunks, int* total_warps) {
+  int blocks_per_sm = 0;
+  CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&blocks_per_sm, kernel, NUC_THREADS, 0));
+  if (blocks_per_sm < 1) return PLK_ERR_CUDA;
+  long resident = (long)in->sm_count * blocks_per_sm * NUC_WARPS;
+  if (resident > NUC_MAX_WALK_WARPS) resident = NUC_MAX_WALK_WARPS;
+  const int per_warp = (int)((n_chunks + resident - 1) / resident);
+  *total_warps = (n_chunks + per_warp - 1) / per_warp;
+  return PLK_SUCCESS;
+}
+
+// Which shape serves a call with `n_ops` operations in `n_levels` dependency levels:
+// the walk costs one dependent global round trip per operation (~1 us) but a single launch and re-reads fresh
+// children from L2; the level shape costs one launch (~4 us) per level.  Once the patterns alone fill the GPU the
+// walk is bandwidth-bound like the level shape and moves fewer bytes, so it wins regardless of the list length.
+bool nuc_use_walk(const plk_instance* in, int n_ops, int n_levels) {
+  const int flags = in->cfg.flags;
+  if (flags & (PLK_FLAG_NO_LEVEL_BATCH | PLK_FLAG_LEVEL_BATCH_ONLY)) return false;
+  if (flags & PLK_FLAG_PATTERN_WALK_ONLY) return true;
+  const NucGeom g = nuc_geom(in->L);
+  if (g.n_chunks >= in->sm_count * 8) return true;
+  return (double)n_ops * 1.0 <= (double)n_levels * 4.0;
+}
+
 template <typename T>
 int launch_post4(plk_instance* in, const DevOp* d_ops, int n_ops) {
   const Layout& L = in->L;
-  dim3 grid(blocks_for(L.P, NUC_THREADS), n_ops);
+  dim3 grid(nuc_geom(L).level_blocks, n_ops);
   switch (L.C) {
 #define CASE(CC) case CC: k_post4<T, CC><<<grid, NUC_THREADS, 0, in->stream>>>(d_ops, L.P); break;
     CASE(1) CASE(2) CASE(3) CASE(4) CASE(5) CASE(6) CASE(7) CASE(8)
@@ -239,20 +289,72 @@ int launch_post4(plk_instance* in, const DevOp* d_ops, int n_ops) {
 }
 
 template <typename T>
-int launch_pre4(plk_instance* in, const DevPreItem* d_items, int n, const T* Q, double* site) {
+int launch_post4_walk(plk_instance* in, const DevOp* d_ops, int n_ops) {
   const Layout& L = in->L;
-  dim3 grid(blocks_for(L.P, NUC_THREADS), n);
-  const double* cw = in->at<double>(L.off_catw);
-  const double* cr = in->at<double>(L.off_rates);
-  const double* wt = in->at<double>(L.off_weights);
-  double* gp = in->at<double>(L.off_grad_partial);
+  const NucGeom g = nuc_geom(L);
+  int tw = 0, rc = PLK_SUCCESS;
   switch (L.C) {
-#define CASE(CC) case CC: k_pre4<T, CC><<<grid, NUC_THREADS, 0, in->stream>>>(d_items, L.P, Q, cw, cr, wt, gp, L.n_tiles, site); break;
+#define CASE(CC)                                                                                             \
+  case CC:                                                                                                   \
+    rc = nuc_walk_warps(in, k_post4_walk<T, CC>, g.n_chunks, &tw);                                           \
+    if (rc) return rc;                                                                                       \
+    k_post4_walk<T, CC><<<(tw + NUC_WARPS - 1) / NUC_WARPS, NUC_THREADS, 0, in->stream>>>(d_ops, n_ops, L.P, \
+                                                                                           g.n_chunks, tw);  \
+    break;
     CASE(1) CASE(2) CASE(3) CASE(4) CASE(5) CASE(6) CASE(7) CASE(8)
 #undef CASE
     default: return PLK_ERR_UNSUPPORTED;
   }
   CHECK_LAUNCH(in);
+  return PLK_SUCCESS;
+}
+
+inline NucModel nuc_model(const plk_instance* in, double* site) {
+  const Layout& L = in->L;
+  return NucModel{in->at<double>(L.off_catw), in->at<double>(L.off_rates), in->at<double>(L.off_weights), site};
+}
+
+template <typename T>
+int launch_pre4(plk_instance* in, const DevPreItem* d_items, int n, const T* Q, double* site) {
+  const Layout& L = in->L;
+  const NucGeom g = nuc_geom(L);
+  dim3 grid(g.level_blocks, n);
+  const NucModel md = nuc_model(in, site);
+  double* gp = in->at<double>(L.off_grad_partial);
+  switch (L.C) {
+#define CASE(CC) case CC: k_pre4<T, CC><<<grid, NUC_THREADS, 0, in->stream>>>(d_items, L.P, Q, md, gp, L.n_tiles); break;
+    CASE(1) CASE(2) CASE(3) CASE(4) CASE(5) CASE(6) CASE(7) CASE(8)
+#undef CASE
+    default: return PLK_ERR_UNSUPPORTED;
+  }
+  CHECK_LAUNCH(in);
+  in->grad_parts = g.level_blocks;
+  return PLK_SUCCESS;
+}
+
+template <typename T>
+int launch_pre4_walk(plk_instance* in, const DevPreItem* d_items, int n, const T* Q, double* site) {
+  const Layout& L = in->L;
+  const NucGeom g = nuc_geom(L);
+  const NucModel md = nuc_model(in, site);
+  double* gp = in->at<double>(L.off_grad_partial);
+  int tw = 0, rc = PLK_SUCCESS;
+  switch (L.C) {
+#define CASE(CC)                                                                                           \
+  case CC:                                                                                                 \
+    rc = nuc_walk_warps(in, k_pre4_walk<T, CC>, g.n_chunks, &tw);                                          \
+    if (rc) return rc;                                                                                     \
+    k_pre4_walk<T, CC><<<(tw + NUC_WARPS - 1) / NUC_WARPS, NUC_THREADS, 0, in->stream>>>(d_items, n, L.P,  \
+                                                                                          g.n_chunks, tw, \
+                                                                                          Q, md, gp,       \
+                                                                                          L.n_tiles);      \
+    break;
+    CASE(1) CASE(2) CASE(3) CASE(4) CASE(5) CASE(6) CASE(7) CASE(8)
+#undef CASE
+    default: return PLK_ERR_UNSUPPORTED;
+  }
+  CHECK_LAUNCH(in);
+  in->grad_parts = tw;
   return PLK_SUCCESS;
 }
 
@@ -271,6 +373,7 @@ int launch_deriv4(plk_instance* in, const DevBranch* d_br, int n, const T* Q, do
     default: return PLK_ERR_UNSUPPORTED;
   }
   CHECK_LAUNCH(in);
+  in->grad_parts = (int)grid.x;
   return PLK_SUCCESS;
 }
 
@@ -303,13 +406,17 @@ int launch_pre64(plk_instance* in, const DevPreItem* d_items, int n, const T* Q,
   double* gp = in->at<double>(L.off_grad_partial);
 #ifdef PLK_WITH_TENSOR
   if (in->cfg.flags & PLK_FLAG_TENSOR_CORES)
+  {
+    in->grad_parts = L.n_tiles;
     return tc_launch_pre<T>(in->stream, d_items, n, L.P, L.S, L.C, Q, cw, cr, wt, gp, L.n_tiles, site, &in->launches);
+  }
 #endif
   int rc = opt_in_smem(k_pre64<T>, pre64_smem<T>());
   if (rc) return rc;
   dim3 grid(L.n_tiles, n);
   k_pre64<T><<<grid, GEN_THREADS, pre64_smem<T>(), in->stream>>>(d_items, L.P, L.S, L.C, Q, cw, cr, wt, gp, L.n_tiles, site);
   CHECK_LAUNCH(in);
+  in->grad_parts = L.n_tiles;
   return PLK_SUCCESS;
 }
 
@@ -323,6 +430,7 @@ int launch_deriv64(plk_instance* in, const DevBranch* d_br, int n, const T* Q, d
       d_br, L.P, L.S, L.C, Q, in->at<double>(L.off_catw), in->at<double>(L.off_rates), in->at<double>(L.off_weights),
       in->at<double>(L.off_grad_partial), L.n_tiles, site);
   CHECK_LAUNCH(in);
+  in->grad_parts = L.n_tiles;
   return PLK_SUCCESS;
 }
 
@@ -363,7 +471,10 @@ int plk_create(const plk_config* cfg, void* d_arena, size_t arena_bytes, void* c
     if (cfg->state_count == 4 && cfg->category_count > 8) return PLK_ERR_UNSUPPORTED;
     return PLK_ERR_OUT_OF_RANGE;
   }
-  if (cfg->flags & ~(PLK_FLAG_TENSOR_CORES | PLK_FLAG_NO_LEVEL_BATCH | PLK_FLAG_SITE_DERIVATIVES)) return PLK_ERR_UNSUPPORTED;
+  if (cfg->flags & ~(PLK_FLAG_TENSOR_CORES | PLK_FLAG_NO_LEVEL_BATCH | PLK_FLAG_SITE_DERIVATIVES | PLK_FLAG_LEVEL_BATCH_ONLY |
+                     PLK_FLAG_PATTERN_WALK_ONLY))
+    return PLK_ERR_UNSUPPORTED;
+  if ((cfg->flags & PLK_FLAG_LEVEL_BATCH_ONLY) && (cfg->flags & PLK_FLAG_PATTERN_WALK_ONLY)) return PLK_ERR_UNSUPPORTED;
 #ifndef PLK_WITH_TENSOR
   if ((cfg->flags & PLK_FLAG_TENSOR_CORES) && L.SP == 64) return PLK_ERR_UNSUPPORTED;
 #endif
@@ -371,6 +482,10 @@ int plk_create(const plk_config* cfg, void* d_arena, size_t arena_bytes, void* c
   if (reinterpret_cast<uintptr_t>(d_arena) % ALIGN != 0) return PLK_ERR_OUT_OF_RANGE;
   int n_dev = 0;
   if (cudaGetDeviceCount(&n_dev) != cudaSuccess || n_dev == 0) return PLK_ERR_CUDA;
+  int dev = 0, sms = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess ||
+      cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || sms < 1)
+    return PLK_ERR_CUDA;
   plk_instance* in = new (std::nothrow) plk_instance();
   if (in == nullptr) return PLK_ERR_OUT_OF_MEMORY;
   in->cfg = *cfg;
@@ -378,6 +493,7 @@ int plk_create(const plk_config* cfg, void* d_arena, size_t arena_bytes, void* c
   in->stream = static_cast<cudaStream_t>(cuda_stream);
   in->arena = static_cast<char*>(d_arena);
   in->f32 = cfg->precision == PLK_FP32;
+  in->sm_count = sms;
   in->deferred = L.SP != 4;
   in->post_slot.assign(cfg->partials_buffer_count, -1);
   in->post_kind.assign(cfg->partials_buffer_count, KIND_PARTIALS);
@@ -695,7 +811,8 @@ int plk_update_partials(plk_instance* in, const plk_op* ops, int count) {
   }
   std::vector<int> order(count);
   std::vector<int> level_start(n_levels + 1, 0);
-  if (cfg.flags & PLK_FLAG_NO_LEVEL_BATCH) {
+  const bool walk = in->L.SP == 4 && nuc_use_walk(in, count, n_levels);
+  if (walk || (cfg.flags & PLK_FLAG_NO_LEVEL_BATCH)) {
     for (int i = 0; i < count; ++i) order[i] = i;
   } else {
     for (int i = 0; i < count; ++i) ++level_start[level[i] + 1];
@@ -717,7 +834,10 @@ int plk_update_partials(plk_instance* in, const plk_op* ops, int count) {
       return in->L.SP == 4 ? launch_post4<T>(in, dops + first, n) : launch_post64<T>(in, dops + first, n);
     });
   };
-  if (cfg.flags & PLK_FLAG_NO_LEVEL_BATCH) {
+  if (walk) {  // one launch, list order (plk_nuc.cuh "walk")
+    rc = by_precision(in, [&](auto tag) -> int { return launch_post4_walk<decltype(tag)>(in, dops, count); });
+    if (rc) return rc;
+  } else if (cfg.flags & PLK_FLAG_NO_LEVEL_BATCH) {
     for (int i = 0; i < count; ++i) {
       rc = launch(i, 1);
       if (rc) return rc;
@@ -947,12 +1067,24 @@ static int pre_impl(plk_instance* in, int eigen, int root_pre, const plk_pre_op*
     rc = ring_alloc(in, (size_t)n_items * sizeof(DevPreItem), &h, &d);
     if (rc) return rc;
     DevPreItem* hit = reinterpret_cast<DevPreItem*>(h);
-    for (const HostItem& hi : items) hit[fill[hi.level]++] = hi.it;
+    const bool walk = L.SP == 4 && nuc_use_walk(in, n_items, n_levels);
+    if (walk) {
+      for (int i = 0; i < n_items; ++i) hit[i] = items[i].it;  // list order (plk_nuc.cuh "walk")
+    } else {
+      for (const HostItem& hi : items) hit[fill[hi.level]++] = hi.it;
+    }
     rc = copy_ring(in, h, d, (size_t)n_items * sizeof(DevPreItem));
     if (rc) return rc;
     const DevPreItem* dit = reinterpret_cast<const DevPreItem*>(d);
     const void* Q = want_grad ? in->eig_QT(eigen) : in->eig_QT(0);
-    for (int l = 0; l < n_levels; ++l) {
+    if (walk) {
+      rc = by_precision(in, [&](auto tag) -> int {
+        using T = decltype(tag);
+        return launch_pre4_walk<T>(in, dit, n_items, static_cast<const T*>(Q), d_site);
+      });
+      if (rc) return rc;
+    }
+    for (int l = 0; l < (walk ? 0 : n_levels); ++l) {
       const int n = level_start[l + 1] - level_start[l];
       for (int first = 0; first < n; first += 32768) {
         const int m = n - first < 32768 ? n - first : 32768;
@@ -967,7 +1099,7 @@ static int pre_impl(plk_instance* in, int eigen, int root_pre, const plk_pre_op*
     }
   }
   if (want_grad && count > 0) {
-    k_sum_rows<<<count, 128, 0, in->stream>>>(in->at<double>(L.off_grad_partial), L.n_tiles, L.n_tiles, d_grad);
+    k_sum_rows<<<count, 128, 0, in->stream>>>(in->at<double>(L.off_grad_partial), in->grad_parts, L.n_tiles, d_grad);
     CHECK_LAUNCH(in);
   }
   return PLK_SUCCESS;
@@ -1046,7 +1178,7 @@ int plk_branch_derivatives(plk_instance* in, int eigen, const int32_t* post_idx,
     });
     if (rc) return rc;
   }
-  k_sum_rows<<<count, 128, 0, in->stream>>>(in->at<double>(L.off_grad_partial), L.n_tiles, L.n_tiles,
+  k_sum_rows<<<count, 128, 0, in->stream>>>(in->at<double>(L.off_grad_partial), in->grad_parts, L.n_tiles,
                                             in->at<double>(L.off_grad_out));
   CHECK_LAUNCH(in);
   return finish_gradient(in, count, out_gradient, out_site, d_site);

@@ -370,14 +370,16 @@ def make_workload(name: str, model_name: str, n_tips: int, n_patterns: int, topo
     return Workload(name, tree, model, Q, pi, U, Uinv, lam, rates, cat_w, np.ascontiguousarray(tips), weights, seed)
 
 
-def config(index: int, n_tips: Optional[int] = None, n_patterns: Optional[int] = None) -> Workload:
+def config(index: int, n_tips: Optional[int] = None, n_patterns: Optional[int] = None,
+           n_categories: int = 4) -> Workload:
     """BASELINE.json configs[index]; `n_tips`/`n_patterns` override the size (sweep points of configs[4], reduced
     parity cases).  Recipes: SURVEY.md section 8(d)."""
     seed = BASE_SEED + index
     if index == 0:
         return make_workload("cfg0_hky_8x1000", "HKY", n_tips or 8, n_patterns or 1000, "coalescent", seed, distinct=True)
     if index == 1:
-        return make_workload("cfg1_gtr_128x100000", "GTR", n_tips or 128, n_patterns or 100_000, "yule", seed, ambiguity=0.05)
+        return make_workload("cfg1_gtr_128x100000", "GTR", n_tips or 128, n_patterns or 100_000, "yule", seed,
+                             n_cat=n_categories, ambiguity=0.05)
     if index == 2:
         return make_workload("cfg2_gy94_32x10000", "GY94", n_tips or 32, n_patterns or 10_000, "coalescent", seed)
     if index == 3:

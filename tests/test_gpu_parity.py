@@ -77,6 +77,15 @@ def test_config1_reduced(precision, as_partials):
 
 
 @pytest.mark.parametrize("precision", PREC)
+@pytest.mark.parametrize("shape", [plk.FLAG_LEVEL_BATCH_ONLY, plk.FLAG_PATTERN_WALK_ONLY], ids=["level", "walk"])
+@pytest.mark.parametrize("n_cat", [1, 2, 3, 4, 6, 8])
+def test_nucleotide_launch_shapes_and_category_counts(precision, shape, n_cat):
+    """Both launch shapes of the 4-state kernels (one launch per level / one pattern-walk launch) for every lane
+    mapping (1, 2 or 4 lanes per pattern); 1237 patterns = a ragged last chunk for each."""
+    _run_case(workloads.config(1, n_tips=24, n_patterns=1237, n_categories=n_cat), precision, flags=shape)
+
+
+@pytest.mark.parametrize("precision", PREC)
 def test_config1_perturbed_branch_lengths(precision):
     wl = workloads.config(1, n_patterns=2000)
     ref, grad = _run_case(wl, precision, t=wl.perturbed_branch_lengths())
