@@ -9,7 +9,7 @@ from paper_2606_27607_b200.client import Evaluator
 pytestmark = pytest.mark.gpu
 
 
-def _compare(wl, precision, t=None, flags=0):
+def _compare(wl, precision, t=None, flags=0, strict_tol=1e-10, cond_tol=None):
     ev = Evaluator(wl, precision=precision, flags=flags)
     try:
         logl, site = ev.log_likelihood(t)
@@ -21,7 +21,9 @@ def _compare(wl, precision, t=None, flags=0):
     assert np.max(np.abs(site - ref["site_logl"]) / np.abs(ref["site_logl"])) <= tol
     strict, rel_cond, norm = orc.gradient_errors(g, ref)
     if precision == plk.FP64:
-        assert strict <= 1e-10
+        assert strict <= strict_tol
+        if cond_tol is not None:
+            assert rel_cond <= cond_tol
     else:
         assert rel_cond <= 1e-4 and norm <= 1e-4
     return site, g, ref
@@ -66,7 +68,11 @@ def test_deep_caterpillar_needs_rescaling(precision, n_tips):
     """Deep tree: unscaled arithmetic underflows (oracle with rescale=False gives -inf), the library stays finite
     and matches the rescaled oracle."""
     wl = workloads.make_workload("deep", "HKY", n_tips, 40, "caterpillar", seed=31)
-    site, g, ref = _compare(wl, precision)
+    # 1499 dependent levels: round-off grows with depth (~ levels * 4 * 2^-53 = 6.6e-13 relative to A_k) and the
+    # strict figure multiplies it by the cancellation ratio A_k / |g_k| (only 40 patterns: up to ~1e3).  The bound
+    # that the arithmetic supports is therefore the A_k-relative one, held two orders tighter than 1e-10
+    # (DESIGN.md "Tolerances").
+    site, g, ref = _compare(wl, precision, strict_tol=1e-8, cond_tol=1e-12)
     assert np.all(np.isfinite(site))
     if precision == plk.FP64:
         unscaled = orc.evaluate(wl, gradient=False, rescale=False)
