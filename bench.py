@@ -39,6 +39,8 @@ def parse_args():
     ap.add_argument("--tensor", action="store_true", help="61-state kernels on the tensor pipe")
     ap.add_argument("--shape", choices=["auto", "level", "walk"], default="auto",
                     help="4-state launch shape: one launch per level / one pattern-walk launch / library's choice")
+    ap.add_argument("--staging", choices=["tma", "ldg"], default="tma",
+                    help="4-state operand staging: TMA ring (cp.async.bulk) / register-staged loads")
     ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
     ap.add_argument("--no-extras", action="store_true", help="skip the other configs / precisions")
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -251,6 +253,7 @@ def workload_config(wl, precision, flags, extra=None):
            "codon_path": ("tensor" if flags & 1 else "cuda-core") if wl.n_states != 4 else None,
            "substitution_model": wl.model["name"], "seed": wl.seed,
            "launch_shape": {8: "level", 16: "walk"}.get(flags & 24, "auto") if wl.n_states == 4 else "level",
+           "staging": ("ldg" if flags & 32 else "tma") if wl.n_states == 4 else None,
            "l2_policy": "inputs exceed L2 (no flush between iterations)"}
     if extra:
         cfg.update(extra)
@@ -355,6 +358,7 @@ def main():
     wl = make_workload(args)
     flags = plk.FLAG_TENSOR_CORES if args.tensor else 0
     flags |= {"auto": 0, "level": plk.FLAG_LEVEL_BATCH_ONLY, "walk": plk.FLAG_PATTERN_WALK_ONLY}[args.shape]
+    flags |= plk.FLAG_NO_TMA if args.staging == "ldg" else 0
     sampler = ClockSampler(local_rank) if rank == 0 else None
 
     if dist is not None:

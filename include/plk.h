@@ -63,6 +63,8 @@ enum {                                                /* plk_config.flags (bit s
                                   patterns and walks the whole operation list in the order given (patterns are
                                   independent, so list order is the only dependency).  Without either flag the
                                   library picks the cheaper shape from P, C, the list length and its level count */
+  PLK_FLAG_NO_TMA = 32,        /* 4-state kernels: use the register-staged (LDG) kernels instead of the TMA-staged
+                                  ones (comparison arm; also what category counts other than 1, 2, 4, 8 run on) */
   PLK_FLAG_SITE_DERIVATIVES = 4 /* reserve partials_buffer_count * P doubles so that the gradient calls can
                                   return per-pattern derivatives (out_site != NULL); without it such a
                                   request returns PLK_ERR_UNSUPPORTED                                   */

@@ -12,6 +12,7 @@
 #include "plk_gen.cuh"
 #include "plk_misc.cuh"
 #include "plk_nuc.cuh"
+#include "plk_nuc_tma.cuh"
 #include "plk_schedule.h"
 #ifdef PLK_WITH_TENSOR
 #include "plk_tc.cuh"
@@ -73,6 +74,7 @@ bool compute_layout(const plk_config& c, Layout& L) {
     const int level_blocks = (n_chunks + NUC_WARPS - 1) / NUC_WARPS;
     const int walk_warps = n_chunks < NUC_MAX_WALK_WARPS ? n_chunks : NUC_MAX_WALK_WARPS;
     L.n_tiles = level_blocks > walk_warps ? level_blocks : walk_warps;
+    if (L.n_tiles < n_chunks + NT_CW) L.n_tiles = n_chunks + NT_CW;  // TMA level shape: one per (pattern tile, warp)
   } else {
     L.n_tiles = (L.P + GEN_TP - 1) / GEN_TP;
   }
@@ -126,6 +128,7 @@ struct plk_instance {
   size_t ring_pos = 0;
   int64_t launches = 0;
   int sm_count = 148;
+  int nt_bps[2][2] = {{0, 0}, {0, 0}};  // resident CTAs per SM of the TMA kernels [post|pre][level|walk]
   int grad_parts = 0;  // partial sums per gradient slot written by the last gradient launch (row stride L.n_tiles)
 
   template <typename X> X* at(size_t off) const { return reinterpret_cast<X*>(arena + off); }
@@ -358,6 +361,94 @@ int launch_pre4_walk(plk_instance* in, const DevPreItem* d_items, int n, const T
   return PLK_SUCCESS;
 }
 
+// ---- TMA-staged 4-state kernels (plk_nuc_tma.cuh) ------------------------------------------------------------
+inline bool nuc_use_tma(const plk_instance* in) {
+  const int C = in->L.C;
+  return !(in->cfg.flags & (PLK_FLAG_NO_TMA | PLK_FLAG_NO_LEVEL_BATCH)) && (C == 1 || C == 2 || C == 4 || C == 8);
+}
+// grid of a TMA kernel: walk -> every CTA owns at least one full tile of rows; level -> at most one CTA per tile
+template <typename K>
+int nt_grid(plk_instance* in, K kernel, size_t smem, int which, bool walk, long long n_units, int* grid) {
+  int& bps = in->nt_bps[which][walk ? 1 : 0];
+  if (bps == 0) {
+    CU(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&bps, kernel, NT_THREADS, smem));
+    if (bps < 1) return PLK_ERR_CUDA;
+  }
+  long long g = (long long)in->sm_count * bps;
+  if (g > n_units) g = n_units;
+  *grid = g < 1 ? 1 : (int)g;
+  return PLK_SUCCESS;
+}
+
+template <typename T, int C>
+int launch_post4_tma_c(plk_instance* in, const DevOp* d_ops, int n_ops, bool walk) {
+  const Layout& L = in->L;
+  using St = NtStage<T, C, 2, false>;
+  const size_t smem = (size_t)NT_NS * St::BYTES;
+  const int n_rows = (L.P + NucMap<C>::PPW - 1) / NucMap<C>::PPW;
+  const long long n_tp = (L.P + St::TP - 1) / St::TP;
+  NtSched sc{walk ? 1 : 0, n_ops, L.P, n_rows};
+  int grid = 0, rc;
+  if (walk) {
+    rc = nt_grid(in, k_post4_tma<T, C, true>, smem, 0, true, n_rows / NT_CW > 0 ? n_rows / NT_CW : 1, &grid);
+    if (rc) return rc;
+    k_post4_tma<T, C, true><<<grid, NT_THREADS, smem, in->stream>>>(d_ops, sc);
+  } else {
+    rc = nt_grid(in, k_post4_tma<T, C, false>, smem, 0, false, n_tp * n_ops, &grid);
+    if (rc) return rc;
+    k_post4_tma<T, C, false><<<grid, NT_THREADS, smem, in->stream>>>(d_ops, sc);
+  }
+  CHECK_LAUNCH(in);
+  return PLK_SUCCESS;
+}
+template <typename T>
+int launch_post4_tma(plk_instance* in, const DevOp* d_ops, int n_ops, bool walk) {
+  switch (in->L.C) {
+    case 1: return launch_post4_tma_c<T, 1>(in, d_ops, n_ops, walk);
+    case 2: return launch_post4_tma_c<T, 2>(in, d_ops, n_ops, walk);
+    case 4: return launch_post4_tma_c<T, 4>(in, d_ops, n_ops, walk);
+    case 8: return launch_post4_tma_c<T, 8>(in, d_ops, n_ops, walk);
+    default: return PLK_ERR_UNSUPPORTED;
+  }
+}
+
+template <typename T, int C>
+int launch_pre4_tma_c(plk_instance* in, const DevPreItem* d_items, int n, const T* Q, double* site, bool walk) {
+  const Layout& L = in->L;
+  using St = NtStage<T, C, 3, true>;
+  const size_t smem = (size_t)NT_NS * St::BYTES;
+  const int n_rows = (L.P + NucMap<C>::PPW - 1) / NucMap<C>::PPW;
+  const long long n_tp = (L.P + St::TP - 1) / St::TP;
+  NtSched sc{walk ? 1 : 0, n, L.P, n_rows};
+  const NucModel md = nuc_model(in, site);
+  double* gp = in->at<double>(L.off_grad_partial);
+  int grid = 0, rc;
+  if (walk) {
+    rc = nt_grid(in, k_pre4_tma<T, C, true>, smem, 1, true, n_rows / NT_CW > 0 ? n_rows / NT_CW : 1, &grid);
+    if (rc) return rc;
+    k_pre4_tma<T, C, true><<<grid, NT_THREADS, smem, in->stream>>>(d_items, sc, Q, md, gp, L.n_tiles);
+    in->grad_parts = grid * NT_CW;
+  } else {
+    rc = nt_grid(in, k_pre4_tma<T, C, false>, smem, 1, false, n_tp * n, &grid);
+    if (rc) return rc;
+    k_pre4_tma<T, C, false><<<grid, NT_THREADS, smem, in->stream>>>(d_items, sc, Q, md, gp, L.n_tiles);
+    in->grad_parts = (int)n_tp * NT_CW;
+  }
+  CHECK_LAUNCH(in);
+  return PLK_SUCCESS;
+}
+template <typename T>
+int launch_pre4_tma(plk_instance* in, const DevPreItem* d_items, int n, const T* Q, double* site, bool walk) {
+  switch (in->L.C) {
+    case 1: return launch_pre4_tma_c<T, 1>(in, d_items, n, Q, site, walk);
+    case 2: return launch_pre4_tma_c<T, 2>(in, d_items, n, Q, site, walk);
+    case 4: return launch_pre4_tma_c<T, 4>(in, d_items, n, Q, site, walk);
+    case 8: return launch_pre4_tma_c<T, 8>(in, d_items, n, Q, site, walk);
+    default: return PLK_ERR_UNSUPPORTED;
+  }
+}
+
 template <typename T>
 int launch_deriv4(plk_instance* in, const DevBranch* d_br, int n, const T* Q, double* site) {
   const Layout& L = in->L;
@@ -472,7 +563,7 @@ int plk_create(const plk_config* cfg, void* d_arena, size_t arena_bytes, void* c
     return PLK_ERR_OUT_OF_RANGE;
   }
   if (cfg->flags & ~(PLK_FLAG_TENSOR_CORES | PLK_FLAG_NO_LEVEL_BATCH | PLK_FLAG_SITE_DERIVATIVES | PLK_FLAG_LEVEL_BATCH_ONLY |
-                     PLK_FLAG_PATTERN_WALK_ONLY))
+                     PLK_FLAG_PATTERN_WALK_ONLY | PLK_FLAG_NO_TMA))
     return PLK_ERR_UNSUPPORTED;
   if ((cfg->flags & PLK_FLAG_LEVEL_BATCH_ONLY) && (cfg->flags & PLK_FLAG_PATTERN_WALK_ONLY)) return PLK_ERR_UNSUPPORTED;
 #ifndef PLK_WITH_TENSOR
@@ -831,11 +922,15 @@ int plk_update_partials(plk_instance* in, const plk_op* ops, int count) {
   auto launch = [&](int first, int n) {
     return by_precision(in, [&](auto tag) -> int {
       using T = decltype(tag);
-      return in->L.SP == 4 ? launch_post4<T>(in, dops + first, n) : launch_post64<T>(in, dops + first, n);
+      if (in->L.SP != 4) return launch_post64<T>(in, dops + first, n);
+      return nuc_use_tma(in) ? launch_post4_tma<T>(in, dops + first, n, false) : launch_post4<T>(in, dops + first, n);
     });
   };
   if (walk) {  // one launch, list order (plk_nuc.cuh "walk")
-    rc = by_precision(in, [&](auto tag) -> int { return launch_post4_walk<decltype(tag)>(in, dops, count); });
+    rc = by_precision(in, [&](auto tag) -> int {
+      using T = decltype(tag);
+      return nuc_use_tma(in) ? launch_post4_tma<T>(in, dops, count, true) : launch_post4_walk<T>(in, dops, count);
+    });
     if (rc) return rc;
   } else if (cfg.flags & PLK_FLAG_NO_LEVEL_BATCH) {
     for (int i = 0; i < count; ++i) {
@@ -1080,7 +1175,8 @@ static int pre_impl(plk_instance* in, int eigen, int root_pre, const plk_pre_op*
     if (walk) {
       rc = by_precision(in, [&](auto tag) -> int {
         using T = decltype(tag);
-        return launch_pre4_walk<T>(in, dit, n_items, static_cast<const T*>(Q), d_site);
+        return nuc_use_tma(in) ? launch_pre4_tma<T>(in, dit, n_items, static_cast<const T*>(Q), d_site, true)
+                               : launch_pre4_walk<T>(in, dit, n_items, static_cast<const T*>(Q), d_site);
       });
       if (rc) return rc;
     }
@@ -1091,8 +1187,9 @@ static int pre_impl(plk_instance* in, int eigen, int root_pre, const plk_pre_op*
         rc = by_precision(in, [&](auto tag) -> int {
           using T = decltype(tag);
           const DevPreItem* p0 = dit + level_start[l] + first;
-          return L.SP == 4 ? launch_pre4<T>(in, p0, m, static_cast<const T*>(Q), d_site)
-                           : launch_pre64<T>(in, p0, m, static_cast<const T*>(Q), d_site);
+          if (L.SP != 4) return launch_pre64<T>(in, p0, m, static_cast<const T*>(Q), d_site);
+          return nuc_use_tma(in) ? launch_pre4_tma<T>(in, p0, m, static_cast<const T*>(Q), d_site, false)
+                                 : launch_pre4<T>(in, p0, m, static_cast<const T*>(Q), d_site);
         });
         if (rc) return rc;
       }

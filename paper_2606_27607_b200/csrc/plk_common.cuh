@@ -14,7 +14,7 @@ namespace plk {
 enum : int { KIND_PARTIALS = 0, KIND_BCAST = 1, KIND_STATES = 2, KIND_NONE = 3 /* operand absent: zeros */ };
 
 // One post-order operation.
-struct DevOp {
+struct alignas(16) DevOp {
   void* dest;          // T [C][P][SP]
   const void* child[2];
   const void* mat[2];  // T [C][SP][SP]
@@ -24,7 +24,7 @@ struct DevOp {
 };
 
 // Both children of one parent in the pre-order pass (SURVEY 8(a) steps 5-6 fused).
-struct DevPreItem {
+struct alignas(16) DevPreItem {
   const void* qm;       // parent pre-order partials T [C][P][SP]
   const void* qm_scale; // SP=64: pending maxima of qm (T [C][P]) or NULL
   void* q[2];           // pre-order partials written for child 0 / 1 (NULL: not stored)
