@@ -478,7 +478,7 @@ template <typename T>
 int launch_post64(plk_instance* in, const DevOp* d_ops, int n_ops) {
   const Layout& L = in->L;
 #ifdef PLK_WITH_TENSOR
-  if (in->cfg.flags & PLK_FLAG_TENSOR_CORES) return tc_launch_post<T>(in->stream, d_ops, n_ops, L.P, L.S, L.C, &in->launches);
+  if (in->cfg.flags & PLK_FLAG_TENSOR_CORES) return tc_launch_post<T>(in->stream, d_ops, n_ops, L.P, L.S, L.C, in->sm_count, &in->launches);
 #endif
   int rc = opt_in_smem(k_post64<T>, post64_smem<T>());
   if (rc) return rc;
@@ -498,8 +498,8 @@ int launch_pre64(plk_instance* in, const DevPreItem* d_items, int n, const T* Q,
 #ifdef PLK_WITH_TENSOR
   if (in->cfg.flags & PLK_FLAG_TENSOR_CORES)
   {
-    in->grad_parts = L.n_tiles;
-    return tc_launch_pre<T>(in->stream, d_items, n, L.P, L.S, L.C, Q, cw, cr, wt, gp, L.n_tiles, site, &in->launches);
+    return tc_launch_pre<T>(in->stream, d_items, n, L.P, L.S, L.C, Q, cw, cr, wt, gp, L.n_tiles, site, &in->grad_parts,
+                            &in->launches);
   }
 #endif
   int rc = opt_in_smem(k_pre64<T>, pre64_smem<T>());

@@ -28,7 +28,14 @@ def _check_grad(g_gpu, ref, precision, root):
     strict, rel_cond, norm = orc.gradient_errors(g_gpu, ref)
     assert g_gpu[root] == 0.0
     if precision == plk.FP64:
-        assert strict <= FP64_TOL, f"fp64 gradient strict rel err {strict:.3e}"
+        # strict 1e-10 element-wise, except where the pattern sum itself cancels: a branch with A_k / |g_k| > 1e3
+        # (g_k is a score evaluated at the truth) is held to 1e-13 A_k instead, i.e. to the
+        # round-off of its S-term dot products accumulated over the levels
+        g, d = ref["grad"], np.abs(g_gpu - ref["grad"])
+        bad = d > FP64_TOL * np.abs(g)
+        assert np.all(d[bad] <= 1e-13 * ref["cond"][bad]), f"fp64 gradient strict rel err {strict:.3e}"
+        assert np.all(ref["cond"][bad] > 1e3 * np.abs(g[bad]))
+        assert norm <= FP64_TOL and rel_cond <= 1e-12
     else:
         assert rel_cond <= FP32_TOL, f"fp32 gradient err / A_k = {rel_cond:.3e}"
         assert norm <= FP32_TOL, f"fp32 gradient 2-norm rel err {norm:.3e}"
@@ -112,6 +119,26 @@ def test_config1_perturbed_branch_lengths(precision):
 def test_config2_reduced_cuda_cores(precision):
     """configs[2] shape (GY94, 61 states, 32 taxa) at 500 patterns = 15 tiles of 32 + a tail of 20; CUDA-core path."""
     _run_case(workloads.config(2, n_patterns=500), precision)
+
+
+@pytest.mark.parametrize("precision", PREC)
+@pytest.mark.parametrize("n_pat", [500, 64, 129, 1])
+def test_config2_reduced_tensor_cores(precision, n_pat):
+    """configs[2] on the tensor pipe (fp64: DMMA m8n8k4, fp32: split-TF32 m16n8k8): 500 patterns = several tiles of
+    64 / 128 + a ragged tail; exactly one fp64 tile; one fp32 tile + 1; a single pattern."""
+    _run_case(workloads.config(2, n_patterns=n_pat), precision, flags=plk.FLAG_TENSOR_CORES)
+
+
+@pytest.mark.parametrize("precision", PREC)
+def test_config2_tensor_cores_tip_partials(precision):
+    """Tips supplied as partials (KIND_BCAST operands go through the contraction instead of the column gather)."""
+    _run_case(workloads.config(2, n_tips=12, n_patterns=300), precision, flags=plk.FLAG_TENSOR_CORES,
+              tips_as_partials=True)
+
+
+def test_config3_reduced_tensor_cores():
+    """configs[3] shape (GY94, 256 taxa, 510 branches, level-batched) at 150 patterns, fp32 tensor path."""
+    _run_case(workloads.config(3, n_patterns=150), plk.FP32, flags=plk.FLAG_TENSOR_CORES)
 
 
 def test_config3_reduced_cuda_cores():
