@@ -37,8 +37,6 @@ namespace plk {
 
 constexpr int TC_THREADS = 256;
 constexpr int TC_WARPS = TC_THREADS / 32;
-constexpr int TC_LD = 68;                       // padded row stride (elements) of tiles and matrices
-constexpr int TC_REGION = 64 * TC_LD * 8;       // bytes of one tile / one matrix, either precision (34 816)
 
 template <typename T>
 struct Tc;
@@ -46,11 +44,15 @@ template <>
 struct Tc<double> {
   static constexpr int MT = 8, KT = 4, CN = 2;  // m-tile rows, k per instruction, accumulator registers per n-tile
   static constexpr int TP = MT * TC_WARPS, RPT = CN / 2;  // patterns per tile (64), rows per thread (1)
+  static constexpr int LD = 68;                            // padded row stride (elements) of tiles and matrices
+  static constexpr int TILE_BYTES = TP * LD * 8, MAT_BYTES = 64 * LD * 8;  // 34 816 each
 };
 template <>
 struct Tc<float> {
   static constexpr int MT = 16, KT = 8, CN = 4;
   static constexpr int TP = MT * TC_WARPS, RPT = CN / 2;  // 128, 2
+  static constexpr int LD = 72;
+  static constexpr int TILE_BYTES = TP * LD * 4, MAT_BYTES = 64 * LD * 4;  // 36 864, 18 432
 };
 
 // ---- PTX ------------------------------------------------------------------------------------------------------
@@ -63,12 +65,12 @@ template <int N>
 __device__ __forceinline__ void tc_cp_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
 
 __device__ __forceinline__ void tc_mma(double (&d)[2], double a, double b) {
-  asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
+  asm("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
                : "+d"(d[0]), "+d"(d[1])
                : "d"(a), "d"(b));
 }
 __device__ __forceinline__ void tc_mma(float (&d)[4], const uint32_t (&a)[4], const uint32_t (&b)[2]) {
-  asm volatile(
+  asm(
       "mma.sync.aligned.m16n8k8.row.col.f32.tf32.tf32.f32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%0,%1,%2,%3};"
       : "+f"(d[0]), "+f"(d[1]), "+f"(d[2]), "+f"(d[3])
       : "r"(a[0]), "r"(a[1]), "r"(a[2]), "r"(a[3]), "r"(b[0]), "r"(b[1]));
@@ -84,13 +86,13 @@ __device__ __forceinline__ void tc_split(float x, uint32_t& hi, uint32_t& lo) {
 }
 
 // ---- staging ---------------------------------------------------------------------------------------------------
-// rows 0..n-1 of `src` ([.][64] row-major in global memory) -> tile rows (stride TC_LD); rows n..TP-1 <- 0
+// rows 0..n-1 of `src` ([.][64] row-major in global memory) -> tile rows (stride Tc<T>::LD); rows n..TP-1 <- 0
 template <typename T>
 __device__ __forceinline__ void tc_load_tile(T* __restrict__ tile, const T* __restrict__ src, int n) {
   constexpr int VEC = 16 / (int)sizeof(T), CPR = SP64 / VEC, TP = Tc<T>::TP;
   for (int idx = threadIdx.x; idx < TP * CPR; idx += TC_THREADS) {
     const int row = idx / CPR, ch = idx % CPR;
-    T* dst = tile + row * TC_LD + ch * VEC;
+    T* dst = tile + row * Tc<T>::LD + ch * VEC;
     if (row < n) {
       tc_cp_async16(dst, src + (size_t)row * SP64 + ch * VEC);
     } else {
@@ -106,32 +108,18 @@ __device__ __forceinline__ void tc_load_operand(T* tile, int kind, const void* p
   else if (kind == KIND_BCAST) tc_load_tile<T>(tile, static_cast<const T*>(ptr) + (size_t)p0 * SP64, n);
 }
 
-// matrix [64][64] row-major in global memory -> shared.  fp64: one plane.  fp32: hi plane, then lo plane.
-__device__ __forceinline__ void tc_load_matrix(double* __restrict__ sM, const double* __restrict__ M) {
-  for (int idx = threadIdx.x; idx < SP64 * SP64 / 2; idx += TC_THREADS) {
-    const int r = idx >> 5, c2 = (idx & 31) * 2;
-    const double2 v = *reinterpret_cast<const double2*>(M + r * SP64 + c2);
-    *reinterpret_cast<double2*>(sM + r * TC_LD + c2) = v;
-  }
-}
-__device__ __forceinline__ void tc_load_matrix(float* __restrict__ sM, const float* __restrict__ M) {
-  for (int idx = threadIdx.x; idx < SP64 * SP64 / 4; idx += TC_THREADS) {
-    const int r = idx >> 4, c4 = (idx & 15) * 4;
-    const float4 v = *reinterpret_cast<const float4*>(M + r * SP64 + c4);
-    uint32_t h[4], l[4];
-    tc_split(v.x, h[0], l[0]);
-    tc_split(v.y, h[1], l[1]);
-    tc_split(v.z, h[2], l[2]);
-    tc_split(v.w, h[3], l[3]);
-    *reinterpret_cast<uint4*>(sM + r * TC_LD + c4) = make_uint4(h[0], h[1], h[2], h[3]);
-    *reinterpret_cast<uint4*>(sM + SP64 * TC_LD + r * TC_LD + c4) = make_uint4(l[0], l[1], l[2], l[3]);
+// matrix [64][64] row-major in global memory -> shared (padded rows), asynchronously (cp.async, 16-byte chunks)
+template <typename T>
+__device__ __forceinline__ void tc_load_matrix(T* __restrict__ sM, const T* __restrict__ M) {
+  constexpr int VEC = 16 / (int)sizeof(T), CPR = SP64 / VEC;
+  for (int idx = threadIdx.x; idx < SP64 * CPR; idx += TC_THREADS) {
+    const int r = idx / CPR, ch = idx % CPR;
+    tc_cp_async16(sM + r * Tc<T>::LD + ch * VEC, M + r * SP64 + ch * VEC);
   }
 }
 // element M[s][x] of a staged matrix (tip gathers)
-__device__ __forceinline__ double tc_mat_at(const double* sM, int s, int x) { return sM[s * TC_LD + x]; }
-__device__ __forceinline__ float tc_mat_at(const float* sM, int s, int x) {
-  return sM[s * TC_LD + x] + sM[SP64 * TC_LD + s * TC_LD + x];
-}
+__device__ __forceinline__ double tc_mat_at(const double* sM, int s, int x) { return sM[s * Tc<double>::LD + x]; }
+__device__ __forceinline__ float tc_mat_at(const float* sM, int s, int x) { return sM[s * Tc<float>::LD + x]; }
 
 // ---- warp-level product: acc[nt][.] = sum_x A[row][x] * B(x, 8 nt + n)  for the warp's MT rows ----------------------
 //   TRANS = false: B(x, s) = M[s][x]  (M . x);   TRANS = true: B(x, s) = M[x][s]  (M^T . x)
@@ -144,37 +132,59 @@ __device__ __forceinline__ void tc_gemm(const double* __restrict__ sA, const dou
   for (int nt = 0; nt < 8; ++nt) acc[nt][0] = acc[nt][1] = 0.0;
 #pragma unroll 4
   for (int k0 = 0; k0 < SP64; k0 += 4) {
-    const double a = sA[r * TC_LD + k0 + c];
+    const double a = sA[r * Tc<double>::LD + k0 + c];
 #pragma unroll
     for (int nt = 0; nt < 8; ++nt) {
-      const double b = TRANS ? sM[(k0 + c) * TC_LD + nt * 8 + r] : sM[(nt * 8 + r) * TC_LD + k0 + c];
+      const double b = TRANS ? sM[(k0 + c) * Tc<double>::LD + nt * 8 + r] : sM[(nt * 8 + r) * Tc<double>::LD + k0 + c];
       tc_mma(acc[nt], a, b);
     }
   }
 }
+// fp32: the k index of an mma is only a summation index, so the non-transposed product assigns lane c the
+// physical columns k0 + 2c, 2c + 1 (instead of k0 + c, c + 4) for BOTH operands: one 64-bit shared-memory load per
+// fragment pair.  hi / lo parts are formed in registers; the three products of one k-step are issued term by term
+// over the 8 independent accumulators so that no mma waits on the one before it.
 template <bool TRANS>
 __device__ __forceinline__ void tc_gemm(const float* __restrict__ sA, const float* __restrict__ sM, float (&acc)[8][4],
                                         int r, int c) {
-  const uint32_t* sH = reinterpret_cast<const uint32_t*>(sM);
-  const uint32_t* sL = sH + SP64 * TC_LD;
+  constexpr int LD = Tc<float>::LD;
 #pragma unroll
   for (int nt = 0; nt < 8; ++nt) acc[nt][0] = acc[nt][1] = acc[nt][2] = acc[nt][3] = 0.0f;
 #pragma unroll 2
   for (int k0 = 0; k0 < SP64; k0 += 8) {
-    uint32_t ah[4], al[4];
-    tc_split(sA[r * TC_LD + k0 + c], ah[0], al[0]);
-    tc_split(sA[(r + 8) * TC_LD + k0 + c], ah[1], al[1]);
-    tc_split(sA[r * TC_LD + k0 + c + 4], ah[2], al[2]);
-    tc_split(sA[(r + 8) * TC_LD + k0 + c + 4], ah[3], al[3]);
+    float av[4];
+    if (!TRANS) {
+      const float2 t0 = *reinterpret_cast<const float2*>(sA + r * LD + k0 + 2 * c);
+      const float2 t1 = *reinterpret_cast<const float2*>(sA + (r + 8) * LD + k0 + 2 * c);
+      av[0] = t0.x; av[1] = t1.x; av[2] = t0.y; av[3] = t1.y;
+    } else {
+      av[0] = sA[r * LD + k0 + c];
+      av[1] = sA[(r + 8) * LD + k0 + c];
+      av[2] = sA[r * LD + k0 + c + 4];
+      av[3] = sA[(r + 8) * LD + k0 + c + 4];
+    }
+    uint32_t ah[4], al[4], bh[8][2], bl[8][2];
+#pragma unroll
+    for (int j = 0; j < 4; ++j) tc_split(av[j], ah[j], al[j]);
 #pragma unroll
     for (int nt = 0; nt < 8; ++nt) {
-      const int i0 = TRANS ? (k0 + c) * TC_LD + nt * 8 + r : (nt * 8 + r) * TC_LD + k0 + c;
-      const int i1 = TRANS ? i0 + 4 * TC_LD : i0 + 4;
-      const uint32_t bh[2] = {sH[i0], sH[i1]}, bl[2] = {sL[i0], sL[i1]};
-      tc_mma(acc[nt], al, bh);
-      tc_mma(acc[nt], ah, bl);
-      tc_mma(acc[nt], ah, bh);
+      float b0, b1;
+      if (!TRANS) {
+        const float2 t = *reinterpret_cast<const float2*>(sM + (nt * 8 + r) * LD + k0 + 2 * c);
+        b0 = t.x; b1 = t.y;
+      } else {
+        b0 = sM[(k0 + c) * LD + nt * 8 + r];
+        b1 = sM[(k0 + c + 4) * LD + nt * 8 + r];
+      }
+      tc_split(b0, bh[nt][0], bl[nt][0]);
+      tc_split(b1, bh[nt][1], bl[nt][1]);
     }
+#pragma unroll
+    for (int nt = 0; nt < 8; ++nt) tc_mma(acc[nt], al, bh[nt]);
+#pragma unroll
+    for (int nt = 0; nt < 8; ++nt) tc_mma(acc[nt], ah, bl[nt]);
+#pragma unroll
+    for (int nt = 0; nt < 8; ++nt) tc_mma(acc[nt], ah, bh[nt]);
   }
 }
 
@@ -206,7 +216,8 @@ __device__ __forceinline__ void tc_gather(const T* __restrict__ sM, int z, int S
 // post-order update (maxima for the deferred step 3)
 // persistent grid over work items (operation, category, tile), tile fastest
 // ---------------------------------------------------------------------------------------------------------------
-constexpr size_t TC_POST_SMEM = 6 * (size_t)TC_REGION;  // 2 matrices + 2 stages x 2 operand tiles
+template <typename T>
+constexpr size_t tc_post_smem() { return 2 * (size_t)Tc<T>::MAT_BYTES + 4 * (size_t)Tc<T>::TILE_BYTES; }  // 2 stages
 
 template <typename T>
 __global__ void __launch_bounds__(TC_THREADS, 1) k_post_tc(const DevOp* __restrict__ ops, int n_ops, int P, int S, int C) {
@@ -214,12 +225,13 @@ __global__ void __launch_bounds__(TC_THREADS, 1) k_post_tc(const DevOp* __restri
   using V2 = typename Vec2Of<T>::type;
   constexpr int TP = Tc<T>::TP, RPT = Tc<T>::RPT;
   extern __shared__ __align__(16) unsigned char tc_smem[];
-  T* sM[2] = {reinterpret_cast<T*>(tc_smem), reinterpret_cast<T*>(tc_smem + TC_REGION)};
+  constexpr int LD = K::LD;
+  T* sM[2] = {reinterpret_cast<T*>(tc_smem), reinterpret_cast<T*>(tc_smem + K::MAT_BYTES)};
   T* sX[2][2];
 #pragma unroll
   for (int st = 0; st < 2; ++st)
 #pragma unroll
-    for (int k = 0; k < 2; ++k) sX[st][k] = reinterpret_cast<T*>(tc_smem + (size_t)(2 + 2 * st + k) * TC_REGION);
+    for (int k = 0; k < 2; ++k) sX[st][k] = reinterpret_cast<T*>(tc_smem + 2 * (size_t)K::MAT_BYTES + (size_t)(2 * st + k) * K::TILE_BYTES);
 
   const int n_tiles = (P + TP - 1) / TP;
   const long long total = (long long)n_ops * C * n_tiles;
@@ -240,31 +252,63 @@ __global__ void __launch_bounds__(TC_THREADS, 1) k_post_tc(const DevOp* __restri
     tc_load_operand<T>(sX[st][0], o.kind[0], o.child[0], c, p0, n, P);
     tc_load_operand<T>(sX[st][1], o.kind[1], o.child[1], c, p0, n, P);
   };
+  // per-row scalars of an item, fetched one item ahead into registers: compact states and pending exponents
+  struct RowMeta {
+    int z[2][RPT], e[2][RPT];
+  };
+  auto fetch = [&](long long i, RowMeta& m) {
+    const int tile = (int)(i % n_tiles);
+    const DevOp& o = ops[i / n_tiles / C];
+#pragma unroll
+    for (int h = 0; h < RPT; ++h) {
+      const int p = tile * TP + m0 + r + 8 * h;
+#pragma unroll
+      for (int k = 0; k < 2; ++k) {
+        m.z[k][h] = (o.kind[k] == KIND_STATES && p < P) ? static_cast<const uint8_t*>(o.child[k])[p] : 0;
+        m.e[k][h] = pending_exp<T>(o.cscale[k], p, P, C);
+      }
+    }
+  };
   issue(i0, 0);
   tc_cp_commit();
+  RowMeta cur, nxt;
+  fetch(i0, cur);
   long long cur_oc = -1;
   for (long long i = i0; i < i1; ++i) {
     const int st = (int)((i - i0) & 1);
-    if (i + 1 < i1) issue(i + 1, st ^ 1);
-    tc_cp_commit();
-    tc_cp_wait<1>();
-    __syncthreads();
     const int tile = (int)(i % n_tiles);
     const long long oc = i / n_tiles;
     const int c = (int)(oc % C);
     const DevOp o = ops[oc / C];
-    if (oc != cur_oc) {
-      tc_load_matrix(sM[0], static_cast<const T*>(o.mat[0]) + (size_t)c * SP64 * SP64);
-      tc_load_matrix(sM[1], static_cast<const T*>(o.mat[1]) + (size_t)c * SP64 * SP64);
-      cur_oc = oc;
+    const bool mma0 = o.kind[0] == KIND_PARTIALS || o.kind[0] == KIND_BCAST;
+    const bool mma1 = o.kind[1] == KIND_PARTIALS || o.kind[1] == KIND_BCAST;
+    const bool new_oc = oc != cur_oc;
+    // One barrier per item: this item's tiles have landed and every warp has left item i-1, so stage st^1 and (on
+    // a change of operation / category) the matrices may be overwritten.  A run of gather-only items (both
+    // children compact tips) of one (operation, category) touches neither and runs barrier-free.
+    if (mma0 || mma1 || new_oc) {
+      tc_cp_wait<0>();
       __syncthreads();
+    }
+    if (new_oc) {
+      tc_load_matrix<T>(sM[0], static_cast<const T*>(o.mat[0]) + (size_t)c * SP64 * SP64);
+      tc_load_matrix<T>(sM[1], static_cast<const T*>(o.mat[1]) + (size_t)c * SP64 * SP64);
+      tc_cp_commit();
+    }
+    if (i + 1 < i1) {
+      issue(i + 1, st ^ 1);
+      fetch(i + 1, nxt);
+    }
+    tc_cp_commit();
+    if (new_oc) {
+      tc_cp_wait<1>();  // the matrices (the older group); the next item's tiles stay in flight
+      __syncthreads();
+      cur_oc = oc;
     }
     const int p0 = tile * TP;
     T acc[2][8][K::CN];
-#pragma unroll
-    for (int k = 0; k < 2; ++k)
-      if (o.kind[k] == KIND_PARTIALS || o.kind[k] == KIND_BCAST)
-        tc_gemm<false>(sX[st][k] + m0 * TC_LD, sM[k], acc[k], r, c4);
+    if (mma0) tc_gemm<false>(sX[st][0] + m0 * LD, sM[0], acc[0], r, c4);
+    if (mma1) tc_gemm<false>(sX[st][1] + m0 * LD, sM[1], acc[1], r, c4);
 #pragma unroll
     for (int h = 0; h < RPT; ++h) {
       const int p = p0 + m0 + r + 8 * h;
@@ -272,15 +316,14 @@ __global__ void __launch_bounds__(TC_THREADS, 1) k_post_tc(const DevOp* __restri
 #pragma unroll
       for (int k = 0; k < 2; ++k) {
         if (o.kind[k] == KIND_STATES) {
-          const int z = live ? static_cast<const uint8_t*>(o.child[k])[p] : 0;
-          tc_gather<T>(sM[k], z, S, T(1), h, c4, acc[k]);
+          tc_gather<T>(sM[k], cur.z[k][h], S, T(1), h, c4, acc[k]);
         } else if (o.kind[k] == KIND_NONE) {
 #pragma unroll
           for (int nt = 0; nt < 8; ++nt) acc[k][nt][h * 2] = acc[k][nt][h * 2 + 1] = T(0);
         }
       }
-      const Pow2Pair<T> f0 = pow2_pair(-pending_exp<T>(o.cscale[0], p, P, C), T(0));
-      const Pow2Pair<T> f1 = pow2_pair(-pending_exp<T>(o.cscale[1], p, P, C), T(0));
+      const Pow2Pair<T> f0 = pow2_pair(-cur.e[0][h], T(0));
+      const Pow2Pair<T> f1 = pow2_pair(-cur.e[1][h], T(0));
       T mx = T(0);
 #pragma unroll
       for (int nt = 0; nt < 8; ++nt)
@@ -304,7 +347,7 @@ __global__ void __launch_bounds__(TC_THREADS, 1) k_post_tc(const DevOp* __restri
         if (c4 == 0 && o.scale != nullptr) static_cast<T*>(o.scale)[(size_t)c * P + p] = mx;
       }
     }
-    __syncthreads();
+    cur = nxt;
   }
 }
 
@@ -317,7 +360,9 @@ __global__ void __launch_bounds__(TC_THREADS, 1) k_post_tc(const DevOp* __restri
 // the owning warp touches, so a __syncwarp is the only barrier between the two products.
 // ---------------------------------------------------------------------------------------------------------------
 template <typename T>
-constexpr size_t tc_pre_smem() { return 6 * (size_t)TC_REGION + 2 * Tc<T>::TP * sizeof(double); }
+constexpr size_t tc_pre_smem() {
+  return 3 * (size_t)Tc<T>::MAT_BYTES + 3 * (size_t)Tc<T>::TILE_BYTES + 2 * Tc<T>::TP * sizeof(double);
+}
 
 template <typename T>
 __global__ void __launch_bounds__(TC_THREADS, 1) k_pre_tc(const DevPreItem* __restrict__ items, int P, int S, int C,
@@ -331,10 +376,12 @@ __global__ void __launch_bounds__(TC_THREADS, 1) k_pre_tc(const DevPreItem* __re
   constexpr int TP = Tc<T>::TP, RPT = Tc<T>::RPT;
   extern __shared__ __align__(16) unsigned char tc_smem[];
   T* sQ = reinterpret_cast<T*>(tc_smem);
-  T* sM[2] = {reinterpret_cast<T*>(tc_smem + TC_REGION), reinterpret_cast<T*>(tc_smem + 2 * (size_t)TC_REGION)};
-  T* tQM = reinterpret_cast<T*>(tc_smem + 3 * (size_t)TC_REGION);
-  T* tX[2] = {reinterpret_cast<T*>(tc_smem + 4 * (size_t)TC_REGION), reinterpret_cast<T*>(tc_smem + 5 * (size_t)TC_REGION)};
-  double* sRed = reinterpret_cast<double*>(tc_smem + 6 * (size_t)TC_REGION);  // [2][TP]
+  constexpr int LD = K::LD;
+  constexpr size_t MB = K::MAT_BYTES, TB = K::TILE_BYTES;
+  T* sM[2] = {reinterpret_cast<T*>(tc_smem + MB), reinterpret_cast<T*>(tc_smem + 2 * MB)};
+  T* tQM = reinterpret_cast<T*>(tc_smem + 3 * MB);
+  T* tX[2] = {reinterpret_cast<T*>(tc_smem + 3 * MB + TB), reinterpret_cast<T*>(tc_smem + 3 * MB + 2 * TB)};
+  double* sRed = reinterpret_cast<double*>(tc_smem + 3 * MB + 3 * TB);  // [2][TP]
 
   const DevPreItem it = items[blockIdx.y];
   const int p0 = blockIdx.x * TP, n = P - p0 < TP ? P - p0 : TP;
@@ -345,7 +392,7 @@ __global__ void __launch_bounds__(TC_THREADS, 1) k_pre_tc(const DevPreItem* __re
   const bool mma_x[2] = {it.kind[0] == KIND_PARTIALS || it.kind[0] == KIND_BCAST,
                          it.kind[1] == KIND_PARTIALS || it.kind[1] == KIND_BCAST};
 
-  if (want[0] || want[1]) tc_load_matrix(sQ, Qg);
+  if (want[0] || want[1]) tc_load_matrix<T>(sQ, Qg);  // joins the first category's cp.async group
 
   int z[2][RPT];
   Pow2Pair<T> fx[2][RPT], fq[RPT];
@@ -363,14 +410,18 @@ __global__ void __launch_bounds__(TC_THREADS, 1) k_pre_tc(const DevPreItem* __re
     }
   }
 
+  // Staging of category c+1 is spread over category c: each buffer is refilled (cp.async) as soon as a barrier
+  // says every warp is done with it -- q_m after the u_k have been formed, M_k and the x_k tile after q_k.
+  auto stage_child = [&](int k, int c) {
+    tc_load_operand<T>(tX[k], it.kind[k], it.p[k], c, p0, n, P);
+    tc_load_matrix<T>(sM[k], static_cast<const T*>(it.mat[k]) + (size_t)c * SP64 * SP64);
+  };
+  tc_load_operand<T>(tQM, KIND_PARTIALS, it.qm, 0, p0, n, P);
+  stage_child(0, 0);
+  stage_child(1, 0);
+  tc_cp_commit();
   for (int c = 0; c < C; ++c) {
-    __syncthreads();  // everyone is done with the previous category's tiles and matrices
-    tc_load_operand<T>(tQM, KIND_PARTIALS, it.qm, c, p0, n, P);
-    tc_load_operand<T>(tX[0], it.kind[0], it.p[0], c, p0, n, P);
-    tc_load_operand<T>(tX[1], it.kind[1], it.p[1], c, p0, n, P);
-    tc_cp_commit();
-    tc_load_matrix(sM[0], static_cast<const T*>(it.mat[0]) + (size_t)c * SP64 * SP64);
-    tc_load_matrix(sM[1], static_cast<const T*>(it.mat[1]) + (size_t)c * SP64 * SP64);
+    const bool more = c + 1 < C;
     tc_cp_wait<0>();
     __syncthreads();
 
@@ -378,8 +429,8 @@ __global__ void __launch_bounds__(TC_THREADS, 1) k_pre_tc(const DevPreItem* __re
 #pragma unroll
     for (int k = 0; k < 2; ++k) {
       if (mma_x[k]) {
-        if (want[k]) tc_gemm<false>(tX[k] + m0 * TC_LD, sQ, qx[k], r, c4);
-        tc_gemm<false>(tX[k] + m0 * TC_LD, sM[k], a[k], r, c4);
+        if (want[k]) tc_gemm<false>(tX[k] + m0 * LD, sQ, qx[k], r, c4);
+        tc_gemm<false>(tX[k] + m0 * LD, sM[k], a[k], r, c4);
       } else {
 #pragma unroll
         for (int h = 0; h < RPT; ++h) {
@@ -403,7 +454,7 @@ __global__ void __launch_bounds__(TC_THREADS, 1) k_pre_tc(const DevPreItem* __re
 #pragma unroll
       for (int nt = 0; nt < 8; ++nt) {
         const int col = nt * 8 + 2 * c4;
-        const V2 qv = *reinterpret_cast<const V2*>(tQM + row * TC_LD + col);
+        const V2 qv = *reinterpret_cast<const V2*>(tQM + row * LD + col);
         const T qm[2] = {(qv.x * fq[h].f1) * fq[h].f2, (qv.y * fq[h].f1) * fq[h].f2};
         V2 u0, u1;
         T t0[2], t1[2];
@@ -417,16 +468,21 @@ __global__ void __launch_bounds__(TC_THREADS, 1) k_pre_tc(const DevPreItem* __re
         }
         u0.x = t0[0]; u0.y = t0[1];
         u1.x = t1[0]; u1.y = t1[1];
-        *reinterpret_cast<V2*>(tX[0] + row * TC_LD + col) = u0;
-        *reinterpret_cast<V2*>(tX[1] + row * TC_LD + col) = u1;
+        *reinterpret_cast<V2*>(tX[0] + row * LD + col) = u0;
+        *reinterpret_cast<V2*>(tX[1] + row * LD + col) = u1;
       }
       den[h] = fma(cw, (double)dd, den[h]);
     }
     __syncwarp();
+    if (more) {
+      __syncthreads();
+      tc_load_operand<T>(tQM, KIND_PARTIALS, it.qm, c + 1, p0, n, P);
+      tc_cp_commit();
+    }
 #pragma unroll
     for (int k = 0; k < 2; ++k) {
-      if (!need_q[k]) continue;
-      tc_gemm<true>(tX[k] + m0 * TC_LD, sM[k], a[k], r, c4);  // a[k] <- q_k
+      if (need_q[k]) {
+      tc_gemm<true>(tX[k] + m0 * LD, sM[k], a[k], r, c4);  // a[k] <- q_k
 #pragma unroll
       for (int h = 0; h < RPT; ++h) {
         const int p = p0 + m0 + r + 8 * h;
@@ -454,6 +510,12 @@ __global__ void __launch_bounds__(TC_THREADS, 1) k_pre_tc(const DevPreItem* __re
             if (c4 == 0) static_cast<T*>(it.q_scale[k])[(size_t)c * P + p] = mx;
           }
         }
+      }
+      }
+      if (more) {
+        __syncthreads();
+        stage_child(k, c + 1);
+        tc_cp_commit();
       }
     }
   }
@@ -497,7 +559,7 @@ int tc_launch_post(cudaStream_t stream, const DevOp* d_ops, int n_ops, int P, in
                    int64_t* launches) {
   static bool opted = false;  // per template instantiation
   if (!opted) {
-    if (cudaFuncSetAttribute(k_post_tc<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)TC_POST_SMEM) != cudaSuccess)
+    if (cudaFuncSetAttribute(k_post_tc<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)tc_post_smem<T>()) != cudaSuccess)
       return PLK_ERR_CUDA;
     opted = true;
   }
@@ -505,7 +567,7 @@ int tc_launch_post(cudaStream_t stream, const DevOp* d_ops, int n_ops, int P, in
   const long long total = (long long)n_ops * C * n_tiles;
   if (total <= 0) return PLK_SUCCESS;
   const int grid = total < sm_count ? (int)total : sm_count;
-  k_post_tc<T><<<grid, TC_THREADS, TC_POST_SMEM, stream>>>(d_ops, n_ops, P, S, C);
+  k_post_tc<T><<<grid, TC_THREADS, tc_post_smem<T>(), stream>>>(d_ops, n_ops, P, S, C);
   if (cudaGetLastError() != cudaSuccess) return PLK_ERR_CUDA;
   ++*launches;
   return PLK_SUCCESS;
