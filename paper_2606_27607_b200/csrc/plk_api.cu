@@ -13,6 +13,7 @@
 #include "plk_misc.cuh"
 #include "plk_nuc.cuh"
 #include "plk_nuc_tma.cuh"
+#include "plk_nuc_lean.cuh"
 #include "plk_schedule.h"
 #ifdef PLK_WITH_TENSOR
 #include "plk_tc.cuh"
@@ -268,10 +269,15 @@ int nuc_walk_warps(const plk_instance* in, K kernel, int n_chunks, int* total_wa
 // the walk costs one dependent global round trip per operation (~1 us) but a single launch and re-reads fresh
 // children from L2; the level shape costs one launch (~4 us) per level.  Once the patterns alone fill the GPU the
 // walk is bandwidth-bound like the level shape and moves fewer bytes, so it wins regardless of the list length.
-bool nuc_use_walk(const plk_instance* in, int n_ops, int n_levels) {
+// The specialised pre-order kernels (plk_nuc_lean.cuh) exist for C = 4 in the level order only.
+inline bool nuc_lean_ok(const plk_instance* in) {
+  return in->L.SP == 4 && in->L.C == 4 && !(in->cfg.flags & (PLK_FLAG_NO_TMA | PLK_FLAG_NO_LEVEL_BATCH | PLK_FLAG_PATTERN_WALK_ONLY));
+}
+bool nuc_use_walk(const plk_instance* in, int n_ops, int n_levels, bool pre_gradient = false) {
   const int flags = in->cfg.flags;
   if (flags & (PLK_FLAG_NO_LEVEL_BATCH | PLK_FLAG_LEVEL_BATCH_ONLY)) return false;
   if (flags & PLK_FLAG_PATTERN_WALK_ONLY) return true;
+  if (pre_gradient && nuc_lean_ok(in)) return false;
   const NucGeom g = nuc_geom(in->L);
   if (g.n_chunks >= in->sm_count * 8) return true;
   return (double)n_ops * 1.0 <= (double)n_levels * 4.0;
@@ -362,8 +368,11 @@ int launch_pre4_walk(plk_instance* in, const DevPreItem* d_items, int n, const T
 }
 
 // ---- TMA-staged 4-state kernels (plk_nuc_tma.cuh) ------------------------------------------------------------
-inline bool nuc_use_tma(const plk_instance* in) {
+// walk = true: the one-launch order, where the register-staged kernels are the faster ones (they re-read fresh
+// children from L2 with plain loads); the TMA walk runs only when the walk order is forced by flag.
+inline bool nuc_use_tma(const plk_instance* in, bool walk = false) {
   const int C = in->L.C;
+  if (walk && !(in->cfg.flags & PLK_FLAG_PATTERN_WALK_ONLY)) return false;
   return !(in->cfg.flags & (PLK_FLAG_NO_TMA | PLK_FLAG_NO_LEVEL_BATCH)) && (C == 1 || C == 2 || C == 4 || C == 8);
 }
 // grid of a TMA kernel: walk -> every CTA owns at least one full tile of rows; level -> at most one CTA per tile
@@ -446,6 +455,37 @@ int launch_pre4_tma(plk_instance* in, const DevPreItem* d_items, int n, const T*
     case 4: return launch_pre4_tma_c<T, 4>(in, d_items, n, Q, site, walk);
     case 8: return launch_pre4_tma_c<T, 8>(in, d_items, n, Q, site, walk);
     default: return PLK_ERR_UNSUPPORTED;
+  }
+}
+
+// specialised fused pre-order + gradient kernels (plk_nuc_lean.cuh): items of one class, level order
+template <typename T, int CLS>
+int launch_pre4_lean_c(plk_instance* in, const DevPreItem* d_items, int n, const T* Q, double* site) {
+  const Layout& L = in->L;
+  using St = NtStage<T, NL_C, 3, true>;
+  const size_t smem = (size_t)NT_NS * St::BYTES;
+  static int bps = 0;  // per instantiation
+  if (bps == 0) {
+    CU(cudaFuncSetAttribute(k_pre4_lean<T, CLS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&bps, k_pre4_lean<T, CLS>, NT_THREADS, smem));
+    if (bps < 1) return PLK_ERR_CUDA;
+  }
+  const long long n_tp = (L.P + St::TP - 1) / St::TP;
+  long long g = (long long)in->sm_count * bps;
+  if (g > n_tp * n) g = n_tp * n;
+  k_pre4_lean<T, CLS><<<(int)g, NT_THREADS, smem, in->stream>>>(d_items, n, L.P, Q, nuc_model(in, site),
+                                                               in->at<double>(L.off_grad_partial), L.n_tiles);
+  in->grad_parts = (int)n_tp * NT_CW;
+  CHECK_LAUNCH(in);
+  return PLK_SUCCESS;
+}
+template <typename T>
+int launch_pre4_lean(plk_instance* in, int cls, const DevPreItem* d_items, int n, const T* Q, double* site) {
+  switch (cls) {
+    case 0: return launch_pre4_lean_c<T, 0>(in, d_items, n, Q, site);
+    case 1: return launch_pre4_lean_c<T, 1>(in, d_items, n, Q, site);
+    case 2: return launch_pre4_lean_c<T, 2>(in, d_items, n, Q, site);
+    default: return PLK_ERR_GENERAL;
   }
 }
 
@@ -929,7 +969,7 @@ int plk_update_partials(plk_instance* in, const plk_op* ops, int count) {
   if (walk) {  // one launch, list order (plk_nuc.cuh "walk")
     rc = by_precision(in, [&](auto tag) -> int {
       using T = decltype(tag);
-      return nuc_use_tma(in) ? launch_post4_tma<T>(in, dops, count, true) : launch_post4_walk<T>(in, dops, count);
+      return nuc_use_tma(in, true) ? launch_post4_tma<T>(in, dops, count, true) : launch_post4_walk<T>(in, dops, count);
     });
     if (rc) return rc;
   } else if (cfg.flags & PLK_FLAG_NO_LEVEL_BATCH) {
@@ -1100,7 +1140,8 @@ static int pre_impl(plk_instance* in, int eigen, int root_pre, const plk_pre_op*
     if (in->next_pre_slot + fresh > L.pre_slots) return PLK_ERR_OUT_OF_MEMORY;
   }
   // build items in list order (bookkeeping), one per pair / unpaired op
-  struct HostItem { DevPreItem it; int level; };
+  struct HostItem { DevPreItem it; int level; int cls; };  // cls 0..2: plk_nuc_lean.cuh classes; 3: general kernel
+  const bool lean = want_grad && nuc_lean_ok(in);
   std::vector<HostItem> items;
   items.reserve(count);
   for (int i = 0; i < count; ++i) {
@@ -1143,7 +1184,24 @@ static int pre_impl(plk_instance* in, int eigen, int root_pre, const plk_pre_op*
         }
       }
     }
-    items.push_back({it, level[i]});
+    int cls = 3;
+    if (lean && it.slot[0] >= 0 && it.slot[1] >= 0) {
+      auto internal = [&](int k) { return it.kind[k] == KIND_PARTIALS && it.q[k] != nullptr; };
+      auto tip = [&](int k) { return it.kind[k] == KIND_STATES && it.q[k] == nullptr; };
+      if (tip(0) && internal(1)) {  // the update is symmetric in the two children: internal child first
+        std::swap(it.q[0], it.q[1]);
+        std::swap(it.q_scale[0], it.q_scale[1]);
+        std::swap(it.p[0], it.p[1]);
+        std::swap(it.p_scale[0], it.p_scale[1]);
+        std::swap(it.mat[0], it.mat[1]);
+        std::swap(it.kind[0], it.kind[1]);
+        std::swap(it.slot[0], it.slot[1]);
+      }
+      if (internal(0) && internal(1)) cls = 0;
+      else if (internal(0) && tip(1)) cls = 1;
+      else if (tip(0) && tip(1)) cls = 2;
+    }
+    items.push_back({it, level[i], cls});
     // bookkeeping after the item's inputs were resolved
     for (int k = 0; k < 2; ++k)
       if (pair[k] != nullptr && pair[k]->dest_pre >= 0) {
@@ -1162,11 +1220,18 @@ static int pre_impl(plk_instance* in, int eigen, int root_pre, const plk_pre_op*
     rc = ring_alloc(in, (size_t)n_items * sizeof(DevPreItem), &h, &d);
     if (rc) return rc;
     DevPreItem* hit = reinterpret_cast<DevPreItem*>(h);
-    const bool walk = L.SP == 4 && nuc_use_walk(in, n_items, n_levels);
+    const bool walk = L.SP == 4 && nuc_use_walk(in, n_items, n_levels, want_grad);
+    std::vector<int> class_start((size_t)n_levels * 5, 0);  // per level: first item of class 0..3, end
     if (walk) {
       for (int i = 0; i < n_items; ++i) hit[i] = items[i].it;  // list order (plk_nuc.cuh "walk")
-    } else {
-      for (const HostItem& hi : items) hit[fill[hi.level]++] = hi.it;
+    } else {  // by level, and inside a level by class
+      for (const HostItem& hi : items) ++class_start[(size_t)hi.level * 5 + hi.cls + 1];
+      for (int l = 0; l < n_levels; ++l) {
+        class_start[(size_t)l * 5] = level_start[l];
+        for (int k = 0; k < 4; ++k) class_start[(size_t)l * 5 + k + 1] += class_start[(size_t)l * 5 + k];
+      }
+      std::vector<int> cfill(class_start);
+      for (const HostItem& hi : items) hit[cfill[(size_t)hi.level * 5 + hi.cls]++] = hi.it;
     }
     rc = copy_ring(in, h, d, (size_t)n_items * sizeof(DevPreItem));
     if (rc) return rc;
@@ -1175,18 +1240,28 @@ static int pre_impl(plk_instance* in, int eigen, int root_pre, const plk_pre_op*
     if (walk) {
       rc = by_precision(in, [&](auto tag) -> int {
         using T = decltype(tag);
-        return nuc_use_tma(in) ? launch_pre4_tma<T>(in, dit, n_items, static_cast<const T*>(Q), d_site, true)
+        return nuc_use_tma(in, true) ? launch_pre4_tma<T>(in, dit, n_items, static_cast<const T*>(Q), d_site, true)
                                : launch_pre4_walk<T>(in, dit, n_items, static_cast<const T*>(Q), d_site);
       });
       if (rc) return rc;
     }
     for (int l = 0; l < (walk ? 0 : n_levels); ++l) {
-      const int n = level_start[l + 1] - level_start[l];
+      for (int k = 0; k < 3; ++k) {  // specialised classes
+        const int c0 = class_start[(size_t)l * 5 + k], m = class_start[(size_t)l * 5 + k + 1] - c0;
+        if (m == 0) continue;
+        rc = by_precision(in, [&](auto tag) -> int {
+          using T = decltype(tag);
+          return launch_pre4_lean<T>(in, k, dit + c0, m, static_cast<const T*>(Q), d_site);
+        });
+        if (rc) return rc;
+      }
+      const int g0 = class_start[(size_t)l * 5 + 3];
+      const int n = level_start[l + 1] - g0;
       for (int first = 0; first < n; first += 32768) {
         const int m = n - first < 32768 ? n - first : 32768;
         rc = by_precision(in, [&](auto tag) -> int {
           using T = decltype(tag);
-          const DevPreItem* p0 = dit + level_start[l] + first;
+          const DevPreItem* p0 = dit + g0 + first;
           if (L.SP != 4) return launch_pre64<T>(in, p0, m, static_cast<const T*>(Q), d_site);
           return nuc_use_tma(in) ? launch_pre4_tma<T>(in, p0, m, static_cast<const T*>(Q), d_site, false)
                                  : launch_pre4<T>(in, p0, m, static_cast<const T*>(Q), d_site);

@@ -1,0 +1,206 @@
+// plk_nuc_lean.cuh -- 4-state fused pre-order + gradient kernel, specialised.
+//
+// Why.  The general TMA-staged kernel (plk_nuc_tma.cuh) spends ~600 warp instructions per (8 patterns x 4
+// categories) cell group, of which 165 are fp64 arithmetic: the rest is operand-kind / slot / store-flag branching,
+// index arithmetic and reductions done once per child (profiles/r01_nuc_pre4_tma.md: issue slots 42 % busy, "wait"
+// the top stall, 2 CTAs per SM at 140 registers).  The hot case has no such variety: C = 4 categories, both
+// derivatives wanted, a child is either an internal node (full partials in, q_k out) or a compact tip (states in,
+// nothing out).  This file compiles exactly those three item classes -- the host sorts the items of a level by
+// class and launches one grid per class -- so that the consumer body is straight-line code:
+//   CLS 0  both children internal          CLS 1  child 0 internal, child 1 compact tip          CLS 2  both tips
+// (a tip / internal pair is stored with the internal child first; the update is symmetric in the two children).
+// Everything else (other category counts, tips given as partials, single-child items, the walk order) stays on
+// the general kernels.
+//
+// Pipeline, stage layout and producer are those of plk_nuc_tma.cuh (cp.async.bulk into an NS-deep ring of stages,
+// mbarrier full / empty pairs, level order: tiles of 32 patterns dealt round-robin to the CTAs).  Lane mapping:
+// lane = 8 g + pl, g = category, pl = pattern within the warp's 8 patterns.  The category sums finish on the lanes
+// of g = 0 (child 0) and g = 1 (child 1), which therefore hold ONE gradient accumulator each: a single 3-step
+// xor reduction per tile serves both children.
+#pragma once
+#include "plk_nuc_tma.cuh"
+
+namespace plk {
+
+constexpr int NL_C = 4;
+
+// tiles of CTA b in level order, without 64-bit division: tile j is (item, t) with item * n_tp + t = b + j * G
+struct NlWalk {
+  uint32_t item, t, step_item, step_t, n_tp;
+  __device__ __forceinline__ void init(uint32_t b, uint32_t G, uint32_t n_tp_) {
+    n_tp = n_tp_;
+    item = b / n_tp;
+    t = b - item * n_tp;
+    step_item = G / n_tp;
+    step_t = G - step_item * n_tp;
+  }
+  __device__ __forceinline__ void next() {
+    item += step_item;
+    t += step_t;
+    if (t >= n_tp) {
+      t -= n_tp;
+      ++item;
+    }
+  }
+};
+
+template <typename T, int CLS>
+__global__ void __launch_bounds__(NT_THREADS, 4) k_pre4_lean(const DevPreItem* __restrict__ items, int n_items, int P,
+                                                             const T* __restrict__ Qg, NucModel md,
+                                                             double* __restrict__ grad_partial, int n_part) {
+  constexpr int C = NL_C;
+  constexpr bool TIP0 = CLS == 2, TIP1 = CLS >= 1;
+  using St = NtStage<T, C, 3, true>;
+  constexpr int MS = St::MS, TP = St::TP;
+  extern __shared__ __align__(128) unsigned char nt_smem[];
+  __shared__ __align__(8) uint64_t full[NT_NS], empty[NT_NS];
+  __shared__ __align__(16) T sQ[16];
+  if (threadIdx.x == 0) {
+#pragma unroll
+    for (int s = 0; s < NT_NS; ++s) {
+      mbar_init(&full[s], 1);
+      mbar_init(&empty[s], NT_CW);
+    }
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    fence_proxy_async();
+  }
+  if (threadIdx.x < 16) sQ[threadIdx.x] = Qg[threadIdx.x];
+  __syncthreads();
+  const uint32_t n_tp = (uint32_t)((P + TP - 1) / TP);
+  const uint32_t total = (uint32_t)n_items * n_tp;
+  const uint32_t G = gridDim.x, b = blockIdx.x;
+  const int J = total > b ? (int)((total - b + G - 1) / G) : 0;
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+
+  if (warp == NT_CW) {  // ---- producer (one lane)
+    if (lane == 0) {
+      NlWalk w;
+      w.init(b, G, n_tp);
+      for (int j = 0; j < J; ++j, w.next()) {
+        if (j >= NT_NS) mbar_wait(&empty[j % NT_NS], (uint32_t)((j / NT_NS - 1) & 1));
+        const DevPreItem* it = items + w.item;
+        const int p0 = (int)w.t * TP;
+        const int n = P - p0 < TP ? P - p0 : TP;
+        const void* ptr[3] = {it->qm, it->p[0], it->p[1]};
+        const int kind[3] = {KIND_PARTIALS, TIP0 ? KIND_STATES : KIND_PARTIALS, TIP1 ? KIND_STATES : KIND_PARTIALS};
+        const void* mat[2] = {it->mat[0], it->mat[1]};
+        nt_fill<T, C, 3, true>(nt_smem + (size_t)(j % NT_NS) * St::BYTES, &full[j % NT_NS], it, sizeof(DevPreItem), ptr,
+                               kind, mat, md.weights, P, p0, n);
+      }
+    }
+    return;
+  }
+  // ---- consumers
+  const int g = lane >> 3, pl = lane & 7;
+  const int r = warp * 8 + pl;
+  const double cw = md.catw[g], cwr = cw * md.catr[g];
+  for (int j = 0; j < J; ++j) {
+    const int s = j % NT_NS;
+    unsigned char* stage = nt_smem + (size_t)s * St::BYTES;
+    mbar_wait(&full[s], (uint32_t)((j / NT_NS) & 1));
+    const NtHdr h = *reinterpret_cast<const NtHdr*>(stage + St::OFF_HDR);
+    const DevPreItem& it = *reinterpret_cast<const DevPreItem*>(stage + St::OFF_DESC);
+    const T* sM0 = reinterpret_cast<const T*>(stage + St::OFF_MATS) + g * MS;
+    const T* sM1 = sM0 + C * MS;
+    const T* sOp = reinterpret_cast<const T*>(stage + St::OFF_OPS);
+    const bool live = r < h.n;
+    const int p = h.p0 + r;
+
+    T a0[4], a1[4], qx0[4], qx1[4];
+    if (TIP0) {
+      const int z = stage[St::OFF_ST + h.soff0 + r];
+#pragma unroll
+      for (int x = 0; x < 4; ++x) {
+        a0[x] = z < 4 ? sM0[x * 4 + z] : T(1);
+        qx0[x] = z < 4 ? sQ[x * 4 + z] : T(0);
+      }
+    } else {
+      T x0[4];
+      ld4(sOp + ((C + g) * TP + r) * 4, x0);
+      mv4<T>(sM0, x0, a0);
+      mv4<T>(sQ, x0, qx0);
+    }
+    if (TIP1) {
+      const int z = stage[St::OFF_ST + (TP + 16) + h.soff1 + r];
+#pragma unroll
+      for (int x = 0; x < 4; ++x) {
+        a1[x] = z < 4 ? sM1[x * 4 + z] : T(1);
+        qx1[x] = z < 4 ? sQ[x * 4 + z] : T(0);
+      }
+    } else {
+      T x1[4];
+      ld4(sOp + ((2 * C + g) * TP + r) * 4, x1);
+      mv4<T>(sM1, x1, a1);
+      mv4<T>(sQ, x1, qx1);
+    }
+    T qm[4], u0[4], u1[4];
+    ld4(sOp + (g * TP + r) * 4, qm);
+    T dd = T(0);
+#pragma unroll
+    for (int x = 0; x < 4; ++x) {
+      u0[x] = qm[x] * a1[x];
+      u1[x] = qm[x] * a0[x];
+      dd = fma(u0[x], a0[x], dd);
+    }
+    T q0[4], q1[4];
+    mvt4<T>(sM0, u0, q0);
+    mvt4<T>(sM1, u1, q1);
+    T n0 = q0[0] * qx0[0], n1 = q1[0] * qx1[0];
+#pragma unroll
+    for (int x = 1; x < 4; ++x) {
+      n0 = fma(q0[x], qx0[x], n0);
+      n1 = fma(q1[x], qx1[x], n1);
+    }
+    // ---- rescaled q_k of the internal children (power-of-two factor, discarded: it cancels in num / den)
+    if (!TIP0) {
+      int key = max(max(max_key(q0[0]), max_key(q0[1])), max(max_key(q0[2]), max_key(q0[3])));
+      key = max(key, 0);
+      key = max(key, __shfl_xor_sync(0xffffffffu, key, 8));
+      key = max(key, __shfl_xor_sync(0xffffffffu, key, 16));
+      const T f = pow2_neg(exp_of_key(key, T(0)), T(0));
+      if (live) {
+        T v[4];
+#pragma unroll
+        for (int x = 0; x < 4; ++x) v[x] = q0[x] * f;
+        st4(static_cast<T*>(it.q[0]) + ((size_t)g * P + p) * 4, v);
+      }
+    }
+    if (!TIP1) {
+      int key = max(max(max_key(q1[0]), max_key(q1[1])), max(max_key(q1[2]), max_key(q1[3])));
+      key = max(key, 0);
+      key = max(key, __shfl_xor_sync(0xffffffffu, key, 8));
+      key = max(key, __shfl_xor_sync(0xffffffffu, key, 16));
+      const T f = pow2_neg(exp_of_key(key, T(0)), T(0));
+      if (live) {
+        T v[4];
+#pragma unroll
+        for (int x = 0; x < 4; ++x) v[x] = q1[x] * f;
+        st4(static_cast<T*>(it.q[1]) + ((size_t)g * P + p) * 4, v);
+      }
+    }
+    // ---- category sums: den on every lane, num_0 on the lanes of g = 0, num_1 on those of g = 1
+    double den = cw * (double)dd, m0 = cwr * (double)n0, m1 = cwr * (double)n1;
+    den += __shfl_xor_sync(0xffffffffu, den, 16);
+    m0 += __shfl_xor_sync(0xffffffffu, m0, 16);
+    m1 += __shfl_xor_sync(0xffffffffu, m1, 16);
+    den += __shfl_xor_sync(0xffffffffu, den, 8);
+    const bool odd = g & 1;
+    const double got = __shfl_xor_sync(0xffffffffu, odd ? m0 : m1, 8);
+    const double num = (odd ? m1 : m0) + got;
+    double contrib = 0.0;
+    if (live && g < 2) {
+      const double ratio = num / den;
+      if (md.site_out != nullptr) md.site_out[(size_t)it.slot[g] * P + p] = ratio;
+      contrib = reinterpret_cast<const double*>(stage + St::OFF_WTS)[r] * ratio;
+    }
+    const int slot = it.slot[g & 1];
+    __syncwarp();
+    if (lane == 0) mbar_arrive(&empty[s]);  // stage no longer needed (slot and weights are in registers)
+    contrib += __shfl_xor_sync(0xffffffffu, contrib, 1);
+    contrib += __shfl_xor_sync(0xffffffffu, contrib, 2);
+    contrib += __shfl_xor_sync(0xffffffffu, contrib, 4);
+    if (pl == 0 && g < 2) grad_partial[(size_t)slot * n_part + (h.p0 / TP) * NT_CW + warp] = contrib;
+  }
+}
+
+}  // namespace plk
