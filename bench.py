@@ -237,6 +237,9 @@ def oracle_time(wl, n_sample, repeats=1):
     return best, int(round(cores)), n_sample
 
 
+# measured DRAM traffic per step (bytes) of the dominant kernel's launches, keyed by (workload, precision, kernel)
+NCU_DRAM_BYTES = {("cfg1_gtr_128x100000", "fp64", "k_pre4_lean"): 4179.5e6}
+
 ORACLE_SAMPLE = {4: 40000, 61: 4000}  # cpu_baseline leg: patterns per oracle evaluation, ~10-30 s of CPU work
 REFERENCE_SAMPLE = {4: 8000, 61: 800}  # --impl reference: patterns per step (a few seconds per step)
 
@@ -388,13 +391,19 @@ def main():
     ph = res["phase_ms"]
     nuc = wl.n_states == 4
     dom = "pre_order_gradient" if ph["pre_order_gradient"] >= ph["post_order"] else "post_order"
-    kname = {"post_order": "k_post4" if nuc else ("tc_post" if args.tensor else "k_post64"),
-             "pre_order_gradient": "k_pre4" if nuc else ("tc_pre" if args.tensor else "k_pre64")}[dom]
-    n_levels_note = "all level launches of the phase"
+    lean = nuc and wl.n_categories == 4 and args.staging == "tma" and args.shape != "walk"
+    kname = {"post_order": ("k_post4_walk" if args.shape != "level" else "k_post4_tma") if nuc
+             else ("k_post_tc" if args.tensor else "k_post64"),
+             "pre_order_gradient": ("k_pre4_lean" if lean else "k_pre4_tma/k_pre4/k_pre4_walk") if nuc
+             else ("k_pre_tc" if args.tensor else "k_pre64")}[dom]
+    n_levels_note = "all launches of the kernel in one step (one per dependency level and item class)"
+    # DRAM bytes (read + write) of those launches from ncu, per step: profiles/r01_launches_cfg1_fp64.md
+    traffic = NCU_DRAM_BYTES.get((wl.name, args.precision, kname))
     if nuc or args.precision == "fp32":
         achieved = res["pre_gbs"] if dom == "pre_order_gradient" else res["post_gbs"]
         roofline = {"bound": "hbm", "kernel": kname, "achieved": achieved, "peak": peaks["hbm_gbs"], "unit": "GB/s",
-                    "frac": achieved / peaks["hbm_gbs"], "traffic": None, "peak_source": peaks["source"] + " hbm_gbs",
+                    "frac": achieved / peaks["hbm_gbs"], "traffic": traffic, "peak_source": peaks["source"] + " hbm_gbs",
+                    "algorithmic_bytes": alg["pre_bytes"] if dom == "pre_order_gradient" else alg["post_bytes"],
                     "over": n_levels_note}
     else:
         # fp64 61-state: tensor (DMMA) / fp64 pipe; nominal B200 fp64 ~ 40 TFLOP/s

@@ -52,7 +52,7 @@ struct Tc<float> {
   static constexpr int MT = 16, KT = 8, CN = 4;
   static constexpr int TP = MT * TC_WARPS, RPT = CN / 2;  // 128, 2
   static constexpr int LD = 72;
-  static constexpr int TILE_BYTES = TP * LD * 4, MAT_BYTES = 64 * LD * 4;  // 36 864, 18 432
+  static constexpr int TILE_BYTES = TP * LD * 4, MAT_BYTES = 2 * 64 * LD * 4;  // 36 864; hi plane + lo plane
 };
 
 // ---- PTX ------------------------------------------------------------------------------------------------------
@@ -119,7 +119,26 @@ __device__ __forceinline__ void tc_load_matrix(T* __restrict__ sM, const T* __re
 }
 // element M[s][x] of a staged matrix (tip gathers)
 __device__ __forceinline__ double tc_mat_at(const double* sM, int s, int x) { return sM[s * Tc<double>::LD + x]; }
-__device__ __forceinline__ float tc_mat_at(const float* sM, int s, int x) { return sM[s * Tc<float>::LD + x]; }
+__device__ __forceinline__ float tc_mat_at(const float* sM, int s, int x) {
+  return sM[s * Tc<float>::LD + x] + sM[SP64 * Tc<float>::LD + s * Tc<float>::LD + x];  // hi + lo: exact
+}
+// fp32: split a landed matrix in place into its TF32 hi plane and the exact remainder (lo plane), once per staging,
+// so that the inner loop of tc_gemm converts nothing on the B side.  Callers put a barrier on both sides.
+__device__ __forceinline__ void tc_split_matrix(double*) {}
+__device__ __forceinline__ void tc_split_matrix(float* sM) {
+  constexpr int LD = Tc<float>::LD;
+  for (int idx = threadIdx.x; idx < SP64 * SP64 / 4; idx += TC_THREADS) {
+    const int r = idx >> 4, c4 = (idx & 15) * 4;
+    float4 v = *reinterpret_cast<float4*>(sM + r * LD + c4);
+    float4 h, l;
+    h.x = __uint_as_float(tc_tf32(v.x)); l.x = v.x - h.x;
+    h.y = __uint_as_float(tc_tf32(v.y)); l.y = v.y - h.y;
+    h.z = __uint_as_float(tc_tf32(v.z)); l.z = v.z - h.z;
+    h.w = __uint_as_float(tc_tf32(v.w)); l.w = v.w - h.w;
+    *reinterpret_cast<float4*>(sM + r * LD + c4) = h;
+    *reinterpret_cast<float4*>(sM + SP64 * LD + r * LD + c4) = l;
+  }
+}
 
 // ---- warp-level product: acc[nt][.] = sum_x A[row][x] * B(x, 8 nt + n)  for the warp's MT rows ----------------------
 //   TRANS = false: B(x, s) = M[s][x]  (M . x);   TRANS = true: B(x, s) = M[x][s]  (M^T . x)
@@ -142,7 +161,7 @@ __device__ __forceinline__ void tc_gemm(const double* __restrict__ sA, const dou
 }
 // fp32: the k index of an mma is only a summation index, so the non-transposed product assigns lane c the
 // physical columns k0 + 2c, 2c + 1 (instead of k0 + c, c + 4) for BOTH operands: one 64-bit shared-memory load per
-// fragment pair.  hi / lo parts are formed in registers; the three products of one k-step are issued term by term
+// fragment pair.  The A side is split into hi / lo in registers, the B side comes pre-split (tc_split_matrix); the three products of one k-step are issued term by term
 // over the 8 independent accumulators so that no mma waits on the one before it.
 template <bool TRANS>
 __device__ __forceinline__ void tc_gemm(const float* __restrict__ sA, const float* __restrict__ sM, float (&acc)[8][4],
@@ -166,18 +185,21 @@ __device__ __forceinline__ void tc_gemm(const float* __restrict__ sA, const floa
     uint32_t ah[4], al[4], bh[8][2], bl[8][2];
 #pragma unroll
     for (int j = 0; j < 4; ++j) tc_split(av[j], ah[j], al[j]);
+    const uint32_t* sH = reinterpret_cast<const uint32_t*>(sM);
+    const uint32_t* sL = sH + SP64 * LD;
 #pragma unroll
     for (int nt = 0; nt < 8; ++nt) {
-      float b0, b1;
       if (!TRANS) {
-        const float2 t = *reinterpret_cast<const float2*>(sM + (nt * 8 + r) * LD + k0 + 2 * c);
-        b0 = t.x; b1 = t.y;
+        const uint2 th = *reinterpret_cast<const uint2*>(sH + (nt * 8 + r) * LD + k0 + 2 * c);
+        const uint2 tl = *reinterpret_cast<const uint2*>(sL + (nt * 8 + r) * LD + k0 + 2 * c);
+        bh[nt][0] = th.x; bh[nt][1] = th.y;
+        bl[nt][0] = tl.x; bl[nt][1] = tl.y;
       } else {
-        b0 = sM[(k0 + c) * LD + nt * 8 + r];
-        b1 = sM[(k0 + c + 4) * LD + nt * 8 + r];
+        bh[nt][0] = sH[(k0 + c) * LD + nt * 8 + r];
+        bh[nt][1] = sH[(k0 + c + 4) * LD + nt * 8 + r];
+        bl[nt][0] = sL[(k0 + c) * LD + nt * 8 + r];
+        bl[nt][1] = sL[(k0 + c + 4) * LD + nt * 8 + r];
       }
-      tc_split(b0, bh[nt][0], bl[nt][0]);
-      tc_split(b1, bh[nt][1], bl[nt][1]);
     }
 #pragma unroll
     for (int nt = 0; nt < 8; ++nt) tc_mma(acc[nt], al, bh[nt]);
@@ -303,6 +325,11 @@ __global__ void __launch_bounds__(TC_THREADS, 1) k_post_tc(const DevOp* __restri
     if (new_oc) {
       tc_cp_wait<1>();  // the matrices (the older group); the next item's tiles stay in flight
       __syncthreads();
+      if (sizeof(T) == 4) {
+        tc_split_matrix(sM[0]);
+        tc_split_matrix(sM[1]);
+        __syncthreads();
+      }
       cur_oc = oc;
     }
     const int p0 = tile * TP;
@@ -424,6 +451,12 @@ __global__ void __launch_bounds__(TC_THREADS, 1) k_pre_tc(const DevPreItem* __re
     const bool more = c + 1 < C;
     tc_cp_wait<0>();
     __syncthreads();
+    if (sizeof(T) == 4) {
+      if (c == 0 && (want[0] || want[1])) tc_split_matrix(sQ);
+      tc_split_matrix(sM[0]);
+      tc_split_matrix(sM[1]);
+      __syncthreads();
+    }
 
     T a[2][8][K::CN], qx[2][8][K::CN];
 #pragma unroll
