@@ -101,6 +101,31 @@ __device__ __forceinline__ void tc_load_tile(T* __restrict__ tile, const T* __re
     }
   }
 }
+// the calling warp's MT rows (first row m0) of the same tile, copied by the warp's own lanes: rows are warp-private
+// (only the owning warp reads them as A fragments), so a cp.async wait + __syncwarp is all the consumer needs
+template <typename T>
+__device__ __forceinline__ void tc_load_rows(T* __restrict__ tile, const T* __restrict__ src, int n, int m0, int lane) {
+  constexpr int VEC = 16 / (int)sizeof(T), CPR = SP64 / VEC, MT = Tc<T>::MT;
+#pragma unroll
+  for (int idx = lane; idx < MT * CPR; idx += 32) {
+    const int row = m0 + idx / CPR, ch = idx % CPR;
+    T* dst = tile + row * Tc<T>::LD + ch * VEC;
+    if (row < n) {
+      tc_cp_async16(dst, src + (size_t)row * SP64 + ch * VEC);
+    } else {
+#pragma unroll
+      for (int j = 0; j < VEC; ++j) dst[j] = T(0);
+    }
+  }
+}
+template <typename T>
+__device__ __forceinline__ void tc_load_operand_rows(T* tile, int kind, const void* ptr, int c, int p0, int n, int P,
+                                                     int m0, int lane) {
+  if (kind == KIND_PARTIALS)
+    tc_load_rows<T>(tile, static_cast<const T*>(ptr) + ((size_t)c * P + p0) * SP64, n, m0, lane);
+  else if (kind == KIND_BCAST)
+    tc_load_rows<T>(tile, static_cast<const T*>(ptr) + (size_t)p0 * SP64, n, m0, lane);
+}
 // operand tile of a child / of the parent's pre-order partials; compact tips and absent operands load nothing
 template <typename T>
 __device__ __forceinline__ void tc_load_operand(T* tile, int kind, const void* ptr, int c, int p0, int n, int P) {
@@ -271,8 +296,8 @@ __global__ void __launch_bounds__(TC_THREADS, 1) k_post_tc(const DevOp* __restri
     const int c = (int)(oc % C);
     const DevOp& o = ops[oc / C];
     const int p0 = tile * TP, n = P - p0 < TP ? P - p0 : TP;
-    tc_load_operand<T>(sX[st][0], o.kind[0], o.child[0], c, p0, n, P);
-    tc_load_operand<T>(sX[st][1], o.kind[1], o.child[1], c, p0, n, P);
+    tc_load_operand_rows<T>(sX[st][0], o.kind[0], o.child[0], c, p0, n, P, m0, lane);
+    tc_load_operand_rows<T>(sX[st][1], o.kind[1], o.child[1], c, p0, n, P, m0, lane);
   };
   // per-row scalars of an item, fetched one item ahead into registers: compact states and pending exponents
   struct RowMeta {
@@ -305,13 +330,12 @@ __global__ void __launch_bounds__(TC_THREADS, 1) k_post_tc(const DevOp* __restri
     const bool mma0 = o.kind[0] == KIND_PARTIALS || o.kind[0] == KIND_BCAST;
     const bool mma1 = o.kind[1] == KIND_PARTIALS || o.kind[1] == KIND_BCAST;
     const bool new_oc = oc != cur_oc;
-    // One barrier per item: this item's tiles have landed and every warp has left item i-1, so stage st^1 and (on
-    // a change of operation / category) the matrices may be overwritten.  A run of gather-only items (both
-    // children compact tips) of one (operation, category) touches neither and runs barrier-free.
-    if (mma0 || mma1 || new_oc) {
-      tc_cp_wait<0>();
-      __syncthreads();
-    }
+    // Tile rows are warp-private (each warp stages and reads its own MT rows), so between items a warp only waits
+    // for its own copies: the warps of a CTA drift apart and one warp's epilogue overlaps another's contraction.
+    // The CTA meets at a barrier only when the (operation, category) run ends and the matrices are replaced.
+    tc_cp_wait<0>();
+    __syncwarp();
+    if (new_oc) __syncthreads();
     if (new_oc) {
       tc_load_matrix<T>(sM[0], static_cast<const T*>(o.mat[0]) + (size_t)c * SP64 * SP64);
       tc_load_matrix<T>(sM[1], static_cast<const T*>(o.mat[1]) + (size_t)c * SP64 * SP64);
