@@ -42,6 +42,9 @@ def parse_args():
     ap.add_argument("--staging", choices=["tma", "ldg"], default="tma",
                     help="4-state operand staging: TMA ring (cp.async.bulk) / register-staged loads")
     ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
+    ap.add_argument("--sweep", action="store_true",
+                    help="BASELINE configs[4]: HKY fp32, taxa {8,32,128,512} x patterns {1e2..5e5}; prints one JSON "
+                         "line with the 20 points instead of the headline line")
     ap.add_argument("--no-extras", action="store_true", help="skip the other configs / precisions")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     return ap.parse_args()
@@ -332,10 +335,41 @@ def run_extras(peaks, steps, warmup):
     return out
 
 
+def run_sweep(peaks, steps, warmup):
+    """BASELINE configs[4]: likelihood and gradient throughput per (taxa, patterns) point, HKY fp32, 4 categories."""
+    from paper_2606_27607_b200 import workloads
+
+    points = []
+    for n in (8, 32, 128, 512):
+        for p in (100, 1_000, 10_000, 100_000, 500_000):
+            wl = workloads.config(4, n_tips=n, n_patterns=p)
+            res, ev = measure_device(wl, "fp32", 0, steps, warmup, peaks)
+            ev.close()
+            ph = res["phase_ms"]
+            lik_ms = ph["matrices"] + ph["post_order"] + ph["root"]
+            points.append({
+                "taxa": n, "patterns": p, "ms_per_step": round(res["ms_per_step"], 4),
+                "likelihood_ms": round(lik_ms, 4), "gradient_ms": round(ph["pre_order_gradient"], 4),
+                "likelihood_updates_per_s": res["alg"]["updates"] / (lik_ms * 1e-3),
+                "gradient_units_per_s": res["grad_units_per_s"],
+                "gradient_evals_per_s": res["gradient_evals_per_s"],
+                "post_hbm_frac": round(res["post_gbs"] / peaks["hbm_gbs"], 4),
+                "pre_hbm_frac": round(res["pre_gbs"] / peaks["hbm_gbs"], 4),
+                "launches_per_step": res["launches"] / steps, "finite": res["finite"]})
+            del wl
+    print(json.dumps({"sweep": "configs[4] HKY fp32", "unit": UNIT, "steps": steps, "points": points}))
+
+
 def main():
     args = parse_args()
     if args.impl == "reference":
         run_reference(args)
+        return
+    if args.sweep:
+        from paper_2606_27607_b200 import build
+
+        build.build()
+        run_sweep(load_peaks(), max(3, min(args.steps, 10)), 3)
         return
     import torch
 
