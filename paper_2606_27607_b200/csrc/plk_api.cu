@@ -17,6 +17,7 @@
 #include "plk_schedule.h"
 #ifdef PLK_WITH_TENSOR
 #include "plk_tc.cuh"
+#include "plk_tc5.cuh"
 #endif
 
 using namespace plk;
@@ -518,7 +519,11 @@ template <typename T>
 int launch_post64(plk_instance* in, const DevOp* d_ops, int n_ops) {
   const Layout& L = in->L;
 #ifdef PLK_WITH_TENSOR
-  if (in->cfg.flags & PLK_FLAG_TENSOR_CORES) return tc_launch_post<T>(in->stream, d_ops, n_ops, L.P, L.S, L.C, in->sm_count, &in->launches);
+  if (in->cfg.flags & PLK_FLAG_TENSOR_CORES) {
+    if (sizeof(T) == 4 && !(in->cfg.flags & PLK_FLAG_NO_TCGEN05))
+      return tc5::launch_post(in->stream, d_ops, n_ops, L.P, L.S, L.C, in->sm_count, &in->launches);
+    return tc_launch_post<T>(in->stream, d_ops, n_ops, L.P, L.S, L.C, in->sm_count, &in->launches);
+  }
 #endif
   int rc = opt_in_smem(k_post64<T>, post64_smem<T>());
   if (rc) return rc;
@@ -603,7 +608,7 @@ int plk_create(const plk_config* cfg, void* d_arena, size_t arena_bytes, void* c
     return PLK_ERR_OUT_OF_RANGE;
   }
   if (cfg->flags & ~(PLK_FLAG_TENSOR_CORES | PLK_FLAG_NO_LEVEL_BATCH | PLK_FLAG_SITE_DERIVATIVES | PLK_FLAG_LEVEL_BATCH_ONLY |
-                     PLK_FLAG_PATTERN_WALK_ONLY | PLK_FLAG_NO_TMA))
+                     PLK_FLAG_PATTERN_WALK_ONLY | PLK_FLAG_NO_TMA | PLK_FLAG_NO_TCGEN05))
     return PLK_ERR_UNSUPPORTED;
   if ((cfg->flags & PLK_FLAG_LEVEL_BATCH_ONLY) && (cfg->flags & PLK_FLAG_PATTERN_WALK_ONLY)) return PLK_ERR_UNSUPPORTED;
 #ifndef PLK_WITH_TENSOR

@@ -1,0 +1,475 @@
+// plk_tc5.cuh -- fp32 codon (61 states padded to SP = 64) post-order kernel on the 5th-generation tensor cores:
+// tcgen05.mma.kind::tf32 with accumulators in tensor memory (TMEM), sm_100a only.
+//
+// What it computes (SURVEY 8(a) steps 2-3; PAPER.md:27 pruning, :59/:71 tensor cores for codon models): for one work
+// item (operation, category c, tile of 128 patterns) and each child k
+//     D_k[p][s] = sum_x X_k[p][x] * M_k[s][x]                      (X_k: child partials, M_k: transition matrix)
+//     dest[p][s] = (D_0[p][s] 2^-e0[p]) * (D_1[p][s] 2^-e1[p]),    mx[c][p] = max_s dest[p][s]   (deferred rescaling)
+// exactly the arithmetic of k_post_tc<float> (plk_tc.cuh): split TF32, x = hi + lo with hi = tf32(x),
+// lo = tf32(x - hi), x.m ~= lo.hi + hi.lo + hi.hi accumulated in fp32 (dropped term 2^-22 relative).
+//
+// Mapping onto tcgen05.  A = X_k tile, 128 x 64, K-major (a pattern row of the [c][p][s] HBM layout IS a K-major
+// operand row); B = M_k, 64 x 64, K-major (row-major M[s][x]); D = 128 x 64 fp32 in TMEM, lane = pattern,
+// column = state.  K = 64 is eight k-steps of 8 (32 bytes); the three split products of both children are
+// 48 tcgen05.mma per item, issued by one thread.  Operands sit in shared memory in the canonical 128-byte-swizzled
+// K-major layout (8-row groups of 1024 B, 16-byte chunk j of row r stored at chunk j ^ (r & 7)); since K = 64 fp32 is
+// 256 B per row, a tile is two such 128 x 32 blocks.
+//
+// Compact tips (uint8 states) take the same route: the producer writes the one-hot (missing: all-ones) rows straight
+// into shared memory, so a tip costs no HBM read and its "gather" M[s][z] = hi + lo is exact on the tensor pipe
+// (its lo.hi product is skipped: lo = 0).
+//
+// Roles (warp-specialised, one persistent CTA per SM, 13 warps):
+//   warps 0-3   epilogue: tcgen05.ld (32 lanes x 32 columns), factors, product, row maximum, transposition through a
+//               small padded shared-memory stage so that global stores are full 128-byte segments
+//   warps 4-11  producers: ld.global (16-byte chunks, register-staged) -> hi/lo split -> st.shared in the swizzled
+//               layout -> fence.proxy.async -> mbarrier arrive; HBM -> L2 streaming runs ahead of them through
+//               cp.async.bulk.prefetch.L2 of the (contiguous, 32 KB) tiles two items ahead
+//   warp 12     TMEM allocation; one lane issues the MMAs and the tcgen05.commit that free the shared-memory stage,
+//               publish the accumulators and release the matrices
+// Pipelines: shared-memory stage per child (full/empty), two TMEM accumulator sets (full/empty), matrices
+// (full/empty; reloaded only when (operation, category) changes: items are dealt tile-fastest in contiguous ranges).
+#pragma once
+#include "plk_common.cuh"
+#include "plk_gen.cuh"
+
+namespace plk {
+namespace tc5 {
+
+constexpr int TP = 128;                    // patterns per tile = MMA M
+constexpr int EPI_WARPS = 4, PROD_WARPS = 8, N_WARPS = EPI_WARPS + PROD_WARPS + 1;
+constexpr int THREADS = N_WARPS * 32;      // 416
+constexpr int PROD_THREADS = PROD_WARPS * 32;
+constexpr int CHUNKS = 8;                  // 16-byte chunks per producer thread and unit (2048 per unit)
+constexpr uint32_t X_PLANE = TP * 64 * 4;  // 32 768: one plane (hi or lo) of a tile
+constexpr uint32_t M_PLANE = 64 * 64 * 4;  // 16 384
+constexpr uint32_t OFF_X = 0;              // [child][hi, lo]
+constexpr uint32_t OFF_M = 4 * X_PLANE;    // [child][hi, lo]
+constexpr uint32_t OFF_STAGE = OFF_M + 4 * M_PLANE;
+constexpr uint32_t STAGE_LD = 144;         // bytes per staged half row (128 + 16: conflict-free 16-byte accesses)
+constexpr uint32_t STAGE_WARP = 32 * STAGE_LD;
+constexpr uint32_t OFF_BAR = OFF_STAGE + EPI_WARPS * STAGE_WARP;
+constexpr uint32_t SMEM_USED = OFF_BAR + 128;
+constexpr size_t SMEM_BYTES = SMEM_USED + 1024;  // + slack for the 1024-byte alignment the swizzle needs
+constexpr int PREFETCH_AHEAD = 2;          // items
+
+// barrier slots (8 bytes each) at OFF_BAR
+enum { B_FULL0 = 0, B_FULL1, B_EMPTY0, B_EMPTY1, B_MFULL, B_MEMPTY, B_TFULL0, B_TFULL1, B_TEMPTY0, B_TEMPTY1, B_TMEM_PTR };
+
+// instruction descriptor: D fp32 (bit 4), A and B TF32 (2 << 7, 2 << 10), both K-major, N = 64 (>> 3 at bit 17),
+// M = 128 (>> 4 at bit 24)
+constexpr uint32_t IDESC = (1u << 4) | (2u << 7) | (2u << 10) | ((64u >> 3) << 17) | ((128u >> 4) << 24);
+
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+// shared-memory matrix descriptor: K-major, 128-byte swizzle, 8-row group stride (SBO) 1024 B, version 1 (sm_100)
+__device__ __forceinline__ uint64_t make_desc(uint32_t saddr) {
+  return (uint64_t)((saddr & 0x3FFFFu) >> 4) | ((uint64_t)1 << 16) | ((uint64_t)(1024 >> 4) << 32) | ((uint64_t)1 << 46) |
+         ((uint64_t)2 << 61);
+}
+__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint32_t bar) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
+  asm volatile(
+      "{\n\t.reg .pred p;\n\t"
+      "WAIT_%=:\n\t"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t"
+      "@p bra DONE_%=;\n\t"
+      "bra WAIT_%=;\n\t"
+      "DONE_%=:\n\t}" ::"r"(bar), "r"(parity)
+      : "memory");
+}
+__device__ __forceinline__ void fence_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+__device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
+__device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
+__device__ __forceinline__ void umma_tf32(uint32_t d_tmem, uint64_t a_desc, uint64_t b_desc, uint32_t accumulate) {
+  asm volatile(
+      "{\n\t.reg .pred p;\n\t"
+      "setp.ne.b32 p, %4, 0;\n\t"
+      "tcgen05.mma.cta_group::1.kind::tf32 [%0], %1, %2, %3, p;\n\t}" ::"r"(d_tmem),
+      "l"(a_desc), "l"(b_desc), "r"(IDESC), "r"(accumulate)
+      : "memory");
+}
+__device__ __forceinline__ void umma_commit(uint32_t bar) {
+  asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void tmem_ld32(uint32_t taddr, uint32_t (&v)[32]) {
+  asm volatile(
+      "tcgen05.ld.sync.aligned.32x32b.x32.b32 "
+      "{%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,%16,%17,%18,%19,%20,%21,%22,%23,%24,%25,%26,%27,%28,%29,"
+      "%30,%31}, [%32];"
+      : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]), "=r"(v[8]),
+        "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15]), "=r"(v[16]),
+        "=r"(v[17]), "=r"(v[18]), "=r"(v[19]), "=r"(v[20]), "=r"(v[21]), "=r"(v[22]), "=r"(v[23]), "=r"(v[24]),
+        "=r"(v[25]), "=r"(v[26]), "=r"(v[27]), "=r"(v[28]), "=r"(v[29]), "=r"(v[30]), "=r"(v[31])
+      : "r"(taddr)
+      : "memory");
+}
+__device__ __forceinline__ void tmem_ld_wait() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
+__device__ __forceinline__ void l2_prefetch_bulk(const void* p, uint32_t bytes) {
+  asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(p), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ float4 ldg_nc(const float* p) {
+  float4 v;
+  asm volatile("ld.global.nc.L1::no_allocate.v4.f32 {%0,%1,%2,%3}, [%4];"
+               : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w)
+               : "l"(p));
+  return v;
+}
+__device__ __forceinline__ float tf32_rna(float x) {
+  uint32_t r;
+  asm("cvt.rna.tf32.f32 %0, %1;" : "=r"(r) : "f"(x));
+  return __uint_as_float(r);
+}
+__device__ __forceinline__ void split4(const float4 v, float4& h, float4& l) {
+  h.x = tf32_rna(v.x); l.x = tf32_rna(v.x - h.x);
+  h.y = tf32_rna(v.y); l.y = tf32_rna(v.y - h.y);
+  h.z = tf32_rna(v.z); l.z = tf32_rna(v.z - h.z);
+  h.w = tf32_rna(v.w); l.w = tf32_rna(v.w - h.w);
+}
+__device__ __forceinline__ void sts128(uint32_t addr, const float4 v) {
+  asm volatile("st.shared.v4.f32 [%0], {%1,%2,%3,%4};" ::"r"(addr), "f"(v.x), "f"(v.y), "f"(v.z), "f"(v.w) : "memory");
+}
+__device__ __forceinline__ float4 lds128(uint32_t addr) {
+  float4 v;
+  asm volatile("ld.shared.v4.f32 {%0,%1,%2,%3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(addr) : "memory");
+  return v;
+}
+// byte offset of 16-byte chunk `ch` (0..15) of row `row` inside a K-major 128B-swizzled plane of `rows` rows x 64 fp32
+__device__ __forceinline__ uint32_t swz_off(int row, int ch, uint32_t rows) {
+  return (uint32_t)(ch >> 3) * rows * 128u + (uint32_t)row * 128u + (uint32_t)(((ch & 7) ^ (row & 7)) << 4);
+}
+
+// work-item decoding shared by the three roles
+struct Item {
+  int tile, c;
+  long long oc;  // operation * C + category: identifies the matrix pair
+  int op;
+};
+__device__ __forceinline__ Item decode(long long i, int n_tiles, int C) {
+  Item it;
+  it.tile = (int)(i % n_tiles);
+  it.oc = i / n_tiles;
+  it.c = (int)(it.oc % C);
+  it.op = (int)(it.oc / C);
+  return it;
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// producer side: one "unit" = 2048 16-byte chunks = 8 per producer thread: either the matrix pair of a new
+// (operation, category) run (sub = 0) or the tile of child sub - 1
+// ---------------------------------------------------------------------------------------------------------------
+struct Cur {
+  long long i;
+  int sub;
+};
+
+struct Ctx {
+  const DevOp* ops;
+  int P, S, C, n_tiles;
+  long long i0, i1;
+  uint32_t smem;  // 1024-aligned shared-memory base (shared-space address)
+  uint32_t bar;   // address of barrier slot 0
+  __device__ __forceinline__ bool new_run(long long i) const { return i == i0 || (i / n_tiles) != ((i - 1) / n_tiles); }
+  __device__ __forceinline__ bool valid(const Cur& u) const { return u.i < i1; }
+  __device__ __forceinline__ Cur first() const { return Cur{i0, 0}; }
+  __device__ __forceinline__ Cur next(const Cur& u) const {
+    if (u.sub < 2) return Cur{u.i, u.sub + 1};
+    return Cur{u.i + 1, (u.i + 1 < i1 && new_run(u.i + 1)) ? 0 : 1};
+  }
+  __device__ __forceinline__ uint32_t barrier(int slot) const { return bar + 8u * slot; }
+};
+
+__device__ __forceinline__ void prefetch_item(const Ctx& cx, long long i) {
+  if (i >= cx.i1) return;
+  const Item it = decode(i, cx.n_tiles, cx.C);
+  const DevOp& o = cx.ops[it.op];
+  const int p0 = it.tile * TP, n = cx.P - p0 < TP ? cx.P - p0 : TP;
+#pragma unroll
+  for (int k = 0; k < 2; ++k) {
+    if (o.kind[k] == KIND_PARTIALS)
+      l2_prefetch_bulk(static_cast<const float*>(o.child[k]) + ((size_t)it.c * cx.P + p0) * SP64, (uint32_t)n * 256u);
+    else if (o.kind[k] == KIND_BCAST)
+      l2_prefetch_bulk(static_cast<const float*>(o.child[k]) + (size_t)p0 * SP64, (uint32_t)n * 256u);
+  }
+}
+
+// global -> registers.  pt = producer thread index 0..255
+__device__ __forceinline__ void prod_load(const Ctx& cx, const Cur& u, int pt, float4 (&r)[CHUNKS]) {
+  const Item it = decode(u.i, cx.n_tiles, cx.C);
+  const DevOp& o = cx.ops[it.op];
+  if (u.sub == 0) {
+#pragma unroll
+    for (int j = 0; j < CHUNKS; ++j) {
+      const int idx = pt + PROD_THREADS * j, k = idx >> 10, rem = idx & 1023;
+      r[j] = ldg_nc(static_cast<const float*>(o.mat[k]) + (size_t)it.c * SP64 * SP64 + rem * 4);
+    }
+    return;
+  }
+  const int k = u.sub - 1, kind = o.kind[k];
+  const int p0 = it.tile * TP, n = cx.P - p0 < TP ? cx.P - p0 : TP;
+  if (k == 0 && pt == 0) prefetch_item(cx, u.i + PREFETCH_AHEAD);
+  if (kind == KIND_PARTIALS || kind == KIND_BCAST) {
+    const float* src = static_cast<const float*>(o.child[k]) + ((kind == KIND_PARTIALS ? (size_t)it.c * cx.P : 0) + p0) * SP64;
+#pragma unroll
+    for (int j = 0; j < CHUNKS; ++j) {
+      const int idx = pt + PROD_THREADS * j, row = idx >> 4;
+      r[j] = row < n ? ldg_nc(src + (size_t)idx * 4) : make_float4(0.f, 0.f, 0.f, 0.f);
+    }
+  } else if (kind == KIND_STATES) {
+    const uint8_t* st = static_cast<const uint8_t*>(o.child[k]) + p0;
+#pragma unroll
+    for (int j = 0; j < CHUNKS; ++j) {
+      const int row = (pt + PROD_THREADS * j) >> 4;
+      r[j].x = __int_as_float(row < n ? (int)st[row] : -1);
+    }
+  }
+}
+
+// registers -> shared memory (swizzled K-major planes), then signal the MMA thread
+__device__ __forceinline__ void prod_store(const Ctx& cx, const Cur& u, int pt, const float4 (&r)[CHUNKS], uint32_t n_item,
+                                           uint32_t n_run) {
+  const Item it = decode(u.i, cx.n_tiles, cx.C);
+  const DevOp& o = cx.ops[it.op];
+  const int lane = pt & 31;
+  if (u.sub == 0) {
+    mbar_wait(cx.barrier(B_MEMPTY), (n_run & 1) ^ 1);
+#pragma unroll
+    for (int j = 0; j < CHUNKS; ++j) {
+      const int idx = pt + PROD_THREADS * j, k = idx >> 10, rem = idx & 1023;
+      const uint32_t off = swz_off(rem >> 4, rem & 15, 64);
+      float4 h, l;
+      split4(r[j], h, l);
+      sts128(cx.smem + OFF_M + (2 * k) * M_PLANE + off, h);
+      sts128(cx.smem + OFF_M + (2 * k + 1) * M_PLANE + off, l);
+    }
+    fence_async_smem();
+    __syncwarp();
+    if (lane == 0) mbar_arrive(cx.barrier(B_MFULL));
+    return;
+  }
+  const int k = u.sub - 1, kind = o.kind[k];
+  mbar_wait(cx.barrier(B_EMPTY0 + k), (n_item & 1) ^ 1);
+  const uint32_t xhi = cx.smem + OFF_X + (2 * k) * X_PLANE, xlo = xhi + X_PLANE;
+  if (kind == KIND_PARTIALS || kind == KIND_BCAST) {
+#pragma unroll
+    for (int j = 0; j < CHUNKS; ++j) {
+      const int idx = pt + PROD_THREADS * j;
+      const uint32_t off = swz_off(idx >> 4, idx & 15, TP);
+      float4 h, l;
+      split4(r[j], h, l);
+      sts128(xhi + off, h);
+      sts128(xlo + off, l);
+    }
+  } else {
+    const int S = cx.S;
+#pragma unroll
+    for (int j = 0; j < CHUNKS; ++j) {
+      const int idx = pt + PROD_THREADS * j, ch = idx & 15, x0 = ch * 4;
+      const int z = kind == KIND_STATES ? __float_as_int(r[j].x) : -1;  // -1: row beyond the tile or operand absent
+      float4 h;
+      if (z < 0) {
+        h = make_float4(0.f, 0.f, 0.f, 0.f);
+      } else if (z < S) {  // one-hot
+        h.x = x0 == z ? 1.f : 0.f; h.y = x0 + 1 == z ? 1.f : 0.f; h.z = x0 + 2 == z ? 1.f : 0.f; h.w = x0 + 3 == z ? 1.f : 0.f;
+      } else {  // missing: every state possible (padding columns stay 0)
+        h.x = x0 < S ? 1.f : 0.f; h.y = x0 + 1 < S ? 1.f : 0.f; h.z = x0 + 2 < S ? 1.f : 0.f; h.w = x0 + 3 < S ? 1.f : 0.f;
+      }
+      sts128(xhi + swz_off(idx >> 4, ch, TP), h);
+    }
+  }
+  fence_async_smem();
+  __syncwarp();
+  if (lane == 0) mbar_arrive(cx.barrier(B_FULL0 + k));
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// the kernel
+// ---------------------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(THREADS, 1) k_post_tc5(const DevOp* __restrict__ ops, int n_ops, int P, int S, int C) {
+  extern __shared__ unsigned char tc5_smem_raw[];
+  Ctx cx;
+  cx.ops = ops; cx.P = P; cx.S = S; cx.C = C;
+  cx.n_tiles = (P + TP - 1) / TP;
+  {
+    const long long total = (long long)n_ops * C * cx.n_tiles;
+    const long long base = total / gridDim.x, rem = total % gridDim.x, b = blockIdx.x;
+    cx.i0 = b * base + (b < rem ? b : rem);
+    cx.i1 = cx.i0 + base + (b < rem ? 1 : 0);
+  }
+  if (cx.i0 >= cx.i1) return;  // whole CTA leaves before any barrier or TMEM allocation
+  cx.smem = (smem_u32(tc5_smem_raw) + 1023u) & ~1023u;
+  cx.bar = cx.smem + OFF_BAR;
+
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  if (threadIdx.x == 0) {
+    mbar_init(cx.barrier(B_FULL0), PROD_WARPS);
+    mbar_init(cx.barrier(B_FULL1), PROD_WARPS);
+    mbar_init(cx.barrier(B_EMPTY0), 1);
+    mbar_init(cx.barrier(B_EMPTY1), 1);
+    mbar_init(cx.barrier(B_MFULL), PROD_WARPS);
+    mbar_init(cx.barrier(B_MEMPTY), 1);
+    mbar_init(cx.barrier(B_TFULL0), 1);
+    mbar_init(cx.barrier(B_TFULL1), 1);
+    mbar_init(cx.barrier(B_TEMPTY0), EPI_WARPS);
+    mbar_init(cx.barrier(B_TEMPTY1), EPI_WARPS);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  if (warp == N_WARPS - 1) {  // 256 TMEM columns: two accumulator sets of (D_0, D_1) = 2 x 64 columns each
+    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], 256;" ::"r"(cx.barrier(B_TMEM_PTR)) : "memory");
+    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+  }
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+  uint32_t tmem_base;
+  asm volatile("ld.shared.b32 %0, [%1];" : "=r"(tmem_base) : "r"(cx.barrier(B_TMEM_PTR)) : "memory");
+
+  if (warp < EPI_WARPS) {
+    // ===== epilogue =====
+    const uint32_t stage = cx.smem + OFF_STAGE + warp * STAGE_WARP;
+    uint32_t n = 0;
+    for (long long i = cx.i0; i < cx.i1; ++i, ++n) {
+      const Item it = decode(i, cx.n_tiles, C);
+      const DevOp& o = ops[it.op];
+      const int p0 = it.tile * TP, prow0 = p0 + 32 * warp, p = prow0 + lane;
+      const Pow2Pair<float> f0 = pow2_pair(-pending_exp<float>(o.cscale[0], p, P, C), 0.f);
+      const Pow2Pair<float> f1 = pow2_pair(-pending_exp<float>(o.cscale[1], p, P, C), 0.f);
+      float* dest = static_cast<float*>(o.dest) + (size_t)it.c * P * SP64;
+      float* scale = static_cast<float*>(o.scale);
+      const uint32_t a = n & 1;
+      mbar_wait(cx.barrier(B_TFULL0 + a), (n >> 1) & 1);
+      tc_fence_after();
+      const uint32_t taddr = tmem_base + ((uint32_t)(32 * warp) << 16) + a * 128;
+      float mx = 0.f;
+#pragma unroll
+      for (int half = 0; half < 2; ++half) {
+        uint32_t d0[32], d1[32];
+        tmem_ld32(taddr + half * 32, d0);
+        tmem_ld32(taddr + 64 + half * 32, d1);
+        tmem_ld_wait();
+        if (half == 1) {  // accumulators are in registers: hand the TMEM set back before the stores
+          tc_fence_before();
+          __syncwarp();
+          if (lane == 0) mbar_arrive(cx.barrier(B_TEMPTY0 + a));
+        }
+#pragma unroll
+        for (int q = 0; q < 8; ++q) {
+          float v[4];
+#pragma unroll
+          for (int j = 0; j < 4; ++j) {
+            v[j] = ((__uint_as_float(d0[4 * q + j]) * f0.f1) * f0.f2) * ((__uint_as_float(d1[4 * q + j]) * f1.f1) * f1.f2);
+            mx = fmaxf(mx, v[j]);
+          }
+          sts128(stage + lane * STAGE_LD + q * 16, make_float4(v[0], v[1], v[2], v[3]));
+        }
+        __syncwarp();
+#pragma unroll
+        for (int j = 0; j < 8; ++j) {
+          const int idx = j * 32 + lane, r = idx >> 3, ch = idx & 7;
+          const float4 v = lds128(stage + r * STAGE_LD + ch * 16);
+          if (prow0 + r < P) *reinterpret_cast<float4*>(dest + (size_t)(prow0 + r) * SP64 + half * 32 + ch * 4) = v;
+        }
+        __syncwarp();
+      }
+      if (p < P && scale != nullptr) scale[(size_t)it.c * P + p] = mx;
+    }
+  } else if (warp < EPI_WARPS + PROD_WARPS) {
+    // ===== producers =====
+    const int pt = threadIdx.x - EPI_WARPS * 32;
+    if (pt == 0)
+      for (int d = 1; d < PREFETCH_AHEAD; ++d) prefetch_item(cx, cx.i0 + d);
+    float4 ra[CHUNKS], rb[CHUNKS];
+    uint32_t n_run = 0;  // matrix runs stored so far
+    Cur cur = cx.first(), nxt;
+    prod_load(cx, cur, pt, ra);
+    while (true) {
+      nxt = cx.next(cur);
+      const bool hn = cx.valid(nxt);
+      if (hn) prod_load(cx, nxt, pt, rb);
+      prod_store(cx, cur, pt, ra, (uint32_t)(cur.i - cx.i0), n_run);
+      n_run += cur.sub == 0;
+      if (!hn) break;
+      cur = cx.next(nxt);
+      const bool hc = cx.valid(cur);
+      if (hc) prod_load(cx, cur, pt, ra);
+      prod_store(cx, nxt, pt, rb, (uint32_t)(nxt.i - cx.i0), n_run);
+      n_run += nxt.sub == 0;
+      if (!hc) break;
+    }
+  } else {
+    // ===== MMA issuer: lane 0 issues, the warp stays converged =====
+    uint32_t n = 0, n_run = 0;
+    for (long long i = cx.i0; i < cx.i1; ++i, ++n) {
+      if (lane == 0) {
+      const Item it = decode(i, cx.n_tiles, C);
+      const DevOp& o = ops[it.op];
+      if (cx.new_run(i)) {
+        mbar_wait(cx.barrier(B_MFULL), n_run & 1);
+        ++n_run;
+      }
+      const uint32_t a = n & 1;
+      mbar_wait(cx.barrier(B_TEMPTY0 + a), ((n >> 1) & 1) ^ 1);
+#pragma unroll
+      for (int k = 0; k < 2; ++k) {
+        mbar_wait(cx.barrier(B_FULL0 + k), n & 1);
+        tc_fence_after();
+        const uint32_t d = tmem_base + a * 128 + k * 64;
+        const uint32_t xhi = cx.smem + OFF_X + (2 * k) * X_PLANE, xlo = xhi + X_PLANE;
+        const uint32_t mhi = cx.smem + OFF_M + (2 * k) * M_PLANE, mlo = mhi + M_PLANE;
+        const bool has_lo = o.kind[k] == KIND_PARTIALS || o.kind[k] == KIND_BCAST;
+        uint32_t acc = 0;
+        // small terms first, hi.hi last (same order as the mma.sync path)
+        if (has_lo) {
+#pragma unroll
+          for (int ks = 0; ks < 8; ++ks) {
+            umma_tf32(d, make_desc(xlo + (ks >> 2) * (TP * 128) + (ks & 3) * 32), make_desc(mhi + (ks >> 2) * (64 * 128) + (ks & 3) * 32), acc);
+            acc = 1;
+          }
+        }
+#pragma unroll
+        for (int ks = 0; ks < 8; ++ks) {
+          umma_tf32(d, make_desc(xhi + (ks >> 2) * (TP * 128) + (ks & 3) * 32), make_desc(mlo + (ks >> 2) * (64 * 128) + (ks & 3) * 32), acc);
+          acc = 1;
+        }
+#pragma unroll
+        for (int ks = 0; ks < 8; ++ks)
+          umma_tf32(d, make_desc(xhi + (ks >> 2) * (TP * 128) + (ks & 3) * 32), make_desc(mhi + (ks >> 2) * (64 * 128) + (ks & 3) * 32), 1);
+        umma_commit(cx.barrier(B_EMPTY0 + k));
+      }
+      umma_commit(cx.barrier(B_TFULL0 + a));
+      if (i + 1 < cx.i1 && cx.new_run(i + 1)) umma_commit(cx.barrier(B_MEMPTY));
+      }
+      __syncwarp();
+    }
+  }
+  tc_fence_before();
+  __syncthreads();
+  if (warp == N_WARPS - 1) {
+    tc_fence_after();
+    asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, 256;" ::"r"(tmem_base) : "memory");
+  }
+}
+
+inline int launch_post(cudaStream_t stream, const DevOp* d_ops, int n_ops, int P, int S, int C, int sm_count,
+                       int64_t* launches) {
+  static bool opted = false;
+  if (!opted) {
+    if (cudaFuncSetAttribute(k_post_tc5, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_BYTES) != cudaSuccess)
+      return PLK_ERR_CUDA;
+    opted = true;
+  }
+  const long long total = (long long)n_ops * C * ((P + TP - 1) / TP);
+  if (total <= 0) return PLK_SUCCESS;
+  const int grid = total < sm_count ? (int)total : sm_count;
+  k_post_tc5<<<grid, THREADS, SMEM_BYTES, stream>>>(d_ops, n_ops, P, S, C);
+  if (cudaGetLastError() != cudaSuccess) return PLK_ERR_CUDA;
+  ++*launches;
+  return PLK_SUCCESS;
+}
+
+}  // namespace tc5
+}  // namespace plk
