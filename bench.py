@@ -41,6 +41,8 @@ def parse_args():
                     help="4-state launch shape: one launch per level / one pattern-walk launch / library's choice")
     ap.add_argument("--staging", choices=["tma", "ldg"], default="tma",
                     help="4-state operand staging: TMA ring (cp.async.bulk) / register-staged loads")
+    ap.add_argument("--codon-fp32", choices=["tcgen05", "mma_sync"], default="tcgen05",
+                    help="fp32 --tensor post-order kernel: tcgen05/TMEM (default) or the legacy mma.sync arm")
     ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
     ap.add_argument("--sweep", action="store_true",
                     help="BASELINE configs[4]: HKY fp32, taxa {8,32,128,512} x patterns {1e2..5e5}; prints one JSON "
@@ -396,6 +398,7 @@ def main():
     flags = plk.FLAG_TENSOR_CORES if args.tensor else 0
     flags |= {"auto": 0, "level": plk.FLAG_LEVEL_BATCH_ONLY, "walk": plk.FLAG_PATTERN_WALK_ONLY}[args.shape]
     flags |= plk.FLAG_NO_TMA if args.staging == "ldg" else 0
+    flags |= plk.FLAG_NO_TCGEN05 if args.codon_fp32 == "mma_sync" else 0
     sampler = ClockSampler(local_rank) if rank == 0 else None
 
     if dist is not None:

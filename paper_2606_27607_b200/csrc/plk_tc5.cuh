@@ -143,49 +143,55 @@ __device__ __forceinline__ uint32_t swz_off(int row, int ch, uint32_t rows) {
   return (uint32_t)(ch >> 3) * rows * 128u + (uint32_t)row * 128u + (uint32_t)(((ch & 7) ^ (row & 7)) << 4);
 }
 
-// work-item decoding shared by the three roles
+// work items (operation, category, tile), tile fastest; each role walks its CTA's contiguous range incrementally
 struct Item {
-  int tile, c;
-  long long oc;  // operation * C + category: identifies the matrix pair
-  int op;
+  int op, c, tile;
+  uint32_t n;  // ordinal inside the CTA's range
 };
-__device__ __forceinline__ Item decode(long long i, int n_tiles, int C) {
-  Item it;
-  it.tile = (int)(i % n_tiles);
-  it.oc = i / n_tiles;
-  it.c = (int)(it.oc % C);
-  it.op = (int)(it.oc / C);
-  return it;
-}
 
 // ---------------------------------------------------------------------------------------------------------------
 // producer side: one "unit" = 2048 16-byte chunks = 8 per producer thread: either the matrix pair of a new
 // (operation, category) run (sub = 0) or the tile of child sub - 1
 // ---------------------------------------------------------------------------------------------------------------
 struct Cur {
-  long long i;
+  Item it;
   int sub;
 };
 
 struct Ctx {
   const DevOp* ops;
   int P, S, C, n_tiles;
-  long long i0, i1;
+  uint32_t n_items;
+  Item first_item;
   uint32_t smem;  // 1024-aligned shared-memory base (shared-space address)
   uint32_t bar;   // address of barrier slot 0
-  __device__ __forceinline__ bool new_run(long long i) const { return i == i0 || (i / n_tiles) != ((i - 1) / n_tiles); }
-  __device__ __forceinline__ bool valid(const Cur& u) const { return u.i < i1; }
-  __device__ __forceinline__ Cur first() const { return Cur{i0, 0}; }
+  __device__ __forceinline__ void advance(Item& it) const {
+    ++it.n;
+    if (++it.tile == n_tiles) {
+      it.tile = 0;
+      if (++it.c == C) {
+        it.c = 0;
+        ++it.op;
+      }
+    }
+  }
+  __device__ __forceinline__ bool valid(const Item& it) const { return it.n < n_items; }
+  // first item of the range or first tile of an (operation, category): the matrix pair changes
+  __device__ __forceinline__ bool new_run(const Item& it) const { return it.n == 0 || it.tile == 0; }
+  __device__ __forceinline__ bool valid(const Cur& u) const { return valid(u.it); }
+  __device__ __forceinline__ Cur first() const { return Cur{first_item, 0}; }
   __device__ __forceinline__ Cur next(const Cur& u) const {
-    if (u.sub < 2) return Cur{u.i, u.sub + 1};
-    return Cur{u.i + 1, (u.i + 1 < i1 && new_run(u.i + 1)) ? 0 : 1};
+    if (u.sub < 2) return Cur{u.it, u.sub + 1};
+    Item t = u.it;
+    advance(t);
+    return Cur{t, (valid(t) && new_run(t)) ? 0 : 1};
   }
   __device__ __forceinline__ uint32_t barrier(int slot) const { return bar + 8u * slot; }
 };
 
-__device__ __forceinline__ void prefetch_item(const Ctx& cx, long long i) {
-  if (i >= cx.i1) return;
-  const Item it = decode(i, cx.n_tiles, cx.C);
+__device__ __forceinline__ void prefetch_item(const Ctx& cx, Item it, int ahead) {
+  for (int d = 0; d < ahead; ++d) cx.advance(it);
+  if (!cx.valid(it)) return;
   const DevOp& o = cx.ops[it.op];
   const int p0 = it.tile * TP, n = cx.P - p0 < TP ? cx.P - p0 : TP;
 #pragma unroll
@@ -199,7 +205,7 @@ __device__ __forceinline__ void prefetch_item(const Ctx& cx, long long i) {
 
 // global -> registers.  pt = producer thread index 0..255
 __device__ __forceinline__ void prod_load(const Ctx& cx, const Cur& u, int pt, float4 (&r)[CHUNKS]) {
-  const Item it = decode(u.i, cx.n_tiles, cx.C);
+  const Item& it = u.it;
   const DevOp& o = cx.ops[it.op];
   if (u.sub == 0) {
 #pragma unroll
@@ -211,7 +217,7 @@ __device__ __forceinline__ void prod_load(const Ctx& cx, const Cur& u, int pt, f
   }
   const int k = u.sub - 1, kind = o.kind[k];
   const int p0 = it.tile * TP, n = cx.P - p0 < TP ? cx.P - p0 : TP;
-  if (k == 0 && pt == 0) prefetch_item(cx, u.i + PREFETCH_AHEAD);
+  if (k == 0 && pt == 0) prefetch_item(cx, it, PREFETCH_AHEAD);
   if (kind == KIND_PARTIALS || kind == KIND_BCAST) {
     const float* src = static_cast<const float*>(o.child[k]) + ((kind == KIND_PARTIALS ? (size_t)it.c * cx.P : 0) + p0) * SP64;
 #pragma unroll
@@ -230,9 +236,9 @@ __device__ __forceinline__ void prod_load(const Ctx& cx, const Cur& u, int pt, f
 }
 
 // registers -> shared memory (swizzled K-major planes), then signal the MMA thread
-__device__ __forceinline__ void prod_store(const Ctx& cx, const Cur& u, int pt, const float4 (&r)[CHUNKS], uint32_t n_item,
-                                           uint32_t n_run) {
-  const Item it = decode(u.i, cx.n_tiles, cx.C);
+__device__ __forceinline__ void prod_store(const Ctx& cx, const Cur& u, int pt, const float4 (&r)[CHUNKS], uint32_t n_run) {
+  const uint32_t n_item = u.it.n;
+  const Item& it = u.it;
   const DevOp& o = cx.ops[it.op];
   const int lane = pt & 31;
   if (u.sub == 0) {
@@ -297,10 +303,12 @@ __global__ void __launch_bounds__(THREADS, 1) k_post_tc5(const DevOp* __restrict
   {
     const long long total = (long long)n_ops * C * cx.n_tiles;
     const long long base = total / gridDim.x, rem = total % gridDim.x, b = blockIdx.x;
-    cx.i0 = b * base + (b < rem ? b : rem);
-    cx.i1 = cx.i0 + base + (b < rem ? 1 : 0);
+    const long long i0 = b * base + (b < rem ? b : rem);
+    cx.n_items = (uint32_t)(base + (b < rem ? 1 : 0));
+    const long long oc = i0 / cx.n_tiles;
+    cx.first_item = Item{(int)(oc / C), (int)(oc % C), (int)(i0 % cx.n_tiles), 0u};
   }
-  if (cx.i0 >= cx.i1) return;  // whole CTA leaves before any barrier or TMEM allocation
+  if (cx.n_items == 0) return;  // whole CTA leaves before any barrier or TMEM allocation
   cx.smem = (smem_u32(tc5_smem_raw) + 1023u) & ~1023u;
   cx.bar = cx.smem + OFF_BAR;
 
@@ -331,9 +339,8 @@ __global__ void __launch_bounds__(THREADS, 1) k_post_tc5(const DevOp* __restrict
   if (warp < EPI_WARPS) {
     // ===== epilogue =====
     const uint32_t stage = cx.smem + OFF_STAGE + warp * STAGE_WARP;
-    uint32_t n = 0;
-    for (long long i = cx.i0; i < cx.i1; ++i, ++n) {
-      const Item it = decode(i, cx.n_tiles, C);
+    for (Item it = cx.first_item; cx.valid(it); cx.advance(it)) {
+      const uint32_t n = it.n;
       const DevOp& o = ops[it.op];
       const int p0 = it.tile * TP, prow0 = p0 + 32 * warp, p = prow0 + lane;
       const Pow2Pair<float> f0 = pow2_pair(-pending_exp<float>(o.cscale[0], p, P, C), 0.f);
@@ -381,7 +388,7 @@ __global__ void __launch_bounds__(THREADS, 1) k_post_tc5(const DevOp* __restrict
     // ===== producers =====
     const int pt = threadIdx.x - EPI_WARPS * 32;
     if (pt == 0)
-      for (int d = 1; d < PREFETCH_AHEAD; ++d) prefetch_item(cx, cx.i0 + d);
+      for (int d = 1; d < PREFETCH_AHEAD; ++d) prefetch_item(cx, cx.first_item, d);
     float4 ra[CHUNKS], rb[CHUNKS];
     uint32_t n_run = 0;  // matrix runs stored so far
     Cur cur = cx.first(), nxt;
@@ -390,24 +397,24 @@ __global__ void __launch_bounds__(THREADS, 1) k_post_tc5(const DevOp* __restrict
       nxt = cx.next(cur);
       const bool hn = cx.valid(nxt);
       if (hn) prod_load(cx, nxt, pt, rb);
-      prod_store(cx, cur, pt, ra, (uint32_t)(cur.i - cx.i0), n_run);
+      prod_store(cx, cur, pt, ra, n_run);
       n_run += cur.sub == 0;
       if (!hn) break;
       cur = cx.next(nxt);
       const bool hc = cx.valid(cur);
       if (hc) prod_load(cx, cur, pt, ra);
-      prod_store(cx, nxt, pt, rb, (uint32_t)(nxt.i - cx.i0), n_run);
+      prod_store(cx, nxt, pt, rb, n_run);
       n_run += nxt.sub == 0;
       if (!hc) break;
     }
   } else {
     // ===== MMA issuer: lane 0 issues, the warp stays converged =====
-    uint32_t n = 0, n_run = 0;
-    for (long long i = cx.i0; i < cx.i1; ++i, ++n) {
+    uint32_t n_run = 0;
+    for (Item it = cx.first_item; cx.valid(it); cx.advance(it)) {
       if (lane == 0) {
-      const Item it = decode(i, cx.n_tiles, C);
+      const uint32_t n = it.n;
       const DevOp& o = ops[it.op];
-      if (cx.new_run(i)) {
+      if (cx.new_run(it)) {
         mbar_wait(cx.barrier(B_MFULL), n_run & 1);
         ++n_run;
       }
@@ -441,7 +448,9 @@ __global__ void __launch_bounds__(THREADS, 1) k_post_tc5(const DevOp* __restrict
         umma_commit(cx.barrier(B_EMPTY0 + k));
       }
       umma_commit(cx.barrier(B_TFULL0 + a));
-      if (i + 1 < cx.i1 && cx.new_run(i + 1)) umma_commit(cx.barrier(B_MEMPTY));
+      Item nx = it;
+      cx.advance(nx);
+      if (cx.valid(nx) && cx.new_run(nx)) umma_commit(cx.barrier(B_MEMPTY));
       }
       __syncwarp();
     }
