@@ -40,7 +40,8 @@ constexpr int TP = 128;                    // patterns per tile = MMA M
 constexpr int EPI_WARPS = 4, PROD_WARPS = 8, N_WARPS = EPI_WARPS + PROD_WARPS + 1;
 constexpr int THREADS = N_WARPS * 32;      // 416
 constexpr int PROD_THREADS = PROD_WARPS * 32;
-constexpr int CHUNKS = 8;                  // 16-byte chunks per producer thread and unit (2048 per unit)
+constexpr int GROUP_THREADS = PROD_THREADS / 2;  // one producer group per child
+constexpr int XCHUNKS = 16, MCHUNKS = 8;   // 16-byte chunks per producer thread: operand tile / matrix
 constexpr uint32_t X_PLANE = TP * 64 * 4;  // 32 768: one plane (hi or lo) of a tile
 constexpr uint32_t M_PLANE = 64 * 64 * 4;  // 16 384
 constexpr uint32_t OFF_X = 0;              // [child][hi, lo]
@@ -149,15 +150,6 @@ struct Item {
   uint32_t n;  // ordinal inside the CTA's range
 };
 
-// ---------------------------------------------------------------------------------------------------------------
-// producer side: one "unit" = 2048 16-byte chunks = 8 per producer thread: either the matrix pair of a new
-// (operation, category) run (sub = 0) or the tile of child sub - 1
-// ---------------------------------------------------------------------------------------------------------------
-struct Cur {
-  Item it;
-  int sub;
-};
-
 struct Ctx {
   const DevOp* ops;
   int P, S, C, n_tiles;
@@ -178,118 +170,94 @@ struct Ctx {
   __device__ __forceinline__ bool valid(const Item& it) const { return it.n < n_items; }
   // first item of the range or first tile of an (operation, category): the matrix pair changes
   __device__ __forceinline__ bool new_run(const Item& it) const { return it.n == 0 || it.tile == 0; }
-  __device__ __forceinline__ bool valid(const Cur& u) const { return valid(u.it); }
-  __device__ __forceinline__ Cur first() const { return Cur{first_item, 0}; }
-  __device__ __forceinline__ Cur next(const Cur& u) const {
-    if (u.sub < 2) return Cur{u.it, u.sub + 1};
-    Item t = u.it;
-    advance(t);
-    return Cur{t, (valid(t) && new_run(t)) ? 0 : 1};
-  }
   __device__ __forceinline__ uint32_t barrier(int slot) const { return bar + 8u * slot; }
 };
 
-__device__ __forceinline__ void prefetch_item(const Ctx& cx, Item it, int ahead) {
+// ---------------------------------------------------------------------------------------------------------------
+// producer side.  Producer group g (4 warps) owns child g: its operand tile (2048 16-byte chunks, 16 per thread) and
+// its transition matrix (1024 chunks, 8 per thread).  Thread gt of a group takes chunk gt % 16 of rows gt / 16 + 8 j,
+// so the swizzled shared-memory offset of its j-th chunk is off0 + 1024 j (row & 7 does not depend on j).
+// ---------------------------------------------------------------------------------------------------------------
+__device__ __forceinline__ void prefetch_child(const Ctx& cx, Item it, int ahead, int k) {
   for (int d = 0; d < ahead; ++d) cx.advance(it);
   if (!cx.valid(it)) return;
   const DevOp& o = cx.ops[it.op];
   const int p0 = it.tile * TP, n = cx.P - p0 < TP ? cx.P - p0 : TP;
-#pragma unroll
-  for (int k = 0; k < 2; ++k) {
-    if (o.kind[k] == KIND_PARTIALS)
-      l2_prefetch_bulk(static_cast<const float*>(o.child[k]) + ((size_t)it.c * cx.P + p0) * SP64, (uint32_t)n * 256u);
-    else if (o.kind[k] == KIND_BCAST)
-      l2_prefetch_bulk(static_cast<const float*>(o.child[k]) + (size_t)p0 * SP64, (uint32_t)n * 256u);
-  }
+  if (o.kind[k] == KIND_PARTIALS)
+    l2_prefetch_bulk(static_cast<const float*>(o.child[k]) + ((size_t)it.c * cx.P + p0) * SP64, (uint32_t)n * 256u);
+  else if (o.kind[k] == KIND_BCAST)
+    l2_prefetch_bulk(static_cast<const float*>(o.child[k]) + (size_t)p0 * SP64, (uint32_t)n * 256u);
 }
 
-// global -> registers.  pt = producer thread index 0..255
-__device__ __forceinline__ void prod_load(const Ctx& cx, const Cur& u, int pt, float4 (&r)[CHUNKS]) {
-  const Item& it = u.it;
+// global -> registers: the tile of child k of item `it` (partials), or its compact states (one per row, in r[j].x)
+__device__ __forceinline__ void prod_load(const Ctx& cx, const Item& it, int k, int gt, float4 (&r)[XCHUNKS]) {
   const DevOp& o = cx.ops[it.op];
-  if (u.sub == 0) {
-#pragma unroll
-    for (int j = 0; j < CHUNKS; ++j) {
-      const int idx = pt + PROD_THREADS * j, k = idx >> 10, rem = idx & 1023;
-      r[j] = ldg_nc(static_cast<const float*>(o.mat[k]) + (size_t)it.c * SP64 * SP64 + rem * 4);
-    }
-    return;
-  }
-  const int k = u.sub - 1, kind = o.kind[k];
+  const int kind = o.kind[k];
   const int p0 = it.tile * TP, n = cx.P - p0 < TP ? cx.P - p0 : TP;
-  if (k == 0 && pt == 0) prefetch_item(cx, it, PREFETCH_AHEAD);
+  const int row0 = gt >> 4;
+  if (gt == 0) prefetch_child(cx, it, PREFETCH_AHEAD, k);
   if (kind == KIND_PARTIALS || kind == KIND_BCAST) {
-    const float* src = static_cast<const float*>(o.child[k]) + ((kind == KIND_PARTIALS ? (size_t)it.c * cx.P : 0) + p0) * SP64;
+    const float* src = static_cast<const float*>(o.child[k]) + ((kind == KIND_PARTIALS ? (size_t)it.c * cx.P : 0) + p0) * SP64 + gt * 4;
 #pragma unroll
-    for (int j = 0; j < CHUNKS; ++j) {
-      const int idx = pt + PROD_THREADS * j, row = idx >> 4;
-      r[j] = row < n ? ldg_nc(src + (size_t)idx * 4) : make_float4(0.f, 0.f, 0.f, 0.f);
-    }
+    for (int j = 0; j < XCHUNKS; ++j)
+      r[j] = row0 + 8 * j < n ? ldg_nc(src + j * 512) : make_float4(0.f, 0.f, 0.f, 0.f);
   } else if (kind == KIND_STATES) {
-    const uint8_t* st = static_cast<const uint8_t*>(o.child[k]) + p0;
+    const uint8_t* st = static_cast<const uint8_t*>(o.child[k]) + p0 + row0;
 #pragma unroll
-    for (int j = 0; j < CHUNKS; ++j) {
-      const int row = (pt + PROD_THREADS * j) >> 4;
-      r[j].x = __int_as_float(row < n ? (int)st[row] : -1);
-    }
+    for (int j = 0; j < XCHUNKS; ++j) r[j].x = __int_as_float(row0 + 8 * j < n ? (int)st[8 * j] : -1);
   }
 }
 
-// registers -> shared memory (swizzled K-major planes), then signal the MMA thread
-__device__ __forceinline__ void prod_store(const Ctx& cx, const Cur& u, int pt, const float4 (&r)[CHUNKS], uint32_t n_run) {
-  const uint32_t n_item = u.it.n;
-  const Item& it = u.it;
-  const DevOp& o = cx.ops[it.op];
-  const int lane = pt & 31;
-  if (u.sub == 0) {
-    mbar_wait(cx.barrier(B_MEMPTY), (n_run & 1) ^ 1);
-#pragma unroll
-    for (int j = 0; j < CHUNKS; ++j) {
-      const int idx = pt + PROD_THREADS * j, k = idx >> 10, rem = idx & 1023;
-      const uint32_t off = swz_off(rem >> 4, rem & 15, 64);
-      float4 h, l;
-      split4(r[j], h, l);
-      sts128(cx.smem + OFF_M + (2 * k) * M_PLANE + off, h);
-      sts128(cx.smem + OFF_M + (2 * k + 1) * M_PLANE + off, l);
-    }
-    fence_async_smem();
-    __syncwarp();
-    if (lane == 0) mbar_arrive(cx.barrier(B_MFULL));
-    return;
-  }
-  const int k = u.sub - 1, kind = o.kind[k];
-  mbar_wait(cx.barrier(B_EMPTY0 + k), (n_item & 1) ^ 1);
-  const uint32_t xhi = cx.smem + OFF_X + (2 * k) * X_PLANE, xlo = xhi + X_PLANE;
+// registers -> shared memory (hi / lo planes, swizzled K-major), then signal the MMA thread
+__device__ __forceinline__ void prod_store(const Ctx& cx, const Item& it, int k, int gt, const float4 (&r)[XCHUNKS]) {
+  const int kind = cx.ops[it.op].kind[k];
+  const uint32_t xhi = cx.smem + OFF_X + (2 * k) * X_PLANE + swz_off(gt >> 4, gt & 15, TP), xlo = xhi + X_PLANE;
+  mbar_wait(cx.barrier(B_EMPTY0 + k), (it.n & 1) ^ 1);
   if (kind == KIND_PARTIALS || kind == KIND_BCAST) {
 #pragma unroll
-    for (int j = 0; j < CHUNKS; ++j) {
-      const int idx = pt + PROD_THREADS * j;
-      const uint32_t off = swz_off(idx >> 4, idx & 15, TP);
+    for (int j = 0; j < XCHUNKS; ++j) {
       float4 h, l;
       split4(r[j], h, l);
-      sts128(xhi + off, h);
-      sts128(xlo + off, l);
+      sts128(xhi + 1024 * j, h);
+      sts128(xlo + 1024 * j, l);
     }
   } else {
-    const int S = cx.S;
+    const int S = cx.S, x0 = (gt & 15) * 4;
 #pragma unroll
-    for (int j = 0; j < CHUNKS; ++j) {
-      const int idx = pt + PROD_THREADS * j, ch = idx & 15, x0 = ch * 4;
+    for (int j = 0; j < XCHUNKS; ++j) {
       const int z = kind == KIND_STATES ? __float_as_int(r[j].x) : -1;  // -1: row beyond the tile or operand absent
+      const bool miss = z >= S;  // missing state: every state possible (padding columns stay 0)
       float4 h;
-      if (z < 0) {
-        h = make_float4(0.f, 0.f, 0.f, 0.f);
-      } else if (z < S) {  // one-hot
-        h.x = x0 == z ? 1.f : 0.f; h.y = x0 + 1 == z ? 1.f : 0.f; h.z = x0 + 2 == z ? 1.f : 0.f; h.w = x0 + 3 == z ? 1.f : 0.f;
-      } else {  // missing: every state possible (padding columns stay 0)
-        h.x = x0 < S ? 1.f : 0.f; h.y = x0 + 1 < S ? 1.f : 0.f; h.z = x0 + 2 < S ? 1.f : 0.f; h.w = x0 + 3 < S ? 1.f : 0.f;
-      }
-      sts128(xhi + swz_off(idx >> 4, ch, TP), h);
+      h.x = (z == x0 || (miss && x0 < S)) ? 1.f : 0.f;
+      h.y = (z == x0 + 1 || (miss && x0 + 1 < S)) ? 1.f : 0.f;
+      h.z = (z == x0 + 2 || (miss && x0 + 2 < S)) ? 1.f : 0.f;
+      h.w = (z == x0 + 3 || (miss && x0 + 3 < S)) ? 1.f : 0.f;
+      sts128(xhi + 1024 * j, h);
     }
   }
   fence_async_smem();
   __syncwarp();
-  if (lane == 0) mbar_arrive(cx.barrier(B_FULL0 + k));
+  if ((gt & 31) == 0) mbar_arrive(cx.barrier(B_FULL0 + k));
+}
+
+__device__ __forceinline__ void prod_load_matrix(const Ctx& cx, const Item& it, int k, int gt, float4 (&m)[MCHUNKS]) {
+  const float* src = static_cast<const float*>(cx.ops[it.op].mat[k]) + (size_t)it.c * SP64 * SP64 + gt * 4;
+#pragma unroll
+  for (int j = 0; j < MCHUNKS; ++j) m[j] = ldg_nc(src + j * 512);
+}
+__device__ __forceinline__ void prod_store_matrix(const Ctx& cx, int k, int gt, const float4 (&m)[MCHUNKS], uint32_t n_run) {
+  const uint32_t mhi = cx.smem + OFF_M + (2 * k) * M_PLANE + swz_off(gt >> 4, gt & 15, 64), mlo = mhi + M_PLANE;
+  mbar_wait(cx.barrier(B_MEMPTY), (n_run & 1) ^ 1);
+#pragma unroll
+  for (int j = 0; j < MCHUNKS; ++j) {
+    float4 h, l;
+    split4(m[j], h, l);
+    sts128(mhi + 1024 * j, h);
+    sts128(mlo + 1024 * j, l);
+  }
+  fence_async_smem();
+  __syncwarp();
+  if ((gt & 31) == 0) mbar_arrive(cx.barrier(B_MFULL));
 }
 
 // ---------------------------------------------------------------------------------------------------------------
@@ -314,8 +282,8 @@ __global__ void __launch_bounds__(THREADS, 1) k_post_tc5(const DevOp* __restrict
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   if (threadIdx.x == 0) {
-    mbar_init(cx.barrier(B_FULL0), PROD_WARPS);
-    mbar_init(cx.barrier(B_FULL1), PROD_WARPS);
+    mbar_init(cx.barrier(B_FULL0), PROD_WARPS / 2);
+    mbar_init(cx.barrier(B_FULL1), PROD_WARPS / 2);
     mbar_init(cx.barrier(B_EMPTY0), 1);
     mbar_init(cx.barrier(B_EMPTY1), 1);
     mbar_init(cx.barrier(B_MFULL), PROD_WARPS);
@@ -345,6 +313,7 @@ __global__ void __launch_bounds__(THREADS, 1) k_post_tc5(const DevOp* __restrict
       const int p0 = it.tile * TP, prow0 = p0 + 32 * warp, p = prow0 + lane;
       const Pow2Pair<float> f0 = pow2_pair(-pending_exp<float>(o.cscale[0], p, P, C), 0.f);
       const Pow2Pair<float> f1 = pow2_pair(-pending_exp<float>(o.cscale[1], p, P, C), 0.f);
+      const bool one_factor = __all_sync(0xffffffffu, f0.f2 == 1.f && f1.f2 == 1.f);
       float* dest = static_cast<float*>(o.dest) + (size_t)it.c * P * SP64;
       float* scale = static_cast<float*>(o.scale);
       const uint32_t a = n & 1;
@@ -363,15 +332,28 @@ __global__ void __launch_bounds__(THREADS, 1) k_post_tc5(const DevOp* __restrict
           __syncwarp();
           if (lane == 0) mbar_arrive(cx.barrier(B_TEMPTY0 + a));
         }
+        if (one_factor) {  // the usual case: each pending exponent fits one power-of-two factor
 #pragma unroll
-        for (int q = 0; q < 8; ++q) {
-          float v[4];
+          for (int q = 0; q < 8; ++q) {
+            float v[4];
 #pragma unroll
-          for (int j = 0; j < 4; ++j) {
-            v[j] = ((__uint_as_float(d0[4 * q + j]) * f0.f1) * f0.f2) * ((__uint_as_float(d1[4 * q + j]) * f1.f1) * f1.f2);
-            mx = fmaxf(mx, v[j]);
+            for (int j = 0; j < 4; ++j) {
+              v[j] = (__uint_as_float(d0[4 * q + j]) * f0.f1) * (__uint_as_float(d1[4 * q + j]) * f1.f1);
+              mx = fmaxf(mx, v[j]);
+            }
+            sts128(stage + lane * STAGE_LD + q * 16, make_float4(v[0], v[1], v[2], v[3]));
           }
-          sts128(stage + lane * STAGE_LD + q * 16, make_float4(v[0], v[1], v[2], v[3]));
+        } else {
+#pragma unroll
+          for (int q = 0; q < 8; ++q) {
+            float v[4];
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+              v[j] = ((__uint_as_float(d0[4 * q + j]) * f0.f1) * f0.f2) * ((__uint_as_float(d1[4 * q + j]) * f1.f1) * f1.f2);
+              mx = fmaxf(mx, v[j]);
+            }
+            sts128(stage + lane * STAGE_LD + q * 16, make_float4(v[0], v[1], v[2], v[3]));
+          }
         }
         __syncwarp();
 #pragma unroll
@@ -385,27 +367,27 @@ __global__ void __launch_bounds__(THREADS, 1) k_post_tc5(const DevOp* __restrict
       if (p < P && scale != nullptr) scale[(size_t)it.c * P + p] = mx;
     }
   } else if (warp < EPI_WARPS + PROD_WARPS) {
-    // ===== producers =====
-    const int pt = threadIdx.x - EPI_WARPS * 32;
-    if (pt == 0)
-      for (int d = 1; d < PREFETCH_AHEAD; ++d) prefetch_item(cx, cx.first_item, d);
-    float4 ra[CHUNKS], rb[CHUNKS];
-    uint32_t n_run = 0;  // matrix runs stored so far
-    Cur cur = cx.first(), nxt;
-    prod_load(cx, cur, pt, ra);
+    // ===== producers: group g = child g =====
+    const int pt = threadIdx.x - EPI_WARPS * 32, g = pt >> 7, gt = pt & 127;
+    if (gt == 0)
+      for (int d = 0; d < PREFETCH_AHEAD; ++d) prefetch_child(cx, cx.first_item, d, g);
+    float4 r[XCHUNKS];
+    uint32_t n_run = 0;
+    Item it = cx.first_item;
+    prod_load(cx, it, g, gt, r);
+#pragma unroll 1
     while (true) {
-      nxt = cx.next(cur);
-      const bool hn = cx.valid(nxt);
-      if (hn) prod_load(cx, nxt, pt, rb);
-      prod_store(cx, cur, pt, ra, n_run);
-      n_run += cur.sub == 0;
-      if (!hn) break;
-      cur = cx.next(nxt);
-      const bool hc = cx.valid(cur);
-      if (hc) prod_load(cx, cur, pt, ra);
-      prod_store(cx, nxt, pt, rb, n_run);
-      n_run += nxt.sub == 0;
-      if (!hc) break;
+      const bool nr = cx.new_run(it);
+      float4 m[MCHUNKS];
+      if (nr) prod_load_matrix(cx, it, g, gt, m);
+      prod_store(cx, it, g, gt, r);
+      if (nr) {
+        prod_store_matrix(cx, g, gt, m, n_run);
+        ++n_run;
+      }
+      cx.advance(it);
+      if (!cx.valid(it)) break;
+      prod_load(cx, it, g, gt, r);
     }
   } else {
     // ===== MMA issuer: lane 0 issues, the warp stays converged =====
