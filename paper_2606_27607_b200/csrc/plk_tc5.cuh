@@ -86,13 +86,32 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
 __device__ __forceinline__ void fence_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 __device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
 __device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
+// COLL: 0 = A read from shared memory and dropped, 1 = A read and kept in the collector buffer (fill),
+//       2 = A taken from the collector buffer filled by the previous MMA (lastuse): the same A k-slice feeds
+//       x_hi . m_lo and x_hi . m_hi, so it crosses the shared-memory port once
+template <int COLL>
 __device__ __forceinline__ void umma_tf32(uint32_t d_tmem, uint64_t a_desc, uint64_t b_desc, uint32_t accumulate) {
-  asm volatile(
-      "{\n\t.reg .pred p;\n\t"
-      "setp.ne.b32 p, %4, 0;\n\t"
-      "tcgen05.mma.cta_group::1.kind::tf32 [%0], %1, %2, %3, p;\n\t}" ::"r"(d_tmem),
-      "l"(a_desc), "l"(b_desc), "r"(IDESC), "r"(accumulate)
-      : "memory");
+  if (COLL == 1)
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "setp.ne.b32 p, %4, 0;\n\t"
+        "tcgen05.mma.cta_group::1.kind::tf32.collector::a::fill [%0], %1, %2, %3, p;\n\t}" ::"r"(d_tmem),
+        "l"(a_desc), "l"(b_desc), "r"(IDESC), "r"(accumulate)
+        : "memory");
+  else if (COLL == 2)
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "setp.ne.b32 p, %4, 0;\n\t"
+        "tcgen05.mma.cta_group::1.kind::tf32.collector::a::lastuse [%0], %1, %2, %3, p;\n\t}" ::"r"(d_tmem),
+        "l"(a_desc), "l"(b_desc), "r"(IDESC), "r"(accumulate)
+        : "memory");
+  else
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "setp.ne.b32 p, %4, 0;\n\t"
+        "tcgen05.mma.cta_group::1.kind::tf32 [%0], %1, %2, %3, p;\n\t}" ::"r"(d_tmem),
+        "l"(a_desc), "l"(b_desc), "r"(IDESC), "r"(accumulate)
+        : "memory");
 }
 __device__ __forceinline__ void umma_commit(uint32_t bar) {
   asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(bar) : "memory");
@@ -143,6 +162,9 @@ __device__ __forceinline__ float4 lds128(uint32_t addr) {
 __device__ __forceinline__ uint32_t swz_off(int row, int ch, uint32_t rows) {
   return (uint32_t)(ch >> 3) * rows * 128u + (uint32_t)row * 128u + (uint32_t)(((ch & 7) ^ (row & 7)) << 4);
 }
+
+// descriptor offset (16-byte units) of k-step ks inside a swizzled plane of `rows` rows
+__host__ __device__ constexpr uint64_t koff(int ks, int rows) { return (uint64_t)(((ks >> 2) * rows * 128 + (ks & 3) * 32) >> 4); }
 
 // work items (operation, category, tile), tile fastest; each role walks its CTA's contiguous range incrementally
 struct Item {
@@ -392,6 +414,8 @@ __global__ void __launch_bounds__(THREADS, 1) k_post_tc5(const DevOp* __restrict
   } else {
     // ===== MMA issuer: lane 0 issues, the warp stays converged =====
     uint32_t n_run = 0;
+    const uint64_t dX[2] = {make_desc(cx.smem + OFF_X), make_desc(cx.smem + OFF_X + 2 * X_PLANE)};
+    const uint64_t dM[2] = {make_desc(cx.smem + OFF_M), make_desc(cx.smem + OFF_M + 2 * M_PLANE)};
     for (Item it = cx.first_item; cx.valid(it); cx.advance(it)) {
       if (lane == 0) {
       const uint32_t n = it.n;
@@ -407,26 +431,23 @@ __global__ void __launch_bounds__(THREADS, 1) k_post_tc5(const DevOp* __restrict
         mbar_wait(cx.barrier(B_FULL0 + k), n & 1);
         tc_fence_after();
         const uint32_t d = tmem_base + a * 128 + k * 64;
-        const uint32_t xhi = cx.smem + OFF_X + (2 * k) * X_PLANE, xlo = xhi + X_PLANE;
-        const uint32_t mhi = cx.smem + OFF_M + (2 * k) * M_PLANE, mlo = mhi + M_PLANE;
+        // descriptors differ from the plane's base descriptor only in the 16-byte-unit address field
+        const uint64_t dxhi = dX[k], dxlo = dX[k] + (X_PLANE >> 4), dmhi = dM[k], dmlo = dM[k] + (M_PLANE >> 4);
         const bool has_lo = o.kind[k] == KIND_PARTIALS || o.kind[k] == KIND_BCAST;
         uint32_t acc = 0;
-        // small terms first, hi.hi last (same order as the mma.sync path)
-        if (has_lo) {
+        if (has_lo) {  // x_lo . m_hi
 #pragma unroll
           for (int ks = 0; ks < 8; ++ks) {
-            umma_tf32(d, make_desc(xlo + (ks >> 2) * (TP * 128) + (ks & 3) * 32), make_desc(mhi + (ks >> 2) * (64 * 128) + (ks & 3) * 32), acc);
+            umma_tf32<0>(d, dxlo + koff(ks, TP), dmhi + koff(ks, 64), acc);
             acc = 1;
           }
         }
 #pragma unroll
-        for (int ks = 0; ks < 8; ++ks) {
-          umma_tf32(d, make_desc(xhi + (ks >> 2) * (TP * 128) + (ks & 3) * 32), make_desc(mlo + (ks >> 2) * (64 * 128) + (ks & 3) * 32), acc);
+        for (int ks = 0; ks < 8; ++ks) {  // x_hi . m_lo + x_hi . m_hi, the A slice fetched once
+          umma_tf32<1>(d, dxhi + koff(ks, TP), dmlo + koff(ks, 64), acc);
+          umma_tf32<2>(d, dxhi + koff(ks, TP), dmhi + koff(ks, 64), 1);
           acc = 1;
         }
-#pragma unroll
-        for (int ks = 0; ks < 8; ++ks)
-          umma_tf32(d, make_desc(xhi + (ks >> 2) * (TP * 128) + (ks & 3) * 32), make_desc(mhi + (ks >> 2) * (64 * 128) + (ks & 3) * 32), 1);
         umma_commit(cx.barrier(B_EMPTY0 + k));
       }
       umma_commit(cx.barrier(B_TFULL0 + a));

@@ -381,9 +381,11 @@ def config(index: int, n_tips: Optional[int] = None, n_patterns: Optional[int] =
         return make_workload("cfg1_gtr_128x100000", "GTR", n_tips or 128, n_patterns or 100_000, "yule", seed,
                              n_cat=n_categories, ambiguity=0.05)
     if index == 2:
-        return make_workload("cfg2_gy94_32x10000", "GY94", n_tips or 32, n_patterns or 10_000, "coalescent", seed)
+        return make_workload("cfg2_gy94_32x10000", "GY94", n_tips or 32, n_patterns or 10_000, "coalescent", seed,
+                             n_cat=n_categories)
     if index == 3:
-        return make_workload("cfg3_gy94_256x20000", "GY94", n_tips or 256, n_patterns or 20_000, "coalescent", seed)
+        return make_workload("cfg3_gy94_256x20000", "GY94", n_tips or 256, n_patterns or 20_000, "coalescent", seed,
+                             n_cat=n_categories)
     if index == 4:
         n = n_tips or 512
         p = n_patterns or 500_000

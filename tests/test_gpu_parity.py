@@ -141,9 +141,34 @@ def test_config2_tensor_cores_tip_partials(precision):
               tips_as_partials=True)
 
 
-def test_config3_reduced_tensor_cores():
-    """configs[3] shape (GY94, 256 taxa, 510 branches, level-batched) at 150 patterns, fp32 tensor path."""
-    _run_case(workloads.config(3, n_patterns=150), plk.FP32, flags=plk.FLAG_TENSOR_CORES)
+@pytest.mark.parametrize("arm", [0, plk.FLAG_NO_TCGEN05], ids=["tcgen05", "mma_sync"])
+def test_config3_reduced_tensor_cores(arm):
+    """configs[3] shape (GY94, 256 taxa, 510 branches, level-batched) at 150 patterns, fp32 tensor path: post-order on
+    tcgen05 / TMEM (default) and on the legacy mma.sync arm."""
+    _run_case(workloads.config(3, n_patterns=150), plk.FP32, flags=plk.FLAG_TENSOR_CORES | arm)
+
+
+@pytest.mark.parametrize("n_pat", [500, 129])
+def test_config2_fp32_mma_sync_arm(n_pat):
+    """The comparison arm PLK_FLAG_NO_TCGEN05 (split-TF32 m16n8k8 post-order) stays parity-green."""
+    _run_case(workloads.config(2, n_patterns=n_pat), plk.FP32, flags=plk.FLAG_TENSOR_CORES | plk.FLAG_NO_TCGEN05)
+
+
+@pytest.mark.parametrize("n_cat,n_pat", [(1, 257), (2, 128), (3, 300), (5, 77), (8, 1000)])
+def test_tcgen05_category_counts_and_tiles(n_cat, n_pat):
+    """tcgen05 post-order kernel: category counts other than 4 (the pending-exponent fetch handles C > 4 separately),
+    exactly one / two tiles, ragged tails, more work items than CTAs (8 categories x 8 tiles x 31 operations)."""
+    _run_case(workloads.config(2, n_patterns=n_pat, n_categories=n_cat), plk.FP32, flags=plk.FLAG_TENSOR_CORES)
+
+
+def test_tcgen05_missing_states_and_deep_tree():
+    """One-hot / all-ones tip rows on the tensor pipe (10 % missing cells) and a 200-taxon caterpillar-like depth
+    where the deferred power-of-two rescaling is necessary in fp32."""
+    wl = workloads.config(2, n_tips=20, n_patterns=200)
+    rng = np.random.default_rng(7)
+    wl.tip_states[rng.random(wl.tip_states.shape) < 0.1] = wl.n_states
+    _run_case(wl, plk.FP32, flags=plk.FLAG_TENSOR_CORES)
+    _run_case(workloads.config(3, n_tips=200, n_patterns=140), plk.FP32, flags=plk.FLAG_TENSOR_CORES)
 
 
 def test_config3_reduced_cuda_cores():
