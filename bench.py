@@ -259,6 +259,8 @@ def workload_config(wl, precision, flags, extra=None):
     cfg = {"workload": wl.name, "taxa": wl.tree.n_tips, "patterns": wl.n_patterns, "states": wl.n_states,
            "categories": wl.n_categories, "branches": 2 * wl.tree.n_tips - 2, "precision": precision,
            "codon_path": ("tensor" if flags & 1 else "cuda-core") if wl.n_states != 4 else None,
+           "codon_fp32_post_order": (("mma.sync" if flags & 64 else "tcgen05") if (flags & 1 and precision == "fp32"
+                                                                                   and wl.n_states != 4) else None),
            "substitution_model": wl.model["name"], "seed": wl.seed,
            "launch_shape": {8: "level", 16: "walk"}.get(flags & 24, "auto") if wl.n_states == 4 else "level",
            "staging": ("ldg" if flags & 32 else "tma") if wl.n_states == 4 else None,
@@ -306,7 +308,8 @@ def run_extras(peaks, steps, warmup):
             ("cfg2_fp64_cuda", 2, None, None, "fp64", 0), ("cfg2_fp32_cuda", 2, None, None, "fp32", 0)]
     if have_tc:
         plan += [("cfg2_fp64_tensor", 2, None, None, "fp64", 1), ("cfg2_fp32_tensor", 2, None, None, "fp32", 1),
-                 ("cfg3_fp32_tensor", 3, None, None, "fp32", 1)]
+                 ("cfg3_fp32_tensor", 3, None, None, "fp32", 1),
+                 ("cfg3_fp32_tensor_mma_sync_post", 3, None, None, "fp32", 1 | 64)]
     else:
         plan += [("cfg3_fp32_cuda", 3, None, None, "fp32", 0)]
     plan += [("cfg4_hky_fp32_512x100000", 4, 512, 100_000, "fp32", 0), ("cfg4_hky_fp32_8x100", 4, 8, 100, "fp32", 0)]
@@ -430,7 +433,8 @@ def main():
     dom = "pre_order_gradient" if ph["pre_order_gradient"] >= ph["post_order"] else "post_order"
     lean = nuc and wl.n_categories == 4 and args.staging == "tma" and args.shape != "walk"
     kname = {"post_order": ("k_post4_walk" if args.shape != "level" else "k_post4_tma") if nuc
-             else ("k_post_tc" if args.tensor else "k_post64"),
+             else (("k_post_tc5" if args.precision == "fp32" and args.codon_fp32 == "tcgen05" else "k_post_tc")
+                   if args.tensor else "k_post64"),
              "pre_order_gradient": ("k_pre4_lean" if lean else "k_pre4_tma/k_pre4/k_pre4_walk") if nuc
              else ("k_pre_tc" if args.tensor else "k_pre64")}[dom]
     n_levels_note = "all launches of the kernel in one step (one per dependency level and item class)"

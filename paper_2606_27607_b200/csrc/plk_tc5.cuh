@@ -86,6 +86,8 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
 __device__ __forceinline__ void fence_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 __device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
 __device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
+// Called by ALL lanes of the (converged) issuing warp: the instruction itself is predicated on elect.sync, so the
+// descriptor arithmetic around it stays on the uniform datapath instead of a divergent branch.
 // COLL: 0 = A read from shared memory and dropped, 1 = A read and kept in the collector buffer (fill),
 //       2 = A taken from the collector buffer filled by the previous MMA (lastuse): the same A k-slice feeds
 //       x_hi . m_lo and x_hi . m_hi, so it crosses the shared-memory port once
@@ -93,28 +95,35 @@ template <int COLL>
 __device__ __forceinline__ void umma_tf32(uint32_t d_tmem, uint64_t a_desc, uint64_t b_desc, uint32_t accumulate) {
   if (COLL == 1)
     asm volatile(
-        "{\n\t.reg .pred p;\n\t"
+        "{\n\t.reg .pred p, e;\n\t"
+        "elect.sync _|e, 0xffffffff;\n\t"
         "setp.ne.b32 p, %4, 0;\n\t"
-        "tcgen05.mma.cta_group::1.kind::tf32.collector::a::fill [%0], %1, %2, %3, p;\n\t}" ::"r"(d_tmem),
+        "@e tcgen05.mma.cta_group::1.kind::tf32.collector::a::fill [%0], %1, %2, %3, p;\n\t}" ::"r"(d_tmem),
         "l"(a_desc), "l"(b_desc), "r"(IDESC), "r"(accumulate)
         : "memory");
   else if (COLL == 2)
     asm volatile(
-        "{\n\t.reg .pred p;\n\t"
+        "{\n\t.reg .pred p, e;\n\t"
+        "elect.sync _|e, 0xffffffff;\n\t"
         "setp.ne.b32 p, %4, 0;\n\t"
-        "tcgen05.mma.cta_group::1.kind::tf32.collector::a::lastuse [%0], %1, %2, %3, p;\n\t}" ::"r"(d_tmem),
+        "@e tcgen05.mma.cta_group::1.kind::tf32.collector::a::lastuse [%0], %1, %2, %3, p;\n\t}" ::"r"(d_tmem),
         "l"(a_desc), "l"(b_desc), "r"(IDESC), "r"(accumulate)
         : "memory");
   else
     asm volatile(
-        "{\n\t.reg .pred p;\n\t"
+        "{\n\t.reg .pred p, e;\n\t"
+        "elect.sync _|e, 0xffffffff;\n\t"
         "setp.ne.b32 p, %4, 0;\n\t"
-        "tcgen05.mma.cta_group::1.kind::tf32 [%0], %1, %2, %3, p;\n\t}" ::"r"(d_tmem),
+        "@e tcgen05.mma.cta_group::1.kind::tf32 [%0], %1, %2, %3, p;\n\t}" ::"r"(d_tmem),
         "l"(a_desc), "l"(b_desc), "r"(IDESC), "r"(accumulate)
         : "memory");
 }
 __device__ __forceinline__ void umma_commit(uint32_t bar) {
-  asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(bar) : "memory");
+  asm volatile(
+      "{\n\t.reg .pred e;\n\t"
+      "elect.sync _|e, 0xffffffff;\n\t"
+      "@e tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];\n\t}" ::"r"(bar)
+      : "memory");
 }
 __device__ __forceinline__ void tmem_ld32(uint32_t taddr, uint32_t (&v)[32]) {
   asm volatile(
@@ -302,7 +311,9 @@ __global__ void __launch_bounds__(THREADS, 1) k_post_tc5(const DevOp* __restrict
   cx.smem = (smem_u32(tc5_smem_raw) + 1023u) & ~1023u;
   cx.bar = cx.smem + OFF_BAR;
 
-  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  // warp index through a shuffle: the compiler then knows it is warp-uniform and keeps the role branches (and the
+  // descriptor arithmetic inside them) on the uniform datapath
+  const int warp = __shfl_sync(0xffffffffu, (int)(threadIdx.x >> 5), 0), lane = threadIdx.x & 31;
   if (threadIdx.x == 0) {
     mbar_init(cx.barrier(B_FULL0), PROD_WARPS / 2);
     mbar_init(cx.barrier(B_FULL1), PROD_WARPS / 2);
@@ -412,12 +423,11 @@ __global__ void __launch_bounds__(THREADS, 1) k_post_tc5(const DevOp* __restrict
       prod_load(cx, it, g, gt, r);
     }
   } else {
-    // ===== MMA issuer: lane 0 issues, the warp stays converged =====
+    // ===== MMA issuer: the whole warp runs the loop, one elected lane executes each tcgen05.mma / commit =====
     uint32_t n_run = 0;
     const uint64_t dX[2] = {make_desc(cx.smem + OFF_X), make_desc(cx.smem + OFF_X + 2 * X_PLANE)};
     const uint64_t dM[2] = {make_desc(cx.smem + OFF_M), make_desc(cx.smem + OFF_M + 2 * M_PLANE)};
     for (Item it = cx.first_item; cx.valid(it); cx.advance(it)) {
-      if (lane == 0) {
       const uint32_t n = it.n;
       const DevOp& o = ops[it.op];
       if (cx.new_run(it)) {
@@ -454,8 +464,6 @@ __global__ void __launch_bounds__(THREADS, 1) k_post_tc5(const DevOp* __restrict
       Item nx = it;
       cx.advance(nx);
       if (cx.valid(nx) && cx.new_run(nx)) umma_commit(cx.barrier(B_MEMPTY));
-      }
-      __syncwarp();
     }
   }
   tc_fence_before();
