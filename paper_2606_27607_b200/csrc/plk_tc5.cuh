@@ -36,6 +36,12 @@
 namespace plk {
 namespace tc5 {
 
+// PLK_TC5_EXP: ablation builds for bottleneck hunting (results are WRONG): 1 = epilogue without staging / global
+// stores, 2 = producers write nothing, 3 = one MMA per child, 4 = no pending-maxima loads in the epilogue
+#ifndef PLK_TC5_EXP
+#define PLK_TC5_EXP 0
+#endif
+
 constexpr int TP = 128;                    // patterns per tile = MMA M
 constexpr int EPI_WARPS = 4, PROD_WARPS = 8, N_WARPS = EPI_WARPS + PROD_WARPS + 1;
 constexpr int THREADS = N_WARPS * 32;      // 416
@@ -244,7 +250,8 @@ __device__ __forceinline__ void prod_store(const Ctx& cx, const Item& it, int k,
   const int kind = cx.ops[it.op].kind[k];
   const uint32_t xhi = cx.smem + OFF_X + (2 * k) * X_PLANE + swz_off(gt >> 4, gt & 15, TP), xlo = xhi + X_PLANE;
   mbar_wait(cx.barrier(B_EMPTY0 + k), (it.n & 1) ^ 1);
-  if (kind == KIND_PARTIALS || kind == KIND_BCAST) {
+  if (PLK_TC5_EXP == 2) {
+  } else if (kind == KIND_PARTIALS || kind == KIND_BCAST) {
 #pragma unroll
     for (int j = 0; j < XCHUNKS; ++j) {
       float4 h, l;
@@ -344,8 +351,8 @@ __global__ void __launch_bounds__(THREADS, 1) k_post_tc5(const DevOp* __restrict
       const uint32_t n = it.n;
       const DevOp& o = ops[it.op];
       const int p0 = it.tile * TP, prow0 = p0 + 32 * warp, p = prow0 + lane;
-      const Pow2Pair<float> f0 = pow2_pair(-pending_exp<float>(o.cscale[0], p, P, C), 0.f);
-      const Pow2Pair<float> f1 = pow2_pair(-pending_exp<float>(o.cscale[1], p, P, C), 0.f);
+      const Pow2Pair<float> f0 = pow2_pair(PLK_TC5_EXP == 4 ? 0 : -pending_exp<float>(o.cscale[0], p, P, C), 0.f);
+      const Pow2Pair<float> f1 = pow2_pair(PLK_TC5_EXP == 4 ? 0 : -pending_exp<float>(o.cscale[1], p, P, C), 0.f);
       const bool one_factor = __all_sync(0xffffffffu, f0.f2 == 1.f && f1.f2 == 1.f);
       float* dest = static_cast<float*>(o.dest) + (size_t)it.c * P * SP64;
       float* scale = static_cast<float*>(o.scale);
@@ -365,6 +372,7 @@ __global__ void __launch_bounds__(THREADS, 1) k_post_tc5(const DevOp* __restrict
           __syncwarp();
           if (lane == 0) mbar_arrive(cx.barrier(B_TEMPTY0 + a));
         }
+        if (PLK_TC5_EXP == 1) continue;
         if (one_factor) {  // the usual case: each pending exponent fits one power-of-two factor
 #pragma unroll
           for (int q = 0; q < 8; ++q) {
@@ -447,15 +455,15 @@ __global__ void __launch_bounds__(THREADS, 1) k_post_tc5(const DevOp* __restrict
         uint32_t acc = 0;
         if (has_lo) {  // x_lo . m_hi
 #pragma unroll
-          for (int ks = 0; ks < 8; ++ks) {
+          for (int ks = 0; ks < (PLK_TC5_EXP == 3 ? 0 : 8); ++ks) {
             umma_tf32<0>(d, dxlo + koff(ks, TP), dmhi + koff(ks, 64), acc);
             acc = 1;
           }
         }
 #pragma unroll
-        for (int ks = 0; ks < 8; ++ks) {  // x_hi . m_lo + x_hi . m_hi, the A slice fetched once
+        for (int ks = 0; ks < (PLK_TC5_EXP == 3 ? 1 : 8); ++ks) {  // x_hi . m_lo + x_hi . m_hi, the A slice fetched once
           umma_tf32<1>(d, dxhi + koff(ks, TP), dmlo + koff(ks, 64), acc);
-          umma_tf32<2>(d, dxhi + koff(ks, TP), dmhi + koff(ks, 64), 1);
+          if (PLK_TC5_EXP != 3) umma_tf32<2>(d, dxhi + koff(ks, TP), dmhi + koff(ks, 64), 1);
           acc = 1;
         }
         umma_commit(cx.barrier(B_EMPTY0 + k));
