@@ -19,13 +19,14 @@
 // into shared memory, so a tip costs no HBM read and its "gather" M[s][z] = hi + lo is exact on the tensor pipe
 // (its lo.hi product is skipped: lo = 0).
 //
-// Roles (warp-specialised, one persistent CTA per SM, 13 warps):
-//   warps 0-3   epilogue: tcgen05.ld (32 lanes x 32 columns), factors, product, row maximum, transposition through a
-//               small padded shared-memory stage so that global stores are full 128-byte segments
-//   warps 4-11  producers: ld.global (16-byte chunks, register-staged) -> hi/lo split -> st.shared in the swizzled
+// Roles (warp-specialised, one persistent CTA per SM, 17 warps):
+//   warps 0-7   epilogue: warp 4h + q takes patterns 32q..32q+31 x states 32h..32h+31: tcgen05.ld (32 lanes x 32
+//               columns), factors, product, row maximum, transposition through a small swizzled shared-memory stage
+//               so that global stores are full 128-byte segments; pending maxima fetched one item ahead
+//   warps 8-15  producers (group g = warps 8+4g .. 11+4g owns child g): ld.global (16-byte chunks, register-staged) -> hi/lo split -> st.shared in the swizzled
 //               layout -> fence.proxy.async -> mbarrier arrive; HBM -> L2 streaming runs ahead of them through
 //               cp.async.bulk.prefetch.L2 of the (contiguous, 32 KB) tiles two items ahead
-//   warp 12     TMEM allocation; one lane issues the MMAs and the tcgen05.commit that free the shared-memory stage,
+//   warp 16     TMEM allocation; one lane issues the MMAs and the tcgen05.commit that free the shared-memory stage,
 //               publish the accumulators and release the matrices
 // Pipelines: shared-memory stage per child (full/empty), two TMEM accumulator sets (full/empty), matrices
 // (full/empty; reloaded only when (operation, category) changes: items are dealt tile-fastest in contiguous ranges).
@@ -43,8 +44,8 @@ namespace tc5 {
 #endif
 
 constexpr int TP = 128;                    // patterns per tile = MMA M
-constexpr int EPI_WARPS = 4, PROD_WARPS = 8, N_WARPS = EPI_WARPS + PROD_WARPS + 1;
-constexpr int THREADS = N_WARPS * 32;      // 416
+constexpr int EPI_WARPS = 8, PROD_WARPS = 8, N_WARPS = EPI_WARPS + PROD_WARPS + 1;
+constexpr int THREADS = N_WARPS * 32;      // 544
 constexpr int PROD_THREADS = PROD_WARPS * 32;
 constexpr int GROUP_THREADS = PROD_THREADS / 2;  // one producer group per child
 constexpr int XCHUNKS = 16, MCHUNKS = 8;   // 16-byte chunks per producer thread: operand tile / matrix
@@ -53,9 +54,9 @@ constexpr uint32_t M_PLANE = 64 * 64 * 4;  // 16 384
 constexpr uint32_t OFF_X = 0;              // [child][hi, lo]
 constexpr uint32_t OFF_M = 4 * X_PLANE;    // [child][hi, lo]
 constexpr uint32_t OFF_STAGE = OFF_M + 4 * M_PLANE;
-constexpr uint32_t STAGE_LD = 144;         // bytes per staged half row (128 + 16: conflict-free 16-byte accesses)
-constexpr uint32_t STAGE_WARP = 32 * STAGE_LD;
-constexpr uint32_t OFF_BAR = OFF_STAGE + EPI_WARPS * STAGE_WARP;
+constexpr uint32_t STAGE_WARP = 32 * 128;  // per epilogue warp: 32 rows x 32 columns, 16-byte chunks XOR-swizzled by row
+constexpr uint32_t OFF_MAX = OFF_STAGE + EPI_WARPS * STAGE_WARP;  // [2][TP] row maxima of the upper column half
+constexpr uint32_t OFF_BAR = OFF_MAX + 2 * TP * 4;
 constexpr uint32_t SMEM_USED = OFF_BAR + 128;
 constexpr size_t SMEM_BYTES = SMEM_USED + 1024;  // + slack for the 1024-byte alignment the swizzle needs
 constexpr int PREFETCH_AHEAD = 2;          // items
@@ -167,6 +168,12 @@ __device__ __forceinline__ void split4(const float4 v, float4& h, float4& l) {
 }
 __device__ __forceinline__ void sts128(uint32_t addr, const float4 v) {
   asm volatile("st.shared.v4.f32 [%0], {%1,%2,%3,%4};" ::"r"(addr), "f"(v.x), "f"(v.y), "f"(v.z), "f"(v.w) : "memory");
+}
+__device__ __forceinline__ void sts32(uint32_t addr, float v) { asm volatile("st.shared.f32 [%0], %1;" ::"r"(addr), "f"(v) : "memory"); }
+__device__ __forceinline__ float lds32(uint32_t addr) {
+  float v;
+  asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v) : "r"(addr) : "memory");
+  return v;
 }
 __device__ __forceinline__ float4 lds128(uint32_t addr) {
   float4 v;
@@ -345,67 +352,104 @@ __global__ void __launch_bounds__(THREADS, 1) k_post_tc5(const DevOp* __restrict
   asm volatile("ld.shared.b32 %0, [%1];" : "=r"(tmem_base) : "r"(cx.barrier(B_TMEM_PTR)) : "memory");
 
   if (warp < EPI_WARPS) {
-    // ===== epilogue =====
+    // ===== epilogue: warp = 4 half + quarter takes patterns 32 quarter .. +31 (TMEM lanes) x states 32 half .. +31 =====
+    const int quarter = warp & 3, half = warp >> 2;
     const uint32_t stage = cx.smem + OFF_STAGE + warp * STAGE_WARP;
-    for (Item it = cx.first_item; cx.valid(it); cx.advance(it)) {
+    // Pending maxima of both children (deferred rescaling) are fetched ONE ITEM AHEAD: the raw loads are issued before
+    // the current item is processed and reduced to exponents after it, so their latency is off the critical path.
+    float raw[2][4];
+    auto load_raw = [&](const Item& t) {
+      const DevOp& o = ops[t.op];
+      const int p = t.tile * TP + 32 * quarter + lane;
+#pragma unroll
+      for (int k = 0; k < 2; ++k) {
+        const float* m = static_cast<const float*>(o.cscale[k]);
+#pragma unroll
+        for (int c = 0; c < 4; ++c)
+          raw[k][c] = (PLK_TC5_EXP != 4 && m != nullptr && p < P && c < C) ? __ldg(m + (size_t)c * P + p) : 0.f;
+      }
+    };
+    auto finish_raw = [&](const Item& t, int k) {
+      float v = fmaxf(fmaxf(raw[k][0], raw[k][1]), fmaxf(raw[k][2], raw[k][3]));
+      if (C > 4) {
+        const float* m = static_cast<const float*>(ops[t.op].cscale[k]);
+        const int p = t.tile * TP + 32 * quarter + lane;
+        if (m != nullptr && p < P)
+          for (int c = 4; c < C; ++c) v = fmaxf(v, m[(size_t)c * P + p]);
+      }
+      return pow2_pair(-exp_of(v), 0.f);
+    };
+    load_raw(cx.first_item);
+    Pow2Pair<float> f0 = finish_raw(cx.first_item, 0), f1 = finish_raw(cx.first_item, 1);
+    for (Item it = cx.first_item; cx.valid(it);) {
       const uint32_t n = it.n;
       const DevOp& o = ops[it.op];
-      const int p0 = it.tile * TP, prow0 = p0 + 32 * warp, p = prow0 + lane;
-      const Pow2Pair<float> f0 = pow2_pair(PLK_TC5_EXP == 4 ? 0 : -pending_exp<float>(o.cscale[0], p, P, C), 0.f);
-      const Pow2Pair<float> f1 = pow2_pair(PLK_TC5_EXP == 4 ? 0 : -pending_exp<float>(o.cscale[1], p, P, C), 0.f);
+      const int p0 = it.tile * TP, prow0 = p0 + 32 * quarter, p = prow0 + lane;
       const bool one_factor = __all_sync(0xffffffffu, f0.f2 == 1.f && f1.f2 == 1.f);
       float* dest = static_cast<float*>(o.dest) + (size_t)it.c * P * SP64;
       float* scale = static_cast<float*>(o.scale);
+      Item nx = it;
+      cx.advance(nx);
+      if (cx.valid(nx)) load_raw(nx);
       const uint32_t a = n & 1;
       mbar_wait(cx.barrier(B_TFULL0 + a), (n >> 1) & 1);
       tc_fence_after();
-      const uint32_t taddr = tmem_base + ((uint32_t)(32 * warp) << 16) + a * 128;
+      const uint32_t taddr = tmem_base + ((uint32_t)(32 * quarter) << 16) + a * 128 + half * 32;
       float mx = 0.f;
-#pragma unroll
-      for (int half = 0; half < 2; ++half) {
+      {
         uint32_t d0[32], d1[32];
-        tmem_ld32(taddr + half * 32, d0);
-        tmem_ld32(taddr + 64 + half * 32, d1);
+        tmem_ld32(taddr, d0);
+        tmem_ld32(taddr + 64, d1);
         tmem_ld_wait();
-        if (half == 1) {  // accumulators are in registers: hand the TMEM set back before the stores
-          tc_fence_before();
-          __syncwarp();
-          if (lane == 0) mbar_arrive(cx.barrier(B_TEMPTY0 + a));
-        }
-        if (PLK_TC5_EXP == 1) continue;
-        if (one_factor) {  // the usual case: each pending exponent fits one power-of-two factor
-#pragma unroll
-          for (int q = 0; q < 8; ++q) {
-            float v[4];
-#pragma unroll
-            for (int j = 0; j < 4; ++j) {
-              v[j] = (__uint_as_float(d0[4 * q + j]) * f0.f1) * (__uint_as_float(d1[4 * q + j]) * f1.f1);
-              mx = fmaxf(mx, v[j]);
-            }
-            sts128(stage + lane * STAGE_LD + q * 16, make_float4(v[0], v[1], v[2], v[3]));
-          }
-        } else {
-#pragma unroll
-          for (int q = 0; q < 8; ++q) {
-            float v[4];
-#pragma unroll
-            for (int j = 0; j < 4; ++j) {
-              v[j] = ((__uint_as_float(d0[4 * q + j]) * f0.f1) * f0.f2) * ((__uint_as_float(d1[4 * q + j]) * f1.f1) * f1.f2);
-              mx = fmaxf(mx, v[j]);
-            }
-            sts128(stage + lane * STAGE_LD + q * 16, make_float4(v[0], v[1], v[2], v[3]));
-          }
-        }
+        // accumulators are in registers: hand the TMEM set back before the stores
+        tc_fence_before();
         __syncwarp();
+        if (lane == 0) mbar_arrive(cx.barrier(B_TEMPTY0 + a));
+        if (PLK_TC5_EXP != 1) {
+          if (one_factor) {  // the usual case: each pending exponent fits one power-of-two factor
+#pragma unroll
+            for (int q = 0; q < 8; ++q) {
+              float v[4];
+#pragma unroll
+              for (int j = 0; j < 4; ++j) {
+                v[j] = (__uint_as_float(d0[4 * q + j]) * f0.f1) * (__uint_as_float(d1[4 * q + j]) * f1.f1);
+                mx = fmaxf(mx, v[j]);
+              }
+              sts128(stage + lane * 128 + ((q ^ (lane & 7)) << 4), make_float4(v[0], v[1], v[2], v[3]));
+            }
+          } else {
+#pragma unroll
+            for (int q = 0; q < 8; ++q) {
+              float v[4];
+#pragma unroll
+              for (int j = 0; j < 4; ++j) {
+                v[j] = ((__uint_as_float(d0[4 * q + j]) * f0.f1) * f0.f2) * ((__uint_as_float(d1[4 * q + j]) * f1.f1) * f1.f2);
+                mx = fmaxf(mx, v[j]);
+              }
+              sts128(stage + lane * 128 + ((q ^ (lane & 7)) << 4), make_float4(v[0], v[1], v[2], v[3]));
+            }
+          }
+        }
+      }
+      // the upper column half's row maximum travels through shared memory (double-buffered by item parity)
+      if (half == 1) sts32(cx.smem + OFF_MAX + (a * TP + 32 * quarter + lane) * 4, mx);
+      __syncwarp();
+      if (PLK_TC5_EXP != 1) {
 #pragma unroll
         for (int j = 0; j < 8; ++j) {
           const int idx = j * 32 + lane, r = idx >> 3, ch = idx & 7;
-          const float4 v = lds128(stage + r * STAGE_LD + ch * 16);
+          const float4 v = lds128(stage + r * 128 + ((ch ^ (r & 7)) << 4));
           if (prow0 + r < P) *reinterpret_cast<float4*>(dest + (size_t)(prow0 + r) * SP64 + half * 32 + ch * 4) = v;
         }
-        __syncwarp();
       }
-      if (p < P && scale != nullptr) scale[(size_t)it.c * P + p] = mx;
+      asm volatile("bar.sync 1, %0;" ::"n"(EPI_WARPS * 32) : "memory");
+      if (half == 0 && p < P && scale != nullptr)
+        scale[(size_t)it.c * P + p] = fmaxf(mx, lds32(cx.smem + OFF_MAX + (a * TP + 32 * quarter + lane) * 4));
+      it = nx;
+      if (cx.valid(it)) {
+        f0 = finish_raw(it, 0);
+        f1 = finish_raw(it, 1);
+      }
     }
   } else if (warp < EPI_WARPS + PROD_WARPS) {
     // ===== producers: group g = child g =====
@@ -415,20 +459,24 @@ __global__ void __launch_bounds__(THREADS, 1) k_post_tc5(const DevOp* __restrict
     float4 r[XCHUNKS];
     uint32_t n_run = 0;
     Item it = cx.first_item;
-    prod_load(cx, it, g, gt, r);
+    bool loaded = false;
 #pragma unroll 1
     while (true) {
-      const bool nr = cx.new_run(it);
-      float4 m[MCHUNKS];
-      if (nr) prod_load_matrix(cx, it, g, gt, m);
-      prod_store(cx, it, g, gt, r);
-      if (nr) {
+      if (cx.new_run(it)) {  // the register pipeline is drained here: r stages the matrix
+        static_assert(MCHUNKS <= XCHUNKS, "r doubles as the matrix staging registers");
+        float4(&m)[MCHUNKS] = reinterpret_cast<float4(&)[MCHUNKS]>(r);
+        prod_load_matrix(cx, it, g, gt, m);
         prod_store_matrix(cx, g, gt, m, n_run);
         ++n_run;
       }
-      cx.advance(it);
-      if (!cx.valid(it)) break;
-      prod_load(cx, it, g, gt, r);
+      if (!loaded) prod_load(cx, it, g, gt, r);
+      prod_store(cx, it, g, gt, r);
+      Item nx = it;
+      cx.advance(nx);
+      if (!cx.valid(nx)) break;
+      loaded = !cx.new_run(nx);
+      if (loaded) prod_load(cx, nx, g, gt, r);
+      it = nx;
     }
   } else {
     // ===== MMA issuer: the whole warp runs the loop, one elected lane executes each tcgen05.mma / commit =====
