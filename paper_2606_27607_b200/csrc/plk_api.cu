@@ -18,6 +18,7 @@
 #ifdef PLK_WITH_TENSOR
 #include "plk_tc.cuh"
 #include "plk_tc5.cuh"
+#include "plk_tc5_pre.cuh"
 #endif
 
 using namespace plk;
@@ -40,7 +41,7 @@ struct Layout {
   int n_tiles, max_grad;
   size_t off_post, off_compact, off_pre, off_pre_mx, off_matrix, off_eigen, off_scale, off_weights, off_pi,
       off_rates, off_catw, off_site, off_block_partial, off_grad_partial, off_grad_out, off_logl, off_site_deriv,
-      off_stage, off_ring, total;
+      off_stage, off_ring, off_matrix_t, total;
   size_t stage_bytes;
 };
 
@@ -103,6 +104,11 @@ bool compute_layout(const plk_config& c, Layout& L) {
   L.stage_bytes = round_up((size_t)L.C * L.P * L.S * 8, ALIGN);
   L.off_stage = take(L.stage_bytes);
   L.off_ring = take(RING_BYTES);
+  // transposed copies of the transition matrices for the tcgen05 pre-order kernel (plk_tc5_pre.cuh, step B)
+  L.off_matrix_t = take((L.SP == 64 && c.precision == PLK_FP32 && (c.flags & PLK_FLAG_TENSOR_CORES) &&
+                         !(c.flags & PLK_FLAG_NO_TCGEN05))
+                            ? (size_t)c.matrix_buffer_count * L.matrix_bytes
+                            : 0);
   L.total = o;
   return true;
 }
@@ -543,6 +549,11 @@ int launch_pre64(plk_instance* in, const DevPreItem* d_items, int n, const T* Q,
 #ifdef PLK_WITH_TENSOR
   if (in->cfg.flags & PLK_FLAG_TENSOR_CORES)
   {
+    if constexpr (sizeof(T) == 4) {
+      if (!(in->cfg.flags & PLK_FLAG_NO_TCGEN05))
+        return tc5::pre::launch_pre(in->stream, d_items, n, L.P, L.S, L.C, Q, (long long)L.off_matrix_t - (long long)L.off_matrix,
+                                    cw, cr, wt, gp, L.n_tiles, site, in->sm_count, &in->grad_parts, &in->launches);
+    }
     return tc_launch_pre<T>(in->stream, d_items, n, L.P, L.S, L.C, Q, cw, cr, wt, gp, L.n_tiles, site, &in->grad_parts,
                             &in->launches);
   }
@@ -1242,6 +1253,14 @@ static int pre_impl(plk_instance* in, int eigen, int root_pre, const plk_pre_op*
     if (rc) return rc;
     const DevPreItem* dit = reinterpret_cast<const DevPreItem*>(d);
     const void* Q = want_grad ? in->eig_QT(eigen) : in->eig_QT(0);
+#ifdef PLK_WITH_TENSOR
+    if (L.SP == 64 && in->f32 && (in->cfg.flags & PLK_FLAG_TENSOR_CORES) && !(in->cfg.flags & PLK_FLAG_NO_TCGEN05)) {
+      // step B of the tcgen05 pre-order kernel contracts over the ROW index of M: it reads transposed copies
+      tc5::pre::k_transpose64<<<in->cfg.matrix_buffer_count * L.C, 256, 0, in->stream>>>(
+          in->at<float>(L.off_matrix), in->at<float>(L.off_matrix_t));
+      CHECK_LAUNCH(in);
+    }
+#endif
     if (walk) {
       rc = by_precision(in, [&](auto tag) -> int {
         using T = decltype(tag);
