@@ -28,9 +28,9 @@ namespace plk {
 namespace tc5 {
 namespace pre {
 
-constexpr int EPI_W = 8, PROD_W = 4, N_W = EPI_W + PROD_W + 1;
-constexpr int THREADS_PRE = N_W * 32;  // 416
-constexpr int PT = PROD_W * 32;        // producer threads
+constexpr int EPI_W = 8, PROD_W = 4, AUX_W = 3, N_W = EPI_W + PROD_W + AUX_W + 1;  // tile producers, matrix / q_m stagers
+constexpr int THREADS_PRE = N_W * 32;  // 512
+constexpr int AT = AUX_W * 32;         // threads of the auxiliary stager group
 constexpr uint32_t OFF_XS = 0;                        // operand stage: hi plane, lo plane
 constexpr uint32_t OFF_MS = 2 * X_PLANE;              // M_0 hi, lo, M_1 hi, lo, Q hi, lo
 constexpr uint32_t OFF_QM = OFF_MS + 6 * M_PLANE;     // q_m tile / store stage
@@ -41,7 +41,7 @@ constexpr uint32_t SMEM_USED_PRE = OFF_BARS + 128;
 constexpr size_t SMEM_BYTES_PRE = SMEM_USED_PRE + 1024;
 enum { P_XFULL = 0, P_XFREE, P_UFULL, P_AFULL, P_QFULL, P_MFULL, P_MFREE, P_QMFULL, P_QMFREE, P_TFREE, P_ADONE, P_MTFULL,
        P_TMEM_PTR };
-constexpr uint32_t T_A0 = 0, T_A1 = 64, T_QX0 = 128, T_QX1 = 192, T_Q = 256;  // TMEM columns
+constexpr uint32_t T_A0 = 0, T_A1 = 64, T_QX0 = 128, T_QX1 = 192, T_Q0 = 256, T_Q1 = 320;  // TMEM columns
 constexpr uint32_t IDESC_BT = IDESC | (1u << 16);  // B operand MN-major: B(n = s, k = x) = M[x][s]
 
 // MN-major B descriptor over a K-major-staged 64 x 64 plane read transposed: 32 n-values per 128-byte row, n-blocks
@@ -132,6 +132,53 @@ __device__ __forceinline__ void pre_stage_matrix(uint32_t ms, const float* M, in
     sts128(mlo + 1024 * j, l);
   }
 }
+// the same with the 96 threads of the auxiliary group (chunks t, t + 96, ...)
+__device__ __forceinline__ void aux_stage_matrix(uint32_t ms, const float* M, int t) {
+  float4 m[11];
+#pragma unroll
+  for (int j = 0; j < 11; ++j) {
+    const int idx = t + AT * j;
+    if (idx < 1024) m[j] = ldg_nc(M + idx * 4);
+  }
+#pragma unroll
+  for (int j = 0; j < 11; ++j) {
+    const int idx = t + AT * j;
+    if (idx < 1024) {
+      float4 h, l;
+      split4(m[j], h, l);
+      const uint32_t o = ms + swz_off(idx >> 4, idx & 15, 64);
+      sts128(o, h);
+      sts128(o + M_PLANE, l);
+    }
+  }
+}
+// raw fp32 tile rows p0 .. p0 + n - 1 of `src` ([.][64]) -> swizzled 128 x 64 plane at `dst` (rows beyond n: zeros)
+__device__ __forceinline__ void aux_stage_tile(uint32_t dst, const float* src, int n, int t) {
+#pragma unroll
+  for (int b = 0; b < 2; ++b) {
+    float4 v[11];
+#pragma unroll
+    for (int j = 0; j < 11; ++j) {
+      const int idx = t + AT * (11 * b + j);
+      v[j] = (idx < 2048 && (idx >> 4) < n) ? ldg_nc(src + idx * 4) : make_float4(0.f, 0.f, 0.f, 0.f);
+    }
+#pragma unroll
+    for (int j = 0; j < 11; ++j) {
+      const int idx = t + AT * (11 * b + j);
+      if (idx < 2048) sts128(dst + swz_off(idx >> 4, idx & 15, TP), v[j]);
+    }
+  }
+}
+__device__ __forceinline__ void prefetch_tiles(const DevPreItem& it, int c, int P, int p0, int n) {
+#pragma unroll
+  for (int k = 0; k < 2; ++k) {
+    if (it.kind[k] == KIND_PARTIALS)
+      l2_prefetch_bulk(static_cast<const float*>(it.p[k]) + ((size_t)c * P + p0) * SP64, (uint32_t)n * 256u);
+    else if (it.kind[k] == KIND_BCAST)
+      l2_prefetch_bulk(static_cast<const float*>(it.p[k]) + (size_t)p0 * SP64, (uint32_t)n * 256u);
+  }
+  l2_prefetch_bulk(static_cast<const float*>(it.qm) + ((size_t)c * P + p0) * SP64, (uint32_t)n * 256u);
+}
 __device__ __forceinline__ void prod_signal(uint32_t bar, int t) {
   fence_async_smem();
   __syncwarp();
@@ -175,13 +222,13 @@ __global__ void __launch_bounds__(THREADS_PRE, 1)
     mbar_init(cx.barrier(P_UFULL), EPI_W);
     mbar_init(cx.barrier(P_AFULL), 1);
     mbar_init(cx.barrier(P_QFULL), 1);
-    mbar_init(cx.barrier(P_MFULL), PROD_W);
+    mbar_init(cx.barrier(P_MFULL), AUX_W);
     mbar_init(cx.barrier(P_MFREE), 1);
-    mbar_init(cx.barrier(P_QMFULL), PROD_W);
+    mbar_init(cx.barrier(P_QMFULL), AUX_W);
     mbar_init(cx.barrier(P_QMFREE), EPI_W);
     mbar_init(cx.barrier(P_TFREE), EPI_W);
     mbar_init(cx.barrier(P_ADONE), 1);
-    mbar_init(cx.barrier(P_MTFULL), PROD_W);
+    mbar_init(cx.barrier(P_MTFULL), AUX_W);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   if (warp == N_W - 1) {
@@ -196,45 +243,67 @@ __global__ void __launch_bounds__(THREADS_PRE, 1)
   const uint32_t xs = cx.smem + OFF_XS;
 
   if (warp >= EPI_W && warp < EPI_W + PROD_W) {
-    // ===== producers =====
+    // ===== tile producers: X_0 and X_1 of every (unit, category); the next tile is always in registers =====
     const int t = threadIdx.x - EPI_W * 32;
     uint32_t uc = 0;
     float4 r[16];
+    {
+      const DevPreItem& it = items[cx.u0 / cx.n_tiles];
+      const int p0 = (int)(cx.u0 % cx.n_tiles) * TP, n = P - p0 < TP ? P - p0 : TP;
+      pre_load_tile(it.p[0], it.kind[0], 0, P, p0, n, t, r);
+    }
     for (uint32_t ui = 0; ui < cx.n_units; ++ui) {
       const uint32_t u = cx.u0 + ui;
       const DevPreItem& it = items[u / cx.n_tiles];
       const int p0 = (int)(u % cx.n_tiles) * TP, n = P - p0 < TP ? P - p0 : TP;
       for (int c = 0; c < C; ++c, ++uc) {
-        // X_0
-        pre_load_tile(it.p[0], it.kind[0], c, P, p0, n, t, r);
         if (uc > 0) mbar_wait(cx.barrier(P_XFREE), 1);  // completion 2 uc - 1: step B of child 1, previous round
         pre_store_x(xs, it.kind[0], S, t, r);
         prod_signal(cx.barrier(P_XFULL), t);
-        // matrices of this category (Q once)
-        if (uc > 0) mbar_wait(cx.barrier(P_MFREE), (uc - 1) & 1);
-        if (uc == 0) pre_stage_matrix(cx.smem + OFF_MS + 4 * M_PLANE, Qg, t);
-        pre_stage_matrix(cx.smem + OFF_MS, static_cast<const float*>(it.mat[0]) + (size_t)c * SP64 * SP64, t);
-        pre_stage_matrix(cx.smem + OFF_MS + 2 * M_PLANE, static_cast<const float*>(it.mat[1]) + (size_t)c * SP64 * SP64, t);
-        prod_signal(cx.barrier(P_MFULL), t);
-        // q_m tile, raw (read by the epilogue threads, generic proxy)
-        pre_load_tile(it.qm, KIND_PARTIALS, c, P, p0, n, t, r);
-        if (uc > 0) mbar_wait(cx.barrier(P_QMFREE), (uc - 1) & 1);
-        {
-          const uint32_t q0 = cx.smem + OFF_QM + swz_off(t >> 4, t & 15, TP);
-#pragma unroll
-          for (int j = 0; j < 16; ++j) sts128(q0 + 1024 * j, r[j]);
-        }
-        __syncwarp();
-        if ((t & 31) == 0) mbar_arrive(cx.barrier(P_QMFULL));
-        // X_1
         pre_load_tile(it.p[1], it.kind[1], c, P, p0, n, t, r);
         mbar_wait(cx.barrier(P_XFREE), 0);  // completion 2 uc: step A of child 0
         pre_store_x(xs, it.kind[1], S, t, r);
         prod_signal(cx.barrier(P_XFULL), t);
+        if (c + 1 < C) {
+          pre_load_tile(it.p[0], it.kind[0], c + 1, P, p0, n, t, r);
+        } else if (ui + 1 < cx.n_units) {
+          const DevPreItem& nt = items[(u + 1) / cx.n_tiles];
+          const int q0 = (int)((u + 1) % cx.n_tiles) * TP, m = P - q0 < TP ? P - q0 : TP;
+          pre_load_tile(nt.p[0], nt.kind[0], 0, P, q0, m, t, r);
+        }
+      }
+    }
+  } else if (warp >= EPI_W + PROD_W && warp < N_W - 1) {
+    // ===== auxiliary stagers: Q once, M_0 / M_1, the q_m tile, the transposed matrices; L2 prefetch of the next round =====
+    const int t = threadIdx.x - (EPI_W + PROD_W) * 32;
+    uint32_t uc = 0;
+    for (uint32_t ui = 0; ui < cx.n_units; ++ui) {
+      const uint32_t u = cx.u0 + ui;
+      const DevPreItem& it = items[u / cx.n_tiles];
+      const int p0 = (int)(u % cx.n_tiles) * TP, n = P - p0 < TP ? P - p0 : TP;
+      for (int c = 0; c < C; ++c, ++uc) {
+        if (t == 0) {
+          if (c + 1 < C) {
+            prefetch_tiles(it, c + 1, P, p0, n);
+          } else if (ui + 1 < cx.n_units) {
+            const int q0 = (int)((u + 1) % cx.n_tiles) * TP;
+            prefetch_tiles(items[(u + 1) / cx.n_tiles], 0, P, q0, P - q0 < TP ? P - q0 : TP);
+          }
+        }
+        if (uc > 0) mbar_wait(cx.barrier(P_MFREE), (uc - 1) & 1);
+        if (uc == 0) aux_stage_matrix(cx.smem + OFF_MS + 4 * M_PLANE, Qg, t);
+        aux_stage_matrix(cx.smem + OFF_MS, static_cast<const float*>(it.mat[0]) + (size_t)c * SP64 * SP64, t);
+        aux_stage_matrix(cx.smem + OFF_MS + 2 * M_PLANE, static_cast<const float*>(it.mat[1]) + (size_t)c * SP64 * SP64, t);
+        prod_signal(cx.barrier(P_MFULL), t);
+        // q_m tile, raw (read by the epilogue threads through the generic proxy)
+        if (uc > 0) mbar_wait(cx.barrier(P_QMFREE), (uc - 1) & 1);
+        aux_stage_tile(cx.smem + OFF_QM, static_cast<const float*>(it.qm) + ((size_t)c * P + p0) * SP64, n, t);
+        __syncwarp();
+        if ((t & 31) == 0) mbar_arrive(cx.barrier(P_QMFULL));
         // step A done with M_0, M_1: their slots take the transposed matrices of step B
         mbar_wait(cx.barrier(P_ADONE), uc & 1);
-        pre_stage_matrix(cx.smem + OFF_MS, reinterpret_cast<const float*>(static_cast<const char*>(it.mat[0]) + mat_t_delta) + (size_t)c * SP64 * SP64, t);
-        pre_stage_matrix(cx.smem + OFF_MS + 2 * M_PLANE, reinterpret_cast<const float*>(static_cast<const char*>(it.mat[1]) + mat_t_delta) + (size_t)c * SP64 * SP64, t);
+        aux_stage_matrix(cx.smem + OFF_MS, reinterpret_cast<const float*>(static_cast<const char*>(it.mat[0]) + mat_t_delta) + (size_t)c * SP64 * SP64, t);
+        aux_stage_matrix(cx.smem + OFF_MS + 2 * M_PLANE, reinterpret_cast<const float*>(static_cast<const char*>(it.mat[1]) + mat_t_delta) + (size_t)c * SP64 * SP64, t);
         prod_signal(cx.barrier(P_MTFULL), t);
       }
     }
@@ -284,7 +353,7 @@ __global__ void __launch_bounds__(THREADS_PRE, 1)
           mbar_wait(cx.barrier(P_UFULL), k);
           tc_fence_after();
           if (need_q[k]) {
-            const uint32_t d = tmem_base + T_Q;
+            const uint32_t d = tmem_base + (k == 0 ? T_Q0 : T_Q1);
             const uint32_t mp = cx.smem + OFF_MS + 2 * k * M_PLANE;
             const uint64_t bhi = make_desc(mp), blo = make_desc(mp + M_PLANE);  // M_k^T, K-major
 #pragma unroll
@@ -363,13 +432,26 @@ __global__ void __launch_bounds__(THREADS_PRE, 1)
         for (int k = 0; k < 2; ++k) {
           mbar_wait(cx.barrier(P_QFULL), k);
           tc_fence_after();
+          if (k == 0) {  // U_0 has been consumed (P_QFULL): hand U_1 to the tensor pipe first, q_1 has its own TMEM columns
+#pragma unroll
+            for (int ch = 0; ch < 8; ++ch) {
+              float4 h, l;
+              split4(make_float4(u1[4 * ch], u1[4 * ch + 1], u1[4 * ch + 2], u1[4 * ch + 3]), h, l);
+              const uint32_t so = (uint32_t)((ch ^ (row & 7)) << 4);
+              sts128(xs_row + so, h);
+              sts128(xs_row + X_PLANE + so, l);
+            }
+            fence_async_smem();
+            __syncwarp();
+            if (lane == 0) mbar_arrive(cx.barrier(P_UFULL));
+          }
           float mx = 0.f;
           if (need_q[k]) {
             float nn = 0.f;
 #pragma unroll
             for (int sub = 0; sub < 2; ++sub) {
               uint32_t qk[16], qx[16];
-              tmem_ld16(lane_tm + T_Q + 16 * sub, qk);
+              tmem_ld16(lane_tm + (k == 0 ? T_Q0 : T_Q1) + 16 * sub, qk);
               tmem_ld16(lane_tm + (k == 0 ? T_QX0 : T_QX1) + 16 * sub, qx);
               tmem_ld_wait();
 #pragma unroll
@@ -388,19 +470,6 @@ __global__ void __launch_bounds__(THREADS_PRE, 1)
             if (want[k]) num[k] = fma(cwr, (double)nn, num[k]);
           }
           tc_fence_before();
-          if (k == 0) {  // q_0 has left TMEM and U_0 has been consumed (P_QFULL): hand U_1 to the tensor pipe
-#pragma unroll
-            for (int ch = 0; ch < 8; ++ch) {
-              float4 h, l;
-              split4(make_float4(u1[4 * ch], u1[4 * ch + 1], u1[4 * ch + 2], u1[4 * ch + 3]), h, l);
-              const uint32_t so = (uint32_t)((ch ^ (row & 7)) << 4);
-              sts128(xs_row + so, h);
-              sts128(xs_row + X_PLANE + so, l);
-            }
-            fence_async_smem();
-            __syncwarp();
-            if (lane == 0) mbar_arrive(cx.barrier(P_UFULL));
-          }
           if (it.q[k] != nullptr) {
             if (half == 1) smx[row] = mx;
             __syncwarp();
