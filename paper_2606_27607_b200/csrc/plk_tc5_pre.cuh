@@ -28,6 +28,14 @@ namespace plk {
 namespace tc5 {
 namespace pre {
 
+#ifdef PLK_TC5_TRACE
+#define TP_T0() long long _t0 = clock64()
+#define TP_ACC(x) do { long long _t1 = clock64(); (x) += _t1 - _t0; _t0 = _t1; } while (0)
+#else
+#define TP_T0() do {} while (0)
+#define TP_ACC(x) do {} while (0)
+#endif
+
 constexpr int EPI_W = 8, PROD_W = 4, AUX_W = 3, N_W = EPI_W + PROD_W + AUX_W + 1;  // tile producers, matrix / q_m stagers
 constexpr int THREADS_PRE = N_W * 32;  // 512
 constexpr int AT = AUX_W * 32;         // threads of the auxiliary stager group
@@ -37,10 +45,10 @@ constexpr uint32_t OFF_QM = OFF_MS + 6 * M_PLANE;     // q_m tile / store stage
 constexpr uint32_t OFF_RED = OFF_QM + X_PLANE;        // doubles: [3][TP] half-1 partial sums, [2][TP] contributions
 constexpr uint32_t OFF_MX = OFF_RED + 5 * TP * 8;     // floats: [TP] half-1 row maxima
 constexpr uint32_t OFF_BARS = OFF_MX + TP * 4;
-constexpr uint32_t SMEM_USED_PRE = OFF_BARS + 128;
+constexpr uint32_t SMEM_USED_PRE = OFF_BARS + 256;
 constexpr size_t SMEM_BYTES_PRE = SMEM_USED_PRE + 1024;
-enum { P_XFULL = 0, P_XFREE, P_UFULL, P_AFULL, P_QFULL, P_MFULL, P_MFREE, P_QMFULL, P_QMFREE, P_TFREE, P_ADONE, P_MTFULL,
-       P_TMEM_PTR };
+enum { P_XFULL = 0, P_XFREE, P_UFULL, P_AFULL, P_QFULL, P_MFULL, P_MFREE, P_TFREE, P_ADONE, P_MTFULL,
+       P_MTFULL1, P_MFULL1, P_M0FREE, P_TMEM_PTR };
 constexpr uint32_t T_A0 = 0, T_A1 = 64, T_QX0 = 128, T_QX1 = 192, T_Q0 = 256, T_Q1 = 320;  // TMEM columns
 constexpr uint32_t IDESC_BT = IDESC | (1u << 16);  // B operand MN-major: B(n = s, k = x) = M[x][s]
 
@@ -132,14 +140,15 @@ __device__ __forceinline__ void pre_stage_matrix(uint32_t ms, const float* M, in
     sts128(mlo + 1024 * j, l);
   }
 }
-// the same with the 96 threads of the auxiliary group (chunks t, t + 96, ...)
-__device__ __forceinline__ void aux_stage_matrix(uint32_t ms, const float* M, int t) {
-  float4 m[11];
+// the same with the 96 threads of the auxiliary group (chunks t, t + 96, ...), as a load half and a store half
+__device__ __forceinline__ void aux_load_matrix(const float* M, int t, float4 (&m)[11]) {
 #pragma unroll
   for (int j = 0; j < 11; ++j) {
     const int idx = t + AT * j;
     if (idx < 1024) m[j] = ldg_nc(M + idx * 4);
   }
+}
+__device__ __forceinline__ void aux_store_matrix(uint32_t ms, int t, const float4 (&m)[11]) {
 #pragma unroll
   for (int j = 0; j < 11; ++j) {
     const int idx = t + AT * j;
@@ -151,6 +160,11 @@ __device__ __forceinline__ void aux_stage_matrix(uint32_t ms, const float* M, in
       sts128(o + M_PLANE, l);
     }
   }
+}
+__device__ __forceinline__ void aux_stage_matrix(uint32_t ms, const float* M, int t) {
+  float4 m[11];
+  aux_load_matrix(M, t, m);
+  aux_store_matrix(ms, t, m);
 }
 // raw fp32 tile rows p0 .. p0 + n - 1 of `src` ([.][64]) -> swizzled 128 x 64 plane at `dst` (rows beyond n: zeros)
 __device__ __forceinline__ void aux_stage_tile(uint32_t dst, const float* src, int n, int t) {
@@ -224,11 +238,12 @@ __global__ void __launch_bounds__(THREADS_PRE, 1)
     mbar_init(cx.barrier(P_QFULL), 1);
     mbar_init(cx.barrier(P_MFULL), AUX_W);
     mbar_init(cx.barrier(P_MFREE), 1);
-    mbar_init(cx.barrier(P_QMFULL), AUX_W);
-    mbar_init(cx.barrier(P_QMFREE), EPI_W);
     mbar_init(cx.barrier(P_TFREE), EPI_W);
     mbar_init(cx.barrier(P_ADONE), 1);
     mbar_init(cx.barrier(P_MTFULL), AUX_W);
+    mbar_init(cx.barrier(P_MTFULL1), AUX_W);
+    mbar_init(cx.barrier(P_MFULL1), AUX_W);
+    mbar_init(cx.barrier(P_M0FREE), 1);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   if (warp == N_W - 1) {
@@ -290,38 +305,66 @@ __global__ void __launch_bounds__(THREADS_PRE, 1)
             prefetch_tiles(items[(u + 1) / cx.n_tiles], 0, P, q0, P - q0 < TP ? P - q0 : TP);
           }
         }
+        // Slot of child 0: M_0 (step A) -> M_0^T (step B of child 0) -> M_0 of the next round as soon as that step B is
+        // done (P_M0FREE), i.e. while child 1 is still in flight.  Slot of child 1: M_1 -> M_1^T -> next M_1 (P_MFREE).
+        float4 mt[11];
+        if (uc == 0) {
+          aux_stage_matrix(cx.smem + OFF_MS + 4 * M_PLANE, Qg, t);
+          aux_stage_matrix(cx.smem + OFF_MS, static_cast<const float*>(it.mat[0]) + (size_t)c * SP64 * SP64, t);
+          prod_signal(cx.barrier(P_MFULL), t);
+        }
+        aux_load_matrix(static_cast<const float*>(it.mat[1]) + (size_t)c * SP64 * SP64, t, mt);
         if (uc > 0) mbar_wait(cx.barrier(P_MFREE), (uc - 1) & 1);
-        if (uc == 0) aux_stage_matrix(cx.smem + OFF_MS + 4 * M_PLANE, Qg, t);
-        aux_stage_matrix(cx.smem + OFF_MS, static_cast<const float*>(it.mat[0]) + (size_t)c * SP64 * SP64, t);
-        aux_stage_matrix(cx.smem + OFF_MS + 2 * M_PLANE, static_cast<const float*>(it.mat[1]) + (size_t)c * SP64 * SP64, t);
-        prod_signal(cx.barrier(P_MFULL), t);
-        // q_m tile, raw (read by the epilogue threads through the generic proxy)
-        if (uc > 0) mbar_wait(cx.barrier(P_QMFREE), (uc - 1) & 1);
-        aux_stage_tile(cx.smem + OFF_QM, static_cast<const float*>(it.qm) + ((size_t)c * P + p0) * SP64, n, t);
-        __syncwarp();
-        if ((t & 31) == 0) mbar_arrive(cx.barrier(P_QMFULL));
-        // step A done with M_0, M_1: their slots take the transposed matrices of step B
+        aux_store_matrix(cx.smem + OFF_MS + 2 * M_PLANE, t, mt);
+        prod_signal(cx.barrier(P_MFULL1), t);
+        aux_load_matrix(reinterpret_cast<const float*>(static_cast<const char*>(it.mat[0]) + mat_t_delta) + (size_t)c * SP64 * SP64, t, mt);
         mbar_wait(cx.barrier(P_ADONE), uc & 1);
-        aux_stage_matrix(cx.smem + OFF_MS, reinterpret_cast<const float*>(static_cast<const char*>(it.mat[0]) + mat_t_delta) + (size_t)c * SP64 * SP64, t);
-        aux_stage_matrix(cx.smem + OFF_MS + 2 * M_PLANE, reinterpret_cast<const float*>(static_cast<const char*>(it.mat[1]) + mat_t_delta) + (size_t)c * SP64 * SP64, t);
+        aux_store_matrix(cx.smem + OFF_MS, t, mt);
         prod_signal(cx.barrier(P_MTFULL), t);
+        aux_stage_matrix(cx.smem + OFF_MS + 2 * M_PLANE, reinterpret_cast<const float*>(static_cast<const char*>(it.mat[1]) + mat_t_delta) + (size_t)c * SP64 * SP64, t);
+        prod_signal(cx.barrier(P_MTFULL1), t);
+        {  // M_0 of the next round
+          const DevPreItem* nt = nullptr;
+          int nc = 0;
+          if (c + 1 < C) {
+            nt = &it;
+            nc = c + 1;
+          } else if (ui + 1 < cx.n_units) {
+            nt = &items[(u + 1) / cx.n_tiles];
+          }
+          if (nt != nullptr) {
+            aux_load_matrix(static_cast<const float*>(nt->mat[0]) + (size_t)nc * SP64 * SP64, t, mt);
+            mbar_wait(cx.barrier(P_M0FREE), uc & 1);
+            aux_store_matrix(cx.smem + OFF_MS, t, mt);
+            prod_signal(cx.barrier(P_MFULL), t);
+          }
+        }
       }
     }
   } else if (warp == N_W - 1) {
     // ===== MMA issuer (whole warp converged; elect.sync inside the asm) =====
     const uint64_t dxhi = make_desc(xs), dxlo = make_desc(xs + X_PLANE);
     uint32_t uc = 0;
+    long long m_tf = 0, m_mf = 0, m_x0 = 0, m_x1 = 0, m_mt = 0, m_u0 = 0, m_u1 = 0, m_is = 0;
+    (void)m_tf; (void)m_mf; (void)m_x0; (void)m_x1; (void)m_mt; (void)m_u0; (void)m_u1; (void)m_is;
+    TP_T0();
     for (uint32_t ui = 0; ui < cx.n_units; ++ui) {
       const DevPreItem& it = items[(cx.u0 + ui) / cx.n_tiles];
       const bool lo[2] = {it.kind[0] == KIND_PARTIALS || it.kind[0] == KIND_BCAST,
                           it.kind[1] == KIND_PARTIALS || it.kind[1] == KIND_BCAST};
       const bool need_q[2] = {it.q[0] != nullptr || it.slot[0] >= 0, it.q[1] != nullptr || it.slot[1] >= 0};
       for (int c = 0; c < C; ++c, ++uc) {
+        TP_ACC(m_is);
         if (uc > 0) mbar_wait(cx.barrier(P_TFREE), (uc - 1) & 1);
-        mbar_wait(cx.barrier(P_MFULL), uc & 1);
+        TP_ACC(m_tf);
+
 #pragma unroll
         for (int k = 0; k < 2; ++k) {  // step A: a_k = X_k M_k^T, Qx_k = X_k Q^T
+          TP_ACC(m_is);
+          mbar_wait(cx.barrier(k == 0 ? P_MFULL : P_MFULL1), uc & 1);
+          TP_ACC(m_mf);
           mbar_wait(cx.barrier(P_XFULL), k);
+          if (k == 0) TP_ACC(m_x0); else TP_ACC(m_x1);
           tc_fence_after();
 #pragma unroll
           for (int w = 0; w < 2; ++w) {  // w = 0: M_k, w = 1: Q
@@ -347,10 +390,13 @@ __global__ void __launch_bounds__(THREADS_PRE, 1)
         }
         umma_commit(cx.barrier(P_AFULL));
         umma_commit(cx.barrier(P_ADONE));
-        mbar_wait(cx.barrier(P_MTFULL), uc & 1);
 #pragma unroll
         for (int k = 0; k < 2; ++k) {  // step B: q_k = U_k M_k (B read MN-major from the same planes)
+          TP_ACC(m_is);
+          mbar_wait(cx.barrier(k == 0 ? P_MTFULL : P_MTFULL1), uc & 1);
+          TP_ACC(m_mt);
           mbar_wait(cx.barrier(P_UFULL), k);
+          if (k == 0) TP_ACC(m_u0); else TP_ACC(m_u1);
           tc_fence_after();
           if (need_q[k]) {
             const uint32_t d = tmem_base + (k == 0 ? T_Q0 : T_Q1);
@@ -366,10 +412,16 @@ __global__ void __launch_bounds__(THREADS_PRE, 1)
           }
           if (k == 1) umma_commit(cx.barrier(P_XFREE));  // the producers' cue for the next X_0
           umma_commit(cx.barrier(P_QFULL));
+          if (k == 0) umma_commit(cx.barrier(P_M0FREE));
         }
         umma_commit(cx.barrier(P_MFREE));
       }
     }
+#ifdef PLK_TC5_TRACE
+    if (blockIdx.x == 0 && lane == 0 && uc > 100)
+      printf("MMA rounds %u: issue %lld | wait tfree %lld, mfull %lld, x0 %lld, x1 %lld, mt %lld, u0 %lld, u1 %lld\n", uc, m_is / uc,
+             m_tf / uc, m_mf / uc, m_x0 / uc, m_x1 / uc, m_mt / uc, m_u0 / uc, m_u1 / uc);
+#endif
   } else {
     // ===== epilogue: warp = 4 half + quarter; thread = pattern row 32 quarter + lane, states 32 half .. 32 half + 31 =====
     const int quarter = warp & 3, half = warp >> 2, row = 32 * quarter + lane;
@@ -380,6 +432,9 @@ __global__ void __launch_bounds__(THREADS_PRE, 1)
     double* red = reinterpret_cast<double*>(tc5p_smem_raw + (cx.smem - smem_u32(tc5p_smem_raw)) + OFF_RED);
     float* smx = reinterpret_cast<float*>(tc5p_smem_raw + (cx.smem - smem_u32(tc5p_smem_raw)) + OFF_MX);
     uint32_t uc = 0;
+    long long e_qm = 0, e_a = 0, e_u = 0, e_q0w = 0, e_u1 = 0, e_q0 = 0, e_q1w = 0, e_q1 = 0, e_end = 0;
+    (void)e_qm; (void)e_a; (void)e_u; (void)e_q0w; (void)e_u1; (void)e_q0; (void)e_q1w; (void)e_q1; (void)e_end;
+    TP_T0();
     for (uint32_t ui = 0; ui < cx.n_units; ++ui) {
       const uint32_t u = cx.u0 + ui;
       const DevPreItem& it = items[u / cx.n_tiles];
@@ -393,8 +448,26 @@ __global__ void __launch_bounds__(THREADS_PRE, 1)
       for (int c = 0; c < C; ++c, ++uc) {
         const double cw = catw[c], cwr = catw[c] * catr[c];
         float u1[32];
-        mbar_wait(cx.barrier(P_QMFULL), uc & 1);
+        TP_ACC(e_end);
+        // the warp's own 32 x 32 slice of q_m, global -> shared (coalesced 128-byte row segments), under step A
+        {
+          const float* src = static_cast<const float*>(it.qm) + ((size_t)c * P + p0 + 32 * quarter) * SP64 + 32 * half;
+          float4 v[8];
+#pragma unroll
+          for (int j = 0; j < 8; ++j) {
+            const int idx = j * 32 + lane, r = idx >> 3, ch = idx & 7;
+            v[j] = (p0 + 32 * quarter + r < P) ? ldg_nc(src + (size_t)r * SP64 + ch * 4) : make_float4(0.f, 0.f, 0.f, 0.f);
+          }
+#pragma unroll
+          for (int j = 0; j < 8; ++j) {
+            const int idx = j * 32 + lane, r = idx >> 3, ch = idx & 7;
+            sts128(slice + (uint32_t)r * 128 + (uint32_t)((ch ^ (r & 7)) << 4), v[j]);
+          }
+          __syncwarp();
+        }
+        TP_ACC(e_qm);
         mbar_wait(cx.barrier(P_AFULL), uc & 1);
+        TP_ACC(e_a);
         tc_fence_after();
         // ---- u_0 = q_m o a_1 (to the operand stage), u_1 = q_m o a_0 (kept), den
         float dd = 0.f;
@@ -428,9 +501,11 @@ __global__ void __launch_bounds__(THREADS_PRE, 1)
         fence_async_smem();
         __syncwarp();
         if (lane == 0) mbar_arrive(cx.barrier(P_UFULL));
+        TP_ACC(e_u);
 #pragma unroll
         for (int k = 0; k < 2; ++k) {
           mbar_wait(cx.barrier(P_QFULL), k);
+          if (k == 0) TP_ACC(e_q0w); else TP_ACC(e_q1w);
           tc_fence_after();
           if (k == 0) {  // U_0 has been consumed (P_QFULL): hand U_1 to the tensor pipe first, q_1 has its own TMEM columns
 #pragma unroll
@@ -444,6 +519,7 @@ __global__ void __launch_bounds__(THREADS_PRE, 1)
             fence_async_smem();
             __syncwarp();
             if (lane == 0) mbar_arrive(cx.barrier(P_UFULL));
+            TP_ACC(e_u1);
           }
           float mx = 0.f;
           if (need_q[k]) {
@@ -470,6 +546,10 @@ __global__ void __launch_bounds__(THREADS_PRE, 1)
             if (want[k]) num[k] = fma(cwr, (double)nn, num[k]);
           }
           tc_fence_before();
+          if (k == 1) {  // every accumulator of this round has been read: step A of the next round may start
+            __syncwarp();
+            if (lane == 0) mbar_arrive(cx.barrier(P_TFREE));
+          }
           if (it.q[k] != nullptr) {
             if (half == 1) smx[row] = mx;
             __syncwarp();
@@ -484,12 +564,10 @@ __global__ void __launch_bounds__(THREADS_PRE, 1)
             if (half == 0 && p < P) static_cast<float*>(it.q_scale[k])[(size_t)c * P + p] = fmaxf(mx, smx[row]);
             epi_bar();  // smx and the slices are free again
           }
+          if (k == 0) TP_ACC(e_q0); else TP_ACC(e_q1);
         }
         __syncwarp();
-        if (lane == 0) {
-          mbar_arrive(cx.barrier(P_QMFREE));
-          mbar_arrive(cx.barrier(P_TFREE));
-        }
+
       }
       // ---- per-pattern derivative and the tile's contribution to each gradient (fixed order)
       if (want[0] || want[1]) {
@@ -523,6 +601,11 @@ __global__ void __launch_bounds__(THREADS_PRE, 1)
         epi_bar();
       }
     }
+#ifdef PLK_TC5_TRACE
+    if (blockIdx.x == 0 && threadIdx.x == 0 && uc > 100)
+      printf("EPI rounds %u: end %lld | wait qm %lld, wait A %lld, u-phase %lld, wait q0 %lld, U1 %lld, q0 %lld, wait q1 %lld, q1 %lld\n", uc,
+             e_end / uc, e_qm / uc, e_a / uc, e_u / uc, e_q0w / uc, e_u1 / uc, e_q0 / uc, e_q1w / uc, e_q1 / uc);
+#endif
   }
   tc_fence_before();
   __syncthreads();
