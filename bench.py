@@ -42,7 +42,7 @@ def parse_args():
     ap.add_argument("--staging", choices=["tma", "ldg"], default="tma",
                     help="4-state operand staging: TMA ring (cp.async.bulk) / register-staged loads")
     ap.add_argument("--codon-fp32", choices=["tcgen05", "mma_sync"], default="tcgen05",
-                    help="fp32 --tensor post-order kernel: tcgen05/TMEM (default) or the legacy mma.sync arm")
+                    help="fp32 --tensor codon kernels: tcgen05/TMEM (default) or the legacy mma.sync arm")
     ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
     ap.add_argument("--sweep", action="store_true",
                     help="BASELINE configs[4]: HKY fp32, taxa {8,32,128,512} x patterns {1e2..5e5}; prints one JSON "
@@ -259,7 +259,7 @@ def workload_config(wl, precision, flags, extra=None):
     cfg = {"workload": wl.name, "taxa": wl.tree.n_tips, "patterns": wl.n_patterns, "states": wl.n_states,
            "categories": wl.n_categories, "branches": 2 * wl.tree.n_tips - 2, "precision": precision,
            "codon_path": ("tensor" if flags & 1 else "cuda-core") if wl.n_states != 4 else None,
-           "codon_fp32_post_order": (("mma.sync" if flags & 64 else "tcgen05") if (flags & 1 and precision == "fp32"
+           "codon_fp32_kernels": (("mma.sync" if flags & 64 else "tcgen05") if (flags & 1 and precision == "fp32"
                                                                                    and wl.n_states != 4) else None),
            "substitution_model": wl.model["name"], "seed": wl.seed,
            "launch_shape": {8: "level", 16: "walk"}.get(flags & 24, "auto") if wl.n_states == 4 else "level",
@@ -309,7 +309,7 @@ def run_extras(peaks, steps, warmup):
     if have_tc:
         plan += [("cfg2_fp64_tensor", 2, None, None, "fp64", 1), ("cfg2_fp32_tensor", 2, None, None, "fp32", 1),
                  ("cfg3_fp32_tensor", 3, None, None, "fp32", 1),
-                 ("cfg3_fp32_tensor_mma_sync_post", 3, None, None, "fp32", 1 | 64)]
+                 ("cfg3_fp32_tensor_mma_sync", 3, None, None, "fp32", 1 | 64)]
     else:
         plan += [("cfg3_fp32_cuda", 3, None, None, "fp32", 0)]
     plan += [("cfg4_hky_fp32_512x100000", 4, 512, 100_000, "fp32", 0), ("cfg4_hky_fp32_8x100", 4, 8, 100, "fp32", 0)]
@@ -436,7 +436,8 @@ def main():
              else (("k_post_tc5" if args.precision == "fp32" and args.codon_fp32 == "tcgen05" else "k_post_tc")
                    if args.tensor else "k_post64"),
              "pre_order_gradient": ("k_pre4_lean" if lean else "k_pre4_tma/k_pre4/k_pre4_walk") if nuc
-             else ("k_pre_tc" if args.tensor else "k_pre64")}[dom]
+             else (("k_pre_tc5" if args.precision == "fp32" and args.codon_fp32 == "tcgen05" else "k_pre_tc")
+                   if args.tensor else "k_pre64")}[dom]
     n_levels_note = "all launches of the kernel in one step (one per dependency level and item class)"
     # DRAM bytes (read + write) of those launches from ncu, per step: profiles/r01_launches_cfg1_fp64.md
     traffic = NCU_DRAM_BYTES.get((wl.name, args.precision, kname))

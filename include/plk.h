@@ -65,8 +65,9 @@ enum {                                                /* plk_config.flags (bit s
                                   library picks the cheaper shape from P, C, the list length and its level count */
   PLK_FLAG_NO_TMA = 32,        /* 4-state kernels: use the register-staged (LDG) kernels instead of the TMA-staged
                                   ones (comparison arm; also what category counts other than 1, 2, 4, 8 run on) */
-  PLK_FLAG_NO_TCGEN05 = 64,    /* fp32 + PLK_FLAG_TENSOR_CORES: run the post-order update on the legacy warp-level
-                                  mma.sync TF32 kernel instead of the tcgen05 / TMEM kernel (comparison arm)  */
+  PLK_FLAG_NO_TCGEN05 = 64,    /* fp32 + PLK_FLAG_TENSOR_CORES: run the post-order and the fused pre-order + derivative
+                                  kernels on the legacy warp-level mma.sync TF32 kernels instead of the tcgen05 /
+                                  TMEM kernels (comparison arm)                                             */
   PLK_FLAG_SITE_DERIVATIVES = 4 /* reserve partials_buffer_count * P doubles so that the gradient calls can
                                   return per-pattern derivatives (out_site != NULL); without it such a
                                   request returns PLK_ERR_UNSUPPORTED                                   */
