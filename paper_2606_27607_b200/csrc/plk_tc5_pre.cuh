@@ -49,7 +49,9 @@ constexpr uint32_t SMEM_USED_PRE = OFF_BARS + 256;
 constexpr size_t SMEM_BYTES_PRE = SMEM_USED_PRE + 1024;
 enum { P_XFULL = 0, P_XFREE, P_UFULL, P_AFULL, P_QFULL, P_MFULL, P_MFREE, P_TFREE, P_ADONE, P_MTFULL,
        P_MTFULL1, P_MFULL1, P_M0FREE, P_TMEM_PTR };
-constexpr uint32_t T_A0 = 0, T_A1 = 64, T_QX0 = 128, T_QX1 = 192, T_Q0 = 256, T_Q1 = 320;  // TMEM columns
+// TMEM columns.  U_0 (hi, lo) has its own 128 columns; U_1 (hi, lo) overwrites a_0 / a_1, which the thread that
+// writes it has just consumed.
+constexpr uint32_t T_A0 = 0, T_A1 = 64, T_QX0 = 128, T_QX1 = 192, T_Q0 = 256, T_Q1 = 320, T_U0 = 384;
 constexpr uint32_t IDESC_BT = IDESC | (1u << 16);  // B operand MN-major: B(n = s, k = x) = M[x][s]
 
 // MN-major B descriptor over a K-major-staged 64 x 64 plane read transposed: 32 n-values per 128-byte row, n-blocks
@@ -207,6 +209,24 @@ __device__ __forceinline__ void tmem_ld16(uint32_t taddr, uint32_t (&v)[16]) {
       : "r"(taddr)
       : "memory");
 }
+__device__ __forceinline__ void tmem_st16(uint32_t taddr, const float (&v)[16]) {
+  asm volatile(
+      "tcgen05.st.sync.aligned.32x32b.x16.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,%16};" ::"r"(taddr),
+      "f"(v[0]), "f"(v[1]), "f"(v[2]), "f"(v[3]), "f"(v[4]), "f"(v[5]), "f"(v[6]), "f"(v[7]), "f"(v[8]), "f"(v[9]), "f"(v[10]),
+      "f"(v[11]), "f"(v[12]), "f"(v[13]), "f"(v[14]), "f"(v[15])
+      : "memory");
+}
+__device__ __forceinline__ void tmem_st_wait() { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
+// D[tmem] (+)= A[tmem] . B[smem]^T : A = 128 lanes x 8 consecutive 32-bit columns (one k-step)
+__device__ __forceinline__ void umma_ta(uint32_t d_tmem, uint32_t a_tmem, uint64_t b_desc, uint32_t accumulate) {
+  asm volatile(
+      "{\n\t.reg .pred p, e;\n\t"
+      "elect.sync _|e, 0xffffffff;\n\t"
+      "setp.ne.b32 p, %4, 0;\n\t"
+      "@e tcgen05.mma.cta_group::1.kind::tf32 [%0], [%1], %2, %3, p;\n\t}" ::"r"(d_tmem),
+      "r"(a_tmem), "l"(b_desc), "r"(IDESC), "r"(accumulate)
+      : "memory");
+}
 __device__ __forceinline__ float scale2(uint32_t bits, const Pow2Pair<float>& f) { return (__uint_as_float(bits) * f.f1) * f.f2; }
 __device__ __forceinline__ void epi_bar() { asm volatile("bar.sync 1, %0;" ::"n"(EPI_W * 32) : "memory"); }
 
@@ -233,7 +253,7 @@ __global__ void __launch_bounds__(THREADS_PRE, 1)
   if (threadIdx.x == 0) {
     mbar_init(cx.barrier(P_XFULL), PROD_W);
     mbar_init(cx.barrier(P_XFREE), 1);
-    mbar_init(cx.barrier(P_UFULL), EPI_W);
+    mbar_init(cx.barrier(P_UFULL), EPI_W);  // one completion per round: both U_0 and U_1 are in TMEM
     mbar_init(cx.barrier(P_AFULL), 1);
     mbar_init(cx.barrier(P_QFULL), 1);
     mbar_init(cx.barrier(P_MFULL), AUX_W);
@@ -386,31 +406,33 @@ __global__ void __launch_bounds__(THREADS_PRE, 1)
               acc = 1;
             }
           }
-          if (k == 0) umma_commit(cx.barrier(P_XFREE));  // the producers' cue for X_1 (after k = 1: P_AFULL)
+          umma_commit(cx.barrier(P_XFREE));  // the producers' cue for X_1 / for X_0 of the next round
         }
         umma_commit(cx.barrier(P_AFULL));
         umma_commit(cx.barrier(P_ADONE));
+        TP_ACC(m_is);
+        mbar_wait(cx.barrier(P_UFULL), uc & 1);
+        TP_ACC(m_u0);
+        tc_fence_after();
 #pragma unroll
-        for (int k = 0; k < 2; ++k) {  // step B: q_k = U_k M_k (B read MN-major from the same planes)
+        for (int k = 0; k < 2; ++k) {  // step B: q_k = U_k M_k, A = U_k (hi, lo) in TMEM, B = M_k^T (K-major)
           TP_ACC(m_is);
           mbar_wait(cx.barrier(k == 0 ? P_MTFULL : P_MTFULL1), uc & 1);
           TP_ACC(m_mt);
-          mbar_wait(cx.barrier(P_UFULL), k);
-          if (k == 0) TP_ACC(m_u0); else TP_ACC(m_u1);
           tc_fence_after();
           if (need_q[k]) {
             const uint32_t d = tmem_base + (k == 0 ? T_Q0 : T_Q1);
+            const uint32_t uhi = tmem_base + (k == 0 ? T_U0 : T_A0), ulo = tmem_base + (k == 0 ? T_U0 + 64 : T_A1);
             const uint32_t mp = cx.smem + OFF_MS + 2 * k * M_PLANE;
             const uint64_t bhi = make_desc(mp), blo = make_desc(mp + M_PLANE);  // M_k^T, K-major
 #pragma unroll
-            for (int ks = 0; ks < 8; ++ks) umma<IDESC>(d, dxlo + koff(ks, TP), bhi + koff(ks, 64), (uint32_t)(ks > 0));
+            for (int ks = 0; ks < 8; ++ks) umma_ta(d, ulo + 8 * ks, bhi + koff(ks, 64), (uint32_t)(ks > 0));
 #pragma unroll
             for (int ks = 0; ks < 8; ++ks) {
-              umma<IDESC>(d, dxhi + koff(ks, TP), blo + koff(ks, 64), 1);
-              umma<IDESC>(d, dxhi + koff(ks, TP), bhi + koff(ks, 64), 1);
+              umma_ta(d, uhi + 8 * ks, blo + koff(ks, 64), 1);
+              umma_ta(d, uhi + 8 * ks, bhi + koff(ks, 64), 1);
             }
           }
-          if (k == 1) umma_commit(cx.barrier(P_XFREE));  // the producers' cue for the next X_0
           umma_commit(cx.barrier(P_QFULL));
           if (k == 0) umma_commit(cx.barrier(P_M0FREE));
         }
@@ -447,7 +469,6 @@ __global__ void __launch_bounds__(THREADS_PRE, 1)
       double den = 0.0, num[2] = {0.0, 0.0};
       for (int c = 0; c < C; ++c, ++uc) {
         const double cw = catw[c], cwr = catw[c] * catr[c];
-        float u1[32];
         TP_ACC(e_end);
         // the warp's own 32 x 32 slice of q_m, global -> shared (coalesced 128-byte row segments), under step A
         {
@@ -469,7 +490,7 @@ __global__ void __launch_bounds__(THREADS_PRE, 1)
         mbar_wait(cx.barrier(P_AFULL), uc & 1);
         TP_ACC(e_a);
         tc_fence_after();
-        // ---- u_0 = q_m o a_1 (to the operand stage), u_1 = q_m o a_0 (kept), den
+        // ---- u_0 = q_m o a_1, u_1 = q_m o a_0 (split, straight into TMEM as the A operands of step B), den
         float dd = 0.f;
 #pragma unroll
         for (int sub = 0; sub < 2; ++sub) {
@@ -477,28 +498,31 @@ __global__ void __launch_bounds__(THREADS_PRE, 1)
           tmem_ld16(lane_tm + T_A0 + 16 * sub, a0);
           tmem_ld16(lane_tm + T_A1 + 16 * sub, a1);
           tmem_ld_wait();
+          float u0h[16], u0l[16], u1h[16], u1l[16];
 #pragma unroll
           for (int q = 0; q < 4; ++q) {
             const int ch = 4 * sub + q;  // 16-byte chunk of the row slice
-            const uint32_t so = (uint32_t)((ch ^ (row & 7)) << 4);
-            const float4 qv = lds128(qm_row + so);
+            const float4 qv = lds128(qm_row + (uint32_t)((ch ^ (row & 7)) << 4));
             const float qm[4] = {(qv.x * fq.f1) * fq.f2, (qv.y * fq.f1) * fq.f2, (qv.z * fq.f1) * fq.f2, (qv.w * fq.f1) * fq.f2};
-            float u0[4];
 #pragma unroll
             for (int j = 0; j < 4; ++j) {
               const float s0 = scale2(a0[4 * q + j], fx[0]), s1 = scale2(a1[4 * q + j], fx[1]);
-              u0[j] = qm[j] * s1;
-              u1[16 * sub + 4 * q + j] = qm[j] * s0;
-              dd = fmaf(u0[j], s0, dd);
+              const float u0 = qm[j] * s1, u1 = qm[j] * s0;
+              dd = fmaf(u0, s0, dd);
+              u0h[4 * q + j] = tf32_rna(u0);
+              u0l[4 * q + j] = tf32_rna(u0 - u0h[4 * q + j]);
+              u1h[4 * q + j] = tf32_rna(u1);
+              u1l[4 * q + j] = tf32_rna(u1 - u1h[4 * q + j]);
             }
-            float4 h, l;
-            split4(make_float4(u0[0], u0[1], u0[2], u0[3]), h, l);
-            sts128(xs_row + so, h);
-            sts128(xs_row + X_PLANE + so, l);
           }
+          tmem_st16(lane_tm + T_U0 + 16 * sub, u0h);
+          tmem_st16(lane_tm + T_U0 + 64 + 16 * sub, u0l);
+          tmem_st16(lane_tm + T_A0 + 16 * sub, u1h);
+          tmem_st16(lane_tm + T_A1 + 16 * sub, u1l);
         }
         den = fma(cw, (double)dd, den);
-        fence_async_smem();
+        tmem_st_wait();
+        tc_fence_before();
         __syncwarp();
         if (lane == 0) mbar_arrive(cx.barrier(P_UFULL));
         TP_ACC(e_u);
@@ -507,20 +531,6 @@ __global__ void __launch_bounds__(THREADS_PRE, 1)
           mbar_wait(cx.barrier(P_QFULL), k);
           if (k == 0) TP_ACC(e_q0w); else TP_ACC(e_q1w);
           tc_fence_after();
-          if (k == 0) {  // U_0 has been consumed (P_QFULL): hand U_1 to the tensor pipe first, q_1 has its own TMEM columns
-#pragma unroll
-            for (int ch = 0; ch < 8; ++ch) {
-              float4 h, l;
-              split4(make_float4(u1[4 * ch], u1[4 * ch + 1], u1[4 * ch + 2], u1[4 * ch + 3]), h, l);
-              const uint32_t so = (uint32_t)((ch ^ (row & 7)) << 4);
-              sts128(xs_row + so, h);
-              sts128(xs_row + X_PLANE + so, l);
-            }
-            fence_async_smem();
-            __syncwarp();
-            if (lane == 0) mbar_arrive(cx.barrier(P_UFULL));
-            TP_ACC(e_u1);
-          }
           float mx = 0.f;
           if (need_q[k]) {
             float nn = 0.f;
