@@ -216,6 +216,17 @@ __device__ __forceinline__ void tmem_st16(uint32_t taddr, const float (&v)[16]) 
       "f"(v[11]), "f"(v[12]), "f"(v[13]), "f"(v[14]), "f"(v[15])
       : "memory");
 }
+__device__ __forceinline__ void tmem_ld8(uint32_t taddr, uint32_t (&v)[8]) {
+  asm volatile("tcgen05.ld.sync.aligned.32x32b.x8.b32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
+               : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7])
+               : "r"(taddr)
+               : "memory");
+}
+__device__ __forceinline__ void tmem_st8(uint32_t taddr, const float (&v)[8]) {
+  asm volatile("tcgen05.st.sync.aligned.32x32b.x8.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8};" ::"r"(taddr), "f"(v[0]), "f"(v[1]),
+               "f"(v[2]), "f"(v[3]), "f"(v[4]), "f"(v[5]), "f"(v[6]), "f"(v[7])
+               : "memory");
+}
 __device__ __forceinline__ void tmem_st_wait() { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
 // D[tmem] (+)= A[tmem] . B[smem]^T : A = 128 lanes x 8 consecutive 32-bit columns (one k-step)
 __device__ __forceinline__ void umma_ta(uint32_t d_tmem, uint32_t a_tmem, uint64_t b_desc, uint32_t accumulate) {
@@ -467,6 +478,7 @@ __global__ void __launch_bounds__(THREADS_PRE, 1)
       const Pow2Pair<float> fx[2] = {pow2_pair(-pending_exp<float>(it.p_scale[0], p, P, C), 0.f),
                                      pow2_pair(-pending_exp<float>(it.p_scale[1], p, P, C), 0.f)};
       double den = 0.0, num[2] = {0.0, 0.0};
+      const bool one_factor = __all_sync(0xffffffffu, fq.f2 == 1.f && fx[0].f2 == 1.f && fx[1].f2 == 1.f);
       for (int c = 0; c < C; ++c, ++uc) {
         const double cw = catw[c], cwr = catw[c] * catr[c];
         TP_ACC(e_end);
@@ -493,32 +505,41 @@ __global__ void __launch_bounds__(THREADS_PRE, 1)
         // ---- u_0 = q_m o a_1, u_1 = q_m o a_0 (split, straight into TMEM as the A operands of step B), den
         float dd = 0.f;
 #pragma unroll
-        for (int sub = 0; sub < 2; ++sub) {
-          uint32_t a0[16], a1[16];
-          tmem_ld16(lane_tm + T_A0 + 16 * sub, a0);
-          tmem_ld16(lane_tm + T_A1 + 16 * sub, a1);
-          tmem_ld_wait();
-          float u0h[16], u0l[16], u1h[16], u1l[16];
+        for (int sub = 0; sub < 4; ++sub) {  // 8 states at a time keeps the split operands in registers
+          uint32_t a0[8], a1[8];
+          tmem_ld8(lane_tm + T_A0 + 8 * sub, a0);
+          tmem_ld8(lane_tm + T_A1 + 8 * sub, a1);
+          float qm[8];
 #pragma unroll
-          for (int q = 0; q < 4; ++q) {
-            const int ch = 4 * sub + q;  // 16-byte chunk of the row slice
-            const float4 qv = lds128(qm_row + (uint32_t)((ch ^ (row & 7)) << 4));
-            const float qm[4] = {(qv.x * fq.f1) * fq.f2, (qv.y * fq.f1) * fq.f2, (qv.z * fq.f1) * fq.f2, (qv.w * fq.f1) * fq.f2};
-#pragma unroll
-            for (int j = 0; j < 4; ++j) {
-              const float s0 = scale2(a0[4 * q + j], fx[0]), s1 = scale2(a1[4 * q + j], fx[1]);
-              const float u0 = qm[j] * s1, u1 = qm[j] * s0;
-              dd = fmaf(u0, s0, dd);
-              u0h[4 * q + j] = tf32_rna(u0);
-              u0l[4 * q + j] = tf32_rna(u0 - u0h[4 * q + j]);
-              u1h[4 * q + j] = tf32_rna(u1);
-              u1l[4 * q + j] = tf32_rna(u1 - u1h[4 * q + j]);
-            }
+          for (int q = 0; q < 2; ++q) {
+            const float4 qv = lds128(qm_row + (uint32_t)(((2 * sub + q) ^ (row & 7)) << 4));
+            qm[4 * q] = qv.x; qm[4 * q + 1] = qv.y; qm[4 * q + 2] = qv.z; qm[4 * q + 3] = qv.w;
           }
-          tmem_st16(lane_tm + T_U0 + 16 * sub, u0h);
-          tmem_st16(lane_tm + T_U0 + 64 + 16 * sub, u0l);
-          tmem_st16(lane_tm + T_A0 + 16 * sub, u1h);
-          tmem_st16(lane_tm + T_A1 + 16 * sub, u1l);
+          tmem_ld_wait();
+          float u0h[8], u0l[8], u1h[8], u1l[8];
+#pragma unroll
+          for (int j = 0; j < 8; ++j) {
+            float s0, s1, qs;
+            if (one_factor) {  // the usual case: every pending exponent fits one power-of-two factor
+              s0 = __uint_as_float(a0[j]) * fx[0].f1;
+              s1 = __uint_as_float(a1[j]) * fx[1].f1;
+              qs = qm[j] * fq.f1;
+            } else {
+              s0 = scale2(a0[j], fx[0]);
+              s1 = scale2(a1[j], fx[1]);
+              qs = (qm[j] * fq.f1) * fq.f2;
+            }
+            const float u0 = qs * s1, u1 = qs * s0;
+            dd = fmaf(u0, s0, dd);
+            u0h[j] = tf32_rna(u0);
+            u0l[j] = tf32_rna(u0 - u0h[j]);
+            u1h[j] = tf32_rna(u1);
+            u1l[j] = tf32_rna(u1 - u1h[j]);
+          }
+          tmem_st8(lane_tm + T_U0 + 8 * sub, u0h);
+          tmem_st8(lane_tm + T_U0 + 64 + 8 * sub, u0l);
+          tmem_st8(lane_tm + T_A0 + 8 * sub, u1h);
+          tmem_st8(lane_tm + T_A1 + 8 * sub, u1l);
         }
         den = fma(cw, (double)dd, den);
         tmem_st_wait();
