@@ -118,3 +118,31 @@ def test_repeatable_bitwise():
         assert a[0] == b[0] and np.array_equal(a[1], b[1]) and np.array_equal(ga, gb)
     finally:
         ev.close()
+
+
+@pytest.mark.parametrize("arm", [0, plk.FLAG_NO_TCGEN05], ids=["tcgen05", "mma_sync"])
+def test_tensor_fp32_unfused_no_level_batch_and_repeatable(arm):
+    """fp32 tensor path (tcgen05 / TMEM kernels and the mma.sync arm): plk_update_pre_partials (no gradient slots, tip
+    pre-order partials stored) + plk_branch_derivatives agrees with the fused call; one launch per operation agrees
+    with level batching bit for bit; two evaluations give identical bits (fixed summation order)."""
+    wl = workloads.config(2, n_tips=10, n_patterns=300)
+    base = plk.FLAG_TENSOR_CORES | arm
+    out = []
+    for flags, unfused in ((base, False), (base, True), (base | plk.FLAG_NO_LEVEL_BATCH, False)):
+        ev = Evaluator(wl, precision=plk.FP32, flags=flags, store_tip_pre=unfused)
+        try:
+            logl, site = ev.log_likelihood()
+            g = ev.gradient_unfused() if unfused else ev.gradient()
+            if not unfused and flags == base:
+                logl2, site2 = ev.log_likelihood()
+                g2 = ev.gradient()
+                assert logl == logl2 and np.array_equal(site, site2) and np.array_equal(g, g2)
+            out.append((logl, site, g))
+        finally:
+            ev.close()
+    for logl, site, g in out[1:]:
+        assert np.array_equal(site, out[0][1])
+        assert np.allclose(g, out[0][2], rtol=1e-5, atol=1e-5 * np.max(np.abs(out[0][2])))
+    ref = orc.evaluate(wl)
+    strict, rel_cond, norm = orc.gradient_errors(out[1][2], ref)
+    assert rel_cond <= 1e-4 and norm <= 1e-4
