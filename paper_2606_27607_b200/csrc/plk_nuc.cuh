@@ -194,6 +194,83 @@ __device__ __forceinline__ void post4_cell(const DevOp& op, const T* __restrict_
   }
 }
 
+// U chunks at once (the walk kernels, fp32): the operand loads of all U patterns are issued before any arithmetic, and
+// a matrix row read from shared memory serves all U of them -- fewer instructions per byte, which is what bounds the
+// 4-byte kernels (same instruction count per cell as fp64 for half the bytes).
+template <typename T, int U>
+__device__ __forceinline__ void contrib4_multi(int kind, const void* ptr, const T* __restrict__ M, int c, const int (&p)[U],
+                                               int P, T (&a)[U][4]) {
+  if (kind == KIND_STATES) {
+#pragma unroll
+    for (int u = 0; u < U; ++u) {
+      const int z = p[u] < P ? static_cast<const uint8_t*>(ptr)[p[u]] : 4;
+#pragma unroll
+      for (int s = 0; s < 4; ++s) a[u][s] = z < 4 ? M[s * 4 + z] : T(1);
+    }
+  } else {
+    T x[U][4];
+#pragma unroll
+    for (int u = 0; u < U; ++u) {
+      if (p[u] < P) {
+        operand4<T>(kind, ptr, c, p[u], P, x[u]);
+      } else {
+#pragma unroll
+        for (int s = 0; s < 4; ++s) x[u][s] = T(0);
+      }
+    }
+#pragma unroll
+    for (int s = 0; s < 4; ++s) {
+      T r[4];
+      ld4(M + 4 * s, r);
+#pragma unroll
+      for (int u = 0; u < U; ++u) a[u][s] = r[0] * x[u][0] + r[1] * x[u][1] + r[2] * x[u][2] + r[3] * x[u][3];
+    }
+  }
+}
+template <typename T, int C, int U>
+__device__ __forceinline__ void post4_cells(const DevOp& op, const T* __restrict__ sM, int P, const int (&p)[U], int g) {
+  using Mp = NucMap<C>;
+  constexpr int MS = NucMat<T>::STRIDE;
+  T r[U][Mp::CPT][4];
+  T mx[U];
+#pragma unroll
+  for (int u = 0; u < U; ++u) mx[u] = T(0);
+#pragma unroll
+  for (int i = 0; i < Mp::CPT; ++i) {
+    const int c = g * Mp::CPT + i;
+    T a[U][4], b[U][4];
+    contrib4_multi<T, U>(op.kind[0], op.child[0], sM + c * MS, c, p, P, a);
+    contrib4_multi<T, U>(op.kind[1], op.child[1], sM + (C + c) * MS, c, p, P, b);
+#pragma unroll
+    for (int u = 0; u < U; ++u)
+#pragma unroll
+      for (int s = 0; s < 4; ++s) {
+        r[u][i][s] = p[u] < P ? a[u][s] * b[u][s] : T(0);
+        mx[u] = fmax(mx[u], r[u][i][s]);
+      }
+  }
+#pragma unroll
+  for (int u = 0; u < U; ++u) {
+    const bool live = p[u] < P;
+    if (op.scale != nullptr) {
+      const int e = exp_of(group_max<T, Mp::LP>(mx[u]));
+      if (e != 0) {
+        const Pow2Pair<T> f = pow2_pair(-e, T(0));
+#pragma unroll
+        for (int i = 0; i < Mp::CPT; ++i)
+#pragma unroll
+          for (int s = 0; s < 4; ++s) r[u][i][s] = (r[u][i][s] * f.f1) * f.f2;
+      }
+      if (live && g == 0) static_cast<int16_t*>(op.scale)[p[u]] = (int16_t)e;
+    }
+    if (live) {
+      T* dest = static_cast<T*>(op.dest);
+#pragma unroll
+      for (int i = 0; i < Mp::CPT; ++i) st4(dest + ((size_t)(g * Mp::CPT + i) * P + p[u]) * 4, r[u][i]);
+    }
+  }
+}
+
 template <typename T, int C>
 __global__ void __launch_bounds__(NUC_THREADS) k_post4(const DevOp* __restrict__ ops, int P) {
   using Mp = NucMap<C>;
@@ -235,8 +312,14 @@ __global__ void __launch_bounds__(NUC_THREADS) k_post4_walk(const DevOp* __restr
       if (threadIdx.x < OP_WORDS) opw = reinterpret_cast<const uint32_t*>(ops + i + 1)[threadIdx.x];
     }
     const DevOp op = sOp[cur];
-    for (int chunk = warp < total_warps ? warp : n_chunks; chunk < n_chunks; chunk += total_warps)
-      post4_cell<T, C>(op, sM[cur], P, chunk * Mp::PPW + pl, g);
+    int chunk = warp < total_warps ? warp : n_chunks;
+    if (sizeof(T) == 4) {  // two chunks per pass (see post4_cells)
+      for (; chunk + total_warps < n_chunks; chunk += 2 * total_warps) {
+        const int pp[2] = {chunk * Mp::PPW + pl, (chunk + total_warps) * Mp::PPW + pl};
+        post4_cells<T, C, 2>(op, sM[cur], P, pp, g);
+      }
+    }
+    for (; chunk < n_chunks; chunk += total_warps) post4_cell<T, C>(op, sM[cur], P, chunk * Mp::PPW + pl, g);
     if (i + 1 < n_ops) {
       st.store(sM[cur ^ 1]);
       if (threadIdx.x < OP_WORDS) reinterpret_cast<uint32_t*>(&sOp[cur ^ 1])[threadIdx.x] = opw;
