@@ -14,13 +14,17 @@
 // deferred power-of-two rescaling, fp64 category / pattern sums.
 //
 // Organisation.  One persistent CTA per SM walks a contiguous range of units.  Shared memory (192 KB): ONE operand
-// stage (hi + lo planes of a 128 x 64 tile, 128-byte-swizzled K-major) that successively holds X_0, X_1, U_0, U_1;
-// M_0, M_1, Q as hi + lo planes; the q_m tile (raw fp32, same swizzle), whose 4 KB slices double as the store stage
-// of the epilogue warp that read them.  TMEM: a_0, a_1, Qx_0, Qx_1 (4 x 64 columns) + q_k (64 columns).
-// Roles: warps 0-7 epilogue (warp 4h + q: patterns 32q.., states 32h..), warps 8-11 producers, warp 12 MMA issue.
-// The phases of one (unit, category) are strictly ordered (X_0 -> A -> X_1 -> A -> u -> U_0 -> B -> q_0 -> U_1 -> B ->
-// q_1); every hand-over is an mbarrier whose completions are counted identically by all roles, and every phase
-// arrives / commits even when it has nothing to do, so parities stay in step.
+// stage (hi + lo planes of a 128 x 64 tile, 128-byte-swizzled K-major) that holds X_0, then X_1; M_0, M_1, Q as hi + lo
+// planes (the M_k slots are re-staged with M_k^T between step A and step B); the q_m tile (raw fp32, same swizzle),
+// each 4 KB slice loaded by the epilogue warp that reads it and reused as that warp's store stage.
+// TMEM (512 columns): a_0, a_1, Qx_0, Qx_1, q_0, q_1 (64 each) + U_0 as hi / lo planes (128); the epilogue writes the
+// split u_k with tcgen05.st -- U_1 over the a_0 / a_1 columns its thread has just consumed -- and step B reads its A
+// operand from tensor memory.
+// Roles (16 warps): 0-7 epilogue (warp 4h + q: patterns 32q.., states 32h..), 8-11 tile producers (X_0, X_1; the next
+// tile is always in registers), 12-14 matrix stagers (Q once, M_k, M_k^T; L2 prefetch of the next round's tiles),
+// 15 MMA issue.  The phases of one (unit, category) are ordered X_0 -> A -> X_1 -> A -> u -> B, B -> q_0, q_1; every
+// hand-over is an mbarrier whose completions all roles count identically, and every phase arrives / commits even when
+// it has nothing to do, so parities stay in step.
 #pragma once
 #include "plk_tc5.cuh"
 
