@@ -402,7 +402,8 @@ __global__ void __launch_bounds__(THREADS_PRE, 1)
           if (k == 0) TP_ACC(m_x0); else TP_ACC(m_x1);
           tc_fence_after();
 #pragma unroll
-          for (int w = 0; w < 2; ++w) {  // w = 0: M_k, w = 1: Q
+          for (int ww = 0; ww < 2; ++ww) {  // w = 0: M_k, w = 1: Q.  Order Qx_0, a_0, a_1, Qx_1: the u-phase needs only the
+            const int w = k == 0 ? 1 - ww : ww;  // a_k, so it is released before Qx_1 is on the pipe
             const uint32_t d = tmem_base + (w == 0 ? (k == 0 ? T_A0 : T_A1) : (k == 0 ? T_QX0 : T_QX1));
             const uint32_t mp = cx.smem + OFF_MS + (w == 0 ? 2 * k : 4) * M_PLANE;
             const uint64_t dmhi = make_desc(mp), dmlo = make_desc(mp + M_PLANE);
@@ -420,11 +421,13 @@ __global__ void __launch_bounds__(THREADS_PRE, 1)
               umma<IDESC>(d, dxhi + koff(ks, TP), dmhi + koff(ks, 64), 1);
               acc = 1;
             }
+            if (k == 1 && w == 0) {  // a_0 and a_1 complete; M_0 / M_1 no longer read
+              umma_commit(cx.barrier(P_AFULL));
+              umma_commit(cx.barrier(P_ADONE));
+            }
           }
           umma_commit(cx.barrier(P_XFREE));  // the producers' cue for X_1 / for X_0 of the next round
         }
-        umma_commit(cx.barrier(P_AFULL));
-        umma_commit(cx.barrier(P_ADONE));
         TP_ACC(m_is);
         mbar_wait(cx.barrier(P_UFULL), uc & 1);
         TP_ACC(m_u0);
