@@ -52,7 +52,7 @@ constexpr uint32_t OFF_BARS = OFF_MX + TP * 4;
 constexpr uint32_t SMEM_USED_PRE = OFF_BARS + 256;
 constexpr size_t SMEM_BYTES_PRE = SMEM_USED_PRE + 1024;
 enum { P_XFULL = 0, P_XFREE, P_UFULL, P_AFULL, P_QFULL, P_MFULL, P_MFREE, P_TFREE, P_ADONE, P_MTFULL,
-       P_MTFULL1, P_MFULL1, P_M0FREE, P_TMEM_PTR };
+       P_MTFULL1, P_MFULL1, P_M0FREE, P_TFREE0, P_TMEM_PTR };
 // TMEM columns.  U_0 (hi, lo) has its own 128 columns; U_1 (hi, lo) overwrites a_0 / a_1, which the thread that
 // writes it has just consumed.
 constexpr uint32_t T_A0 = 0, T_A1 = 64, T_QX0 = 128, T_QX1 = 192, T_Q0 = 256, T_Q1 = 320, T_U0 = 384;
@@ -279,6 +279,7 @@ __global__ void __launch_bounds__(THREADS_PRE, 1)
     mbar_init(cx.barrier(P_MTFULL1), AUX_W);
     mbar_init(cx.barrier(P_MFULL1), AUX_W);
     mbar_init(cx.barrier(P_M0FREE), 1);
+    mbar_init(cx.barrier(P_TFREE0), EPI_W);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   if (warp == N_W - 1) {
@@ -390,7 +391,9 @@ __global__ void __launch_bounds__(THREADS_PRE, 1)
       const bool need_q[2] = {it.q[0] != nullptr || it.slot[0] >= 0, it.q[1] != nullptr || it.slot[1] >= 0};
       for (int c = 0; c < C; ++c, ++uc) {
         TP_ACC(m_is);
-        if (uc > 0) mbar_wait(cx.barrier(P_TFREE), (uc - 1) & 1);
+        // Qx_0 (first product of step A) may be overwritten once the previous round's q_0 epilogue has read it; a_0 / a_1
+        // are free as soon as the previous step B has run (in-order pipe); Qx_1 waits for the q_1 epilogue further down
+        if (uc > 0) mbar_wait(cx.barrier(P_TFREE0), (uc - 1) & 1);
         TP_ACC(m_tf);
 
 #pragma unroll
@@ -404,6 +407,10 @@ __global__ void __launch_bounds__(THREADS_PRE, 1)
 #pragma unroll
           for (int ww = 0; ww < 2; ++ww) {  // w = 0: M_k, w = 1: Q.  Order Qx_0, a_0, a_1, Qx_1: the u-phase needs only the
             const int w = k == 0 ? 1 - ww : ww;  // a_k, so it is released before Qx_1 is on the pipe
+            if (k == 1 && w == 1 && uc > 0) {
+              mbar_wait(cx.barrier(P_TFREE), (uc - 1) & 1);
+              tc_fence_after();
+            }
             const uint32_t d = tmem_base + (w == 0 ? (k == 0 ? T_A0 : T_A1) : (k == 0 ? T_QX0 : T_QX1));
             const uint32_t mp = cx.smem + OFF_MS + (w == 0 ? 2 * k : 4) * M_PLANE;
             const uint64_t dmhi = make_desc(mp), dmlo = make_desc(mp + M_PLANE);
@@ -584,10 +591,8 @@ __global__ void __launch_bounds__(THREADS_PRE, 1)
             if (want[k]) num[k] = fma(cwr, (double)nn, num[k]);
           }
           tc_fence_before();
-          if (k == 1) {  // every accumulator of this round has been read: step A of the next round may start
-            __syncwarp();
-            if (lane == 0) mbar_arrive(cx.barrier(P_TFREE));
-          }
+          __syncwarp();  // q_k and Qx_k of this round have been read: their columns may be overwritten
+          if (lane == 0) mbar_arrive(cx.barrier(k == 0 ? P_TFREE0 : P_TFREE));
           if (it.q[k] != nullptr) {
             if (half == 1) smx[row] = mx;
             __syncwarp();
