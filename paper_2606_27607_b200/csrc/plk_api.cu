@@ -469,7 +469,7 @@ int launch_pre4_tma(plk_instance* in, const DevPreItem* d_items, int n, const T*
 template <typename T, int CLS>
 int launch_pre4_lean_c(plk_instance* in, const DevPreItem* d_items, int n, const T* Q, double* site) {
   const Layout& L = in->L;
-  using St = NtStage<T, NL_C, 3, true>;
+  using St = NtStage<T, NL_C, 3, true, NlRows<T>::R>;
   const size_t smem = (size_t)NT_NS * St::BYTES;
   static int bps = 0;  // per instantiation
   if (bps == 0) {

@@ -44,13 +44,51 @@ struct NlWalk {
   }
 };
 
+// rows per consumer lane: the 4-byte instantiation takes two patterns per lane (tile = 64 patterns), so that a matrix
+// row read from shared memory serves both and twice the operand bytes are in flight per instruction -- the fp32
+// kernels are bound by instructions per byte (same instruction count per cell as fp64 for half the bytes)
+template <typename T>
+struct NlRows {
+  static constexpr int R = sizeof(T) == 4 ? 2 : 1;
+};
+
+// a[u][s] = sum_x M[s][x] v[u][x] / sum_x M[x][s] v[u][x] for R vectors at once
+template <typename T, int R>
+__device__ __forceinline__ void mv4r(const T* __restrict__ M, const T (&v)[R][4], T (&a)[R][4]) {
+#pragma unroll
+  for (int s = 0; s < 4; ++s) {
+    T r[4];
+    ld4(M + 4 * s, r);
+#pragma unroll
+    for (int u = 0; u < R; ++u) a[u][s] = r[0] * v[u][0] + r[1] * v[u][1] + r[2] * v[u][2] + r[3] * v[u][3];
+  }
+}
+template <typename T, int R>
+__device__ __forceinline__ void mvt4r(const T* __restrict__ M, const T (&v)[R][4], T (&a)[R][4]) {
+  T r[4];
+  ld4(M, r);
+#pragma unroll
+  for (int u = 0; u < R; ++u)
+#pragma unroll
+    for (int s = 0; s < 4; ++s) a[u][s] = r[s] * v[u][0];
+#pragma unroll
+  for (int x = 1; x < 4; ++x) {
+    ld4(M + 4 * x, r);
+#pragma unroll
+    for (int u = 0; u < R; ++u)
+#pragma unroll
+      for (int s = 0; s < 4; ++s) a[u][s] = fma(r[s], v[u][x], a[u][s]);
+  }
+}
+
 template <typename T, int CLS>
 __global__ void __launch_bounds__(NT_THREADS, 4) k_pre4_lean(const DevPreItem* __restrict__ items, int n_items, int P,
                                                              const T* __restrict__ Qg, NucModel md,
                                                              double* __restrict__ grad_partial, int n_part) {
   constexpr int C = NL_C;
+  constexpr int R = NlRows<T>::R;
   constexpr bool TIP0 = CLS == 2, TIP1 = CLS >= 1;
-  using St = NtStage<T, C, 3, true>;
+  using St = NtStage<T, C, 3, true, R>;
   constexpr int MS = St::MS, TP = St::TP;
   extern __shared__ __align__(128) unsigned char nt_smem[];
   __shared__ __align__(8) uint64_t full[NT_NS], empty[NT_NS];
@@ -84,15 +122,14 @@ __global__ void __launch_bounds__(NT_THREADS, 4) k_pre4_lean(const DevPreItem* _
         const void* ptr[3] = {it->qm, it->p[0], it->p[1]};
         const int kind[3] = {KIND_PARTIALS, TIP0 ? KIND_STATES : KIND_PARTIALS, TIP1 ? KIND_STATES : KIND_PARTIALS};
         const void* mat[2] = {it->mat[0], it->mat[1]};
-        nt_fill<T, C, 3, true>(nt_smem + (size_t)(j % NT_NS) * St::BYTES, &full[j % NT_NS], it, sizeof(DevPreItem), ptr,
-                               kind, mat, md.weights, P, p0, n);
+        nt_fill<T, C, 3, true, R>(nt_smem + (size_t)(j % NT_NS) * St::BYTES, &full[j % NT_NS], it, sizeof(DevPreItem),
+                                  ptr, kind, mat, md.weights, P, p0, n);
       }
     }
     return;
   }
-  // ---- consumers
+  // ---- consumers: lane = 8 g + pl takes category g of patterns warp * 8 + pl + 32 u, u < R
   const int g = lane >> 3, pl = lane & 7;
-  const int r = warp * 8 + pl;
   const double cw = md.catw[g], cwr = cw * md.catr[g];
   for (int j = 0; j < J; ++j) {
     const int s = j % NT_NS;
@@ -103,95 +140,116 @@ __global__ void __launch_bounds__(NT_THREADS, 4) k_pre4_lean(const DevPreItem* _
     const T* sM0 = reinterpret_cast<const T*>(stage + St::OFF_MATS) + g * MS;
     const T* sM1 = sM0 + C * MS;
     const T* sOp = reinterpret_cast<const T*>(stage + St::OFF_OPS);
-    const bool live = r < h.n;
-    const int p = h.p0 + r;
-
-    T a0[4], a1[4], qx0[4], qx1[4];
-    if (TIP0) {
-      const int z = stage[St::OFF_ST + h.soff0 + r];
+    int r[R], p[R];
+    bool live[R];
 #pragma unroll
-      for (int x = 0; x < 4; ++x) {
-        a0[x] = z < 4 ? sM0[x * 4 + z] : T(1);
-        qx0[x] = z < 4 ? sQ[x * 4 + z] : T(0);
+    for (int u = 0; u < R; ++u) {
+      r[u] = warp * 8 + pl + 32 * u;
+      live[u] = r[u] < h.n;
+      p[u] = h.p0 + r[u];
+    }
+
+    T a0[R][4], a1[R][4], qx0[R][4], qx1[R][4];
+    if (TIP0) {
+#pragma unroll
+      for (int u = 0; u < R; ++u) {
+        const int z = stage[St::OFF_ST + h.soff0 + r[u]];
+#pragma unroll
+        for (int x = 0; x < 4; ++x) {
+          a0[u][x] = z < 4 ? sM0[x * 4 + z] : T(1);
+          qx0[u][x] = z < 4 ? sQ[x * 4 + z] : T(0);
+        }
       }
     } else {
-      T x0[4];
-      ld4(sOp + ((C + g) * TP + r) * 4, x0);
-      mv4<T>(sM0, x0, a0);
-      mv4<T>(sQ, x0, qx0);
+      T x0[R][4];
+#pragma unroll
+      for (int u = 0; u < R; ++u) ld4(sOp + ((C + g) * TP + r[u]) * 4, x0[u]);
+      mv4r<T, R>(sM0, x0, a0);
+      mv4r<T, R>(sQ, x0, qx0);
     }
     if (TIP1) {
-      const int z = stage[St::OFF_ST + (TP + 16) + h.soff1 + r];
 #pragma unroll
-      for (int x = 0; x < 4; ++x) {
-        a1[x] = z < 4 ? sM1[x * 4 + z] : T(1);
-        qx1[x] = z < 4 ? sQ[x * 4 + z] : T(0);
+      for (int u = 0; u < R; ++u) {
+        const int z = stage[St::OFF_ST + (TP + 16) + h.soff1 + r[u]];
+#pragma unroll
+        for (int x = 0; x < 4; ++x) {
+          a1[u][x] = z < 4 ? sM1[x * 4 + z] : T(1);
+          qx1[u][x] = z < 4 ? sQ[x * 4 + z] : T(0);
+        }
       }
     } else {
-      T x1[4];
-      ld4(sOp + ((2 * C + g) * TP + r) * 4, x1);
-      mv4<T>(sM1, x1, a1);
-      mv4<T>(sQ, x1, qx1);
-    }
-    T qm[4], u0[4], u1[4];
-    ld4(sOp + (g * TP + r) * 4, qm);
-    T dd = T(0);
+      T x1[R][4];
 #pragma unroll
-    for (int x = 0; x < 4; ++x) {
-      u0[x] = qm[x] * a1[x];
-      u1[x] = qm[x] * a0[x];
-      dd = fma(u0[x], a0[x], dd);
+      for (int u = 0; u < R; ++u) ld4(sOp + ((2 * C + g) * TP + r[u]) * 4, x1[u]);
+      mv4r<T, R>(sM1, x1, a1);
+      mv4r<T, R>(sQ, x1, qx1);
     }
-    T q0[4], q1[4];
-    mvt4<T>(sM0, u0, q0);
-    mvt4<T>(sM1, u1, q1);
-    T n0 = q0[0] * qx0[0], n1 = q1[0] * qx1[0];
+    T u0[R][4], u1[R][4], dd[R];
 #pragma unroll
-    for (int x = 1; x < 4; ++x) {
-      n0 = fma(q0[x], qx0[x], n0);
-      n1 = fma(q1[x], qx1[x], n1);
-    }
-    // ---- rescaled q_k of the internal children (power-of-two factor, discarded: it cancels in num / den)
-    if (!TIP0) {
-      int key = max(max(max_key(q0[0]), max_key(q0[1])), max(max_key(q0[2]), max_key(q0[3])));
-      key = max(key, 0);
-      key = max(key, __shfl_xor_sync(0xffffffffu, key, 8));
-      key = max(key, __shfl_xor_sync(0xffffffffu, key, 16));
-      const T f = pow2_neg(exp_of_key(key, T(0)), T(0));
-      if (live) {
-        T v[4];
+    for (int u = 0; u < R; ++u) {
+      T qm[4];
+      ld4(sOp + (g * TP + r[u]) * 4, qm);
+      dd[u] = T(0);
 #pragma unroll
-        for (int x = 0; x < 4; ++x) v[x] = q0[x] * f;
-        st4(static_cast<T*>(it.q[0]) + ((size_t)g * P + p) * 4, v);
+      for (int x = 0; x < 4; ++x) {
+        u0[u][x] = qm[x] * a1[u][x];
+        u1[u][x] = qm[x] * a0[u][x];
+        dd[u] = fma(u0[u][x], a0[u][x], dd[u]);
       }
     }
-    if (!TIP1) {
-      int key = max(max(max_key(q1[0]), max_key(q1[1])), max(max_key(q1[2]), max_key(q1[3])));
-      key = max(key, 0);
-      key = max(key, __shfl_xor_sync(0xffffffffu, key, 8));
-      key = max(key, __shfl_xor_sync(0xffffffffu, key, 16));
-      const T f = pow2_neg(exp_of_key(key, T(0)), T(0));
-      if (live) {
-        T v[4];
-#pragma unroll
-        for (int x = 0; x < 4; ++x) v[x] = q1[x] * f;
-        st4(static_cast<T*>(it.q[1]) + ((size_t)g * P + p) * 4, v);
-      }
-    }
-    // ---- category sums: den on every lane, num_0 on the lanes of g = 0, num_1 on those of g = 1
-    double den = cw * (double)dd, m0 = cwr * (double)n0, m1 = cwr * (double)n1;
-    den += __shfl_xor_sync(0xffffffffu, den, 16);
-    m0 += __shfl_xor_sync(0xffffffffu, m0, 16);
-    m1 += __shfl_xor_sync(0xffffffffu, m1, 16);
-    den += __shfl_xor_sync(0xffffffffu, den, 8);
-    const bool odd = g & 1;
-    const double got = __shfl_xor_sync(0xffffffffu, odd ? m0 : m1, 8);
-    const double num = (odd ? m1 : m0) + got;
+    T q0[R][4], q1[R][4];
+    mvt4r<T, R>(sM0, u0, q0);
+    mvt4r<T, R>(sM1, u1, q1);
     double contrib = 0.0;
-    if (live && g < 2) {
-      const double ratio = num / den;
-      if (md.site_out != nullptr) md.site_out[(size_t)it.slot[g] * P + p] = ratio;
-      contrib = reinterpret_cast<const double*>(stage + St::OFF_WTS)[r] * ratio;
+#pragma unroll
+    for (int u = 0; u < R; ++u) {
+      T n0 = q0[u][0] * qx0[u][0], n1 = q1[u][0] * qx1[u][0];
+#pragma unroll
+      for (int x = 1; x < 4; ++x) {
+        n0 = fma(q0[u][x], qx0[u][x], n0);
+        n1 = fma(q1[u][x], qx1[u][x], n1);
+      }
+      // ---- rescaled q_k of the internal children (power-of-two factor, discarded: it cancels in num / den)
+      if (!TIP0) {
+        int key = max(max(max_key(q0[u][0]), max_key(q0[u][1])), max(max_key(q0[u][2]), max_key(q0[u][3])));
+        key = max(key, 0);
+        key = max(key, __shfl_xor_sync(0xffffffffu, key, 8));
+        key = max(key, __shfl_xor_sync(0xffffffffu, key, 16));
+        const T f = pow2_neg(exp_of_key(key, T(0)), T(0));
+        if (live[u]) {
+          T v[4];
+#pragma unroll
+          for (int x = 0; x < 4; ++x) v[x] = q0[u][x] * f;
+          st4(static_cast<T*>(it.q[0]) + ((size_t)g * P + p[u]) * 4, v);
+        }
+      }
+      if (!TIP1) {
+        int key = max(max(max_key(q1[u][0]), max_key(q1[u][1])), max(max_key(q1[u][2]), max_key(q1[u][3])));
+        key = max(key, 0);
+        key = max(key, __shfl_xor_sync(0xffffffffu, key, 8));
+        key = max(key, __shfl_xor_sync(0xffffffffu, key, 16));
+        const T f = pow2_neg(exp_of_key(key, T(0)), T(0));
+        if (live[u]) {
+          T v[4];
+#pragma unroll
+          for (int x = 0; x < 4; ++x) v[x] = q1[u][x] * f;
+          st4(static_cast<T*>(it.q[1]) + ((size_t)g * P + p[u]) * 4, v);
+        }
+      }
+      // ---- category sums: den on every lane, num_0 on the lanes of g = 0, num_1 on those of g = 1
+      double den = cw * (double)dd[u], m0 = cwr * (double)n0, m1 = cwr * (double)n1;
+      den += __shfl_xor_sync(0xffffffffu, den, 16);
+      m0 += __shfl_xor_sync(0xffffffffu, m0, 16);
+      m1 += __shfl_xor_sync(0xffffffffu, m1, 16);
+      den += __shfl_xor_sync(0xffffffffu, den, 8);
+      const bool odd = g & 1;
+      const double got = __shfl_xor_sync(0xffffffffu, odd ? m0 : m1, 8);
+      const double num = (odd ? m1 : m0) + got;
+      if (live[u] && g < 2) {
+        const double ratio = num / den;
+        if (md.site_out != nullptr) md.site_out[(size_t)it.slot[g] * P + p[u]] = ratio;
+        contrib += reinterpret_cast<const double*>(stage + St::OFF_WTS)[r[u]] * ratio;
+      }
     }
     const int slot = it.slot[g & 1];
     __syncwarp();

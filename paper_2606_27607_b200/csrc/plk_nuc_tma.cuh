@@ -108,10 +108,10 @@ struct NtHdr {
   int32_t p0, n, soff0, soff1;  // first pattern, pattern count, offset of pattern p0 inside st[0] / st[1]
 };
 
-template <typename T, int C, int NOPS, bool WTS>
+template <typename T, int C, int NOPS, bool WTS, int R = 1>  // R = pattern rows per consumer lane
 struct NtStage {
   using Mp = NucMap<C>;
-  static constexpr int TP = Mp::PPW * NT_CW;       // patterns per tile
+  static constexpr int TP = Mp::PPW * NT_CW * R;   // patterns per tile
   static constexpr int SEG = TP * 4;               // reals per (operand, category) segment
   static constexpr int MS = NucMat<T>::STRIDE;
   static constexpr int OFF_HDR = 0;
@@ -173,11 +173,11 @@ struct NtTiles {
 // ---- producer: fill one stage with one tile (single lane) ------------------------------------------------------
 // operand o of NOPS: ptr[o], kind[o]; operands NOPS-2 and NOPS-1 are the two children (their compact states go to
 // st[0] / st[1]); an operand before them (the parent's pre-order partials) is always KIND_PARTIALS.
-template <typename T, int C, int NOPS, bool WTS>
+template <typename T, int C, int NOPS, bool WTS, int R = 1>
 __device__ __forceinline__ void nt_fill(unsigned char* stage, uint64_t* full, const void* desc, uint32_t desc_bytes,
                                         const void* const* ptr, const int* kind, const void* const* mat,
                                         const double* weights, int P, int p0, int n) {
-  using St = NtStage<T, C, NOPS, WTS>;
+  using St = NtStage<T, C, NOPS, WTS, R>;
   const uint32_t seg_bytes = (uint32_t)n * 4 * sizeof(T);
   const uint32_t mat_bytes = 16 * sizeof(T);
   NtHdr h;
