@@ -41,7 +41,7 @@ struct Layout {
   int n_tiles, max_grad;
   size_t off_post, off_compact, off_pre, off_pre_mx, off_matrix, off_eigen, off_scale, off_weights, off_pi,
       off_rates, off_catw, off_site, off_block_partial, off_grad_partial, off_grad_out, off_logl, off_site_deriv,
-      off_stage, off_ring, off_matrix_t, total;
+      off_stage, off_ring, off_matrix_t, off_matrix_d, total;
   size_t stage_bytes;
 };
 
@@ -109,6 +109,8 @@ bool compute_layout(const plk_config& c, Layout& L) {
                          !(c.flags & PLK_FLAG_NO_TCGEN05))
                             ? (size_t)c.matrix_buffer_count * L.matrix_bytes
                             : 0);
+  // derivative matrices D = M Q of the 4-state specialised gradient kernels (plk_nuc_lean.cuh, compact-tip children)
+  L.off_matrix_d = take(L.SP == 4 ? (size_t)c.matrix_buffer_count * L.matrix_bytes : 0);
   L.total = o;
   return true;
 }
@@ -480,7 +482,9 @@ int launch_pre4_lean_c(plk_instance* in, const DevPreItem* d_items, int n, const
   const long long n_tp = (L.P + St::TP - 1) / St::TP;
   long long g = (long long)in->sm_count * bps;
   if (g > n_tp * n) g = n_tp * n;
-  k_pre4_lean<T, CLS><<<(int)g, NT_THREADS, smem, in->stream>>>(d_items, n, L.P, Q, nuc_model(in, site),
+  k_pre4_lean<T, CLS><<<(int)g, NT_THREADS, smem, in->stream>>>(d_items, n, L.P, Q,
+                                                               (long long)L.off_matrix_d - (long long)L.off_matrix,
+                                                               nuc_model(in, site),
                                                                in->at<double>(L.off_grad_partial), L.n_tiles);
   in->grad_parts = (int)n_tp * NT_CW;
   CHECK_LAUNCH(in);
@@ -1266,6 +1270,20 @@ static int pre_impl(plk_instance* in, int eigen, int root_pre, const plk_pre_op*
         using T = decltype(tag);
         return nuc_use_tma(in, true) ? launch_pre4_tma<T>(in, dit, n_items, static_cast<const T*>(Q), d_site, true)
                                : launch_pre4_walk<T>(in, dit, n_items, static_cast<const T*>(Q), d_site);
+      });
+      if (rc) return rc;
+    }
+    if (!walk && L.SP == 4 && class_start[(size_t)(n_levels - 1) * 5 + 3] > 0) {
+      // some items run on the class-specialised kernels: their compact-tip children read D = M Q (one 4 x 4 product
+      // per matrix and category, every matrix buffer; unwritten buffers give unused garbage)
+      rc = by_precision(in, [&](auto tag) -> int {
+        using T = decltype(tag);
+        const int n_buf = in->cfg.matrix_buffer_count;
+        k_deriv_matrices4<T><<<(n_buf * L.C * 16 + 255) / 256, 256, 0, in->stream>>>(
+            in->at<T>(L.off_matrix), static_cast<const T*>(Q), in->at<T>(L.off_matrix_d), n_buf, L.C,
+            L.matrix_bytes / sizeof(T));
+        CHECK_LAUNCH(in);
+        return PLK_SUCCESS;
       });
       if (rc) return rc;
     }

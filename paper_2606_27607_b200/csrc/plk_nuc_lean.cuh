@@ -44,6 +44,20 @@ struct NlWalk {
   }
 };
 
+// D[m] = M[m] Q for every 4 x 4 matrix m (16 threads each): the derivative matrices of the compact-tip children.
+// With x_k = e_z:  num_k = q_k . (Q e_z) = u_k^T M_k Q e_z = sum_x u_k[x] D_k[x][z]  -- a 4-term gather-dot instead of
+// the transposed product q_k = M_k^T u_k (which a tip never stores) followed by a dot with column z of Q.
+template <typename T>
+__global__ void __launch_bounds__(256) k_deriv_matrices4(const T* __restrict__ M, const T* __restrict__ Q, T* __restrict__ D,
+                                                         int n_buffers, int C, size_t buffer_stride /* elements */) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n_buffers * C * 16) return;
+  const int m = i >> 4, x = (i >> 2) & 3, z = i & 3;
+  const size_t base = (size_t)(m / C) * buffer_stride + (size_t)(m % C) * 16;
+  const T* Mm = M + base;
+  D[base + x * 4 + z] = Mm[x * 4] * Q[z] + Mm[x * 4 + 1] * Q[4 + z] + Mm[x * 4 + 2] * Q[8 + z] + Mm[x * 4 + 3] * Q[12 + z];
+}
+
 // rows per consumer lane: the 4-byte instantiation takes two patterns per lane (tile = 64 patterns), so that a matrix
 // row read from shared memory serves both and twice the operand bytes are in flight per instruction -- the fp32
 // kernels are bound by instructions per byte (same instruction count per cell as fp64 for half the bytes)
@@ -83,7 +97,7 @@ __device__ __forceinline__ void mvt4r(const T* __restrict__ M, const T (&v)[R][4
 
 template <typename T, int CLS>
 __global__ void __launch_bounds__(NT_THREADS, 4) k_pre4_lean(const DevPreItem* __restrict__ items, int n_items, int P,
-                                                             const T* __restrict__ Qg, NucModel md,
+                                                             const T* __restrict__ Qg, long long dmat_delta, NucModel md,
                                                              double* __restrict__ grad_partial, int n_part) {
   constexpr int C = NL_C;
   constexpr int R = NlRows<T>::R;
@@ -149,15 +163,18 @@ __global__ void __launch_bounds__(NT_THREADS, 4) k_pre4_lean(const DevPreItem* _
       p[u] = h.p0 + r[u];
     }
 
+    // compact-tip child k: a_k = column z of M_k; qx_k holds column z of D_k = M_k Q (0 for a missing state), so that
+    // num_k = u_k . qx_k and no q_k is formed (k_deriv_matrices4)
     T a0[R][4], a1[R][4], qx0[R][4], qx1[R][4];
     if (TIP0) {
+      const T* D0 = reinterpret_cast<const T*>(static_cast<const char*>(it.mat[0]) + dmat_delta) + g * 16;
 #pragma unroll
       for (int u = 0; u < R; ++u) {
         const int z = stage[St::OFF_ST + h.soff0 + r[u]];
 #pragma unroll
         for (int x = 0; x < 4; ++x) {
           a0[u][x] = z < 4 ? sM0[x * 4 + z] : T(1);
-          qx0[u][x] = z < 4 ? sQ[x * 4 + z] : T(0);
+          qx0[u][x] = z < 4 ? __ldg(D0 + x * 4 + z) : T(0);
         }
       }
     } else {
@@ -168,13 +185,14 @@ __global__ void __launch_bounds__(NT_THREADS, 4) k_pre4_lean(const DevPreItem* _
       mv4r<T, R>(sQ, x0, qx0);
     }
     if (TIP1) {
+      const T* D1 = reinterpret_cast<const T*>(static_cast<const char*>(it.mat[1]) + dmat_delta) + g * 16;
 #pragma unroll
       for (int u = 0; u < R; ++u) {
         const int z = stage[St::OFF_ST + (TP + 16) + h.soff1 + r[u]];
 #pragma unroll
         for (int x = 0; x < 4; ++x) {
           a1[u][x] = z < 4 ? sM1[x * 4 + z] : T(1);
-          qx1[u][x] = z < 4 ? sQ[x * 4 + z] : T(0);
+          qx1[u][x] = z < 4 ? __ldg(D1 + x * 4 + z) : T(0);
         }
       }
     } else {
@@ -198,8 +216,22 @@ __global__ void __launch_bounds__(NT_THREADS, 4) k_pre4_lean(const DevPreItem* _
       }
     }
     T q0[R][4], q1[R][4];
-    mvt4r<T, R>(sM0, u0, q0);
-    mvt4r<T, R>(sM1, u1, q1);
+    if (TIP0) {
+#pragma unroll
+      for (int u = 0; u < R; ++u)
+#pragma unroll
+        for (int x = 0; x < 4; ++x) q0[u][x] = u0[u][x];  // num_0 = u_0 . D_0[:, z]
+    } else {
+      mvt4r<T, R>(sM0, u0, q0);
+    }
+    if (TIP1) {
+#pragma unroll
+      for (int u = 0; u < R; ++u)
+#pragma unroll
+        for (int x = 0; x < 4; ++x) q1[u][x] = u1[u][x];
+    } else {
+      mvt4r<T, R>(sM1, u1, q1);
+    }
     double contrib = 0.0;
 #pragma unroll
     for (int u = 0; u < R; ++u) {
