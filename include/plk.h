@@ -140,6 +140,13 @@ PLK_API const char* plk_error_string(int status);
  * contributes 1 for every state (S8c row 15).  Uses one compact slot. */
 PLK_API int plk_set_tip_states(plk_instance* inst, int tip, const int32_t* states);
 
+/* The same with one BYTE per pattern (values >= S: missing), which is the layout the kernels read: a plain
+ * host -> device copy, enqueued on the instance's stream WITHOUT synchronising.  `states` (P bytes, host memory) is
+ * therefore the one exception to the ownership rule above: when it is pinned memory it must stay unchanged until the
+ * next call that returns values to the host (or plk_synchronize).  This is the upload an application repeats per
+ * evaluation when its alignment changes (bench.py's end-to-end leg). */
+PLK_API int plk_set_tip_states_u8(plk_instance* inst, int tip, const uint8_t* states);
+
 /* Tip `tip` as partials [P][S], the same for every category (e.g. one-hot rows, all-ones rows for missing). */
 PLK_API int plk_set_tip_partials(plk_instance* inst, int tip, const double* partials);
 

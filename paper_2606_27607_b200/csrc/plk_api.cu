@@ -719,6 +719,22 @@ int plk_set_tip_states(plk_instance* in, int tip, const int32_t* states) {
   return PLK_SUCCESS;
 }
 
+int plk_set_tip_states_u8(plk_instance* in, int tip, const uint8_t* states) {
+  if (in == nullptr || states == nullptr) return PLK_ERR_OUT_OF_RANGE;
+  if (tip < 0 || tip >= in->cfg.tip_count) return PLK_ERR_OUT_OF_RANGE;
+  const Layout& L = in->L;
+  if (!(in->post_slot[tip] >= 0 && in->post_kind[tip] == KIND_STATES)) {
+    if (in->post_slot[tip] >= 0) return PLK_ERR_OUT_OF_RANGE;  // already bound as partials
+    if (in->next_compact_slot >= L.compact_slots) return PLK_ERR_OUT_OF_MEMORY;
+    in->post_slot[tip] = in->next_compact_slot++;
+    in->post_kind[tip] = KIND_STATES;
+  }
+  CU(cudaMemcpyAsync(in->post_ptr(tip), states, (size_t)L.P, cudaMemcpyHostToDevice, in->stream));
+  in->post_written[tip] = 1;
+  in->post_pending_scale[tip] = -1;
+  return PLK_SUCCESS;
+}
+
 int plk_set_tip_partials(plk_instance* in, int tip, const double* partials) {
   if (in == nullptr || partials == nullptr) return PLK_ERR_OUT_OF_RANGE;
   if (tip < 0 || tip >= in->cfg.tip_count) return PLK_ERR_OUT_OF_RANGE;

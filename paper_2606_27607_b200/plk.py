@@ -53,6 +53,7 @@ _SIGNATURES = {
     "plk_destroy": (_I, [_P]),
     "plk_error_string": (C.c_char_p, [_I]),
     "plk_set_tip_states": (_I, [_P, _I, _P]),
+    "plk_set_tip_states_u8": (_I, [_P, _I, _P]),
     "plk_set_tip_partials": (_I, [_P, _I, _P]),
     "plk_set_partials": (_I, [_P, _I, _P]),
     "plk_set_pattern_weights": (_I, [_P, _P]),
@@ -237,6 +238,14 @@ class Instance:
         if s.size != self.P:
             raise ValueError("states must have pattern_count entries")
         self._call("plk_set_tip_states", tip, _ptr(s))
+
+    def set_tip_states_u8(self, tip, states):
+        """One byte per pattern (values >= S: missing); enqueued without synchronising: `states` (a contiguous uint8
+        array, ideally pinned) must stay unchanged until the next call that returns values to the host."""
+        s = np.ascontiguousarray(states, dtype=np.uint8)
+        if s.size != self.P:
+            raise ValueError("states must have pattern_count entries")
+        self._call("plk_set_tip_states_u8", tip, _ptr(s))
 
     def set_tip_partials(self, tip, partials):
         self._call("plk_set_tip_partials", tip, _ptr(_f64(partials, self.P * self.S)))

@@ -146,3 +146,20 @@ def test_tensor_fp32_unfused_no_level_batch_and_repeatable(arm):
     ref = orc.evaluate(wl)
     strict, rel_cond, norm = orc.gradient_errors(out[1][2], ref)
     assert rel_cond <= 1e-4 and norm <= 1e-4
+
+
+def test_tip_states_u8_matches_int32():
+    """plk_set_tip_states_u8 (byte states, asynchronous copy) gives the same bits as plk_set_tip_states."""
+    wl = workloads.config(1, n_tips=16, n_patterns=700)
+    ev = Evaluator(wl, precision=plk.FP64)
+    try:
+        a = ev.log_likelihood()
+        ga = ev.gradient()
+        u8 = np.ascontiguousarray(np.minimum(wl.tip_states, 255).astype(np.uint8))
+        for k in range(wl.tree.n_tips):
+            ev.inst.set_tip_states_u8(k, u8[k])
+        b = ev.log_likelihood()
+        gb = ev.gradient()
+        assert a[0] == b[0] and np.array_equal(a[1], b[1]) and np.array_equal(ga, gb)
+    finally:
+        ev.close()
