@@ -243,7 +243,8 @@ def oracle_time(wl, n_sample, repeats=1):
 
 
 # measured DRAM traffic per step (bytes) of the dominant kernel's launches, keyed by (workload, precision, kernel)
-NCU_DRAM_BYTES = {("cfg1_gtr_128x100000", "fp64", "k_pre4_lean"): 4179.5e6}
+NCU_DRAM_BYTES = {("cfg1_gtr_128x100000", "fp64", "k_pre4_lean"): 4193.0e6,
+                  ("cfg3_gy94_256x20000", "fp32", "k_pre_tc5"): 17075.1e6}
 
 ORACLE_SAMPLE = {4: 40000, 61: 4000}  # cpu_baseline leg: patterns per oracle evaluation, ~10-30 s of CPU work
 REFERENCE_SAMPLE = {4: 8000, 61: 800}  # --impl reference: patterns per step (a few seconds per step)
