@@ -495,7 +495,22 @@ int launch_pre4_lean(plk_instance* in, int cls, const DevPreItem* d_items, int n
   switch (cls) {
     case 0: return launch_pre4_lean_c<T, 0>(in, d_items, n, Q, site);
     case 1: return launch_pre4_lean_c<T, 1>(in, d_items, n, Q, site);
-    case 2: return launch_pre4_lean_c<T, 2>(in, d_items, n, Q, site);
+    case 2: {  // both children compact tips: lane-per-pattern kernel, no staging ring
+      if (in->cfg.flags & PLK_FLAG_NO_TMA) return launch_pre4_lean_c<T, 2>(in, d_items, n, Q, site);
+      const Layout& L = in->L;
+      const int n_tp = (L.P + 32 * NlRows<T>::R - 1) / (32 * NlRows<T>::R);
+      for (int first = 0; first < n; first += 32768) {
+        const int m = n - first < 32768 ? n - first : 32768;
+        dim3 grid((n_tp + NT_CW - 1) / NT_CW, m);
+        k_grad4_tips<T><<<grid, NT_CW * 32, 0, in->stream>>>(d_items + first, L.P,
+                                                             (long long)L.off_matrix_d - (long long)L.off_matrix,
+                                                             nuc_model(in, site), in->at<double>(L.off_grad_partial),
+                                                             L.n_tiles);
+        CHECK_LAUNCH(in);
+      }
+      in->grad_parts = n_tp * NT_CW;
+      return PLK_SUCCESS;
+    }
     default: return PLK_ERR_GENERAL;
   }
 }

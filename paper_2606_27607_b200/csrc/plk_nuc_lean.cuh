@@ -293,4 +293,102 @@ __global__ void __launch_bounds__(NT_THREADS, 4) k_pre4_lean(const DevPreItem* _
   }
 }
 
+// ---------------------------------------------------------------------------------------------------------------
+// Class 2 (both children compact tips) without the staging ring: the item reads only q_m (one cell per pattern and
+// category) and writes nothing, so it is instruction-bound in the lane-per-cell mapping above.  Here a lane owns a
+// whole PATTERN (R of them: p and p + 32, like the tiles of k_pre4_lean) and loops over the categories: the category
+// sums stay in registers (no shuffles), a_k and the derivative column D_k[:, z] come as one vector each from small
+// transposed tables in shared memory, and there is one division per pattern and child.
+//   den = sum_c w_c sum_x q_m[x] a_1[x] a_0[x],  num_k = sum_c w_c r_c sum_x (q_m[x] a_{1-k}[x]) D_k[x][z_k]
+// Gradient partial sums land exactly where k_pre4_lean puts them (entry = tile * NT_CW + lane / 8, tile = 32 R patterns).
+// ---------------------------------------------------------------------------------------------------------------
+template <typename T>
+__global__ void __launch_bounds__(NT_CW * 32) k_grad4_tips(const DevPreItem* __restrict__ items, int P, long long dmat_delta,
+                                                           NucModel md, double* __restrict__ grad_partial, int n_part) {
+  constexpr int C = NL_C, R = NlRows<T>::R;
+  __shared__ __align__(16) T tabA[2][C][5][4];  // [child][category][state z (4 = missing)][x]: M_k[x][z]; missing: 1
+  __shared__ __align__(16) T tabD[2][C][5][4];  // D_k[x][z]; missing: 0 (Q . 1 = 0)
+  const DevPreItem& it = items[blockIdx.y];
+  for (int i = threadIdx.x; i < 2 * C * 16; i += blockDim.x) {
+    const int k = i / (C * 16), c = (i / 16) % C, x = (i >> 2) & 3, z = i & 3;
+    const T* M = static_cast<const T*>(it.mat[k]) + c * 16;
+    const T* D = reinterpret_cast<const T*>(static_cast<const char*>(it.mat[k]) + dmat_delta) + c * 16;
+    tabA[k][c][z][x] = M[x * 4 + z];
+    tabD[k][c][z][x] = D[x * 4 + z];
+  }
+  for (int i = threadIdx.x; i < 2 * C * 4; i += blockDim.x) {
+    const int k = i / (C * 4), c = (i >> 2) % C, x = i & 3;
+    tabA[k][c][4][x] = T(1);
+    tabD[k][c][4][x] = T(0);
+  }
+  __syncthreads();
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int tile = blockIdx.x * NT_CW + warp;  // 32 R patterns
+  const int n_tp = (P + 32 * R - 1) / (32 * R);
+  if (tile >= n_tp) return;
+  const uint8_t* st0 = static_cast<const uint8_t*>(it.p[0]);
+  const uint8_t* st1 = static_cast<const uint8_t*>(it.p[1]);
+  const T* qmp = static_cast<const T*>(it.qm);
+  double contrib[2] = {0.0, 0.0};
+  int p[R], z0[R], z1[R];
+  T qm[R][C][4];
+#pragma unroll
+  for (int u = 0; u < R; ++u) {  // every load of the lane is issued before any arithmetic
+    p[u] = tile * 32 * R + lane + 32 * u;
+    const bool live = p[u] < P;
+    z0[u] = live ? min((int)st0[p[u]], 4) : 4;
+    z1[u] = live ? min((int)st1[p[u]], 4) : 4;
+#pragma unroll
+    for (int c = 0; c < C; ++c) {
+      if (live) {
+        ld4(qmp + ((size_t)c * P + p[u]) * 4, qm[u][c]);
+      } else {
+#pragma unroll
+        for (int x = 0; x < 4; ++x) qm[u][c][x] = T(0);
+      }
+    }
+  }
+#pragma unroll
+  for (int u = 0; u < R; ++u) {
+    double den = 0.0, num0 = 0.0, num1 = 0.0;
+#pragma unroll
+    for (int c = 0; c < C; ++c) {
+      T a0[4], a1[4], d0[4], d1[4];
+      ld4(&tabA[0][c][z0[u]][0], a0);
+      ld4(&tabA[1][c][z1[u]][0], a1);
+      ld4(&tabD[0][c][z0[u]][0], d0);
+      ld4(&tabD[1][c][z1[u]][0], d1);
+      T dd = T(0), n0 = T(0), n1 = T(0);
+#pragma unroll
+      for (int x = 0; x < 4; ++x) {
+        const T u0 = qm[u][c][x] * a1[x], u1 = qm[u][c][x] * a0[x];
+        dd = fma(u0, a0[x], dd);
+        n0 = fma(u0, d0[x], n0);
+        n1 = fma(u1, d1[x], n1);
+      }
+      const double cw = md.catw[c], cwr = cw * md.catr[c];
+      den = fma(cw, (double)dd, den);
+      num0 = fma(cwr, (double)n0, num0);
+      num1 = fma(cwr, (double)n1, num1);
+    }
+    if (p[u] < P) {
+      const double w = md.weights[p[u]], r0 = num0 / den, r1 = num1 / den;
+      if (md.site_out != nullptr) {
+        md.site_out[(size_t)it.slot[0] * P + p[u]] = r0;
+        md.site_out[(size_t)it.slot[1] * P + p[u]] = r1;
+      }
+      contrib[0] += w * r0;
+      contrib[1] += w * r1;
+    }
+  }
+#pragma unroll
+  for (int k = 0; k < 2; ++k) {
+    double v = contrib[k];
+    v += __shfl_xor_sync(0xffffffffu, v, 1);
+    v += __shfl_xor_sync(0xffffffffu, v, 2);
+    v += __shfl_xor_sync(0xffffffffu, v, 4);
+    if ((lane & 7) == 0) grad_partial[(size_t)it.slot[k] * n_part + tile * NT_CW + (lane >> 3)] = v;
+  }
+}
+
 }  // namespace plk
