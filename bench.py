@@ -243,7 +243,7 @@ def oracle_time(wl, n_sample, repeats=1):
 
 
 # measured DRAM traffic per step (bytes) of the dominant kernel's launches, keyed by (workload, precision, kernel)
-NCU_DRAM_BYTES = {("cfg1_gtr_128x100000", "fp64", "k_pre4_lean"): 4193.0e6,
+NCU_DRAM_BYTES = {("cfg1_gtr_128x100000", "fp64", "k_pre4_lean+k_grad4_tips"): 4193.0e6,
                   ("cfg3_gy94_256x20000", "fp32", "k_pre_tc5"): 17075.1e6}
 
 ORACLE_SAMPLE = {4: 40000, 61: 4000}  # cpu_baseline leg: patterns per oracle evaluation, ~10-30 s of CPU work
@@ -436,7 +436,7 @@ def main():
     kname = {"post_order": ("k_post4_walk" if args.shape != "level" else "k_post4_tma") if nuc
              else (("k_post_tc5" if args.precision == "fp32" and args.codon_fp32 == "tcgen05" else "k_post_tc")
                    if args.tensor else "k_post64"),
-             "pre_order_gradient": ("k_pre4_lean" if lean else "k_pre4_tma/k_pre4/k_pre4_walk") if nuc
+             "pre_order_gradient": ("k_pre4_lean+k_grad4_tips" if lean else "k_pre4_tma/k_pre4/k_pre4_walk") if nuc
              else (("k_pre_tc5" if args.precision == "fp32" and args.codon_fp32 == "tcgen05" else "k_pre_tc")
                    if args.tensor else "k_pre64")}[dom]
     n_levels_note = "all launches of the kernel in one step (one per dependency level and item class)"
