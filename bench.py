@@ -41,6 +41,9 @@ def parse_args():
                     help="4-state launch shape: one launch per level / one pattern-walk launch / library's choice")
     ap.add_argument("--staging", choices=["tma", "ldg"], default="tma",
                     help="4-state operand staging: TMA ring (cp.async.bulk) / register-staged loads")
+    ap.add_argument("--no-pdl", action="store_true",
+                    help="4-state gradient pass: plain stream-ordered launches (comparison arm of the programmatic "
+                         "dependent launch chain)")
     ap.add_argument("--codon-fp32", choices=["tcgen05", "mma_sync"], default="tcgen05",
                     help="fp32 --tensor codon kernels: tcgen05/TMEM (default) or the legacy mma.sync arm")
     ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
@@ -265,6 +268,7 @@ def workload_config(wl, precision, flags, extra=None):
            "substitution_model": wl.model["name"], "seed": wl.seed,
            "launch_shape": {8: "level", 16: "walk"}.get(flags & 24, "auto") if wl.n_states == 4 else "level",
            "staging": ("ldg" if flags & 32 else "tma") if wl.n_states == 4 else None,
+           "dependent_launch": (not flags & 128) if wl.n_states == 4 else None,
            "l2_policy": "inputs exceed L2 (no flush between iterations)"}
     if extra:
         cfg.update(extra)
@@ -403,6 +407,7 @@ def main():
     flags |= {"auto": 0, "level": plk.FLAG_LEVEL_BATCH_ONLY, "walk": plk.FLAG_PATTERN_WALK_ONLY}[args.shape]
     flags |= plk.FLAG_NO_TMA if args.staging == "ldg" else 0
     flags |= plk.FLAG_NO_TCGEN05 if args.codon_fp32 == "mma_sync" else 0
+    flags |= plk.FLAG_NO_PDL if args.no_pdl else 0
     sampler = ClockSampler(local_rank) if rank == 0 else None
 
     if dist is not None:

@@ -68,6 +68,9 @@ enum {                                                /* plk_config.flags (bit s
   PLK_FLAG_NO_TCGEN05 = 64,    /* fp32 + PLK_FLAG_TENSOR_CORES: run the post-order and the fused pre-order + derivative
                                   kernels on the legacy warp-level mma.sync TF32 kernels instead of the tcgen05 /
                                   TMEM kernels (comparison arm)                                             */
+  PLK_FLAG_NO_PDL = 128,       /* 4-state gradient pass: plain stream-ordered launches instead of programmatic
+                                  dependent launches (the item classes of one dependency level are independent of
+                                  each other and otherwise overlap one another's tail; comparison arm)       */
   PLK_FLAG_SITE_DERIVATIVES = 4 /* reserve partials_buffer_count * P doubles so that the gradient calls can
                                   return per-pattern derivatives (out_site != NULL); without it such a
                                   request returns PLK_ERR_UNSUPPORTED                                   */

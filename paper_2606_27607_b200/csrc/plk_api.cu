@@ -467,9 +467,30 @@ int launch_pre4_tma(plk_instance* in, const DevPreItem* d_items, int n, const T*
   }
 }
 
-// specialised fused pre-order + gradient kernels (plk_nuc_lean.cuh): items of one class, level order
+// Launch with the programmatic-stream-serialisation attribute (programmatic dependent launch): the grid may become
+// resident while the previous launch of the stream drains; the kernels order themselves with griddepcontrol
+// (plk_nuc_lean.cuh).  pdl = false is a plain stream-ordered launch.
+template <typename... KArgs, typename... Args>
+cudaError_t launch_chain(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t stream, bool pdl,
+                         Args... args) {
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = grid;
+  cfg.blockDim = block;
+  cfg.dynamicSmemBytes = smem;
+  cfg.stream = stream;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  attr[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = attr;
+  cfg.numAttrs = pdl ? 1 : 0;
+  return cudaLaunchKernelEx(&cfg, kernel, KArgs(args)...);
+}
+
+// specialised fused pre-order + gradient kernels (plk_nuc_lean.cuh): items of one class, level order.  `first`: the
+// first launch of its dependency level (it waits for the previous level before it reads; the other classes of the
+// level are independent of it and overlap its tail).
 template <typename T, int CLS>
-int launch_pre4_lean_c(plk_instance* in, const DevPreItem* d_items, int n, const T* Q, double* site) {
+int launch_pre4_lean_c(plk_instance* in, const DevPreItem* d_items, int n, const T* Q, double* site, bool first) {
   const Layout& L = in->L;
   using St = NtStage<T, NL_C, 3, true, NlRows<T>::R>;
   const size_t smem = (size_t)NT_NS * St::BYTES;
@@ -482,30 +503,31 @@ int launch_pre4_lean_c(plk_instance* in, const DevPreItem* d_items, int n, const
   const long long n_tp = (L.P + St::TP - 1) / St::TP;
   long long g = (long long)in->sm_count * bps;
   if (g > n_tp * n) g = n_tp * n;
-  k_pre4_lean<T, CLS><<<(int)g, NT_THREADS, smem, in->stream>>>(d_items, n, L.P, Q,
-                                                               (long long)L.off_matrix_d - (long long)L.off_matrix,
-                                                               nuc_model(in, site),
-                                                               in->at<double>(L.off_grad_partial), L.n_tiles);
+  const bool pdl = !(in->cfg.flags & PLK_FLAG_NO_PDL);
+  CU(launch_chain(k_pre4_lean<T, CLS>, dim3((unsigned)g), dim3(NT_THREADS), smem, in->stream, pdl, d_items, n, L.P, Q,
+                  (long long)L.off_matrix_d - (long long)L.off_matrix, nuc_model(in, site),
+                  in->at<double>(L.off_grad_partial), L.n_tiles, (first || !pdl) ? 1 : 0));
   in->grad_parts = (int)n_tp * NT_CW;
   CHECK_LAUNCH(in);
   return PLK_SUCCESS;
 }
 template <typename T>
-int launch_pre4_lean(plk_instance* in, int cls, const DevPreItem* d_items, int n, const T* Q, double* site) {
+int launch_pre4_lean(plk_instance* in, int cls, const DevPreItem* d_items, int n, const T* Q, double* site,
+                     bool first_launch) {
   switch (cls) {
-    case 0: return launch_pre4_lean_c<T, 0>(in, d_items, n, Q, site);
-    case 1: return launch_pre4_lean_c<T, 1>(in, d_items, n, Q, site);
+    case 0: return launch_pre4_lean_c<T, 0>(in, d_items, n, Q, site, first_launch);
+    case 1: return launch_pre4_lean_c<T, 1>(in, d_items, n, Q, site, first_launch);
     case 2: {  // both children compact tips: lane-per-pattern kernel, no staging ring
-      if (in->cfg.flags & PLK_FLAG_NO_TMA) return launch_pre4_lean_c<T, 2>(in, d_items, n, Q, site);
+      if (in->cfg.flags & PLK_FLAG_NO_TMA) return launch_pre4_lean_c<T, 2>(in, d_items, n, Q, site, first_launch);
       const Layout& L = in->L;
+      const bool pdl = !(in->cfg.flags & PLK_FLAG_NO_PDL);
       const int n_tp = (L.P + 32 * NlRows<T>::R - 1) / (32 * NlRows<T>::R);
       for (int first = 0; first < n; first += 32768) {
         const int m = n - first < 32768 ? n - first : 32768;
         dim3 grid((n_tp + NT_CW - 1) / NT_CW, m);
-        k_grad4_tips<T><<<grid, NT_CW * 32, 0, in->stream>>>(d_items + first, L.P,
-                                                             (long long)L.off_matrix_d - (long long)L.off_matrix,
-                                                             nuc_model(in, site), in->at<double>(L.off_grad_partial),
-                                                             L.n_tiles);
+        CU(launch_chain(k_grad4_tips<T>, grid, dim3(NT_CW * 32), 0, in->stream, pdl, d_items + first, L.P,
+                        (long long)L.off_matrix_d - (long long)L.off_matrix, nuc_model(in, site),
+                        in->at<double>(L.off_grad_partial), L.n_tiles, ((first_launch && first == 0) || !pdl) ? 1 : 0));
         CHECK_LAUNCH(in);
       }
       in->grad_parts = n_tp * NT_CW;
@@ -638,7 +660,7 @@ int plk_create(const plk_config* cfg, void* d_arena, size_t arena_bytes, void* c
     return PLK_ERR_OUT_OF_RANGE;
   }
   if (cfg->flags & ~(PLK_FLAG_TENSOR_CORES | PLK_FLAG_NO_LEVEL_BATCH | PLK_FLAG_SITE_DERIVATIVES | PLK_FLAG_LEVEL_BATCH_ONLY |
-                     PLK_FLAG_PATTERN_WALK_ONLY | PLK_FLAG_NO_TMA | PLK_FLAG_NO_TCGEN05))
+                     PLK_FLAG_PATTERN_WALK_ONLY | PLK_FLAG_NO_TMA | PLK_FLAG_NO_TCGEN05 | PLK_FLAG_NO_PDL))
     return PLK_ERR_UNSUPPORTED;
   if ((cfg->flags & PLK_FLAG_LEVEL_BATCH_ONLY) && (cfg->flags & PLK_FLAG_PATTERN_WALK_ONLY)) return PLK_ERR_UNSUPPORTED;
 #ifndef PLK_WITH_TENSOR
@@ -1319,14 +1341,16 @@ static int pre_impl(plk_instance* in, int eigen, int root_pre, const plk_pre_op*
       if (rc) return rc;
     }
     for (int l = 0; l < (walk ? 0 : n_levels); ++l) {
+      bool first_launch = true;  // of this level: see launch_pre4_lean_c
       for (int k = 0; k < 3; ++k) {  // specialised classes
         const int c0 = class_start[(size_t)l * 5 + k], m = class_start[(size_t)l * 5 + k + 1] - c0;
         if (m == 0) continue;
         rc = by_precision(in, [&](auto tag) -> int {
           using T = decltype(tag);
-          return launch_pre4_lean<T>(in, k, dit + c0, m, static_cast<const T*>(Q), d_site);
+          return launch_pre4_lean<T>(in, k, dit + c0, m, static_cast<const T*>(Q), d_site, first_launch);
         });
         if (rc) return rc;
+        first_launch = false;
       }
       const int g0 = class_start[(size_t)l * 5 + 3];
       const int n = level_start[l + 1] - g0;

@@ -98,7 +98,8 @@ __device__ __forceinline__ void mvt4r(const T* __restrict__ M, const T (&v)[R][4
 template <typename T, int CLS>
 __global__ void __launch_bounds__(NT_THREADS, 4) k_pre4_lean(const DevPreItem* __restrict__ items, int n_items, int P,
                                                              const T* __restrict__ Qg, long long dmat_delta, NucModel md,
-                                                             double* __restrict__ grad_partial, int n_part) {
+                                                             double* __restrict__ grad_partial, int n_part,
+                                                             int wait_first) {
   constexpr int C = NL_C;
   constexpr int R = NlRows<T>::R;
   constexpr bool TIP0 = CLS == 2, TIP1 = CLS >= 1;
@@ -116,6 +117,11 @@ __global__ void __launch_bounds__(NT_THREADS, 4) k_pre4_lean(const DevPreItem* _
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     fence_proxy_async();
   }
+  // Launch chain of one level (plk_api.cu): the first kernel of a level waits for the previous level and only then
+  // lets the next launch in; the other classes of the level are independent of it, start as its CTAs drain and
+  // wait at their END, so that a grid never completes before the one it overlaps.
+  if (wait_first) pdl_wait();
+  pdl_trigger();
   if (threadIdx.x < 16) sQ[threadIdx.x] = Qg[threadIdx.x];
   __syncthreads();
   const uint32_t n_tp = (uint32_t)((P + TP - 1) / TP);
@@ -140,6 +146,7 @@ __global__ void __launch_bounds__(NT_THREADS, 4) k_pre4_lean(const DevPreItem* _
                                   ptr, kind, mat, md.weights, P, p0, n);
       }
     }
+    if (!wait_first) pdl_wait();
     return;
   }
   // ---- consumers: lane = 8 g + pl takes category g of patterns warp * 8 + pl + 32 u, u < R
@@ -291,6 +298,7 @@ __global__ void __launch_bounds__(NT_THREADS, 4) k_pre4_lean(const DevPreItem* _
     contrib += __shfl_xor_sync(0xffffffffu, contrib, 4);
     if (pl == 0 && g < 2) grad_partial[(size_t)slot * n_part + (h.p0 / TP) * NT_CW + warp] = contrib;
   }
+  if (!wait_first) pdl_wait();
 }
 
 // ---------------------------------------------------------------------------------------------------------------
@@ -304,10 +312,13 @@ __global__ void __launch_bounds__(NT_THREADS, 4) k_pre4_lean(const DevPreItem* _
 // ---------------------------------------------------------------------------------------------------------------
 template <typename T>
 __global__ void __launch_bounds__(NT_CW * 32) k_grad4_tips(const DevPreItem* __restrict__ items, int P, long long dmat_delta,
-                                                           NucModel md, double* __restrict__ grad_partial, int n_part) {
+                                                           NucModel md, double* __restrict__ grad_partial, int n_part,
+                                                           int wait_first) {
   constexpr int C = NL_C, R = NlRows<T>::R;
   __shared__ __align__(16) T tabA[2][C][5][4];  // [child][category][state z (4 = missing)][x]: M_k[x][z]; missing: 1
   __shared__ __align__(16) T tabD[2][C][5][4];  // D_k[x][z]; missing: 0 (Q . 1 = 0)
+  if (wait_first) pdl_wait();  // launch chain: see k_pre4_lean
+  pdl_trigger();
   const DevPreItem& it = items[blockIdx.y];
   for (int i = threadIdx.x; i < 2 * C * 16; i += blockDim.x) {
     const int k = i / (C * 16), c = (i / 16) % C, x = (i >> 2) & 3, z = i & 3;
@@ -325,7 +336,10 @@ __global__ void __launch_bounds__(NT_CW * 32) k_grad4_tips(const DevPreItem* __r
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int tile = blockIdx.x * NT_CW + warp;  // 32 R patterns
   const int n_tp = (P + 32 * R - 1) / (32 * R);
-  if (tile >= n_tp) return;
+  if (tile >= n_tp) {
+    if (!wait_first) pdl_wait();
+    return;
+  }
   const uint8_t* st0 = static_cast<const uint8_t*>(it.p[0]);
   const uint8_t* st1 = static_cast<const uint8_t*>(it.p[1]);
   const T* qmp = static_cast<const T*>(it.qm);
@@ -389,6 +403,7 @@ __global__ void __launch_bounds__(NT_CW * 32) k_grad4_tips(const DevPreItem* __r
     v += __shfl_xor_sync(0xffffffffu, v, 4);
     if ((lane & 7) == 0) grad_partial[(size_t)it.slot[k] * n_part + tile * NT_CW + (lane >> 3)] = v;
   }
+  if (!wait_first) pdl_wait();
 }
 
 }  // namespace plk

@@ -61,6 +61,11 @@ __device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t by
                : "memory");
 }
 __device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async;" ::: "memory"); }
+// programmatic dependent launch (griddepcontrol): `pdl_trigger` lets the next launch of the stream become resident
+// as this grid's CTAs drain; `pdl_wait` blocks until the grids this launch depends on have completed and flushed.
+// Both are no-ops in a launch without the programmatic-serialisation attribute.
+__device__ __forceinline__ void pdl_trigger() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
 
 // ---- exponent of a non-negative maximum from its bit pattern (integer max instead of fp compares) ---------------
 // key(v) is monotone in v for v >= 0; negative values and -0 give keys <= 0 and never win against 0.

@@ -23,6 +23,7 @@ FP64, FP32 = 0, 1
 FLAG_TENSOR_CORES, FLAG_NO_LEVEL_BATCH, FLAG_SITE_DERIVATIVES = 1, 2, 4
 FLAG_LEVEL_BATCH_ONLY, FLAG_PATTERN_WALK_ONLY, FLAG_NO_TMA = 8, 16, 32
 FLAG_NO_TCGEN05 = 64
+FLAG_NO_PDL = 128
 NUCLEOTIDE, CODON = 0, 1
 
 

@@ -111,6 +111,23 @@ def test_nucleotide_walk_small_and_ragged_pattern_counts(precision, n_pat):
 
 
 @pytest.mark.parametrize("precision", PREC)
+def test_gradient_launch_chain_matches_plain_launches(precision):
+    """4-state gradient pass: the programmatic dependent launch chain (the item classes of a dependency level
+    overlap one another's tail; a level still waits for the one before it) against plain stream-ordered launches
+    (PLK_FLAG_NO_PDL).  Same kernels, fixed summation order: the gradients must be bitwise equal, repeatedly (an
+    ordering bug would show as a stale q_parent).  Deep tree = many short levels."""
+    wl = workloads.config(1, n_tips=96, n_patterns=20000)
+    _, g_plain = _run_case(wl, precision, flags=plk.FLAG_NO_PDL | plk.FLAG_LEVEL_BATCH_ONLY)
+    ev = Evaluator(wl, precision=precision, flags=plk.FLAG_LEVEL_BATCH_ONLY)
+    try:
+        for _ in range(20):
+            ev.log_likelihood()
+            assert np.array_equal(ev.gradient(), g_plain)
+    finally:
+        ev.close()
+
+
+@pytest.mark.parametrize("precision", PREC)
 def test_config1_perturbed_branch_lengths(precision):
     wl = workloads.config(1, n_patterns=2000)
     ref, grad = _run_case(wl, precision, t=wl.perturbed_branch_lengths())
