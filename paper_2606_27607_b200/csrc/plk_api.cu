@@ -130,6 +130,7 @@ struct plk_instance {
   std::vector<int> pre_slot;
   std::vector<char> pre_written, pre_has_mx;
   std::vector<char> matrix_written, scale_written, eigen_written, q_written;
+  std::vector<double> h_q4;  // 4-state instances: host copy of every Q [eigen][16] (working precision, widened)
   int next_post_slot = 0, next_compact_slot = 0, next_pre_slot = 0;
   bool have_weights = false, have_pi = false, have_rates = false, have_catw = false;
   int root_pre_filled = -1;
@@ -490,7 +491,8 @@ cudaError_t launch_chain(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t
 // first launch of its dependency level (it waits for the previous level before it reads; the other classes of the
 // level are independent of it and overlap its tail).
 template <typename T, int CLS>
-int launch_pre4_lean_c(plk_instance* in, const DevPreItem* d_items, int n, const T* Q, double* site, bool first) {
+int launch_pre4_lean_c(plk_instance* in, const DevPreItem* d_items, int n, const double* h_q, double* site,
+                       bool first) {
   const Layout& L = in->L;
   using St = NtStage<T, NL_C, 3, true, NlRows<T>::R>;
   const size_t smem = (size_t)NT_NS * St::BYTES;
@@ -504,6 +506,8 @@ int launch_pre4_lean_c(plk_instance* in, const DevPreItem* d_items, int n, const
   long long g = (long long)in->sm_count * bps;
   if (g > n_tp * n) g = n_tp * n;
   const bool pdl = !(in->cfg.flags & PLK_FLAG_NO_PDL);
+  NlQ<T> Q;
+  for (int i = 0; i < 16; ++i) Q.v[i] = (T)h_q[i];
   CU(launch_chain(k_pre4_lean<T, CLS>, dim3((unsigned)g), dim3(NT_THREADS), smem, in->stream, pdl, d_items, n, L.P, Q,
                   (long long)L.off_matrix_d - (long long)L.off_matrix, nuc_model(in, site),
                   in->at<double>(L.off_grad_partial), L.n_tiles, (first || !pdl) ? 1 : 0));
@@ -512,7 +516,7 @@ int launch_pre4_lean_c(plk_instance* in, const DevPreItem* d_items, int n, const
   return PLK_SUCCESS;
 }
 template <typename T>
-int launch_pre4_lean(plk_instance* in, int cls, const DevPreItem* d_items, int n, const T* Q, double* site,
+int launch_pre4_lean(plk_instance* in, int cls, const DevPreItem* d_items, int n, const double* Q, double* site,
                      bool first_launch) {
   switch (cls) {
     case 0: return launch_pre4_lean_c<T, 0>(in, d_items, n, Q, site, first_launch);
@@ -524,7 +528,7 @@ int launch_pre4_lean(plk_instance* in, int cls, const DevPreItem* d_items, int n
       const int n_tp = (L.P + 32 * NlRows<T>::R - 1) / (32 * NlRows<T>::R);
       for (int first = 0; first < n; first += 32768) {
         const int m = n - first < 32768 ? n - first : 32768;
-        dim3 grid((n_tp + NT_CW - 1) / NT_CW, m);
+        dim3 grid((n_tp + NT_CW * NL_TIPS_TPW - 1) / (NT_CW * NL_TIPS_TPW), m);
         CU(launch_chain(k_grad4_tips<T>, grid, dim3(NT_CW * 32), 0, in->stream, pdl, d_items + first, L.P,
                         (long long)L.off_matrix_d - (long long)L.off_matrix, nuc_model(in, site),
                         in->at<double>(L.off_grad_partial), L.n_tiles, ((first_launch && first == 0) || !pdl) ? 1 : 0));
@@ -694,6 +698,7 @@ int plk_create(const plk_config* cfg, void* d_arena, size_t arena_bytes, void* c
   in->scale_written.assign(cfg->scale_buffer_count, 0);
   in->eigen_written.assign(cfg->eigen_buffer_count, 0);
   in->q_written.assign(cfg->eigen_buffer_count, 0);
+  in->h_q4.assign((size_t)cfg->eigen_buffer_count * 16, 0.0);
   if (cudaHostAlloc(reinterpret_cast<void**>(&in->h_ring), RING_BYTES, cudaHostAllocDefault) != cudaSuccess) {
     delete in;
     return PLK_ERR_CUDA;
@@ -850,6 +855,23 @@ static int rebuild_rate_matrix(plk_instance* in, int eigen) {
   return PLK_SUCCESS;
 }
 
+// 4-state instances keep a host copy of Q in working precision: the class-specialised gradient kernels take it by
+// value (plk_nuc_lean.cuh NlQ).  Called by the two setters of Q, which synchronise anyway.
+static int fetch_q4(plk_instance* in, int eigen) {
+  if (in->L.SP != 4) return PLK_SUCCESS;
+  double* dst = in->h_q4.data() + (size_t)eigen * 16;
+  if (in->f32) {
+    float q[16];
+    CU(cudaMemcpyAsync(q, in->eig_QT(eigen), sizeof(q), cudaMemcpyDeviceToHost, in->stream));
+    CU(cudaStreamSynchronize(in->stream));
+    for (int i = 0; i < 16; ++i) dst[i] = q[i];
+  } else {
+    CU(cudaMemcpyAsync(dst, in->eig_QT(eigen), 16 * sizeof(double), cudaMemcpyDeviceToHost, in->stream));
+    CU(cudaStreamSynchronize(in->stream));
+  }
+  return PLK_SUCCESS;
+}
+
 int plk_set_eigen_decomposition(plk_instance* in, int eigen, const double* U, const double* Uinv, const double* lam) {
   if (in == nullptr || U == nullptr || Uinv == nullptr || lam == nullptr) return PLK_ERR_OUT_OF_RANGE;
   if (eigen < 0 || eigen >= in->cfg.eigen_buffer_count) return PLK_ERR_OUT_OF_RANGE;
@@ -864,6 +886,8 @@ int plk_set_eigen_decomposition(plk_instance* in, int eigen, const double* U, co
   int rc = rebuild_rate_matrix(in, eigen);
   if (rc) return rc;
   CU(cudaStreamSynchronize(in->stream));
+  rc = fetch_q4(in, eigen);
+  if (rc) return rc;
   in->eigen_written[eigen] = 1;
   in->q_written[eigen] = 1;
   return PLK_SUCCESS;
@@ -884,6 +908,8 @@ int plk_set_rate_matrix(plk_instance* in, int eigen, const double* Q) {
   });
   CHECK_LAUNCH(in);
   CU(cudaStreamSynchronize(in->stream));
+  int rc = fetch_q4(in, eigen);
+  if (rc) return rc;
   in->q_written[eigen] = 1;
   return PLK_SUCCESS;
 }
@@ -1347,7 +1373,8 @@ static int pre_impl(plk_instance* in, int eigen, int root_pre, const plk_pre_op*
         if (m == 0) continue;
         rc = by_precision(in, [&](auto tag) -> int {
           using T = decltype(tag);
-          return launch_pre4_lean<T>(in, k, dit + c0, m, static_cast<const T*>(Q), d_site, first_launch);
+          return launch_pre4_lean<T>(in, k, dit + c0, m, in->h_q4.data() + (size_t)(want_grad ? eigen : 0) * 16, d_site,
+                                     first_launch);
         });
         if (rc) return rc;
         first_launch = false;

@@ -77,6 +77,21 @@ __device__ __forceinline__ void mv4r(const T* __restrict__ M, const T (&v)[R][4]
     for (int u = 0; u < R; ++u) a[u][s] = r[0] * v[u][0] + r[1] * v[u][1] + r[2] * v[u][2] + r[3] * v[u][3];
   }
 }
+// the rate matrix Q of the pass by value: a kernel parameter sits in the constant bank, so the products with Q take
+// their matrix operand straight from there (no shared-memory reads: the l1tex pipe is the busiest unit of this
+// kernel, profiles/r01_nuc_pre4_lean_fp64.txt)
+template <typename T>
+struct NlQ {
+  T v[16];
+};
+template <typename T, int R>
+__device__ __forceinline__ void mvq4r(const NlQ<T>& Q, const T (&v)[R][4], T (&a)[R][4]) {
+#pragma unroll
+  for (int s = 0; s < 4; ++s)
+#pragma unroll
+    for (int u = 0; u < R; ++u)
+      a[u][s] = Q.v[4 * s] * v[u][0] + Q.v[4 * s + 1] * v[u][1] + Q.v[4 * s + 2] * v[u][2] + Q.v[4 * s + 3] * v[u][3];
+}
 template <typename T, int R>
 __device__ __forceinline__ void mvt4r(const T* __restrict__ M, const T (&v)[R][4], T (&a)[R][4]) {
   T r[4];
@@ -97,7 +112,7 @@ __device__ __forceinline__ void mvt4r(const T* __restrict__ M, const T (&v)[R][4
 
 template <typename T, int CLS>
 __global__ void __launch_bounds__(NT_THREADS, 4) k_pre4_lean(const DevPreItem* __restrict__ items, int n_items, int P,
-                                                             const T* __restrict__ Qg, long long dmat_delta, NucModel md,
+                                                             const NlQ<T> Qc, long long dmat_delta, NucModel md,
                                                              double* __restrict__ grad_partial, int n_part,
                                                              int wait_first) {
   constexpr int C = NL_C;
@@ -107,7 +122,6 @@ __global__ void __launch_bounds__(NT_THREADS, 4) k_pre4_lean(const DevPreItem* _
   constexpr int MS = St::MS, TP = St::TP;
   extern __shared__ __align__(128) unsigned char nt_smem[];
   __shared__ __align__(8) uint64_t full[NT_NS], empty[NT_NS];
-  __shared__ __align__(16) T sQ[16];
   if (threadIdx.x == 0) {
 #pragma unroll
     for (int s = 0; s < NT_NS; ++s) {
@@ -122,7 +136,6 @@ __global__ void __launch_bounds__(NT_THREADS, 4) k_pre4_lean(const DevPreItem* _
   // wait at their END, so that a grid never completes before the one it overlaps.
   if (wait_first) pdl_wait();
   pdl_trigger();
-  if (threadIdx.x < 16) sQ[threadIdx.x] = Qg[threadIdx.x];
   __syncthreads();
   const uint32_t n_tp = (uint32_t)((P + TP - 1) / TP);
   const uint32_t total = (uint32_t)n_items * n_tp;
@@ -189,7 +202,7 @@ __global__ void __launch_bounds__(NT_THREADS, 4) k_pre4_lean(const DevPreItem* _
 #pragma unroll
       for (int u = 0; u < R; ++u) ld4(sOp + ((C + g) * TP + r[u]) * 4, x0[u]);
       mv4r<T, R>(sM0, x0, a0);
-      mv4r<T, R>(sQ, x0, qx0);
+      mvq4r<T, R>(Qc, x0, qx0);
     }
     if (TIP1) {
       const T* D1 = reinterpret_cast<const T*>(static_cast<const char*>(it.mat[1]) + dmat_delta) + g * 16;
@@ -207,7 +220,7 @@ __global__ void __launch_bounds__(NT_THREADS, 4) k_pre4_lean(const DevPreItem* _
 #pragma unroll
       for (int u = 0; u < R; ++u) ld4(sOp + ((2 * C + g) * TP + r[u]) * 4, x1[u]);
       mv4r<T, R>(sM1, x1, a1);
-      mv4r<T, R>(sQ, x1, qx1);
+      mvq4r<T, R>(Qc, x1, qx1);
     }
     T u0[R][4], u1[R][4], dd[R];
 #pragma unroll
@@ -310,16 +323,58 @@ __global__ void __launch_bounds__(NT_THREADS, 4) k_pre4_lean(const DevPreItem* _
 //   den = sum_c w_c sum_x q_m[x] a_1[x] a_0[x],  num_k = sum_c w_c r_c sum_x (q_m[x] a_{1-k}[x]) D_k[x][z_k]
 // Gradient partial sums land exactly where k_pre4_lean puts them (entry = tile * NT_CW + lane / 8, tile = 32 R patterns).
 // ---------------------------------------------------------------------------------------------------------------
+// tiles of 32 R patterns a warp takes per launch: a CTA lives long enough to amortise its table set-up (item
+// descriptor -> matrix pointers -> table entries: dependent global loads), and the loads of tile t + 1 are in flight
+// while tile t is computed
+#ifndef PLK_TIPS_TPW
+#define PLK_TIPS_TPW 1
+#endif
+constexpr int NL_TIPS_TPW = PLK_TIPS_TPW;
+
+template <typename T>
+struct NlTipsTile {  // what a lane reads for its R patterns of one tile
+  static constexpr int C = NL_C, R = NlRows<T>::R;
+  int p[R], z0[R], z1[R];
+  T qm[R][C][4];
+  __device__ __forceinline__ void load(int tile, int lane, int P, const T* __restrict__ qmp,
+                                       const uint8_t* __restrict__ st0, const uint8_t* __restrict__ st1) {
+#pragma unroll
+    for (int u = 0; u < R; ++u) {  // every load of the lane is issued before any arithmetic
+      p[u] = tile * 32 * R + lane + 32 * u;
+      const bool live = p[u] < P;
+      z0[u] = live ? min((int)st0[p[u]], 4) : 4;
+      z1[u] = live ? min((int)st1[p[u]], 4) : 4;
+#pragma unroll
+      for (int c = 0; c < C; ++c) {
+        if (live) {
+          ld4(qmp + ((size_t)c * P + p[u]) * 4, qm[u][c]);
+        } else {
+#pragma unroll
+          for (int x = 0; x < 4; ++x) qm[u][c][x] = T(0);
+        }
+      }
+    }
+  }
+};
+
 template <typename T>
 __global__ void __launch_bounds__(NT_CW * 32) k_grad4_tips(const DevPreItem* __restrict__ items, int P, long long dmat_delta,
                                                            NucModel md, double* __restrict__ grad_partial, int n_part,
                                                            int wait_first) {
-  constexpr int C = NL_C, R = NlRows<T>::R;
+  constexpr int C = NL_C, R = NlRows<T>::R, TPW = NL_TIPS_TPW;
   __shared__ __align__(16) T tabA[2][C][5][4];  // [child][category][state z (4 = missing)][x]: M_k[x][z]; missing: 1
   __shared__ __align__(16) T tabD[2][C][5][4];  // D_k[x][z]; missing: 0 (Q . 1 = 0)
   if (wait_first) pdl_wait();  // launch chain: see k_pre4_lean
   pdl_trigger();
   const DevPreItem& it = items[blockIdx.y];
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int n_tp = (P + 32 * R - 1) / (32 * R);
+  const int tile0 = blockIdx.x * (NT_CW * TPW) + warp;  // the warp's tiles: tile0 + t NT_CW, t < TPW
+  const uint8_t* st0 = static_cast<const uint8_t*>(it.p[0]);
+  const uint8_t* st1 = static_cast<const uint8_t*>(it.p[1]);
+  const T* qmp = static_cast<const T*>(it.qm);
+  NlTipsTile<T> buf[2];
+  buf[0].load(tile0, lane, P, qmp, st0, st1);  // in flight under the table set-up (a tile past the end loads nothing)
   for (int i = threadIdx.x; i < 2 * C * 16; i += blockDim.x) {
     const int k = i / (C * 16), c = (i / 16) % C, x = (i >> 2) & 3, z = i & 3;
     const T* M = static_cast<const T*>(it.mat[k]) + c * 16;
@@ -333,75 +388,55 @@ __global__ void __launch_bounds__(NT_CW * 32) k_grad4_tips(const DevPreItem* __r
     tabD[k][c][4][x] = T(0);
   }
   __syncthreads();
-  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  const int tile = blockIdx.x * NT_CW + warp;  // 32 R patterns
-  const int n_tp = (P + 32 * R - 1) / (32 * R);
-  if (tile >= n_tp) {
-    if (!wait_first) pdl_wait();
-    return;
-  }
-  const uint8_t* st0 = static_cast<const uint8_t*>(it.p[0]);
-  const uint8_t* st1 = static_cast<const uint8_t*>(it.p[1]);
-  const T* qmp = static_cast<const T*>(it.qm);
-  double contrib[2] = {0.0, 0.0};
-  int p[R], z0[R], z1[R];
-  T qm[R][C][4];
+  const int slot0 = it.slot[0], slot1 = it.slot[1];
 #pragma unroll
-  for (int u = 0; u < R; ++u) {  // every load of the lane is issued before any arithmetic
-    p[u] = tile * 32 * R + lane + 32 * u;
-    const bool live = p[u] < P;
-    z0[u] = live ? min((int)st0[p[u]], 4) : 4;
-    z1[u] = live ? min((int)st1[p[u]], 4) : 4;
+  for (int t = 0; t < TPW; ++t) {
+    const int tile = tile0 + t * NT_CW;
+    if (tile >= n_tp) break;
+    if (t + 1 < TPW) buf[(t + 1) & 1].load(tile + NT_CW, lane, P, qmp, st0, st1);
+    const NlTipsTile<T>& b = buf[t & 1];
+    double contrib[2] = {0.0, 0.0};
 #pragma unroll
-    for (int c = 0; c < C; ++c) {
-      if (live) {
-        ld4(qmp + ((size_t)c * P + p[u]) * 4, qm[u][c]);
-      } else {
+    for (int u = 0; u < R; ++u) {
+      double den = 0.0, num0 = 0.0, num1 = 0.0;
 #pragma unroll
-        for (int x = 0; x < 4; ++x) qm[u][c][x] = T(0);
+      for (int c = 0; c < C; ++c) {
+        T a0[4], a1[4], d0[4], d1[4];
+        ld4(&tabA[0][c][b.z0[u]][0], a0);
+        ld4(&tabA[1][c][b.z1[u]][0], a1);
+        ld4(&tabD[0][c][b.z0[u]][0], d0);
+        ld4(&tabD[1][c][b.z1[u]][0], d1);
+        T dd = T(0), n0 = T(0), n1 = T(0);
+#pragma unroll
+        for (int x = 0; x < 4; ++x) {
+          const T u0 = b.qm[u][c][x] * a1[x], u1 = b.qm[u][c][x] * a0[x];
+          dd = fma(u0, a0[x], dd);
+          n0 = fma(u0, d0[x], n0);
+          n1 = fma(u1, d1[x], n1);
+        }
+        const double cw = md.catw[c], cwr = cw * md.catr[c];
+        den = fma(cw, (double)dd, den);
+        num0 = fma(cwr, (double)n0, num0);
+        num1 = fma(cwr, (double)n1, num1);
+      }
+      if (b.p[u] < P) {
+        const double w = md.weights[b.p[u]], r0 = num0 / den, r1 = num1 / den;
+        if (md.site_out != nullptr) {
+          md.site_out[(size_t)slot0 * P + b.p[u]] = r0;
+          md.site_out[(size_t)slot1 * P + b.p[u]] = r1;
+        }
+        contrib[0] += w * r0;
+        contrib[1] += w * r1;
       }
     }
-  }
 #pragma unroll
-  for (int u = 0; u < R; ++u) {
-    double den = 0.0, num0 = 0.0, num1 = 0.0;
-#pragma unroll
-    for (int c = 0; c < C; ++c) {
-      T a0[4], a1[4], d0[4], d1[4];
-      ld4(&tabA[0][c][z0[u]][0], a0);
-      ld4(&tabA[1][c][z1[u]][0], a1);
-      ld4(&tabD[0][c][z0[u]][0], d0);
-      ld4(&tabD[1][c][z1[u]][0], d1);
-      T dd = T(0), n0 = T(0), n1 = T(0);
-#pragma unroll
-      for (int x = 0; x < 4; ++x) {
-        const T u0 = qm[u][c][x] * a1[x], u1 = qm[u][c][x] * a0[x];
-        dd = fma(u0, a0[x], dd);
-        n0 = fma(u0, d0[x], n0);
-        n1 = fma(u1, d1[x], n1);
-      }
-      const double cw = md.catw[c], cwr = cw * md.catr[c];
-      den = fma(cw, (double)dd, den);
-      num0 = fma(cwr, (double)n0, num0);
-      num1 = fma(cwr, (double)n1, num1);
+    for (int k = 0; k < 2; ++k) {
+      double v = contrib[k];
+      v += __shfl_xor_sync(0xffffffffu, v, 1);
+      v += __shfl_xor_sync(0xffffffffu, v, 2);
+      v += __shfl_xor_sync(0xffffffffu, v, 4);
+      if ((lane & 7) == 0) grad_partial[(size_t)(k ? slot1 : slot0) * n_part + tile * NT_CW + (lane >> 3)] = v;
     }
-    if (p[u] < P) {
-      const double w = md.weights[p[u]], r0 = num0 / den, r1 = num1 / den;
-      if (md.site_out != nullptr) {
-        md.site_out[(size_t)it.slot[0] * P + p[u]] = r0;
-        md.site_out[(size_t)it.slot[1] * P + p[u]] = r1;
-      }
-      contrib[0] += w * r0;
-      contrib[1] += w * r1;
-    }
-  }
-#pragma unroll
-  for (int k = 0; k < 2; ++k) {
-    double v = contrib[k];
-    v += __shfl_xor_sync(0xffffffffu, v, 1);
-    v += __shfl_xor_sync(0xffffffffu, v, 2);
-    v += __shfl_xor_sync(0xffffffffu, v, 4);
-    if ((lane & 7) == 0) grad_partial[(size_t)it.slot[k] * n_part + tile * NT_CW + (lane >> 3)] = v;
   }
   if (!wait_first) pdl_wait();
 }
