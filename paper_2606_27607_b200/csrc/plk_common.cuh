@@ -95,6 +95,13 @@ __device__ __forceinline__ void ld4(const float* p, float v[4]) {
   const float4 a = *reinterpret_cast<const float4*>(p);
   v[0] = a.x; v[1] = a.y; v[2] = a.z; v[3] = a.w;
 }
+// the same from GLOBAL memory in one 256-bit request per lane (sm_100: ld.global.v4.f64; 32-byte aligned): a warp whose
+// lanes take consecutive cells then touches every 128-byte line once instead of twice (two 16-byte halves at a
+// 32-byte stride).  volatile: stays behind griddepcontrol.wait.
+__device__ __forceinline__ void ldg4(const double* p, double v[4]) {
+  asm volatile("ld.global.v4.f64 {%0,%1,%2,%3}, [%4];" : "=d"(v[0]), "=d"(v[1]), "=d"(v[2]), "=d"(v[3]) : "l"(p));
+}
+__device__ __forceinline__ void ldg4(const float* p, float v[4]) { ld4(p, v); }
 __device__ __forceinline__ void st4(double* p, const double v[4]) {
   reinterpret_cast<double2*>(p)[0] = make_double2(v[0], v[1]);
   reinterpret_cast<double2*>(p)[1] = make_double2(v[2], v[3]);

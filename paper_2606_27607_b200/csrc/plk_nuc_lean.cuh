@@ -347,7 +347,7 @@ struct NlTipsTile {  // what a lane reads for its R patterns of one tile
 #pragma unroll
       for (int c = 0; c < C; ++c) {
         if (live) {
-          ld4(qmp + ((size_t)c * P + p[u]) * 4, qm[u][c]);
+          ldg4(qmp + ((size_t)c * P + p[u]) * 4, qm[u][c]);
         } else {
 #pragma unroll
           for (int x = 0; x < 4; ++x) qm[u][c][x] = T(0);
