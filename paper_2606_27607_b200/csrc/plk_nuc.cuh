@@ -76,9 +76,9 @@ __device__ __forceinline__ void mvt4(const T* __restrict__ M, const T v[4], T a[
 template <typename T>
 __device__ __forceinline__ void operand4(int kind, const void* ptr, int c, int p, int P, T x[4]) {
   if (kind == KIND_PARTIALS) {
-    ld4(static_cast<const T*>(ptr) + ((size_t)c * P + p) * 4, x);
+    ldg4c(static_cast<const T*>(ptr) + ((size_t)c * P + p) * 4, x);
   } else if (kind == KIND_BCAST) {
-    ld4(static_cast<const T*>(ptr) + (size_t)p * 4, x);
+    ldg4c(static_cast<const T*>(ptr) + (size_t)p * 4, x);
   } else if (kind == KIND_STATES) {
     const int z = static_cast<const uint8_t*>(ptr)[p];
 #pragma unroll
@@ -190,7 +190,7 @@ __device__ __forceinline__ void post4_cell(const DevOp& op, const T* __restrict_
   if (live) {
     T* dest = static_cast<T*>(op.dest);
 #pragma unroll
-    for (int i = 0; i < Mp::CPT; ++i) st4(dest + ((size_t)(g * Mp::CPT + i) * P + p) * 4, r[i]);
+    for (int i = 0; i < Mp::CPT; ++i) stg4c(dest + ((size_t)(g * Mp::CPT + i) * P + p) * 4, r[i]);
   }
 }
 
