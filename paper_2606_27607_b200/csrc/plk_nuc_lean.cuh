@@ -272,7 +272,7 @@ __global__ void __launch_bounds__(NT_THREADS, 4) k_pre4_lean(const DevPreItem* _
           T v[4];
 #pragma unroll
           for (int x = 0; x < 4; ++x) v[x] = q0[u][x] * f;
-          st4(static_cast<T*>(it.q[0]) + ((size_t)g * P + p[u]) * 4, v);
+          stg4c(static_cast<T*>(it.q[0]) + ((size_t)g * P + p[u]) * 4, v);
         }
       }
       if (!TIP1) {
@@ -285,7 +285,7 @@ __global__ void __launch_bounds__(NT_THREADS, 4) k_pre4_lean(const DevPreItem* _
           T v[4];
 #pragma unroll
           for (int x = 0; x < 4; ++x) v[x] = q1[u][x] * f;
-          st4(static_cast<T*>(it.q[1]) + ((size_t)g * P + p[u]) * 4, v);
+          stg4c(static_cast<T*>(it.q[1]) + ((size_t)g * P + p[u]) * 4, v);
         }
       }
       // ---- category sums: den on every lane, num_0 on the lanes of g = 0, num_1 on those of g = 1
