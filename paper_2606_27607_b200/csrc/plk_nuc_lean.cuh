@@ -66,6 +66,20 @@ struct NlRows {
   static constexpr int R = sizeof(T) == 4 ? 2 : 1;
 };
 
+// one cell of a staged operand tile.  fp64: a cell is 32 bytes and a 128-bit shared-memory load serves 8 lanes per
+// phase, so 8 consecutive cells read half by half hit every bank group twice (2-way conflict: a third of all the
+// kernel's shared-memory wavefronts, profiles/r01_nuc_pre4_lean_fp64.txt).  Lanes 4..7 of each group of 8 therefore
+// read the upper half first: each phase then covers 8 distinct 16-byte bank groups.
+__device__ __forceinline__ void ld4_cell(const double* p, double v[4], bool swap) {
+  const double2* q = reinterpret_cast<const double2*>(p);
+  const double2 a = q[swap ? 1 : 0], b = q[swap ? 0 : 1];
+  v[0] = swap ? b.x : a.x;
+  v[1] = swap ? b.y : a.y;
+  v[2] = swap ? a.x : b.x;
+  v[3] = swap ? a.y : b.y;
+}
+__device__ __forceinline__ void ld4_cell(const float* p, float v[4], bool) { ld4(p, v); }
+
 // a[u][s] = sum_x M[s][x] v[u][x] / sum_x M[x][s] v[u][x] for R vectors at once
 template <typename T, int R>
 __device__ __forceinline__ void mv4r(const T* __restrict__ M, const T (&v)[R][4], T (&a)[R][4]) {
@@ -200,7 +214,7 @@ __global__ void __launch_bounds__(NT_THREADS, 4) k_pre4_lean(const DevPreItem* _
     } else {
       T x0[R][4];
 #pragma unroll
-      for (int u = 0; u < R; ++u) ld4(sOp + ((C + g) * TP + r[u]) * 4, x0[u]);
+      for (int u = 0; u < R; ++u) ld4_cell(sOp + ((C + g) * TP + r[u]) * 4, x0[u], (pl & 4) != 0);
       mv4r<T, R>(sM0, x0, a0);
       mvq4r<T, R>(Qc, x0, qx0);
     }
@@ -218,7 +232,7 @@ __global__ void __launch_bounds__(NT_THREADS, 4) k_pre4_lean(const DevPreItem* _
     } else {
       T x1[R][4];
 #pragma unroll
-      for (int u = 0; u < R; ++u) ld4(sOp + ((2 * C + g) * TP + r[u]) * 4, x1[u]);
+      for (int u = 0; u < R; ++u) ld4_cell(sOp + ((2 * C + g) * TP + r[u]) * 4, x1[u], (pl & 4) != 0);
       mv4r<T, R>(sM1, x1, a1);
       mvq4r<T, R>(Qc, x1, qx1);
     }
@@ -226,7 +240,7 @@ __global__ void __launch_bounds__(NT_THREADS, 4) k_pre4_lean(const DevPreItem* _
 #pragma unroll
     for (int u = 0; u < R; ++u) {
       T qm[4];
-      ld4(sOp + (g * TP + r[u]) * 4, qm);
+      ld4_cell(sOp + (g * TP + r[u]) * 4, qm, (pl & 4) != 0);
       dd[u] = T(0);
 #pragma unroll
       for (int x = 0; x < 4; ++x) {
