@@ -247,7 +247,7 @@ def oracle_time(wl, n_sample, repeats=1):
 
 # measured DRAM traffic per step (bytes) of the dominant kernel's launches, keyed by (workload, precision, kernel)
 # (profiles/r01_launches_cfg1_fp64.md: dram__bytes_read.sum + dram__bytes_write.sum summed over the launches of one step)
-NCU_DRAM_BYTES = {("cfg1_gtr_128x100000", "fp64", "k_pre4_lean+k_grad4_tips"): 4191.7e6,
+NCU_DRAM_BYTES = {("cfg1_gtr_128x100000", "fp64", "k_pre4_lean+k_grad4_tips"): 4194.4e6,
                   ("cfg1_gtr_128x100000", "fp32", "k_pre4_lean+k_grad4_tips"): 1871.9e6,
                   ("cfg3_gy94_256x20000", "fp32", "k_pre_tc5"): 17075.1e6}
 
