@@ -35,7 +35,6 @@ def build(force: bool = False, verbose: bool = False) -> str:
     flags = [f for f in NVCC_FLAGS if not f.startswith("--use_fast_math")]
     if os.path.exists(os.path.join(CSRC, "plk_tc.cuh")):
         flags.append("-DPLK_WITH_TENSOR")
-    flags += os.environ.get("PLK_NVCC_EXTRA", "").split()  # e.g. -DPLK_TC5_EXP=1 for ablation builds
     cmd = [nvcc] + flags + ["-o", LIB] + [os.path.join(CSRC, s) for s in SOURCES]
     if verbose:
         cmd.insert(1, "-Xptxas=-v")

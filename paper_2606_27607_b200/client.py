@@ -40,19 +40,23 @@ def pre_order_ops(tree, store_tips: bool = False) -> np.ndarray:
 class Evaluator:
     """Holds one library instance loaded with a workload; evaluates logL and the branch-length gradient."""
 
-    def __init__(self, wl, precision=plk.FP64, flags=0, tips_as_partials: bool = False, device="cuda:0",
-                 stream=None, store_tip_pre: bool = False):
+    def __init__(self, wl, precision=plk.FP64, flags=0, tips_as_partials=False, device="cuda:0",
+                 stream=None, store_tip_pre: bool = False, eigen=None):
+        """`tips_as_partials`: False (all tips compact states), True (all tips one-hot / all-ones partials) or a
+        boolean sequence per tip (mixed).  `eigen`: (U, Uinv, lam) handed to plk_set_eigen_decomposition instead of the
+        workload's own (the eigendecomposition is a client-side input)."""
         self.wl = wl
+        self.eigen = eigen
         tree = wl.tree
         self.tree = tree
         N = tree.n_tips
         S = wl.n_states
         self.inst = plk.Instance(
             N, S, wl.n_patterns, wl.n_categories,
-            compact_buffer_count=0 if tips_as_partials else N,
+            compact_buffer_count=N - int(np.sum(np.broadcast_to(np.asarray(tips_as_partials, dtype=bool), (N,)))),
             preorder_slot_count=0 if store_tip_pre else N,  # root + internal nodes (N-1) rounded up
             precision=precision, flags=flags, device=device, stream=stream)
-        self.tips_as_partials = tips_as_partials
+        self.tips_as_partials = np.broadcast_to(np.asarray(tips_as_partials, dtype=bool), (N,)).copy()
         self.ops = post_order_ops(tree)
         self.pre_ops = pre_order_ops(tree, store_tips=store_tip_pre)
         self.branch_nodes = self.pre_ops["node_post"].copy()  # gradient order of pre_order_gradient
@@ -68,14 +72,15 @@ class Evaluator:
         inst.set_state_frequencies(wl.pi)
         inst.set_category_rates(wl.rates)
         inst.set_category_weights(wl.cat_weights)
-        inst.set_eigen_decomposition(0, wl.U, wl.Uinv, wl.lam)
+        U, Uinv, lam = self.eigen if self.eigen is not None else (wl.U, wl.Uinv, wl.lam)
+        inst.set_eigen_decomposition(0, U, Uinv, lam)
         inst.set_rate_matrix(0, wl.Q)
 
     def upload_tips(self):
         wl, inst = self.wl, self.inst
         S = wl.n_states
         for k in range(self.tree.n_tips):
-            if self.tips_as_partials:
+            if self.tips_as_partials[k]:
                 st = wl.tip_states[k]
                 part = np.zeros((wl.n_patterns, S))
                 known = st < S
@@ -86,9 +91,16 @@ class Evaluator:
                 inst.set_tip_states(k, wl.tip_states[k].astype(np.int32))
 
     # -- evaluation with host inputs / outputs
-    def log_likelihood(self, branch_lengths: Optional[np.ndarray] = None, want_site=True, allow_nonfinite=False):
+    def log_likelihood(self, branch_lengths: Optional[np.ndarray] = None, want_site=True, allow_nonfinite=False,
+                       matrices=None):
+        """`matrices`: {node: [C, S, S]} transition matrices supplied by the client (plk_set_transition_matrix)
+        instead of being formed from the eigendecomposition and `branch_lengths`."""
         t = self.tree.branch_length if branch_lengths is None else branch_lengths
-        self.inst.update_transition_matrices(0, self.matrix_idx, np.asarray(t)[self.matrix_idx])
+        if matrices is not None:
+            for k in self.matrix_idx:
+                self.inst.set_transition_matrix(int(k), matrices[int(k)])
+        else:
+            self.inst.update_transition_matrices(0, self.matrix_idx, np.asarray(t)[self.matrix_idx])
         self.inst.update_partials(self.ops)
         return self.inst.root_log_likelihoods(self.tree.root, self.scale_idx, want_site, allow_nonfinite)
 

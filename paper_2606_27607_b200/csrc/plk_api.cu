@@ -96,7 +96,8 @@ bool compute_layout(const plk_config& c, Layout& L) {
   L.off_rates = take((size_t)L.C * 8);
   L.off_catw = take((size_t)L.C * 8);
   L.off_site = take((size_t)L.P * 8);
-  L.off_block_partial = take((size_t)(L.P / 32 + 2) * 8);
+  // one partial per block of k_root (128 threads, G threads per pattern: G = 1 for SP = 4, 16 for SP = 64)
+  L.off_block_partial = take(((size_t)L.P * (L.SP == 4 ? 1 : 16) + 127) / 128 * 8 + 8);
   L.off_grad_partial = take((size_t)L.max_grad * L.n_tiles * 8);
   L.off_grad_out = take((size_t)L.max_grad * 8);
   L.off_logl = take(64);
@@ -140,7 +141,8 @@ struct plk_instance {
   int64_t launches = 0;
   int sm_count = 148;
   int nt_bps[2][2] = {{0, 0}, {0, 0}};  // resident CTAs per SM of the TMA kernels [post|pre][level|walk]
-  int grad_parts = 0;  // partial sums per gradient slot written by the last gradient launch (row stride L.n_tiles)
+  int lean_bps[3] = {0, 0, 0};          // the same for k_pre4_lean<T, CLS> (T is fixed per instance)
+  int grad_parts = 0;  // partial sums per gradient slot written by the LAST gradient launch (row stride L.n_tiles)
 
   template <typename X> X* at(size_t off) const { return reinterpret_cast<X*>(arena + off); }
   void* post_ptr(int idx) const {
@@ -496,7 +498,7 @@ int launch_pre4_lean_c(plk_instance* in, const DevPreItem* d_items, int n, const
   const Layout& L = in->L;
   using St = NtStage<T, NL_C, 3, true, NlRows<T>::R>;
   const size_t smem = (size_t)NT_NS * St::BYTES;
-  static int bps = 0;  // per instantiation
+  int& bps = in->lean_bps[CLS];
   if (bps == 0) {
     CU(cudaFuncSetAttribute(k_pre4_lean<T, CLS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&bps, k_pre4_lean<T, CLS>, NT_THREADS, smem));
@@ -675,9 +677,10 @@ int plk_create(const plk_config* cfg, void* d_arena, size_t arena_bytes, void* c
   int n_dev = 0;
   if (cudaGetDeviceCount(&n_dev) != cudaSuccess || n_dev == 0) return PLK_ERR_CUDA;
   int dev = 0, sms = 0;
-  if (cudaGetDevice(&dev) != cudaSuccess ||
-      cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || sms < 1)
-    return PLK_ERR_CUDA;
+  cudaPointerAttributes pa;
+  if (cudaPointerGetAttributes(&pa, d_arena) != cudaSuccess || pa.type != cudaMemoryTypeDevice) return PLK_ERR_CUDA;
+  dev = pa.device;  // the arena's device (the caller keeps it current while it uses the instance)
+  if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || sms < 1) return PLK_ERR_CUDA;
   plk_instance* in = new (std::nothrow) plk_instance();
   if (in == nullptr) return PLK_ERR_OUT_OF_MEMORY;
   in->cfg = *cfg;
@@ -1147,7 +1150,7 @@ static int root_impl(plk_instance* in, int root, const int32_t* scale_idx, int s
     return PLK_SUCCESS;
   });
   CHECK_LAUNCH(in);
-  k_sum_rows<<<1, 128, 0, in->stream>>>(bp, n_blocks, n_blocks, d_sum);
+  k_sum_rows<<<1, 128, 0, in->stream>>>(bp, nullptr, n_blocks, n_blocks, d_sum);
   CHECK_LAUNCH(in);
   return PLK_SUCCESS;
 }
@@ -1310,6 +1313,7 @@ static int pre_impl(plk_instance* in, int eigen, int root_pre, const plk_pre_op*
       }
   }
   const int n_items = (int)items.size();
+  std::vector<int> slot_parts(count > 0 ? count : 0, 0);  // partial sums per gradient slot (0: nothing written)
   if (n_items > 0) {
     std::vector<int> level_start(n_levels + 1, 0);
     for (const HostItem& hi : items) ++level_start[hi.level + 1];
@@ -1344,6 +1348,13 @@ static int pre_impl(plk_instance* in, int eigen, int root_pre, const plk_pre_op*
       CHECK_LAUNCH(in);
     }
 #endif
+    // Every gradient kernel writes its own number of partial sums per slot (tile geometry differs between the
+    // class-specialised, the general TMA and the register-staged kernels): remember it per slot for k_sum_rows.
+    auto mark_parts = [&](int first, int n) {
+      for (int i = first; i < first + n; ++i)
+        for (int k = 0; k < 2; ++k)
+          if (hit[i].slot[k] >= 0) slot_parts[hit[i].slot[k]] = in->grad_parts;
+    };
     if (walk) {
       rc = by_precision(in, [&](auto tag) -> int {
         using T = decltype(tag);
@@ -1351,6 +1362,7 @@ static int pre_impl(plk_instance* in, int eigen, int root_pre, const plk_pre_op*
                                : launch_pre4_walk<T>(in, dit, n_items, static_cast<const T*>(Q), d_site);
       });
       if (rc) return rc;
+      mark_parts(0, n_items);
     }
     if (!walk && L.SP == 4 && class_start[(size_t)(n_levels - 1) * 5 + 3] > 0) {
       // some items run on the class-specialised kernels: their compact-tip children read D = M Q (one 4 x 4 product
@@ -1377,6 +1389,7 @@ static int pre_impl(plk_instance* in, int eigen, int root_pre, const plk_pre_op*
                                      first_launch);
         });
         if (rc) return rc;
+        mark_parts(c0, m);
         first_launch = false;
       }
       const int g0 = class_start[(size_t)l * 5 + 3];
@@ -1391,11 +1404,19 @@ static int pre_impl(plk_instance* in, int eigen, int root_pre, const plk_pre_op*
                                  : launch_pre4<T>(in, p0, m, static_cast<const T*>(Q), d_site);
         });
         if (rc) return rc;
+        mark_parts(g0 + first, m);
       }
     }
   }
   if (want_grad && count > 0) {
-    k_sum_rows<<<count, 128, 0, in->stream>>>(in->at<double>(L.off_grad_partial), in->grad_parts, L.n_tiles, d_grad);
+    char *h, *d;
+    rc = ring_alloc(in, (size_t)count * sizeof(int), &h, &d);
+    if (rc) return rc;
+    std::memcpy(h, slot_parts.data(), (size_t)count * sizeof(int));
+    rc = copy_ring(in, h, d, (size_t)count * sizeof(int));
+    if (rc) return rc;
+    k_sum_rows<<<count, 128, 0, in->stream>>>(in->at<double>(L.off_grad_partial), reinterpret_cast<const int*>(d), 0,
+                                              L.n_tiles, d_grad);
     CHECK_LAUNCH(in);
   }
   return PLK_SUCCESS;
@@ -1474,7 +1495,7 @@ int plk_branch_derivatives(plk_instance* in, int eigen, const int32_t* post_idx,
     });
     if (rc) return rc;
   }
-  k_sum_rows<<<count, 128, 0, in->stream>>>(in->at<double>(L.off_grad_partial), in->grad_parts, L.n_tiles,
+  k_sum_rows<<<count, 128, 0, in->stream>>>(in->at<double>(L.off_grad_partial), nullptr, in->grad_parts, L.n_tiles,
                                             in->at<double>(L.off_grad_out));
   CHECK_LAUNCH(in);
   return finish_gradient(in, count, out_gradient, out_site, d_site);

@@ -384,10 +384,12 @@ __global__ void __launch_bounds__(128) k_root(const T* __restrict__ root, int ki
 }
 
 // out[slot] = sum_i partial[slot][i] in a fixed order (deterministic: SURVEY section 7 hard part 8)
-__global__ void __launch_bounds__(128) k_sum_rows(const double* __restrict__ partial, int n, int stride,
-                                                  double* __restrict__ out) {
+// n_per_row[r] (or n when n_per_row == NULL) = how many partial sums the kernel that served row r has written.
+__global__ void __launch_bounds__(128) k_sum_rows(const double* __restrict__ partial, const int* __restrict__ n_per_row,
+                                                  int n, int stride, double* __restrict__ out) {
   __shared__ double red[4];
   const double* row = partial + (size_t)blockIdx.x * stride;
+  if (n_per_row != nullptr) n = n_per_row[blockIdx.x];
   double v = 0.0;
   for (int i = threadIdx.x; i < n; i += 128) v += row[i];
   const double s = block_sum(v, red);

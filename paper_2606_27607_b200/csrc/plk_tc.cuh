@@ -614,12 +614,9 @@ __global__ void __launch_bounds__(TC_THREADS, 1) k_pre_tc(const DevPreItem* __re
 template <typename T>
 int tc_launch_post(cudaStream_t stream, const DevOp* d_ops, int n_ops, int P, int S, int C, int sm_count,
                    int64_t* launches) {
-  static bool opted = false;  // per template instantiation
-  if (!opted) {
-    if (cudaFuncSetAttribute(k_post_tc<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)tc_post_smem<T>()) != cudaSuccess)
-      return PLK_ERR_CUDA;
-    opted = true;
-  }
+  // per device and cheap: no process-wide "done" flag (instances may live on several GPUs)
+  if (cudaFuncSetAttribute(k_post_tc<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)tc_post_smem<T>()) != cudaSuccess)
+    return PLK_ERR_CUDA;
   const int n_tiles = (P + Tc<T>::TP - 1) / Tc<T>::TP;
   const long long total = (long long)n_ops * C * n_tiles;
   if (total <= 0) return PLK_SUCCESS;
@@ -635,13 +632,10 @@ template <typename T>
 int tc_launch_pre(cudaStream_t stream, const DevPreItem* d_items, int n, int P, int S, int C, const T* Q,
                   const double* catw, const double* catr, const double* weights, double* grad_partial, int n_part,
                   double* site, int* n_parts, int64_t* launches) {
-  static bool opted = false;
-  if (!opted) {
-    if (cudaFuncSetAttribute(k_pre_tc<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)tc_pre_smem<T>()) !=
-        cudaSuccess)
-      return PLK_ERR_CUDA;
-    opted = true;
-  }
+  // per device and cheap: no process-wide "done" flag (instances may live on several GPUs)
+  if (cudaFuncSetAttribute(k_pre_tc<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)tc_pre_smem<T>()) !=
+      cudaSuccess)
+    return PLK_ERR_CUDA;
   const int n_tiles = (P + Tc<T>::TP - 1) / Tc<T>::TP;
   *n_parts = n_tiles;
   if (n <= 0) return PLK_SUCCESS;

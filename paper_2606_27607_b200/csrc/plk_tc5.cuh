@@ -37,12 +37,6 @@
 namespace plk {
 namespace tc5 {
 
-// PLK_TC5_EXP: ablation builds for bottleneck hunting (results are WRONG): 1 = epilogue without staging / global
-// stores, 2 = producers write nothing, 3 = one MMA per child, 4 = no pending-maxima loads in the epilogue
-#ifndef PLK_TC5_EXP
-#define PLK_TC5_EXP 0
-#endif
-
 constexpr int TP = 128;                    // patterns per tile = MMA M
 constexpr int EPI_WARPS = 8, PROD_WARPS = 8, N_WARPS = EPI_WARPS + PROD_WARPS + 1;
 constexpr int THREADS = N_WARPS * 32;      // 544
@@ -257,8 +251,7 @@ __device__ __forceinline__ void prod_store(const Ctx& cx, const Item& it, int k,
   const int kind = cx.ops[it.op].kind[k];
   const uint32_t xhi = cx.smem + OFF_X + (2 * k) * X_PLANE + swz_off(gt >> 4, gt & 15, TP), xlo = xhi + X_PLANE;
   mbar_wait(cx.barrier(B_EMPTY0 + k), (it.n & 1) ^ 1);
-  if (PLK_TC5_EXP == 2) {
-  } else if (kind == KIND_PARTIALS || kind == KIND_BCAST) {
+  if (kind == KIND_PARTIALS || kind == KIND_BCAST) {
 #pragma unroll
     for (int j = 0; j < XCHUNKS; ++j) {
       float4 h, l;
@@ -366,7 +359,7 @@ __global__ void __launch_bounds__(THREADS, 1) k_post_tc5(const DevOp* __restrict
         const float* m = static_cast<const float*>(o.cscale[k]);
 #pragma unroll
         for (int c = 0; c < 4; ++c)
-          raw[k][c] = (PLK_TC5_EXP != 4 && m != nullptr && p < P && c < C) ? __ldg(m + (size_t)c * P + p) : 0.f;
+          raw[k][c] = (m != nullptr && p < P && c < C) ? __ldg(m + (size_t)c * P + p) : 0.f;
       }
     };
     auto finish_raw = [&](const Item& t, int k) {
@@ -405,42 +398,38 @@ __global__ void __launch_bounds__(THREADS, 1) k_post_tc5(const DevOp* __restrict
         tc_fence_before();
         __syncwarp();
         if (lane == 0) mbar_arrive(cx.barrier(B_TEMPTY0 + a));
-        if (PLK_TC5_EXP != 1) {
-          if (one_factor) {  // the usual case: each pending exponent fits one power-of-two factor
+        if (one_factor) {  // the usual case: each pending exponent fits one power-of-two factor
 #pragma unroll
-            for (int q = 0; q < 8; ++q) {
-              float v[4];
+          for (int q = 0; q < 8; ++q) {
+            float v[4];
 #pragma unroll
-              for (int j = 0; j < 4; ++j) {
-                v[j] = (__uint_as_float(d0[4 * q + j]) * f0.f1) * (__uint_as_float(d1[4 * q + j]) * f1.f1);
-                mx = fmaxf(mx, v[j]);
-              }
-              sts128(stage + lane * 128 + ((q ^ (lane & 7)) << 4), make_float4(v[0], v[1], v[2], v[3]));
+            for (int j = 0; j < 4; ++j) {
+              v[j] = (__uint_as_float(d0[4 * q + j]) * f0.f1) * (__uint_as_float(d1[4 * q + j]) * f1.f1);
+              mx = fmaxf(mx, v[j]);
             }
-          } else {
+            sts128(stage + lane * 128 + ((q ^ (lane & 7)) << 4), make_float4(v[0], v[1], v[2], v[3]));
+          }
+        } else {
 #pragma unroll
-            for (int q = 0; q < 8; ++q) {
-              float v[4];
+          for (int q = 0; q < 8; ++q) {
+            float v[4];
 #pragma unroll
-              for (int j = 0; j < 4; ++j) {
-                v[j] = ((__uint_as_float(d0[4 * q + j]) * f0.f1) * f0.f2) * ((__uint_as_float(d1[4 * q + j]) * f1.f1) * f1.f2);
-                mx = fmaxf(mx, v[j]);
-              }
-              sts128(stage + lane * 128 + ((q ^ (lane & 7)) << 4), make_float4(v[0], v[1], v[2], v[3]));
+            for (int j = 0; j < 4; ++j) {
+              v[j] = ((__uint_as_float(d0[4 * q + j]) * f0.f1) * f0.f2) * ((__uint_as_float(d1[4 * q + j]) * f1.f1) * f1.f2);
+              mx = fmaxf(mx, v[j]);
             }
+            sts128(stage + lane * 128 + ((q ^ (lane & 7)) << 4), make_float4(v[0], v[1], v[2], v[3]));
           }
         }
       }
       // the upper column half's row maximum travels through shared memory (double-buffered by item parity)
       if (half == 1) sts32(cx.smem + OFF_MAX + (a * TP + 32 * quarter + lane) * 4, mx);
       __syncwarp();
-      if (PLK_TC5_EXP != 1) {
 #pragma unroll
-        for (int j = 0; j < 8; ++j) {
-          const int idx = j * 32 + lane, r = idx >> 3, ch = idx & 7;
-          const float4 v = lds128(stage + r * 128 + ((ch ^ (r & 7)) << 4));
-          if (prow0 + r < P) *reinterpret_cast<float4*>(dest + (size_t)(prow0 + r) * SP64 + half * 32 + ch * 4) = v;
-        }
+      for (int j = 0; j < 8; ++j) {
+        const int idx = j * 32 + lane, r = idx >> 3, ch = idx & 7;
+        const float4 v = lds128(stage + r * 128 + ((ch ^ (r & 7)) << 4));
+        if (prow0 + r < P) *reinterpret_cast<float4*>(dest + (size_t)(prow0 + r) * SP64 + half * 32 + ch * 4) = v;
       }
       asm volatile("bar.sync 1, %0;" ::"n"(EPI_WARPS * 32) : "memory");
       if (half == 0 && p < P && scale != nullptr)
@@ -503,15 +492,15 @@ __global__ void __launch_bounds__(THREADS, 1) k_post_tc5(const DevOp* __restrict
         uint32_t acc = 0;
         if (has_lo) {  // x_lo . m_hi
 #pragma unroll
-          for (int ks = 0; ks < (PLK_TC5_EXP == 3 ? 0 : 8); ++ks) {
+          for (int ks = 0; ks < 8; ++ks) {
             umma_tf32<0>(d, dxlo + koff(ks, TP), dmhi + koff(ks, 64), acc);
             acc = 1;
           }
         }
 #pragma unroll
-        for (int ks = 0; ks < (PLK_TC5_EXP == 3 ? 1 : 8); ++ks) {  // x_hi . m_lo + x_hi . m_hi, the A slice fetched once
+        for (int ks = 0; ks < 8; ++ks) {  // x_hi . m_lo + x_hi . m_hi, the A slice fetched once
           umma_tf32<1>(d, dxhi + koff(ks, TP), dmlo + koff(ks, 64), acc);
-          if (PLK_TC5_EXP != 3) umma_tf32<2>(d, dxhi + koff(ks, TP), dmhi + koff(ks, 64), 1);
+          umma_tf32<2>(d, dxhi + koff(ks, TP), dmhi + koff(ks, 64), 1);
           acc = 1;
         }
         umma_commit(cx.barrier(B_EMPTY0 + k));
@@ -532,12 +521,9 @@ __global__ void __launch_bounds__(THREADS, 1) k_post_tc5(const DevOp* __restrict
 
 inline int launch_post(cudaStream_t stream, const DevOp* d_ops, int n_ops, int P, int S, int C, int sm_count,
                        int64_t* launches) {
-  static bool opted = false;
-  if (!opted) {
-    if (cudaFuncSetAttribute(k_post_tc5, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_BYTES) != cudaSuccess)
-      return PLK_ERR_CUDA;
-    opted = true;
-  }
+  // per device and cheap: no process-wide "done" flag (instances may live on several GPUs)
+  if (cudaFuncSetAttribute(k_post_tc5, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_BYTES) != cudaSuccess)
+    return PLK_ERR_CUDA;
   const long long total = (long long)n_ops * C * ((P + TP - 1) / TP);
   if (total <= 0) return PLK_SUCCESS;
   const int grid = total < sm_count ? (int)total : sm_count;

@@ -663,12 +663,9 @@ inline int launch_pre(cudaStream_t stream, const DevPreItem* d_items, int n, int
                       long long mat_t_delta,
                       const double* catw, const double* catr, const double* weights, double* grad_partial, int n_part,
                       double* site, int sm_count, int* n_parts, int64_t* launches) {
-  static bool opted = false;
-  if (!opted) {
-    if (cudaFuncSetAttribute(k_pre_tc5, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_BYTES_PRE) != cudaSuccess)
-      return PLK_ERR_CUDA;
-    opted = true;
-  }
+  // per device and cheap: no process-wide "done" flag (instances may live on several GPUs)
+  if (cudaFuncSetAttribute(k_pre_tc5, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_BYTES_PRE) != cudaSuccess)
+    return PLK_ERR_CUDA;
   const int n_tiles = (P + TP - 1) / TP;
   *n_parts = n_tiles;
   const long long total = (long long)n * n_tiles;
