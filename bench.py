@@ -6,9 +6,12 @@
 One "step" = one full evaluation as an HMC step needs it: transition matrices for all 2N-2 branches,
 post-order partials over the whole tree with rescaling, root log-likelihood, pre-order partials fused with all 2N-2
 branch-length derivatives.  Default workload: BASELINE.json configs[1] (GTR, 128 taxa, 100 000 patterns, 4 gamma
-categories, 5% tip ambiguity), fp64.  Prints ONE JSON line (rank 0).  Multi-GPU: the path does not shard
-(north_star: "no sharding or collectives across GPUs") -> N independent replicas, scaling "weak".
-The oracle (oracle/) is executed only by the cpu_baseline leg and by --impl reference.
+categories, 5% tip ambiguity), fp64.  Prints ONE JSON line (rank 0).  Multi-GPU (--gpus N; the driver launches N
+ranks with torchrun, a plain `python bench.py --gpus N` re-launches itself that way): by default N independent
+replicas, scaling "weak" (north_star: "no sharding or collectives across GPUs"); with --shard-patterns the pattern
+axis is split into N contiguous ranges, one instance per GPU, and logL + the 2N-2 derivatives are summed with ONE
+all-reduce per evaluation, scaling "strong".
+The oracle (oracle/) is executed only by the cpu_baseline / parity leg and by --impl reference.
 """
 import argparse
 import json
@@ -52,6 +55,9 @@ def parse_args():
                          "line with the 20 points instead of the headline line")
     ap.add_argument("--no-extras", action="store_true", help="skip the other configs / precisions")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--shard-patterns", action="store_true",
+                    help="N > 1: split the pattern axis over the ranks (one all-reduce of 1 + 2N-2 doubles per "
+                         "evaluation) instead of running N independent replicas")
     return ap.parse_args()
 
 

@@ -129,13 +129,18 @@ class Evaluator:
         return grad
 
     # -- device-resident step used by bench.py: nothing but launches, outputs stay on the device
-    def make_device_io(self):
+    def make_device_io(self, out=None):
+        """`out`: optional fp64 device tensor [1 + 2N-2] that receives [logL, gradient] (one buffer, so that a
+        multi-GPU caller can all-reduce it as it is: sharded.py)."""
         torch = self.inst.torch
         dev = self.inst.device
         t = np.asarray(self.tree.branch_length)[self.matrix_idx]
         self.d_t = torch.from_numpy(np.ascontiguousarray(t)).to(dev)
-        self.d_logl = torch.zeros(1, dtype=torch.float64, device=dev)
-        self.d_grad = torch.zeros(len(self.pre_ops), dtype=torch.float64, device=dev)
+        if out is None:
+            out = torch.zeros(1 + len(self.pre_ops), dtype=torch.float64, device=dev)
+        self.d_out = out
+        self.d_logl = out[:1]
+        self.d_grad = out[1:]
 
     def step_matrices(self):
         self.inst.update_transition_matrices_device(0, self.matrix_idx, self.d_t)

@@ -150,6 +150,26 @@ def test_worked_example_w1():
     _worked(W1, TREE4, 6, T4, Q, pi, 4, lambda x: int(x))
 
 
+def test_weighted_sums_and_conditioning_from_the_printed_w1_values():
+    """evaluate() on all five W1 patterns at once with pattern weights != 1: logL = sum_p omega_p logl_p,
+    grad_k = sum_p omega_p d_kp and cond_k = A_k = sum_p omega_p |d_kp| must equal the same sums
+    formed from the PRINTED per-pattern values (tests/golden/w1_nucleotide.txt).  Patterns 0, 2, 4 have negative and
+    positive derivatives on the same branch, so dropping the weight, the absolute value or the sign shows."""
+    Q, pi = models.hky(2.0, [0.1, 0.2, 0.3, 0.4])
+    omega = np.array([3.0, 1.0, 7.0, 2.0, 5.0])
+    for cn, (rates, w) in {"c1": (np.ones(1), np.ones(1)), "c4": _gamma4()}.items():
+        tips = np.array([[int(x) for x in W1[f"case{i}.tips"]] for i in range(5)]).T  # [tip][pattern]
+        d = np.array([W1[f"case{i}.{cn}.grad"] for i in range(5)])                      # [pattern][branch 0..5]
+        ll = np.array([W1[f"case{i}.{cn}.logl"][0] for i in range(5)])
+        r = lk.evaluate(TREE4, 6, T4, Q, pi, rates, w, _tips(tips, 4), omega, chunk=2, keep_site_derivatives=True)
+        assert abs(r["logL"] - np.dot(omega, ll)) < 1e-11
+        assert np.abs(r["grad"][:6] - omega @ d).max() < 1e-11
+        assert np.abs(r["cond"][:6] - omega @ np.abs(d)).max() < 1e-11
+        assert np.all(r["cond"][:6] > np.abs(r["grad"][:6]) + 1.0)  # mixed signs: A_k is not |g_k|
+        assert r["grad"][6] == 0.0 and r["cond"][6] == 0.0
+        assert np.abs(r["site_derivs"][:6].T - d).max() < 2e-12
+
+
 def test_worked_example_w2():
     Q, pi = models.gy94(2.0, 0.3, (0.1, 0.2, 0.3, 0.4), (0.4, 0.3, 0.2, 0.1), (0.25,) * 4)
     cod = models.codon_states()
