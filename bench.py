@@ -71,6 +71,45 @@ def load_peaks():
     return {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "bf16_tflops_sustained": 1400.0, "source": "fallback"}
 
 
+HBM_NOMINAL_GBS = 8000.0  # the "~8 TB/s" BASELINE.json north_star names (report against both)
+
+
+def measure_matmul_peaks(device):
+    """fp64 and TF32 dense matmul throughput of THIS box, measured the way MEASURED_PEAKS.json measured bf16
+    (torch.matmul 8192^3 = cuBLAS, best of 5, CUDA events): the denominators of the codon rooflines (SURVEY 8(d):
+    "peaks for fp64 and TF32 are not in MEASURED_PEAKS.json -- measure them in the same run").  A library GEMM used as
+    a yardstick only; nothing on the product path calls it."""
+    import torch
+
+    out = {}
+    n = 8192
+    flops = 2.0 * n ** 3
+    prev = torch.backends.cuda.matmul.allow_tf32
+    try:
+        for name, dtype, tf32 in (("fp64_tflops", torch.float64, False), ("tf32_tflops", torch.float32, True),
+                                  ("fp32_simt_tflops", torch.float32, False)):
+            torch.backends.cuda.matmul.allow_tf32 = tf32
+            a = torch.randn(n, n, dtype=dtype, device=device)
+            b = torch.randn(n, n, dtype=dtype, device=device)
+            c = torch.empty(n, n, dtype=dtype, device=device)
+            torch.matmul(a, b, out=c)
+            best = None
+            for _ in range(5):
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                e0.record()
+                torch.matmul(a, b, out=c)
+                e1.record()
+                torch.cuda.synchronize()
+                ms = e0.elapsed_time(e1)
+                best = ms if best is None else min(best, ms)
+            out[name] = flops / (best * 1e-3) / 1e12
+            del a, b, c
+    finally:
+        torch.backends.cuda.matmul.allow_tf32 = prev
+    out["how"] = "torch.matmul 8192^3 (2 n^3 flops), best of 5, CUDA events, this run"
+    return out
+
+
 # ---- algorithmic traffic / work of one evaluation (DESIGN.md "Roofline accounting"; SURVEY 8(d)) ----------------
 def algorithmic(N, P, S, C, w):
     SP = 4 if S == 4 else 64
@@ -83,6 +122,27 @@ def algorithmic(N, P, S, C, w):
     pre_flops = 3 * (N - 2) * P * C * mv   # recompute P_j p_j, apply P_k^T, apply Q
     return {"W": W, "post_bytes": post_bytes, "pre_bytes": pre_bytes, "post_flops": post_flops,
             "pre_flops": pre_flops, "updates": (N - 1) * P * C, "grad_units": (2 * N - 2) * P * C}
+
+
+def issued_tensor_flops(N, P, C, precision, kernels):
+    """Flops the 64-state tensor-pipe kernels ISSUE per evaluation (padding 61 -> 64, the three split-TF32 passes of
+    the fp32 kernels, tip edges that travel through the pipe as one-hot rows), as opposed to the algorithmic count
+    above ("report issued flops separately").  Edges: N - 2 internal child edges, N tip edges (compact).
+      mma.sync (plk_tc.cuh)    post: internal edges only (tips are column gathers); pre: a_k, Q x_k, M_k^T u_k for every
+                               edge with partials; fp32 = 3 passes
+      tcgen05 (plk_tc5*.cuh)   post: every edge (one-hot tips: 2 of the 3 passes); pre: a_k and D_k x_k for internal
+                               edges (3 passes), a_k for tip edges through the pipe (2 passes), M_k^T u_k for internal
+                               edges only (3 passes)"""
+    mv = 2.0 * 64 * 64 * P * C
+    n_int, n_tip = N - 2, N
+    passes = 1 if precision == "fp64" else 3
+    if kernels == "tcgen05":
+        post = mv * (3 * n_int + 2 * n_tip)
+        pre = mv * (3 * (2 * n_int) + 2 * n_tip + 3 * n_int)
+    else:
+        post = mv * passes * n_int
+        pre = mv * passes * 3 * n_int
+    return {"post": post, "pre": pre}
 
 
 # ---- nvidia-smi clock sampler (B200_PROFILING.md "clocks DURING the timed region") -------------------------------
@@ -136,21 +196,38 @@ class ClockSampler:
 
 
 # ---- one workload on the GPU -------------------------------------------------------------------------------------
-def measure_device(wl, precision, flags, steps, warmup, peaks, sampler=None, device="cuda:0"):
-    """Device-resident timing: K full evaluations, CUDA events on the launching stream; per-phase events inside."""
+def measure_device(wl, precision, flags, steps, warmup, peaks, sampler=None, device="cuda:0", keep_site=False,
+                   shard=None):
+    """Device-resident timing: K full evaluations, CUDA events on the launching stream; per-phase events inside.
+    shard = (rank, world, dist): this rank evaluates its pattern range and every step ends with the all-reduce of
+    [logL, gradient] (sharded.py); the algorithmic work reported is then this rank's share."""
     import torch
 
-    from paper_2606_27607_b200 import plk
+    from paper_2606_27607_b200 import plk, sharded
     from paper_2606_27607_b200.client import Evaluator
 
-    ev = Evaluator(wl, precision=plk.FP64 if precision == "fp64" else plk.FP32, flags=flags, device=device)
-    ev.make_device_io()
+    prec = plk.FP64 if precision == "fp64" else plk.FP32
+    sh = None
+    if shard is not None:
+        sh = sharded.ShardedEvaluator(wl, shard[0], shard[1], dist=shard[2], device=device, precision=prec, flags=flags)
+        ev = sh.local
+        assert ev is not None, "empty shard: fewer pattern tiles than ranks"
+    else:
+        ev = Evaluator(wl, precision=prec, flags=flags, device=device)
+        ev.make_device_io()
     stream = ev.inst.stream
+    d_site = torch.zeros(ev.wl.n_patterns, dtype=torch.float64, device=device) if keep_site else None
+
+    def reduce_step():
+        if sh is not None and sh.world > 1:
+            sh.dist.all_reduce(sh.result, op=sh.dist.ReduceOp.SUM)
+
     for _ in range(max(warmup, 3)):
         ev.step_device()
+        reduce_step()
     torch.cuda.synchronize()
     l0 = ev.inst.kernel_launch_count()
-    marks = [[torch.cuda.Event(enable_timing=True) for _ in range(5)] for _ in range(steps)]
+    marks = [[torch.cuda.Event(enable_timing=True) for _ in range(6)] for _ in range(steps)]
     if sampler is not None:
         sampler.start()
         time.sleep(0.3)
@@ -165,18 +242,26 @@ def measure_device(wl, precision, flags, steps, warmup, peaks, sampler=None, dev
         marks[s][3].record(stream)
         ev.step_pre_gradient()
         marks[s][4].record(stream)
+        reduce_step()
+        marks[s][5].record(stream)
     torch.cuda.synchronize()
     clocks = sampler.stop() if sampler is not None else None
     launches = ev.inst.kernel_launch_count() - l0
-    total_ms = marks[0][0].elapsed_time(marks[-1][4])
-    phase = np.zeros(4)
+    total_ms = marks[0][0].elapsed_time(marks[-1][5])
+    phase = np.zeros(5)
     for s in range(steps):
-        for i in range(4):
+        for i in range(5):
             phase[i] += marks[s][i].elapsed_time(marks[s][i + 1])
     phase /= steps
+    site = None
+    if keep_site:  # one extra (untimed) root reduction that also writes the per-pattern log-likelihoods
+        ev.inst.root_log_likelihoods_device(ev.tree.root, ev.scale_idx, ev.d_logl, d_site)
+        ev.step_pre_gradient()  # the gradient of the last timed step was all-reduced in place when sharded
+        torch.cuda.synchronize()
+        site = d_site.cpu().numpy()
     logl = float(ev.d_logl.cpu()[0])
     grad = ev.d_grad.cpu().numpy()
-    N, P, S, C = wl.tree.n_tips, wl.n_patterns, wl.n_states, wl.n_categories
+    N, P, S, C = ev.wl.tree.n_tips, ev.wl.n_patterns, ev.wl.n_states, ev.wl.n_categories
     w = 8 if precision == "fp64" else 4
     alg = algorithmic(N, P, S, C, w)
     ms_step = total_ms / steps
@@ -187,12 +272,14 @@ def measure_device(wl, precision, flags, steps, warmup, peaks, sampler=None, dev
         "bls_gradients_per_s": (2 * N - 2) * 1e3 / ms_step,
         "post_order_updates_per_s": alg["updates"] / (phase[1] * 1e-3),
         "grad_units_per_s": alg["grad_units"] / (phase[3] * 1e-3),
-        "phase_ms": {"matrices": phase[0], "post_order": phase[1], "root": phase[2], "pre_order_gradient": phase[3]},
+        "phase_ms": {"matrices": phase[0], "post_order": phase[1], "root": phase[2], "pre_order_gradient": phase[3],
+                     "all_reduce": phase[4]},
         "post_gbs": alg["post_bytes"] / (phase[1] * 1e-3) / 1e9,
         "pre_gbs": alg["pre_bytes"] / (phase[3] * 1e-3) / 1e9,
         "post_tflops": alg["post_flops"] / (phase[1] * 1e-3) / 1e12,
         "pre_tflops": alg["pre_flops"] / (phase[3] * 1e-3) / 1e12,
-        "launches": int(launches), "logL": logl, "grad_norm": float(np.linalg.norm(grad)),
+        "launches": int(launches), "logL": logl, "grad": grad, "site": site,
+        "grad_norm": float(np.linalg.norm(grad)),
         "finite": bool(np.isfinite(logl) and np.all(np.isfinite(grad))),
         "alg": alg, "clocks": clocks,
     }
@@ -231,33 +318,107 @@ def measure_e2e(ev, wl, steps, warmup):
 
 
 # ---- the oracle on the host cores ------------------------------------------------------------------------------------
-def oracle_time(wl, n_sample, repeats=1):
+def cpu_model_string():
+    try:
+        with open("/proc/cpuinfo") as fh:
+            for line in fh:
+                if line.lower().startswith("model name"):
+                    return line.split(":", 1)[1].strip()
+    except OSError:
+        pass
+    return "unknown"
+
+
+def oracle_time(wl, n_sample, workers=1):
     """The fp64 CPU oracle as it stands on the first `n_sample` patterns of the workload (full evaluation incl. the
-    gradient).  Returns (seconds per evaluation, threads actually used = CPU time / wall time)."""
+    gradient): in this process (workers = 1; `cores` = CPU time / wall time, i.e. the threads numpy's BLAS really
+    used) or by pattern chunks in `workers` processes.  Returns (seconds, cores used, patterns, oracle result)."""
     sys.path.insert(0, os.path.join(ROOT, "tests"))
     import oracle_runner as orc
 
     n_sample = min(n_sample, wl.n_patterns)
-    best = None
-    cores = 1.0
-    for _ in range(repeats):
-        c0, t0 = os.times(), time.perf_counter()
-        orc.evaluate(wl, lo=0, hi=n_sample)
-        dt = time.perf_counter() - t0
-        c1 = os.times()
+    c0, t0 = os.times(), time.perf_counter()
+    if workers <= 1:
+        ref = orc.evaluate(wl, lo=0, hi=n_sample)
+        used = None
+    else:
+        ref = orc.evaluate_pool(wl, lo=0, hi=n_sample, workers=workers, chunk=4096 if wl.n_states == 4 else 512)
+        used = ref["workers"]
+    dt = time.perf_counter() - t0
+    c1 = os.times()
+    if used is None:
         cpu = (c1.user - c0.user) + (c1.system - c0.system)
-        if best is None or dt < best:
-            best, cores = dt, max(1.0, cpu / dt)
-    return best, int(round(cores)), n_sample
+        used = max(1, int(round(cpu / dt)))
+    return dt, used, n_sample, ref
 
 
-# measured DRAM traffic per step (bytes) of the dominant kernel's launches, keyed by (workload, precision, kernel)
-# (profiles/r01_launches_cfg1_fp64.md: dram__bytes_read.sum + dram__bytes_write.sum summed over the launches of one step)
-NCU_DRAM_BYTES = {("cfg1_gtr_128x100000", "fp64", "k_pre4_lean+k_grad4_tips"): 4194.4e6,
-                  ("cfg1_gtr_128x100000", "fp32", "k_pre4_lean+k_grad4_tips"): 1871.9e6,
-                  ("cfg3_gy94_256x20000", "fp32", "k_pre_tc5"): 17075.1e6}
+def parity_against_oracle(ref, n_used, gpu_site, gpu_logl, gpu_grad, wl, branch_nodes):
+    """The GPU's outputs of the timed workload against the oracle result of the cpu_baseline leg, on the oracle's
+    patterns: every site log-likelihood; when the oracle covered ALL patterns also logL and every branch gradient
+    (the three figures of SURVEY 8(c) row 18)."""
+    out = {"patterns": n_used, "of": wl.n_patterns,
+           "site_rel": float(np.max(np.abs(gpu_site[:n_used] - ref["site_logl"]) / np.abs(ref["site_logl"]))),
+           "logL_rel_on_sample": float(abs(np.dot(wl.pattern_weights[:n_used], gpu_site[:n_used]) - ref["logL"])
+                                       / abs(ref["logL"]))}
+    if n_used == wl.n_patterns:
+        g_ref, cond = ref["grad"][branch_nodes], ref["cond"][branch_nodes]
+        d = np.abs(gpu_grad - g_ref)
+        nz = np.abs(g_ref) > 1e-13 * np.max(np.abs(g_ref))
+        out.update({"logL_rel": float(abs(gpu_logl - ref["logL"]) / abs(ref["logL"])),
+                    "grad_strict_rel": float(np.max(d[nz] / np.abs(g_ref[nz]))),
+                    "grad_rel_to_A_k": float(np.max(d[cond > 0] / cond[cond > 0])),
+                    "grad_2norm_rel": float(np.linalg.norm(gpu_grad - g_ref) / np.linalg.norm(g_ref)),
+                    "eigendecomposition": "workload's own (independent of the oracle's: DESIGN.md section 3)"})
+    return out
 
-ORACLE_SAMPLE = {4: 40000, 61: 4000}  # cpu_baseline leg: patterns per oracle evaluation, ~10-30 s of CPU work
+
+def ncu_dram_bytes_per_step(csv_name, kernel_pattern):
+    """DRAM bytes (read + write) per evaluation of the kernels whose name matches `kernel_pattern`, from a committed
+    ncu launch list (profiles/*.csv, `--metrics gpu__time_duration.sum,dram__bytes_read.sum,dram__bytes_write.sum`):
+    summed over every matching launch of the capture and divided by the number of evaluations in it (= launches of
+    k_transition over more than one branch).  None when the list is absent."""
+    import csv
+    import re
+
+    path = os.path.join(ROOT, "profiles", csv_name)
+    if not os.path.exists(path):
+        return None
+    pat = re.compile(kernel_pattern)
+    total, evals, seen = 0.0, 0, set()
+    with open(path, newline="") as fh:
+        rows = (ln for ln in fh if ln.startswith('"'))
+        for row in csv.DictReader(rows):
+            name, metric = row["Kernel Name"], row["Metric Name"]
+            if metric in ("dram__bytes_read.sum", "dram__bytes_write.sum") and pat.search(name):
+                val = float(row["Metric Value"].replace(",", ""))
+                unit = row["Metric Unit"].lower()
+                total += val * {"byte": 1.0, "kbyte": 1e3, "mbyte": 1e6, "gbyte": 1e9}.get(unit, 1.0)
+            if "k_transition" in name and row["ID"] not in seen and row["Grid Size"].replace(" ", "") != "(1,1,1)":
+                seen.add(row["ID"])
+                evals += 1
+    return total / evals if evals else None
+
+
+# committed launch lists by (workload, precision); the newest capture of each is used
+NCU_LISTS = {("cfg1_gtr_128x100000", "fp64"): ["r02_launches_cfg1_fp64.csv", "r01_launches_cfg1_fp64.csv"],
+             ("cfg1_gtr_128x100000", "fp32"): ["r02_launches_cfg1_fp32.csv", "r01_launches_cfg1_fp32.csv"],
+             ("cfg3_gy94_256x20000", "fp32"): ["r02_launches_cfg3_fp32_tensor.csv", "r01_launches_cfg3_fp32_tensor.csv"],
+             ("cfg2_gy94_32x10000", "fp64"): ["r02_launches_cfg2_fp64_tensor.csv"]}
+KERNEL_PATTERNS = {"k_pre4_lean+k_grad4_tips": r"k_pre4_lean|k_grad4_tips", "k_post4_walk": r"k_post4_walk",
+                   "k_pre_tc5": r"k_pre_tc5", "k_post_tc5": r"k_post_tc5", "k_pre_tc": r"k_pre_tc<",
+                   "k_post_tc": r"k_post_tc<"}
+
+
+def measured_traffic(wl_name, precision, kname):
+    for csv_name in NCU_LISTS.get((wl_name, precision), []):
+        if kname in KERNEL_PATTERNS:
+            v = ncu_dram_bytes_per_step(csv_name, KERNEL_PATTERNS[kname])
+            if v:
+                return v, "profiles/" + csv_name
+    return None, None
+
+
+ORACLE_1CORE_BUDGET_S = 25.0  # cpu_baseline, one process: the largest pattern prefix that fits this budget
 REFERENCE_SAMPLE = {4: 8000, 61: 800}  # --impl reference: patterns per step (a few seconds per step)
 
 
@@ -284,7 +445,7 @@ def workload_config(wl, precision, flags, extra=None):
 
 
 def run_reference(args):
-    """--impl reference: the CPU oracle as it stands, each step a bounded sample of the workload."""
+    """--impl reference: the CPU oracle as it stands (one process), each step a bounded sample of the workload."""
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
@@ -293,9 +454,9 @@ def run_reference(args):
     N, C = wl.tree.n_tips, wl.n_categories
     for _ in range(min(args.warmup, 1)):
         oracle_time(wl, min(n_sample, 2000 if wl.n_states == 4 else 50))
-    times, cores = [], 1
+    times, cores, n_used = [], 1, n_sample
     for _ in range(args.steps):
-        dt, cores, n_used = oracle_time(wl, n_sample)
+        dt, cores, n_used, _ = oracle_time(wl, n_sample)
         times.append(dt)
     dt = float(np.mean(times))
     value = (N - 1) * n_used * C / dt
@@ -303,8 +464,8 @@ def run_reference(args):
         "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": dt * 1e3, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": workload_config(wl, "fp64", 0, {"sample": f"first {n_used} of {wl.n_patterns} patterns per step"}),
-        "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle",
+        "config": workload_config(wl, args.precision, 0, {"parallelism": "single GPU" if args.gpus == 1 else "replicas only"}),
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "cpu": cpu_model_string(),
                          "sample": f"first {n_used} of {wl.n_patterns} patterns, full logL + gradient, per step"},
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
@@ -312,21 +473,36 @@ def run_reference(args):
     print(json.dumps(line))
 
 
-def run_extras(peaks, steps, warmup):
+def codon_roofline(name, wl, precision, kernels, res, peaks, mm):
+    """Both rooflines of a 64-state run (SURVEY 8(d) "report both, state which binds"): tensor pipe against the
+    matmul peak of its precision MEASURED in this run (fp64: DMMA; fp32: TF32), with algorithmic and issued flops
+    separately, and HBM against the measured copy rate."""
+    N, P, C = wl.tree.n_tips, wl.n_patterns, wl.n_categories
+    iss = issued_tensor_flops(N, P, C, precision, kernels)
+    peak = mm["fp64_tflops"] if precision == "fp64" else mm["tf32_tflops"]
+    ph = res["phase_ms"]
+    out = {"workload": wl.name, "precision": precision, "kernels": kernels,
+           "peak_tflops": peak, "peak_source": ("fp64" if precision == "fp64" else "tf32") + " torch.matmul 8192^3, this run"}
+    for tag, key, alg_fl, alg_by in (("post_order", "post", res["alg"]["post_flops"], res["alg"]["post_bytes"]),
+                                     ("pre_order_gradient", "pre", res["alg"]["pre_flops"], res["alg"]["pre_bytes"])):
+        t = ph[tag] * 1e-3
+        out[tag] = {"ms": ph[tag], "alg_tflops": alg_fl / t / 1e12, "issued_tflops": iss[key] / t / 1e12,
+                    "frac_tensor_alg": alg_fl / t / 1e12 / peak, "frac_tensor_issued": iss[key] / t / 1e12 / peak,
+                    "hbm_gbs": alg_by / t / 1e9, "frac_hbm": alg_by / t / 1e9 / peaks["hbm_gbs"]}
+        out[tag]["binds"] = "tensor" if out[tag]["frac_tensor_issued"] >= out[tag]["frac_hbm"] else "hbm"
+    return out
+
+
+def run_extras(peaks, steps, warmup, mm):
     """The other BASELINE configs / precisions, a few steps each (context for the headline line)."""
     from paper_2606_27607_b200 import workloads
 
-    have_tc = os.path.exists(os.path.join(ROOT, "paper_2606_27607_b200", "csrc", "plk_tc.cuh"))
     plan = [("cfg1_fp32", 1, None, None, "fp32", 0), ("cfg0_fp64", 0, None, None, "fp64", 0),
-            ("cfg2_fp64_cuda", 2, None, None, "fp64", 0), ("cfg2_fp32_cuda", 2, None, None, "fp32", 0)]
-    if have_tc:
-        plan += [("cfg2_fp64_tensor", 2, None, None, "fp64", 1), ("cfg2_fp32_tensor", 2, None, None, "fp32", 1),
-                 ("cfg3_fp32_tensor", 3, None, None, "fp32", 1),
-                 ("cfg3_fp32_tensor_mma_sync", 3, None, None, "fp32", 1 | 64)]
-    else:
-        plan += [("cfg3_fp32_cuda", 3, None, None, "fp32", 0)]
-    plan += [("cfg4_hky_fp32_512x100000", 4, 512, 100_000, "fp32", 0), ("cfg4_hky_fp32_8x100", 4, 8, 100, "fp32", 0)]
-    out = {}
+            ("cfg2_fp64_cuda", 2, None, None, "fp64", 0), ("cfg2_fp32_cuda", 2, None, None, "fp32", 0),
+            ("cfg2_fp64_tensor", 2, None, None, "fp64", 1), ("cfg2_fp32_tensor", 2, None, None, "fp32", 1),
+            ("cfg3_fp32_tensor", 3, None, None, "fp32", 1), ("cfg3_fp32_tensor_mma_sync", 3, None, None, "fp32", 1 | 64),
+            ("cfg4_hky_fp32_512x100000", 4, 512, 100_000, "fp32", 0), ("cfg4_hky_fp32_8x100", 4, 8, 100, "fp32", 0)]
+    out, codon = {}, []
     cache = {}
     for name, idx, n, p, prec, flags in plan:
         key = (idx, n, p)
@@ -347,10 +523,14 @@ def run_extras(peaks, steps, warmup):
             "gradient_evals_per_s": res["gradient_evals_per_s"],
             "phase_ms": {k: round(v, 4) for k, v in res["phase_ms"].items()},
             "post_hbm_frac": res["post_gbs"] / hbm, "pre_hbm_frac": res["pre_gbs"] / hbm,
+            "post_hbm_frac_of_8TBs": res["post_gbs"] / HBM_NOMINAL_GBS, "pre_hbm_frac_of_8TBs": res["pre_gbs"] / HBM_NOMINAL_GBS,
             "post_alg_tflops": res["post_tflops"], "pre_alg_tflops": res["pre_tflops"],
             "launches_per_step": res["launches"] / steps, "finite": res["finite"],
         }
-    return out
+        if flags & 1 and mm is not None:
+            codon.append(codon_roofline(name, wl, prec, "mma.sync" if (prec == "fp64" or flags & 64) else "tcgen05",
+                                        res, peaks, mm))
+    return out, codon
 
 
 def run_sweep(peaks, steps, warmup):
@@ -378,8 +558,31 @@ def run_sweep(peaks, steps, warmup):
     print(json.dumps({"sweep": "configs[4] HKY fp32", "unit": UNIT, "steps": steps, "points": points}))
 
 
+def respawn_under_torchrun(args):
+    """`python bench.py --gpus N` without a launcher: start N ranks of this very command line with torchrun (what the
+    driver does itself), so that --gpus N never silently measures one GPU."""
+    import torch
+
+    have = torch.cuda.device_count()
+    if have < args.gpus:
+        raise SystemExit(f"bench.py --gpus {args.gpus}: only {have} CUDA device(s) visible")
+    import socket
+
+    with socket.socket() as sk:
+        sk.bind(("127.0.0.1", 0))
+        port = sk.getsockname()[1]
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}",
+           "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+    raise SystemExit(subprocess.call(cmd))
+
+
 def main():
     args = parse_args()
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    if args.gpus > 1 and world == 1 and args.impl == "ours":
+        respawn_under_torchrun(args)
+    if args.impl == "ours" and world != args.gpus:
+        raise SystemExit(f"bench.py: --gpus {args.gpus} but WORLD_SIZE={world}")
     if args.impl == "reference":
         run_reference(args)
         return
@@ -395,13 +598,13 @@ def main():
 
     rank = int(os.environ.get("RANK", "0"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
-    world = int(os.environ.get("WORLD_SIZE", "1"))
     if rank == 0:
         build.build()
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a CUDA device: the product path has no CPU fallback "
                          "(use --impl reference for the oracle)")
     torch.cuda.set_device(local_rank)
+    device = f"cuda:{local_rank}"
     dist = None
     if world > 1:
         import torch.distributed as dist
@@ -417,21 +620,24 @@ def main():
     flags |= plk.FLAG_NO_TCGEN05 if args.codon_fp32 == "mma_sync" else 0
     flags |= plk.FLAG_NO_PDL if args.no_pdl else 0
     sampler = ClockSampler(local_rank) if rank == 0 else None
+    sharded_run = args.shard_patterns and world > 1
+    want_parity = rank == 0 and not args.no_cpu_baseline and not sharded_run
 
     if dist is not None:
         dist.barrier()
     torch.cuda.synchronize()
-    res, ev = measure_device(wl, args.precision, flags, args.steps, args.warmup, peaks, sampler,
-                             device=f"cuda:{local_rank}")
-    ms = torch.tensor([res["ms_per_step"]], dtype=torch.float64, device=f"cuda:{local_rank}")
+    res, ev = measure_device(wl, args.precision, flags, args.steps, args.warmup, peaks, sampler, device=device,
+                             keep_site=want_parity, shard=(rank, world, dist) if sharded_run else None)
+    ms = torch.tensor([res["ms_per_step"]], dtype=torch.float64, device=device)
     if dist is not None:
         dist.barrier()
         dist.all_reduce(ms, op=dist.ReduceOp.MAX)
     ms_step = float(ms[0])
-    e2e_dt, h2d, d2h = measure_e2e(ev, wl, max(2, min(args.steps, 5)), args.warmup)
-    e2e_t = torch.tensor([e2e_dt], dtype=torch.float64, device=f"cuda:{local_rank}")
+    e2e_dt, h2d, d2h = measure_e2e(ev, ev.wl, max(2, min(args.steps, 5)), args.warmup)
+    e2e_t = torch.tensor([e2e_dt], dtype=torch.float64, device=device)
     if dist is not None:
         dist.all_reduce(e2e_t, op=dist.ReduceOp.MAX)
+    branch_nodes = ev.branch_nodes.copy()
     ev.close()
     if rank != 0:
         if dist is not None:
@@ -439,8 +645,10 @@ def main():
             dist.destroy_process_group()
         return
 
-    alg = res["alg"]
-    updates_all = alg["updates"] * world
+    alg = algorithmic(wl.tree.n_tips, wl.n_patterns, wl.n_states, wl.n_categories, 8 if args.precision == "fp64" else 4)
+    # whole job: N replicas each do the full workload (weak); N shards together do it once (strong)
+    updates_all = alg["updates"] * (1 if sharded_run else world)
+    evals_all = 1 if sharded_run else world
     # roofline of the dominant kernel (largest share of the step)
     ph = res["phase_ms"]
     nuc = wl.n_states == 4
@@ -453,33 +661,37 @@ def main():
              else (("k_pre_tc5" if args.precision == "fp32" and args.codon_fp32 == "tcgen05" else "k_pre_tc")
                    if args.tensor else "k_pre64")}[dom]
     n_levels_note = "all launches of the kernel in one step (one per dependency level and item class)"
-    # DRAM bytes (read + write) of those launches from ncu, per step: profiles/r01_launches_cfg1_fp64.md
-    traffic = NCU_DRAM_BYTES.get((wl.name, args.precision, kname))
+    traffic, traffic_src = measured_traffic(wl.name, args.precision, kname)
+    mm = measure_matmul_peaks(device) if (not nuc or not args.no_extras) else None
+    ralg = res["alg"]  # this rank's share when sharded
     if nuc or args.precision == "fp32":
         achieved = res["pre_gbs"] if dom == "pre_order_gradient" else res["post_gbs"]
         roofline = {"bound": "hbm", "kernel": kname, "achieved": achieved, "peak": peaks["hbm_gbs"], "unit": "GB/s",
-                    "frac": achieved / peaks["hbm_gbs"], "traffic": traffic, "peak_source": peaks["source"] + " hbm_gbs",
-                    "algorithmic_bytes": alg["pre_bytes"] if dom == "pre_order_gradient" else alg["post_bytes"],
+                    "frac": achieved / peaks["hbm_gbs"], "traffic": traffic, "traffic_source": traffic_src,
+                    "peak_source": peaks["source"] + " hbm_gbs (copy rate, burst)",
+                    "frac_of_nominal_8TBs": achieved / HBM_NOMINAL_GBS,
+                    "algorithmic_bytes": ralg["pre_bytes"] if dom == "pre_order_gradient" else ralg["post_bytes"],
                     "over": n_levels_note}
     else:
-        # fp64 61-state: tensor (DMMA) / fp64 pipe; nominal B200 fp64 ~ 40 TFLOP/s
+        # fp64 61-state: DMMA / fp64 pipe against the fp64 matmul rate measured in this run
         achieved = res["pre_tflops"] if dom == "pre_order_gradient" else res["post_tflops"]
-        roofline = {"bound": "tensor", "kernel": kname, "achieved": achieved, "peak": 40.0, "unit": "TFLOP/s",
-                    "frac": achieved / 40.0, "traffic": None, "peak_source": "nominal fp64 (DESIGN.md)",
-                    "over": n_levels_note}
-    roofline["post_order"] = {"GB/s": res["post_gbs"], "frac_hbm": res["post_gbs"] / peaks["hbm_gbs"],
-                              "alg_TFLOP/s": res["post_tflops"], "ms": ph["post_order"]}
-    roofline["pre_order_gradient"] = {"GB/s": res["pre_gbs"], "frac_hbm": res["pre_gbs"] / peaks["hbm_gbs"],
-                                      "alg_TFLOP/s": res["pre_tflops"], "ms": ph["pre_order_gradient"]}
+        roofline = {"bound": "tensor", "kernel": kname, "achieved": achieved, "peak": mm["fp64_tflops"], "unit": "TFLOP/s",
+                    "frac": achieved / mm["fp64_tflops"], "traffic": traffic, "traffic_source": traffic_src,
+                    "peak_source": "fp64 torch.matmul 8192^3 measured in this run", "over": n_levels_note}
+    for tag, gb, tf in (("post_order", "post_gbs", "post_tflops"), ("pre_order_gradient", "pre_gbs", "pre_tflops")):
+        roofline[tag] = {"GB/s": res[gb], "frac_hbm": res[gb] / peaks["hbm_gbs"],
+                         "frac_hbm_of_nominal_8TBs": res[gb] / HBM_NOMINAL_GBS, "alg_TFLOP/s": res[tf], "ms": ph[tag]}
 
     line = {
         "metric": METRIC, "value": updates_all / (ms_step * 1e-3), "unit": UNIT, "n_gpus": world, "steps": args.steps,
-        "warmup": max(args.warmup, 3), "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak",
+        "warmup": max(args.warmup, 3), "ms_per_step": ms_step, "higher_is_better": True,
+        "scaling": "strong" if sharded_run else "weak",
         "vs_baseline": None, "dtype": "f64" if args.precision == "fp64" else "f32", "data": "synthetic",
         "config": workload_config(wl, args.precision, flags,
-                                  {"parallelism": "replicas only" if world > 1 else "single GPU"}),
-        "gradient_evals_per_s": world * 1e3 / ms_step,
-        "bls_gradients_per_s": world * (2 * wl.tree.n_tips - 2) * 1e3 / ms_step,
+                                  {"parallelism": ("pattern shards + one all-reduce" if sharded_run else "replicas only")
+                                   if world > 1 else "single GPU"}),
+        "gradient_evals_per_s": evals_all * 1e3 / ms_step,
+        "bls_gradients_per_s": evals_all * (2 * wl.tree.n_tips - 2) * 1e3 / ms_step,
         "post_order_updates_per_s": res["post_order_updates_per_s"] * world,
         "phase_ms": {k: round(v, 5) for k, v in ph.items()},
         "logL": res["logL"], "finite": res["finite"],
@@ -490,14 +702,37 @@ def main():
         "gpu_launches": res["launches"],
         "roofline": roofline,
     }
+    if mm is not None:
+        line["matmul_peaks"] = mm
+    if not nuc and args.tensor and mm is not None:
+        line["roofline_codon"] = [codon_roofline("headline", wl, args.precision,
+                                                 "tcgen05" if (args.precision == "fp32" and args.codon_fp32 == "tcgen05")
+                                                 else "mma.sync", res, peaks, mm)]
     if not args.no_cpu_baseline:
-        n_sample = ORACLE_SAMPLE[4 if nuc else 61]
-        dt, cores, n_used = oracle_time(wl, n_sample)
-        line["cpu_baseline"] = {"value": (wl.tree.n_tips - 1) * n_used * wl.n_categories / dt, "unit": UNIT,
-                                "cores": cores, "kind": "oracle", "seconds": dt,
-                                "sample": f"first {n_used} of {wl.n_patterns} patterns, full logL + gradient, once"}
+        # (a) one process on the largest pattern prefix that fits the budget (rate probed on a small prefix)
+        probe_n = min(wl.n_patterns, 4000 if nuc else 200)
+        dt_probe, _, _, _ = oracle_time(wl, probe_n)
+        n1 = int(min(wl.n_patterns, max(probe_n, ORACLE_1CORE_BUDGET_S / dt_probe * probe_n)))
+        dt1, cores1, n1, ref1 = oracle_time(wl, n1)
+        per_update = (wl.tree.n_tips - 1) * wl.n_categories
+        line["cpu_baseline"] = {"value": per_update * n1 / dt1, "unit": UNIT, "cores": cores1, "kind": "oracle",
+                                "seconds": dt1, "cpu": cpu_model_string(), "host_cores": os.cpu_count(),
+                                "sample": f"first {n1} of {wl.n_patterns} patterns, full logL + gradient, once, one process"}
+        # (b) all host cores, pattern chunks in a process pool: the full pattern set if that takes < ~60 s
+        ncpu = os.cpu_count() or 1
+        ref_all, n_all = ref1, n1
+        if ncpu > 1:
+            est_full = dt1 / n1 * wl.n_patterns / max(1, 0.7 * ncpu)
+            n_all = wl.n_patterns if est_full < 60.0 else int(wl.n_patterns * 60.0 / est_full)
+            dta, used, n_all, ref_all = oracle_time(wl, n_all, workers=ncpu)
+            line["cpu_baseline_all_cores"] = {"value": per_update * n_all / dta, "unit": UNIT, "cores": used,
+                                              "kind": "oracle", "seconds": dta,
+                                              "sample": f"first {n_all} of {wl.n_patterns} patterns by chunks in {used} processes"}
+        if res["site"] is not None:
+            line["parity"] = parity_against_oracle(ref_all, n_all, res["site"], res["logL"], res["grad"], wl, branch_nodes)
     if not args.no_extras and world == 1:
-        line["extras"] = run_extras(peaks, max(3, min(args.steps, 5)), 3)
+        line["extras"], codon = run_extras(peaks, max(3, min(args.steps, 5)), 3, mm)
+        line["roofline_codon"] = line.get("roofline_codon", []) + codon
     print(json.dumps(line))
     if dist is not None:
         dist.barrier()
