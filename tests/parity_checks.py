@@ -72,15 +72,18 @@ def check_grad(g_gpu, ref, precision, root):
 
 
 def check_site_derivs(site_d, ref, precision, root, cols=None):
-    """Per-pattern derivatives, norm-wise per branch (last sentence).  A branch above an
-    all-missing tip has derivative 0 analytically; both sides then hold pure round-off, which has no relative
-    meaning: such a branch is measured against the largest branch scale."""
+    """Per-pattern derivatives, norm-wise per branch (last sentence): max_p |dd_kp| <= tol *
+    max_p |d_kp|.  d_kp = num / den is a quotient whose numerator is a sum of terms of both signs (Q has a negative
+    diagonal), so a single d_kp can be small by cancellation; the norm over the patterns of a branch absorbs that,
+    but it degenerates when a branch has one pattern (P = 1) or is analytically zero (branch above an all-missing
+    tip: pure round-off on both sides).  Hence a floor: a branch whose largest |d_kp| is below 1e-3 of the largest
+    branch's is measured against that floor."""
     tol = tol_of(precision)
     sd = ref["site_derivs"]
     got = site_d if cols is None else site_d[:, cols]
     scale = np.max(np.abs(sd), axis=1)
     scale[root] = 0.0
-    scale = np.maximum(scale, 1e-6 * np.max(scale))
+    scale = np.maximum(scale, 1e-3 * np.max(scale))
     err = np.max(np.abs(got - sd), axis=1) / scale
     err[root] = 0.0
     k = int(np.argmax(err))
