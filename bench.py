@@ -130,15 +130,15 @@ def issued_tensor_flops(N, P, C, precision, kernels):
     above ("report issued flops separately").  Edges: N - 2 internal child edges, N tip edges (compact).
       mma.sync (plk_tc.cuh)    post: internal edges only (tips are column gathers); pre: a_k, Q x_k, M_k^T u_k for every
                                edge with partials; fp32 = 3 passes
-      tcgen05 (plk_tc5*.cuh)   post: every edge (one-hot tips: 2 of the 3 passes); pre: a_k and D_k x_k for internal
-                               edges (3 passes), a_k for tip edges through the pipe (2 passes), M_k^T u_k for internal
-                               edges only (3 passes)"""
+      tcgen05 (plk_tc5*.cuh)   post: every edge (one-hot tips: 2 of the 3 passes); pre (plk_tc5_pre2.cuh): a_k and
+                               D_k x_k for internal edges (3 passes each) and M_k^T u_k for internal edges (3 passes);
+                               tip edges are table gathers on the CUDA cores"""
     mv = 2.0 * 64 * 64 * P * C
     n_int, n_tip = N - 2, N
     passes = 1 if precision == "fp64" else 3
     if kernels == "tcgen05":
         post = mv * (3 * n_int + 2 * n_tip)
-        pre = mv * (3 * (2 * n_int) + 2 * n_tip + 3 * n_int)
+        pre = mv * (3 * (2 * n_int) + 3 * n_int)
     else:
         post = mv * passes * n_int
         pre = mv * passes * 3 * n_int

@@ -19,6 +19,7 @@
 #include "plk_tc.cuh"
 #include "plk_tc5.cuh"
 #include "plk_tc5_pre.cuh"
+#include "plk_tc5_pre2.cuh"
 #endif
 
 using namespace plk;
@@ -41,7 +42,7 @@ struct Layout {
   int n_tiles, max_grad;
   size_t off_post, off_compact, off_pre, off_pre_mx, off_matrix, off_eigen, off_scale, off_weights, off_pi,
       off_rates, off_catw, off_site, off_block_partial, off_grad_partial, off_grad_out, off_logl, off_site_deriv,
-      off_stage, off_ring, off_matrix_t, off_matrix_d, total;
+      off_stage, off_ring, off_matrix_t, off_matrix_d, off_matrix_dt, off_cat_scratch, total;
   size_t stage_bytes;
 };
 
@@ -105,13 +106,14 @@ bool compute_layout(const plk_config& c, Layout& L) {
   L.stage_bytes = round_up((size_t)L.C * L.P * L.S * 8, ALIGN);
   L.off_stage = take(L.stage_bytes);
   L.off_ring = take(RING_BYTES);
-  // transposed copies of the transition matrices for the tcgen05 pre-order kernel (plk_tc5_pre.cuh, step B)
-  L.off_matrix_t = take((L.SP == 64 && c.precision == PLK_FP32 && (c.flags & PLK_FLAG_TENSOR_CORES) &&
-                         !(c.flags & PLK_FLAG_NO_TCGEN05))
-                            ? (size_t)c.matrix_buffer_count * L.matrix_bytes
-                            : 0);
-  // derivative matrices D = M Q of the 4-state specialised gradient kernels (plk_nuc_lean.cuh, compact-tip children)
-  L.off_matrix_d = take(L.SP == 4 ? (size_t)c.matrix_buffer_count * L.matrix_bytes : 0);
+  // fp32 tensor-core instances (tcgen05 pre-order kernels, plk_tc5_pre*.cuh): per matrix buffer M^T, D = M Q and D^T,
+  // and the per-category num / den scratch of the class-specialised kernels ([slot][num, den][C][P] floats)
+  const bool tc5 = L.SP == 64 && c.precision == PLK_FP32 && (c.flags & PLK_FLAG_TENSOR_CORES) && !(c.flags & PLK_FLAG_NO_TCGEN05);
+  L.off_matrix_t = take(tc5 ? (size_t)c.matrix_buffer_count * L.matrix_bytes : 0);
+  // derivative matrices D = M Q: 4-state specialised gradient kernels (plk_nuc_lean.cuh, compact-tip children) and tc5
+  L.off_matrix_d = take((L.SP == 4 || tc5) ? (size_t)c.matrix_buffer_count * L.matrix_bytes : 0);
+  L.off_matrix_dt = take(tc5 ? (size_t)c.matrix_buffer_count * L.matrix_bytes : 0);
+  L.off_cat_scratch = take((tc5 && c.preorder_buffer_count > 0) ? (size_t)L.max_grad * 2 * L.C * L.P * 4 : 0);
   L.total = o;
   return true;
 }
@@ -284,6 +286,15 @@ int nuc_walk_warps(const plk_instance* in, K kernel, int n_chunks, int* total_wa
 // The specialised pre-order kernels (plk_nuc_lean.cuh) exist for C = 4 in the level order only.
 inline bool nuc_lean_ok(const plk_instance* in) {
   return in->L.SP == 4 && in->L.C == 4 && !(in->cfg.flags & (PLK_FLAG_NO_TMA | PLK_FLAG_NO_LEVEL_BATCH | PLK_FLAG_PATTERN_WALK_ONLY));
+}
+// fp32 codon instances on tcgen05: the class-specialised, pipelined gradient kernels of plk_tc5_pre2.cuh
+inline bool tc5_classes_ok(const plk_instance* in) {
+#ifdef PLK_WITH_TENSOR
+  return in->L.SP == 64 && in->f32 && (in->cfg.flags & PLK_FLAG_TENSOR_CORES) &&
+         !(in->cfg.flags & (PLK_FLAG_NO_TCGEN05 | PLK_FLAG_NO_LEVEL_BATCH));
+#else
+  return false;
+#endif
 }
 bool nuc_use_walk(const plk_instance* in, int n_ops, int n_levels, bool pre_gradient = false) {
   const int flags = in->cfg.flags;
@@ -1243,7 +1254,7 @@ static int pre_impl(plk_instance* in, int eigen, int root_pre, const plk_pre_op*
   }
   // build items in list order (bookkeeping), one per pair / unpaired op
   struct HostItem { DevPreItem it; int level; int cls; };  // cls 0..2: plk_nuc_lean.cuh classes; 3: general kernel
-  const bool lean = want_grad && nuc_lean_ok(in);
+  const bool lean = want_grad && (nuc_lean_ok(in) || tc5_classes_ok(in));
   std::vector<HostItem> items;
   items.reserve(count);
   for (int i = 0; i < count; ++i) {
@@ -1341,11 +1352,20 @@ static int pre_impl(plk_instance* in, int eigen, int root_pre, const plk_pre_op*
     const DevPreItem* dit = reinterpret_cast<const DevPreItem*>(d);
     const void* Q = want_grad ? in->eig_QT(eigen) : in->eig_QT(0);
 #ifdef PLK_WITH_TENSOR
+    std::vector<int> fin_slots;  // gradient slots served by the class-specialised tcgen05 kernels (per-category scratch)
     if (L.SP == 64 && in->f32 && (in->cfg.flags & PLK_FLAG_TENSOR_CORES) && !(in->cfg.flags & PLK_FLAG_NO_TCGEN05)) {
-      // step B of the tcgen05 pre-order kernel contracts over the ROW index of M: it reads transposed copies
-      tc5::pre::k_transpose64<<<in->cfg.matrix_buffer_count * L.C, 256, 0, in->stream>>>(
-          in->at<float>(L.off_matrix), in->at<float>(L.off_matrix_t));
-      CHECK_LAUNCH(in);
+      // step B of the tcgen05 pre-order kernels contracts over the ROW index of M: it reads transposed copies; the
+      // class-specialised kernels also read D = M Q and D^T (plk_tc5_pre2.cuh).  Every matrix buffer, once per pass.
+      if (want_grad) {
+        rc = tc5::pre2::launch_prep(in->stream, in->at<float>(L.off_matrix), static_cast<const float*>(Q),
+                                    in->at<float>(L.off_matrix_d), in->at<float>(L.off_matrix_t),
+                                    in->at<float>(L.off_matrix_dt), in->cfg.matrix_buffer_count * L.C, &in->launches);
+        if (rc) return rc;
+      } else {
+        tc5::pre::k_transpose64<<<in->cfg.matrix_buffer_count * L.C, 256, 0, in->stream>>>(
+            in->at<float>(L.off_matrix), in->at<float>(L.off_matrix_t));
+        CHECK_LAUNCH(in);
+      }
     }
 #endif
     // Every gradient kernel writes its own number of partial sums per slot (tile geometry differs between the
@@ -1383,6 +1403,26 @@ static int pre_impl(plk_instance* in, int eigen, int root_pre, const plk_pre_op*
       for (int k = 0; k < 3; ++k) {  // specialised classes
         const int c0 = class_start[(size_t)l * 5 + k], m = class_start[(size_t)l * 5 + k + 1] - c0;
         if (m == 0) continue;
+#ifdef PLK_WITH_TENSOR
+        if (L.SP == 64) {  // tcgen05 classes: results go through the per-category scratch, finished after the last level
+          const tc5::pre2::MatDeltas mdl{(long long)L.off_matrix_d - (long long)L.off_matrix,
+                                         (long long)L.off_matrix_t - (long long)L.off_matrix,
+                                         (long long)L.off_matrix_dt - (long long)L.off_matrix};
+          float* scr = in->at<float>(L.off_cat_scratch);
+          if (k == 0)
+            rc = tc5::pre2::launch_class<0>(in->stream, dit + c0, m, L.P, L.S, L.C, mdl, scr, in->sm_count, &in->launches);
+          else if (k == 1)
+            rc = tc5::pre2::launch_class<1>(in->stream, dit + c0, m, L.P, L.S, L.C, mdl, scr, in->sm_count, &in->launches);
+          else
+            rc = tc5::pre2::launch_tips(in->stream, dit + c0, m, L.P, L.S, L.C, mdl, scr, &in->launches);
+          if (rc) return rc;
+          for (int i = c0; i < c0 + m; ++i) {
+            fin_slots.push_back(hit[i].slot[0]);
+            fin_slots.push_back(hit[i].slot[1]);
+          }
+          continue;
+        }
+#endif
         rc = by_precision(in, [&](auto tag) -> int {
           using T = decltype(tag);
           return launch_pre4_lean<T>(in, k, dit + c0, m, in->h_q4.data() + (size_t)(want_grad ? eigen : 0) * 16, d_site,
@@ -1407,6 +1447,23 @@ static int pre_impl(plk_instance* in, int eigen, int root_pre, const plk_pre_op*
         mark_parts(g0 + first, m);
       }
     }
+#ifdef PLK_WITH_TENSOR
+    if (!fin_slots.empty()) {  // d_k[p] = sum_c w_c r_c num / sum_c w_c den and the weighted pattern sums of those slots
+      char *hs, *ds;
+      rc = ring_alloc(in, fin_slots.size() * sizeof(int), &hs, &ds);
+      if (rc) return rc;
+      std::memcpy(hs, fin_slots.data(), fin_slots.size() * sizeof(int));
+      rc = copy_ring(in, hs, ds, fin_slots.size() * sizeof(int));
+      if (rc) return rc;
+      int parts = 0;
+      rc = tc5::pre2::launch_finish(in->stream, in->at<float>(L.off_cat_scratch), reinterpret_cast<const int*>(ds),
+                                    (int)fin_slots.size(), L.P, L.C, in->at<double>(L.off_catw), in->at<double>(L.off_rates),
+                                    in->at<double>(L.off_weights), in->at<double>(L.off_grad_partial), L.n_tiles, d_site,
+                                    &parts, &in->launches);
+      if (rc) return rc;
+      for (int sl : fin_slots) slot_parts[sl] = parts;
+    }
+#endif
   }
   if (want_grad && count > 0) {
     char *h, *d;

@@ -32,14 +32,6 @@ namespace plk {
 namespace tc5 {
 namespace pre {
 
-#ifdef PLK_TC5_TRACE
-#define TP_T0() long long _t0 = clock64()
-#define TP_ACC(x) do { long long _t1 = clock64(); (x) += _t1 - _t0; _t0 = _t1; } while (0)
-#else
-#define TP_T0() do {} while (0)
-#define TP_ACC(x) do {} while (0)
-#endif
-
 constexpr int EPI_W = 8, PROD_W = 4, AUX_W = 3, N_W = EPI_W + PROD_W + AUX_W + 1;  // tile producers, matrix / q_m stagers
 constexpr int THREADS_PRE = N_W * 32;  // 512
 constexpr int AT = AUX_W * 32;         // threads of the auxiliary stager group
@@ -52,7 +44,7 @@ constexpr uint32_t OFF_BARS = OFF_MX + TP * 4;
 constexpr uint32_t SMEM_USED_PRE = OFF_BARS + 256;
 constexpr size_t SMEM_BYTES_PRE = SMEM_USED_PRE + 1024;
 enum { P_XFULL = 0, P_XFREE, P_UFULL, P_AFULL, P_QFULL, P_MFULL, P_MFREE, P_TFREE, P_ADONE, P_MTFULL,
-       P_MTFULL1, P_MFULL1, P_M0FREE, P_TFREE0, P_TMEM_PTR };
+       P_MTFULL1, P_MFULL1, P_M0FREE, P_TFREE0, P_TMEM_PTR, P_QFULL1 };
 // TMEM columns.  U_0 (hi, lo) has its own 128 columns; U_1 (hi, lo) overwrites a_0 / a_1, which the thread that
 // writes it has just consumed.
 constexpr uint32_t T_A0 = 0, T_A1 = 64, T_QX0 = 128, T_QX1 = 192, T_Q0 = 256, T_Q1 = 320, T_U0 = 384;
@@ -270,7 +262,10 @@ __global__ void __launch_bounds__(THREADS_PRE, 1)
     mbar_init(cx.barrier(P_XFREE), 1);
     mbar_init(cx.barrier(P_UFULL), EPI_W);  // one completion per round: both U_0 and U_1 are in TMEM
     mbar_init(cx.barrier(P_AFULL), 1);
-    mbar_init(cx.barrier(P_QFULL), 1);
+    mbar_init(cx.barrier(P_QFULL), 1);   // q_0 complete (one completion per round)
+    mbar_init(cx.barrier(P_QFULL1), 1);  // q_1 complete.  Two barriers: when step B of child 1 has nothing to do both
+                                         // commits land together, and a single barrier would run two phases ahead of
+                                         // its waiter (an unpaired op hung here)
     mbar_init(cx.barrier(P_MFULL), AUX_W);
     mbar_init(cx.barrier(P_MFREE), 1);
     mbar_init(cx.barrier(P_TFREE), EPI_W);
@@ -381,28 +376,20 @@ __global__ void __launch_bounds__(THREADS_PRE, 1)
     // ===== MMA issuer (whole warp converged; elect.sync inside the asm) =====
     const uint64_t dxhi = make_desc(xs), dxlo = make_desc(xs + X_PLANE);
     uint32_t uc = 0;
-    long long m_tf = 0, m_mf = 0, m_x0 = 0, m_x1 = 0, m_mt = 0, m_u0 = 0, m_u1 = 0, m_is = 0;
-    (void)m_tf; (void)m_mf; (void)m_x0; (void)m_x1; (void)m_mt; (void)m_u0; (void)m_u1; (void)m_is;
-    TP_T0();
     for (uint32_t ui = 0; ui < cx.n_units; ++ui) {
       const DevPreItem& it = items[(cx.u0 + ui) / cx.n_tiles];
       const bool lo[2] = {it.kind[0] == KIND_PARTIALS || it.kind[0] == KIND_BCAST,
                           it.kind[1] == KIND_PARTIALS || it.kind[1] == KIND_BCAST};
       const bool need_q[2] = {it.q[0] != nullptr || it.slot[0] >= 0, it.q[1] != nullptr || it.slot[1] >= 0};
       for (int c = 0; c < C; ++c, ++uc) {
-        TP_ACC(m_is);
         // Qx_0 (first product of step A) may be overwritten once the previous round's q_0 epilogue has read it; a_0 / a_1
         // are free as soon as the previous step B has run (in-order pipe); Qx_1 waits for the q_1 epilogue further down
         if (uc > 0) mbar_wait(cx.barrier(P_TFREE0), (uc - 1) & 1);
-        TP_ACC(m_tf);
 
 #pragma unroll
         for (int k = 0; k < 2; ++k) {  // step A: a_k = X_k M_k^T, Qx_k = X_k Q^T
-          TP_ACC(m_is);
           mbar_wait(cx.barrier(k == 0 ? P_MFULL : P_MFULL1), uc & 1);
-          TP_ACC(m_mf);
           mbar_wait(cx.barrier(P_XFULL), k);
-          if (k == 0) TP_ACC(m_x0); else TP_ACC(m_x1);
           tc_fence_after();
 #pragma unroll
           for (int ww = 0; ww < 2; ++ww) {  // w = 0: M_k, w = 1: Q.  Order Qx_0, a_0, a_1, Qx_1: the u-phase needs only the
@@ -435,15 +422,11 @@ __global__ void __launch_bounds__(THREADS_PRE, 1)
           }
           umma_commit(cx.barrier(P_XFREE));  // the producers' cue for X_1 / for X_0 of the next round
         }
-        TP_ACC(m_is);
         mbar_wait(cx.barrier(P_UFULL), uc & 1);
-        TP_ACC(m_u0);
         tc_fence_after();
 #pragma unroll
         for (int k = 0; k < 2; ++k) {  // step B: q_k = U_k M_k, A = U_k (hi, lo) in TMEM, B = M_k^T (K-major)
-          TP_ACC(m_is);
           mbar_wait(cx.barrier(k == 0 ? P_MTFULL : P_MTFULL1), uc & 1);
-          TP_ACC(m_mt);
           tc_fence_after();
           if (need_q[k]) {
             const uint32_t d = tmem_base + (k == 0 ? T_Q0 : T_Q1);
@@ -458,17 +441,12 @@ __global__ void __launch_bounds__(THREADS_PRE, 1)
               umma_ta(d, uhi + 8 * ks, bhi + koff(ks, 64), 1);
             }
           }
-          umma_commit(cx.barrier(P_QFULL));
+          umma_commit(cx.barrier(k == 0 ? P_QFULL : P_QFULL1));
           if (k == 0) umma_commit(cx.barrier(P_M0FREE));
         }
         umma_commit(cx.barrier(P_MFREE));
       }
     }
-#ifdef PLK_TC5_TRACE
-    if (blockIdx.x == 0 && lane == 0 && uc > 100)
-      printf("MMA rounds %u: issue %lld | wait tfree %lld, mfull %lld, x0 %lld, x1 %lld, mt %lld, u0 %lld, u1 %lld\n", uc, m_is / uc,
-             m_tf / uc, m_mf / uc, m_x0 / uc, m_x1 / uc, m_mt / uc, m_u0 / uc, m_u1 / uc);
-#endif
   } else {
     // ===== epilogue: warp = 4 half + quarter; thread = pattern row 32 quarter + lane, states 32 half .. 32 half + 31 =====
     const int quarter = warp & 3, half = warp >> 2, row = 32 * quarter + lane;
@@ -479,9 +457,6 @@ __global__ void __launch_bounds__(THREADS_PRE, 1)
     double* red = reinterpret_cast<double*>(tc5p_smem_raw + (cx.smem - smem_u32(tc5p_smem_raw)) + OFF_RED);
     float* smx = reinterpret_cast<float*>(tc5p_smem_raw + (cx.smem - smem_u32(tc5p_smem_raw)) + OFF_MX);
     uint32_t uc = 0;
-    long long e_qm = 0, e_a = 0, e_u = 0, e_q0w = 0, e_u1 = 0, e_q0 = 0, e_q1w = 0, e_q1 = 0, e_end = 0;
-    (void)e_qm; (void)e_a; (void)e_u; (void)e_q0w; (void)e_u1; (void)e_q0; (void)e_q1w; (void)e_q1; (void)e_end;
-    TP_T0();
     for (uint32_t ui = 0; ui < cx.n_units; ++ui) {
       const uint32_t u = cx.u0 + ui;
       const DevPreItem& it = items[u / cx.n_tiles];
@@ -495,7 +470,6 @@ __global__ void __launch_bounds__(THREADS_PRE, 1)
       const bool one_factor = __all_sync(0xffffffffu, fq.f2 == 1.f && fx[0].f2 == 1.f && fx[1].f2 == 1.f);
       for (int c = 0; c < C; ++c, ++uc) {
         const double cw = catw[c], cwr = catw[c] * catr[c];
-        TP_ACC(e_end);
         // the warp's own 32 x 32 slice of q_m, global -> shared (coalesced 128-byte row segments), under step A
         {
           const float* src = static_cast<const float*>(it.qm) + ((size_t)c * P + p0 + 32 * quarter) * SP64 + 32 * half;
@@ -512,9 +486,7 @@ __global__ void __launch_bounds__(THREADS_PRE, 1)
           }
           __syncwarp();
         }
-        TP_ACC(e_qm);
         mbar_wait(cx.barrier(P_AFULL), uc & 1);
-        TP_ACC(e_a);
         tc_fence_after();
         // ---- u_0 = q_m o a_1, u_1 = q_m o a_0 (split, straight into TMEM as the A operands of step B), den
         float dd = 0.f;
@@ -560,11 +532,9 @@ __global__ void __launch_bounds__(THREADS_PRE, 1)
         tc_fence_before();
         __syncwarp();
         if (lane == 0) mbar_arrive(cx.barrier(P_UFULL));
-        TP_ACC(e_u);
 #pragma unroll
         for (int k = 0; k < 2; ++k) {
-          mbar_wait(cx.barrier(P_QFULL), k);
-          if (k == 0) TP_ACC(e_q0w); else TP_ACC(e_q1w);
+          mbar_wait(cx.barrier(k == 0 ? P_QFULL : P_QFULL1), uc & 1);
           tc_fence_after();
           float mx = 0.f;
           if (need_q[k]) {
@@ -607,7 +577,6 @@ __global__ void __launch_bounds__(THREADS_PRE, 1)
             if (half == 0 && p < P) static_cast<float*>(it.q_scale[k])[(size_t)c * P + p] = fmaxf(mx, smx[row]);
             epi_bar();  // smx and the slices are free again
           }
-          if (k == 0) TP_ACC(e_q0); else TP_ACC(e_q1);
         }
         __syncwarp();
 
@@ -644,11 +613,6 @@ __global__ void __launch_bounds__(THREADS_PRE, 1)
         epi_bar();
       }
     }
-#ifdef PLK_TC5_TRACE
-    if (blockIdx.x == 0 && threadIdx.x == 0 && uc > 100)
-      printf("EPI rounds %u: end %lld | wait qm %lld, wait A %lld, u-phase %lld, wait q0 %lld, U1 %lld, q0 %lld, wait q1 %lld, q1 %lld\n", uc,
-             e_end / uc, e_qm / uc, e_a / uc, e_u / uc, e_q0w / uc, e_u1 / uc, e_q0 / uc, e_q1w / uc, e_q1 / uc);
-#endif
   }
   tc_fence_before();
   __syncthreads();
