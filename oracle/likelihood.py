@@ -6,6 +6,9 @@ layout [category c, pattern p, state s]; the only library primitive is a matrix 
 S x S matrix-vector products, one per (node, category).  No blocking, fusion or reordering beyond a loop over
 chunks of independent patterns (to bound host memory) in `evaluate`.
 
+Also the approximate gradient with respect to the elements of the rate matrix and its chain rule
+to substitution-model parameters, see `rate_matrix_cross_products`.
+
 Passages followed: PAPER.md:27 (Felsenstein's pruning algorithm gives the likelihood of the data on a tree);
 PAPER.md:43 (a pre-order traversal complements the post-order one; the likelihood is the inner product of post- and
 pre-order partials; the gradient w.r.t. all branch-length-specific parameters takes one pre-order traversal);
@@ -139,6 +142,52 @@ def branch_site_derivatives(qk, pk, Q, rates, cat_weights):
         den = den + cat_weights[c] * np.sum(qk[c] * pk[c], axis=1)
     with np.errstate(divide="ignore", invalid="ignore"):
         return num / den, num, den
+
+
+# ---------------------------------------------------------------------------------------------- 8(f)-1
+def rate_matrix_cross_products(children, root, branch_lengths, Q, pi, rates, cat_weights, tip_partials,
+                               pattern_weights, eigen=None):
+    """Approximate gradient of logL with respect to every ELEMENT of the rate matrix ("the gradient
+    w.r.t. elements of the rate matrix ... exploiting a first-order approximation of the derivative of the matrix
+    exponential"; DESIGN.md section 2 reading 14).
+
+    The likelihood of pattern p is, for ANY branch b (node b below its parent m, sibling j),
+        l_p = sum_c w_c u_b[c,p]^T P_{b,c} p_b[c,p],   u_b = q_m o (P_j p_j),   q_b = P_{b,c}^T u_b
+    and P_{b,c} = exp(Q r_c t_b) enters l_p once per branch, so d l_p / d Q_ij = sum_b sum_c w_c u_b^T (d P_{b,c} / d Q_ij) p_b.
+    First-order approximation (the commutator terms of the exact integral are dropped):
+        d exp(Q tau) / d Q_ij  ~=  tau exp(Q tau) E_ij           (E_ij = unit matrix element, tau = r_c t_b)
+    which turns the sandwich into an outer product of the pre- and post-order partials of the SAME node:
+        G_ij = sum_b t_b sum_p omega_p ( sum_c w_c r_c q_b[c,p,i] p_b[c,p,j] ) / ( sum_c w_c q_b[c,p]^T p_b[c,p] ).
+    It is exact in every direction dQ that commutes with Q (e.g. dQ = Q: the derivative with respect to an overall
+    rate).  Per-pattern scale factors of q_b and p_b cancel in the quotient.  Returns G [S, S] (diagonal included: the
+    chain rule below decides how the diagonal depends on the parameters)."""
+    from .models import eigen_decomposition
+
+    n_nodes = len(children)
+    n_tips = (n_nodes + 1) // 2
+    C = len(rates)
+    S = Q.shape[0]
+    U, Uinv, lam = eigen if eigen is not None else eigen_decomposition(Q, pi)
+    P = {k: transition_matrices(U, Uinv, lam, rates, branch_lengths[k]) for k in range(n_nodes) if k != root}
+    tips = {k: tip_partials[k] for k in range(n_tips)}
+    p, _ = post_order(children, root, P, tips, C)
+    q, _ = pre_order(children, root, P, p, pi)
+    G = np.zeros((S, S))
+    for b in range(n_nodes):
+        if b == root:
+            continue
+        den = np.zeros(p[b].shape[1])
+        for c in range(C):
+            den = den + cat_weights[c] * np.sum(q[b][c] * p[b][c], axis=1)
+        for c in range(C):
+            scale = pattern_weights * (cat_weights[c] * rates[c] * branch_lengths[b]) / den  # [Pn]
+            G = G + (q[b][c] * scale[:, None]).T @ p[b][c]  # sum_p scale_p q[p, i] p[p, j]
+    return G
+
+
+def substitution_parameter_gradient(G, dQ):
+    """Chain rule: d logL / d theta_k ~= sum_ij G_ij dQ_ij / d theta_k, dQ [K, S, S] (O(K S^2))."""
+    return np.einsum("ij,kij->k", G, np.asarray(dQ))
 
 
 # ---------------------------------------------------------------------------------------------- driver
