@@ -223,6 +223,18 @@ PLK_API int plk_pre_order_gradient_device(plk_instance* inst, int eigen, int roo
                                           const plk_pre_op* ops, int count, double* d_out_gradient,
                                           double* d_out_site);
 
+/* S8f-1 / P:29.  Approximate gradient of logL with respect to every element of the rate matrix: the gradient
+ * "w.r.t. elements of the rate matrix" evaluated with "a first-order approximation of the derivative of the matrix
+ * exponential", d exp(Q tau) / d Q_ij ~= tau exp(Q tau) E_ij, which reduces the sandwich of branch b to an outer product
+ * of the pre- and post-order partials of node b (reading 14).  For i in 0..count-1 with
+ * p = post-order buffer post_idx[i], q = pre-order buffer pre_idx[i] of the same node and t = branch_lengths[i]:
+ *   out_G[a][b] = sum_i t_i sum_p omega_p ( sum_c w_c r_c q[c,p,a] p[c,p,b] ) / ( sum_c w_c q[c,p]^T p[c,p] )
+ * out_G: HOST [S][S] row-major (diagonal included).  branch_lengths: HOST [count], finite and >= 0.  Needs the
+ * pre-order partials of every listed node (plk_update_pre_partials, or plk_pre_order_gradient with dest_pre >= 0).
+ * Exact in every direction dQ that commutes with Q (an overall rate).  _FLOATING_POINT if an element is not finite. */
+PLK_API int plk_rate_matrix_gradient(plk_instance* inst, const int32_t* post_idx, const int32_t* pre_idx,
+                                     const double* branch_lengths, int count, double* out_G);
+
 /* ---- read-back (tests) -------------------------------------------------------------------------------------- */
 
 /* Partials [C][P][S] of a post-order (pre = 0) or pre-order (pre = 1) buffer; compact tips are expanded to
@@ -248,6 +260,12 @@ PLK_API int plk_schedule_levels(const plk_op* ops, int count, int32_t* out_level
 /* Same for pre-order ops (dependency: parent_pre written by an earlier op); additionally out_partner[i] = index
  * of the other op with the same parent_pre in the same call (the two are fused into one launch item), or -1. */
 PLK_API int plk_schedule_pre_levels(const plk_pre_op* ops, int count, int32_t* out_level, int32_t* out_partner);
+
+/* S8f-1 / P:45 chain rule ("the product of the gradient w.r.t. elements of the rate matrix and the gradient of the matrix
+ * elements w.r.t. substitution model parameters", O(K S^2)): out[k] = sum_ab G[a][b] dQ[k][a][b].  G: [S][S] from
+ * plk_rate_matrix_gradient; dQ: [K][S][S] = d Q / d theta_k of the client's model (diagonal and normalisation
+ * included); out: [K].  Runs on the host. */
+PLK_API int plk_chain_rule_rate_matrix(const double* G, const double* dQ, int state_count, int param_count, double* out);
 
 /* S8a step 0.  Encode `taxa` character sequences of `sites` characters each (nucleotide: one site per character;
  * codon: sites must be divisible by 3, one site per triplet) and merge identical columns.

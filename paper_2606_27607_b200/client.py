@@ -128,6 +128,14 @@ class Evaluator:
             return grad, full
         return grad
 
+    def rate_matrix_gradient(self, branch_lengths: Optional[np.ndarray] = None):
+        """After log_likelihood() and a pre-order pass that stored EVERY node's pre-order partials
+        (gradient_unfused(), store_tip_pre=True): the S x S approximate gradient with respect to the rate-matrix
+        elements (plk_rate_matrix_gradient)."""
+        t = self.tree.branch_length if branch_lengths is None else branch_lengths
+        nodes = self.matrix_idx
+        return self.inst.rate_matrix_gradient(nodes, nodes, np.asarray(t)[nodes])
+
     # -- device-resident step used by bench.py: nothing but launches, outputs stay on the device
     def make_device_io(self, out=None):
         """`out`: optional fp64 device tensor [1 + 2N-2] that receives [logL, gradient] (one buffer, so that a

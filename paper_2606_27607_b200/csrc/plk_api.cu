@@ -14,6 +14,7 @@
 #include "plk_nuc.cuh"
 #include "plk_nuc_tma.cuh"
 #include "plk_nuc_lean.cuh"
+#include "plk_cross.cuh"
 #include "plk_schedule.h"
 #ifdef PLK_WITH_TENSOR
 #include "plk_tc.cuh"
@@ -42,7 +43,7 @@ struct Layout {
   int n_tiles, max_grad;
   size_t off_post, off_compact, off_pre, off_pre_mx, off_matrix, off_eigen, off_scale, off_weights, off_pi,
       off_rates, off_catw, off_site, off_block_partial, off_grad_partial, off_grad_out, off_logl, off_site_deriv,
-      off_stage, off_ring, off_matrix_t, off_matrix_d, off_matrix_dt, off_cat_scratch, total;
+      off_stage, off_ring, off_matrix_t, off_matrix_d, off_matrix_dt, off_cat_scratch, off_cross_partial, off_cross_out, total;
   size_t stage_bytes;
 };
 
@@ -114,6 +115,12 @@ bool compute_layout(const plk_config& c, Layout& L) {
   L.off_matrix_d = take((L.SP == 4 || tc5) ? (size_t)c.matrix_buffer_count * L.matrix_bytes : 0);
   L.off_matrix_dt = take(tc5 ? (size_t)c.matrix_buffer_count * L.matrix_bytes : 0);
   L.off_cat_scratch = take((tc5 && c.preorder_buffer_count > 0) ? (size_t)L.max_grad * 2 * L.C * L.P * 4 : 0);
+  // rate-matrix gradient (plk_cross.cuh): per-block partial sums and the S x S result
+  L.off_cross_partial = take(c.preorder_buffer_count > 0
+                                 ? (L.SP == 4 ? (size_t)16 * ((L.P + CROSS4_THREADS - 1) / CROSS4_THREADS)
+                                              : (size_t)((L.P + CROSS64_TP - 1) / CROSS64_TP) * L.SP * L.SP) * 8
+                                 : 0);
+  L.off_cross_out = take((size_t)L.SP * L.SP * 8);
   L.total = o;
   return true;
 }
@@ -1556,6 +1563,98 @@ int plk_branch_derivatives(plk_instance* in, int eigen, const int32_t* post_idx,
                                             in->at<double>(L.off_grad_out));
   CHECK_LAUNCH(in);
   return finish_gradient(in, count, out_gradient, out_site, d_site);
+}
+
+// ---- 8(f)-1: approximate gradient with respect to the rate-matrix elements --------------------------------------------
+
+int plk_rate_matrix_gradient(plk_instance* in, const int32_t* post_idx, const int32_t* pre_idx,
+                             const double* branch_lengths, int count, double* out_G) {
+  if (in == nullptr || count < 0 || out_G == nullptr) return PLK_ERR_OUT_OF_RANGE;
+  const Layout& L = in->L;
+  const plk_config& cfg = in->cfg;
+  if (cfg.preorder_buffer_count == 0) return PLK_ERR_UNSUPPORTED;
+  if (count > 0 && (post_idx == nullptr || pre_idx == nullptr || branch_lengths == nullptr)) return PLK_ERR_OUT_OF_RANGE;
+  int rc = check_model_ready(in, true);
+  if (rc) return rc;
+  const int n_elem = L.SP * L.SP;
+  double* d_out = in->at<double>(L.off_cross_out);
+  if (count == 0) {
+    for (int i = 0; i < L.S * L.S; ++i) out_G[i] = 0.0;
+    return PLK_SUCCESS;
+  }
+  char *h, *d;
+  rc = ring_alloc(in, (size_t)count * sizeof(DevCrossBranch), &h, &d);
+  if (rc) return rc;
+  DevCrossBranch* hb = reinterpret_cast<DevCrossBranch*>(h);
+  for (int i = 0; i < count; ++i) {
+    if (pre_idx[i] < 0 || pre_idx[i] >= cfg.preorder_buffer_count) return PLK_ERR_OUT_OF_RANGE;
+    if (in->pre_slot[pre_idx[i]] < 0 || !in->pre_written[pre_idx[i]]) return PLK_ERR_UNINITIALIZED;
+    if (!(branch_lengths[i] >= 0.0 && std::isfinite(branch_lengths[i]))) return PLK_ERR_OUT_OF_RANGE;
+    const void* pending;
+    rc = operand_of(in, post_idx[i], &hb[i].p, &hb[i].kind, &pending);
+    if (rc) return rc;
+    hb[i].q = in->pre_ptr(pre_idx[i]);
+    hb[i].t = branch_lengths[i];
+    hb[i].pad = 0;
+  }
+  rc = copy_ring(in, h, d, (size_t)count * sizeof(DevCrossBranch));
+  if (rc) return rc;
+  const DevCrossBranch* db = reinterpret_cast<const DevCrossBranch*>(d);
+  const double* cw = in->at<double>(L.off_catw);
+  const double* cr = in->at<double>(L.off_rates);
+  const double* wt = in->at<double>(L.off_weights);
+  double* part = in->at<double>(L.off_cross_partial);
+  if (L.SP == 4) {
+    const int n_blocks = (L.P + CROSS4_THREADS - 1) / CROSS4_THREADS;
+    rc = by_precision(in, [&](auto tag) -> int {
+      using T = decltype(tag);
+      switch (L.C) {
+#define CASE(CC) case CC: k_cross4<T, CC><<<n_blocks, CROSS4_THREADS, 0, in->stream>>>(db, count, L.P, cw, cr, wt, part, n_blocks); break;
+        CASE(1) CASE(2) CASE(3) CASE(4) CASE(5) CASE(6) CASE(7) CASE(8)
+#undef CASE
+        default: return PLK_ERR_UNSUPPORTED;
+      }
+      return PLK_SUCCESS;
+    });
+    if (rc) return rc;
+    CHECK_LAUNCH(in);
+    k_sum_rows<<<16, 128, 0, in->stream>>>(part, nullptr, n_blocks, n_blocks, d_out);
+    CHECK_LAUNCH(in);
+  } else {
+    const int n_blocks = (L.P + CROSS64_TP - 1) / CROSS64_TP;
+    rc = by_precision(in, [&](auto tag) -> int {
+      using T = decltype(tag);
+      int r2 = opt_in_smem(k_cross64<T>, cross64_smem<T>());
+      if (r2) return r2;
+      k_cross64<T><<<n_blocks, CROSS64_THREADS, cross64_smem<T>(), in->stream>>>(db, count, L.P, L.S, L.C, cw, cr, wt, part);
+      return PLK_SUCCESS;
+    });
+    if (rc) return rc;
+    CHECK_LAUNCH(in);
+    k_sum_blocks<<<(n_elem + 255) / 256, 256, 0, in->stream>>>(part, n_blocks, n_elem, d_out);
+    CHECK_LAUNCH(in);
+  }
+  std::vector<double> tmp(n_elem);
+  rc = download(in, tmp.data(), d_out, n_elem);
+  if (rc) return rc;
+  for (int i = 0; i < L.S; ++i)
+    for (int j = 0; j < L.S; ++j) {
+      out_G[i * L.S + j] = tmp[i * L.SP + j];
+      if (!std::isfinite(out_G[i * L.S + j])) rc = PLK_ERR_FLOATING_POINT;
+    }
+  return rc;
+}
+
+int plk_chain_rule_rate_matrix(const double* G, const double* dQ, int state_count, int param_count, double* out) {
+  if (G == nullptr || out == nullptr || state_count < 1 || param_count < 0 || (param_count > 0 && dQ == nullptr))
+    return PLK_ERR_OUT_OF_RANGE;
+  const size_t n = (size_t)state_count * state_count;
+  for (int k = 0; k < param_count; ++k) {
+    double s = 0.0;
+    for (size_t e = 0; e < n; ++e) s += G[e] * dQ[(size_t)k * n + e];
+    out[k] = s;
+  }
+  return PLK_SUCCESS;
 }
 
 // ---- read-back -------------------------------------------------------------------------------------------------------

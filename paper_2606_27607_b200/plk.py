@@ -73,6 +73,8 @@ _SIGNATURES = {
     "plk_branch_derivatives": (_I, [_P, _I, _P, _P, _I, _P, _P]),
     "plk_pre_order_gradient": (_I, [_P, _I, _I, _P, _I, _P, _P]),
     "plk_pre_order_gradient_device": (_I, [_P, _I, _I, _P, _I, _P, _P]),
+    "plk_rate_matrix_gradient": (_I, [_P, _P, _P, _P, _I, _P]),
+    "plk_chain_rule_rate_matrix": (_I, [_P, _P, _I, _I, _P]),
     "plk_get_partials": (_I, [_P, _I, _I, _P]),
     "plk_get_scale_factors": (_I, [_P, _I, _P]),
     "plk_get_transition_matrix": (_I, [_P, _I, _P]),
@@ -155,6 +157,17 @@ def schedule_pre_levels(ops: np.ndarray):
     n = lib().plk_schedule_pre_levels(_ptr(ops), len(ops), _ptr(level), _ptr(partner))
     _check(min(n, 0), "plk_schedule_pre_levels")
     return n, level, partner
+
+
+def chain_rule_rate_matrix(G, dQ):
+    """plk_chain_rule_rate_matrix: out[k] = sum_ab G[a][b] dQ[k][a][b] (host only)."""
+    G = _f64(G)
+    S = int(round(np.sqrt(G.size)))
+    dQ = _f64(dQ)
+    K = dQ.size // (S * S)
+    out = np.zeros(K)
+    _check(lib().plk_chain_rule_rate_matrix(_ptr(G), _ptr(dQ), S, K, _ptr(out)), "plk_chain_rule_rate_matrix")
+    return out
 
 
 def encode_and_compress(state_kind: int, seqs: Sequence[bytes]):
@@ -329,6 +342,13 @@ class Instance:
         self._call("plk_pre_order_gradient_device", eigen, root_pre_buffer, _ptr(ops), len(ops),
                    C.c_void_p(d_out_gradient.data_ptr()),
                    None if d_out_site is None else C.c_void_p(d_out_site.data_ptr()))
+
+    def rate_matrix_gradient(self, post_idx, pre_idx, branch_lengths):
+        a, b = _i32(post_idx), _i32(pre_idx)
+        t = _f64(branch_lengths, a.size)
+        out = np.zeros((self.S, self.S))
+        self._call("plk_rate_matrix_gradient", _ptr(a), _ptr(b), _ptr(t), a.size, _ptr(out))
+        return out
 
     # -- read-back
     def get_partials(self, buffer, pre=False):

@@ -106,3 +106,13 @@ def test_encode_errors():
     s, w, m = plk.encode_and_compress(plk.NUCLEOTIDE, [b"", b""])
     assert s.shape == (2, 0) and w.size == 0 and m.size == 0
     assert lib.plk_destroy(None) == 0
+
+
+def test_chain_rule_rate_matrix_host_helper():
+    """plk_chain_rule_rate_matrix: out[k] = sum_ab G[a][b] dQ[k][a][b]; no device needed."""
+    rng = np.random.default_rng(11)
+    G = rng.normal(size=(61, 61))
+    dQ = rng.normal(size=(7, 61, 61))
+    out = plk.chain_rule_rate_matrix(G, dQ)
+    assert np.allclose(out, [np.sum(G * dQ[k]) for k in range(7)], rtol=1e-13, atol=0)
+    assert plk.chain_rule_rate_matrix(G, np.zeros((0, 61, 61))).shape == (0,)
