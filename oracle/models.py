@@ -68,6 +68,23 @@ def gtr(rho, pi):
     return _finish(sym * pi[None, :], pi), pi
 
 
+def general_reversible(rho_upper, pi):
+    """General time-reversible model on S = len(pi) states (the 20-state amino-acid models the paper's tensor-core
+    claim covers): q_ij = rho_ij pi_j with rho symmetric, its S(S-1)/2 upper-triangle
+    entries given row by row ((0,1), (0,2), ..., (S-2,S-1)).  GTR (8(c) row 5) is the case S = 4."""
+    pi = np.asarray(pi, dtype=np.float64)
+    S = pi.shape[0]
+    rho = np.asarray(rho_upper, dtype=np.float64)
+    assert rho.shape[0] == S * (S - 1) // 2
+    sym = np.zeros((S, S))
+    n = 0
+    for i in range(S):
+        for j in range(i + 1, S):
+            sym[i, j] = sym[j, i] = rho[n]
+            n += 1
+    return _finish(sym * pi[None, :], pi), pi
+
+
 def gy94(kappa, omega, f1, f2, f3):
     """GY94 with F3x4 frequencies (8(c) row 6): q_ij = 0 unless codons i, j differ at exactly one position; then
     pi_j, times kappa for a transition, times omega for a non-synonymous change.  pi_j ~ f1[n1] f2[n2] f3[n3]
@@ -103,6 +120,8 @@ def rate_matrix(model):
         return hky(model["kappa"], model["pi"])
     if name == "GTR":
         return gtr(model["rho"], model["pi"])
+    if name == "AA20":
+        return general_reversible(model["rho"], model["pi"])
     if name == "GY94":
         return gy94(model["kappa"], model["omega"], model["f1"], model["f2"], model["f3"])
     raise ValueError(name)

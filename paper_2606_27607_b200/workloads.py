@@ -171,7 +171,13 @@ def _is_transition(a: str, b: str) -> bool:
 def client_rate_matrix(model: dict) -> Tuple[np.ndarray, np.ndarray]:
     """Model parameters -> (Q, pi), Q normalised to one expected substitution per unit time."""
     name = model["name"]
-    if name in ("HKY", "GTR"):
+    if name == "AA20":  # 20-state reversible model: exchangeabilities (upper triangle, row by row) x frequencies
+        pi = np.asarray(model["pi"], dtype=np.float64)
+        S = len(pi)
+        R = np.zeros((S, S))
+        R[np.triu_indices(S, 1)] = model["rho"]
+        Q = (R + R.T) * pi[None, :]
+    elif name in ("HKY", "GTR"):
         pi = np.asarray(model["pi"], dtype=np.float64)
         R = np.zeros((4, 4))
         if name == "HKY":
@@ -333,6 +339,8 @@ def draw_model(name: str, rng: np.random.Generator) -> dict:
     if name == "GTR":
         rho = rng.gamma(2.0, 1.0, size=6).tolist()
         return {"name": "GTR", "rho": rho, "pi": rng.dirichlet([10.0] * 4).tolist()}
+    if name == "AA20":
+        return {"name": "AA20", "rho": rng.gamma(2.0, 1.0, size=190).tolist(), "pi": rng.dirichlet([10.0] * 20).tolist()}
     if name == "GY94":
         return {"name": "GY94", "kappa": 2.0, "omega": 0.3,
                 "f1": rng.dirichlet([10.0] * 4).tolist(), "f2": rng.dirichlet([10.0] * 4).tolist(),
@@ -385,6 +393,9 @@ def config(index: int, n_tips: Optional[int] = None, n_patterns: Optional[int] =
                              n_cat=n_categories)
     if index == 3:
         return make_workload("cfg3_gy94_256x20000", "GY94", n_tips or 256, n_patterns or 20_000, "coalescent", seed,
+                             n_cat=n_categories)
+    if index == 5:  # not a BASELINE config: the 20-state amino-acid shape of SURVEY 8(f)-2
+        return make_workload("aa20_64x20000", "AA20", n_tips or 64, n_patterns or 20_000, "coalescent", seed,
                              n_cat=n_categories)
     if index == 4:
         n = n_tips or 512

@@ -149,3 +149,27 @@ def test_transition_matrices(name):
         assert np.abs(Ps[c] @ Pt[c] - Pst[c]).max() < 1e-13  # Chapman-Kolmogorov
     Pinf = lk.transition_matrices(U, Uinv, lam, np.ones(1), 1e4)[0]
     assert np.abs(Pinf - pi[None, :]).max() < 1e-12  # rows -> stationary distribution
+
+
+def test_general_reversible_20_states():
+    """SURVEY 8(f)-2 (PAPER.md:59 amino-acid models): the S-state reversible model reduces to GTR at S = 4 (same
+    exchangeability order AC, AG, AT, CG, CT, GT), and at S = 20 satisfies the defining properties -- rows sum to 0,
+    detailed balance pi_i q_ij = pi_j q_ji, pi Q = 0, unit normalisation, q_ij / pi_j symmetric and equal to the given
+    exchangeability up to the common normalisation -- and its eigendecomposition reconstructs it."""
+    rng = np.random.default_rng(77)
+    rho4, pi4 = rng.gamma(2, 1, 6), rng.dirichlet([10] * 4)
+    assert np.array_equal(models.general_reversible(rho4, pi4)[0], models.gtr(rho4, pi4)[0])
+    rho, pi = rng.gamma(2, 1, 190), rng.dirichlet([10] * 20)
+    Q, pi_out = models.general_reversible(rho, pi)
+    assert Q.shape == (20, 20) and np.array_equal(pi_out, pi)
+    assert np.max(np.abs(Q.sum(axis=1))) < 1e-14 and np.max(np.abs(pi @ Q)) < 1e-15
+    F = pi[:, None] * Q
+    assert np.max(np.abs(F - F.T)) < 1e-16
+    assert abs(-np.sum(pi * np.diag(Q)) - 1.0) < 1e-14
+    ratio = Q / pi[None, :]
+    mu = ratio[0, 1] / rho[0]
+    assert abs(ratio[0, 19] / rho[18] - mu) < 1e-13 * mu and abs(ratio[1, 2] / rho[19] - mu) < 1e-13 * mu
+    assert abs(ratio[18, 19] / rho[189] - mu) < 1e-13 * mu
+    U, Uinv, lam = models.eigen_decomposition(Q, pi)
+    assert np.max(np.abs(U @ np.diag(lam) @ Uinv - Q)) < 1e-13 and np.max(np.abs(U @ Uinv - np.eye(20))) < 1e-13
+    assert abs(np.max(lam)) < 1e-14 and np.all(np.sort(lam)[:-1] < 0)
