@@ -21,7 +21,7 @@
  *                  that stream before returning; calls with only device outputs (`*_device`) never synchronise.
  *   Layout         every exposed array is row-major with the state index fastest, then pattern, then category:
  *                  partials[c][p][s]; matrices M[c][s_parent][s_child].  Internally states are padded
- *                  (61 -> 64) with zeros; padding never appears at this boundary.
+ *                  (20 -> 32, 61 -> 64) with zeros; padding never appears at this boundary.
  *   Indices        partials buffers 0..partials_buffer_count-1 (tips are 0..tip_count-1); pre-order buffers
  *                  0..preorder_buffer_count-1; matrix / scale / eigen buffers likewise.  Any index out of range
  *                  -> PLK_ERR_OUT_OF_RANGE; a buffer read before it was written -> PLK_ERR_UNINITIALIZED.
@@ -82,7 +82,8 @@ typedef struct plk_instance plk_instance;            /* opaque */
 /* All sizes are fixed at creation (S8b). */
 typedef struct {
   int32_t tip_count;              /* N >= 2                                                              */
-  int32_t state_count;            /* S: 4 (nucleotide, bandwidth kernels) or 5..64 (padded to 64; 61 = codon) */
+  int32_t state_count;            /* S: 4 (nucleotide, bandwidth kernels), 5..32 (padded to 32; 20 = amino acids,
+                                     CUDA cores) or 33..64 (padded to 64; 61 = codon)                       */
   int32_t pattern_count;          /* P >= 1                                                              */
   int32_t category_count;         /* C >= 1 (<= 16)                                                      */
   int32_t partials_buffer_count;  /* size of the post-order index space (tips first), usually 2N-1       */

@@ -58,7 +58,7 @@ bool compute_layout(const plk_config& c, Layout& L) {
     return false;
   if (c.precision != PLK_FP64 && c.precision != PLK_FP32) return false;
   L.S = c.state_count;
-  L.SP = c.state_count == 4 ? 4 : 64;
+  L.SP = c.state_count == 4 ? 4 : (c.state_count <= 32 ? 32 : 64);  // 5..32 states (amino acids: 20) pad to 32
   L.C = c.category_count;
   L.P = c.pattern_count;
   L.w = c.precision == PLK_FP64 ? 8 : 4;
@@ -98,8 +98,8 @@ bool compute_layout(const plk_config& c, Layout& L) {
   L.off_rates = take((size_t)L.C * 8);
   L.off_catw = take((size_t)L.C * 8);
   L.off_site = take((size_t)L.P * 8);
-  // one partial per block of k_root (128 threads, G threads per pattern: G = 1 for SP = 4, 16 for SP = 64)
-  L.off_block_partial = take(((size_t)L.P * (L.SP == 4 ? 1 : 16) + 127) / 128 * 8 + 8);
+  // one partial per block of k_root (128 threads, G threads per pattern: G = 1 for SP = 4, SP / 4 otherwise)
+  L.off_block_partial = take(((size_t)L.P * (L.SP == 4 ? 1 : L.SP / 4) + 127) / 128 * 8 + 8);
   L.off_grad_partial = take((size_t)L.max_grad * L.n_tiles * 8);
   L.off_grad_out = take((size_t)L.max_grad * 8);
   L.off_logl = take(64);
@@ -589,6 +589,14 @@ int opt_in_smem(K kernel, size_t bytes) {
 template <typename T>
 int launch_post64(plk_instance* in, const DevOp* d_ops, int n_ops) {
   const Layout& L = in->L;
+  if (L.SP == 32) {  // 5..32 states: the CUDA-core kernels instantiated for 32 padded states (plk_gen.cuh)
+    int rc = opt_in_smem(k_post64<T, 32>, post64_smem<T, 32>());
+    if (rc) return rc;
+    dim3 grid(L.n_tiles, L.C, n_ops);
+    k_post64<T, 32><<<grid, GEN_THREADS, post64_smem<T, 32>(), in->stream>>>(d_ops, L.P, L.S, L.C);
+    CHECK_LAUNCH(in);
+    return PLK_SUCCESS;
+  }
 #ifdef PLK_WITH_TENSOR
   if (in->cfg.flags & PLK_FLAG_TENSOR_CORES) {
     if (sizeof(T) == 4 && !(in->cfg.flags & PLK_FLAG_NO_TCGEN05))
@@ -611,6 +619,15 @@ int launch_pre64(plk_instance* in, const DevPreItem* d_items, int n, const T* Q,
   const double* cr = in->at<double>(L.off_rates);
   const double* wt = in->at<double>(L.off_weights);
   double* gp = in->at<double>(L.off_grad_partial);
+  if (L.SP == 32) {
+    int rc = opt_in_smem(k_pre64<T, 32>, pre64_smem<T, 32>());
+    if (rc) return rc;
+    dim3 grid(L.n_tiles, n);
+    k_pre64<T, 32><<<grid, GEN_THREADS, pre64_smem<T, 32>(), in->stream>>>(d_items, L.P, L.S, L.C, Q, cw, cr, wt, gp, L.n_tiles, site);
+    CHECK_LAUNCH(in);
+    in->grad_parts = L.n_tiles;
+    return PLK_SUCCESS;
+  }
 #ifdef PLK_WITH_TENSOR
   if (in->cfg.flags & PLK_FLAG_TENSOR_CORES)
   {
@@ -635,6 +652,17 @@ int launch_pre64(plk_instance* in, const DevPreItem* d_items, int n, const T* Q,
 template <typename T>
 int launch_deriv64(plk_instance* in, const DevBranch* d_br, int n, const T* Q, double* site) {
   const Layout& L = in->L;
+  if (L.SP == 32) {
+    int r2 = opt_in_smem(k_deriv64<T, 32>, deriv64_smem<T, 32>());
+    if (r2) return r2;
+    dim3 grid32(L.n_tiles, n);
+    k_deriv64<T, 32><<<grid32, GEN_THREADS, deriv64_smem<T, 32>(), in->stream>>>(
+        d_br, L.P, L.S, L.C, Q, in->at<double>(L.off_catw), in->at<double>(L.off_rates), in->at<double>(L.off_weights),
+        in->at<double>(L.off_grad_partial), L.n_tiles, site);
+    CHECK_LAUNCH(in);
+    in->grad_parts = L.n_tiles;
+    return PLK_SUCCESS;
+  }
   int rc = opt_in_smem(k_deriv64<T>, deriv64_smem<T>());
   if (rc) return rc;
   dim3 grid(L.n_tiles, n);
@@ -1150,7 +1178,7 @@ static int root_impl(plk_instance* in, int root, const int32_t* scale_idx, int s
     if (rc) return rc;
   }
   double* bp = in->at<double>(L.off_block_partial);
-  const int G = L.SP == 4 ? 1 : 16;
+  const int G = L.SP == 4 ? 1 : L.SP / 4;  // threads per pattern, 4 states each
   const int n_blocks = (int)blocks_for((size_t)L.P * G, 128);
   by_precision(in, [&](auto tag) -> int {
     using T = decltype(tag);
@@ -1160,6 +1188,11 @@ static int root_impl(plk_instance* in, int root, const int32_t* scale_idx, int s
                                                         in->at<double>(L.off_catw),
                                                         reinterpret_cast<const void* const*>(d), (int)list.size(),
                                                         in->at<double>(L.off_weights), d_site, bp);
+    else if (L.SP == 32)
+      k_root<T, 32, 8><<<n_blocks, 128, 0, in->stream>>>(r, kind, L.P, L.C, in->at<double>(L.off_pi),
+                                                         in->at<double>(L.off_catw),
+                                                         reinterpret_cast<const void* const*>(d), (int)list.size(),
+                                                         in->at<double>(L.off_weights), d_site, bp);
     else
       k_root<T, 64, 16><<<n_blocks, 128, 0, in->stream>>>(r, kind, L.P, L.C, in->at<double>(L.off_pi),
                                                           in->at<double>(L.off_catw),
@@ -1624,6 +1657,12 @@ int plk_rate_matrix_gradient(plk_instance* in, const int32_t* post_idx, const in
     const int n_blocks = (L.P + CROSS64_TP - 1) / CROSS64_TP;
     rc = by_precision(in, [&](auto tag) -> int {
       using T = decltype(tag);
+      if (L.SP == 32) {
+        int r3 = opt_in_smem(k_cross64<T, 32>, cross64_smem<T, 32>());
+        if (r3) return r3;
+        k_cross64<T, 32><<<n_blocks, CROSS64_THREADS, cross64_smem<T, 32>(), in->stream>>>(db, count, L.P, L.S, L.C, cw, cr, wt, part);
+        return PLK_SUCCESS;
+      }
       int r2 = opt_in_smem(k_cross64<T>, cross64_smem<T>());
       if (r2) return r2;
       k_cross64<T><<<n_blocks, CROSS64_THREADS, cross64_smem<T>(), in->stream>>>(db, count, L.P, L.S, L.C, cw, cr, wt, part);

@@ -72,22 +72,22 @@ __global__ void __launch_bounds__(CROSS4_THREADS) k_cross4(const DevCrossBranch*
   }
 }
 
-// ---- 64 padded states ------------------------------------------------------------------------------------------
+// ---- 32 / 64 padded states ----------------------------------------------------------------------------------------
 constexpr int CROSS64_TP = 32, CROSS64_THREADS = 256;
-template <typename T>
+template <typename T, int SP = SP64>
 constexpr size_t cross64_smem() {
-  return (size_t)2 * CROSS64_TP * Gen<T>::TS * sizeof(T) + (size_t)2 * CROSS64_TP * sizeof(double);
+  return (size_t)2 * CROSS64_TP * Gen<T, SP>::TS * sizeof(T) + (size_t)2 * CROSS64_TP * sizeof(double);
 }
 
-// grid.x = pattern chunks of 32; thread (ti, tj) = (tid >> 4, tid & 15) owns G[4 ti .. 4 ti + 3][4 tj .. 4 tj + 3].
-// partial[block][i * 64 + j] (padded rows / columns stay 0).
-template <typename T>
+// grid.x = pattern chunks of 32; thread (ti, tj) = (tid >> 4, tid & 15) owns the B x B block G[B ti ..][B tj ..],
+// B = SP / 16.  partial[block][i * SP + j] (padded rows / columns stay 0).
+template <typename T, int SP = SP64>
 __global__ void __launch_bounds__(CROSS64_THREADS) k_cross64(const DevCrossBranch* __restrict__ br, int n_br, int P, int S,
                                                              int C, const double* __restrict__ catw,
                                                              const double* __restrict__ catr,
                                                              const double* __restrict__ weights,
                                                              double* __restrict__ partial) {
-  constexpr int TS = Gen<T>::TS;
+  constexpr int TS = Gen<T, SP>::TS, B = SP / 16, NPT = SP / 8;
   extern __shared__ __align__(16) unsigned char smem_raw[];
   T* tQ = reinterpret_cast<T*>(smem_raw);
   T* tX = tQ + CROSS64_TP * TS;
@@ -96,62 +96,62 @@ __global__ void __launch_bounds__(CROSS64_THREADS) k_cross64(const DevCrossBranc
   static_assert(CROSS64_TP == GEN_TP && CROSS64_THREADS == GEN_THREADS, "load_tile geometry");
   const int p0 = blockIdx.x * CROSS64_TP;
   const int ti = threadIdx.x >> 4, tj = threadIdx.x & 15;
-  const int pp = threadIdx.x >> 3, sb = threadIdx.x & 7;  // den pass: 8 lanes per pattern, 8 states each
-  double g[16];
+  const int pp = threadIdx.x >> 3, sb = threadIdx.x & 7;  // den pass: 8 lanes per pattern, NPT states each
+  double g[B * B];
 #pragma unroll
-  for (int e = 0; e < 16; ++e) g[e] = 0.0;
+  for (int e = 0; e < B * B; ++e) g[e] = 0.0;
   for (int b = 0; b < n_br; ++b) {
-    const DevCrossBranch B = br[b];
+    const DevCrossBranch Br = br[b];
     // pass 1: den_p = sum_c w_c q^T p
     if (threadIdx.x < CROSS64_TP) sDen[threadIdx.x] = 0.0;
     for (int c = 0; c < C; ++c) {
       __syncthreads();
-      load_tile<T>(tQ, KIND_PARTIALS, B.q, c, p0, P, S);
-      load_tile<T>(tX, B.kind, B.p, c, p0, P, S);
+      load_tile<T, SP>(tQ, KIND_PARTIALS, Br.q, c, p0, P, S);
+      load_tile<T, SP>(tX, Br.kind, Br.p, c, p0, P, S);
       __syncthreads();
       T d = T(0);
 #pragma unroll
-      for (int k = 0; k < 8; ++k) d = fma(tQ[pp * TS + 8 * sb + k], tX[pp * TS + 8 * sb + k], d);
+      for (int k = 0; k < NPT; ++k) d = fma(tQ[pp * TS + NPT * sb + k], tX[pp * TS + NPT * sb + k], d);
       d = lane8_sum(d);
       if (sb == 0) sDen[pp] += catw[c] * (double)d;
     }
     // pass 2: G += sum_c sum_p (omega_p w_c r_c t_b / den_p) q[p, i] p[p, j]   (the chunk's tiles come back from L2)
     for (int c = 0; c < C; ++c) {
       __syncthreads();
-      load_tile<T>(tQ, KIND_PARTIALS, B.q, c, p0, P, S);
-      load_tile<T>(tX, B.kind, B.p, c, p0, P, S);
+      load_tile<T, SP>(tQ, KIND_PARTIALS, Br.q, c, p0, P, S);
+      load_tile<T, SP>(tX, Br.kind, Br.p, c, p0, P, S);
       if (threadIdx.x < CROSS64_TP) {
         const int p = p0 + threadIdx.x;
-        sScale[threadIdx.x] = p < P ? weights[p] * catw[c] * catr[c] * B.t / sDen[threadIdx.x] : 0.0;
+        sScale[threadIdx.x] = p < P ? weights[p] * catw[c] * catr[c] * Br.t / sDen[threadIdx.x] : 0.0;
       }
       __syncthreads();
-      T acc[16];  // working-precision sum over the 32 patterns of the chunk, widened once per (branch, category)
+      T acc[B * B];  // working-precision sum over the 32 patterns of the chunk, widened once per (branch, category)
 #pragma unroll
-      for (int e = 0; e < 16; ++e) acc[e] = T(0);
+      for (int e = 0; e < B * B; ++e) acc[e] = T(0);
 #pragma unroll 4
       for (int r = 0; r < CROSS64_TP; ++r) {
         const T sc = (T)sScale[r];
-        T qi[4], xj[4];
+        T qi[B], xj[B];
 #pragma unroll
-        for (int k = 0; k < 4; ++k) {
-          qi[k] = tQ[r * TS + 4 * ti + k] * sc;
-          xj[k] = tX[r * TS + 4 * tj + k];
+        for (int k = 0; k < B; ++k) {
+          qi[k] = tQ[r * TS + B * ti + k] * sc;
+          xj[k] = tX[r * TS + B * tj + k];
         }
 #pragma unroll
-        for (int i = 0; i < 4; ++i)
+        for (int i = 0; i < B; ++i)
 #pragma unroll
-          for (int j = 0; j < 4; ++j) acc[4 * i + j] = fma(qi[i], xj[j], acc[4 * i + j]);
+          for (int j = 0; j < B; ++j) acc[B * i + j] = fma(qi[i], xj[j], acc[B * i + j]);
       }
 #pragma unroll
-      for (int e = 0; e < 16; ++e) g[e] += (double)acc[e];
+      for (int e = 0; e < B * B; ++e) g[e] += (double)acc[e];
     }
     __syncthreads();
   }
-  double* out = partial + (size_t)blockIdx.x * SP64 * SP64;
+  double* out = partial + (size_t)blockIdx.x * SP * SP;
 #pragma unroll
-  for (int i = 0; i < 4; ++i)
+  for (int i = 0; i < B; ++i)
 #pragma unroll
-    for (int j = 0; j < 4; ++j) out[(4 * ti + i) * SP64 + 4 * tj + j] = g[4 * i + j];
+    for (int j = 0; j < B; ++j) out[(B * ti + i) * SP + B * tj + j] = g[B * i + j];
 }
 
 // out[e] = sum over blocks of partial[block][e] in block order (fixed order)

@@ -1,6 +1,8 @@
 // plk_gen.cuh -- CUDA-core kernels for state counts padded to SP = 64 (61-state codon models): the comparison arm
 // BASELINE.json configs[2] asks for ("CUDA-core vs tensor-core partials update") and the path used when the
-// instance was created without PLK_FLAG_TENSOR_CORES.
+// instance was created without PLK_FLAG_TENSOR_CORES -- and, instantiated with SP = 32, the kernels of the 20-state
+// amino-acid models (5..32 states): a quarter of the flops and half of the bytes of
+// padding them to 64.  Everything below is templated on the padded state count SP (a multiple of 32), default 64.
 //
 // A block of 256 threads handles one (operation, category, tile of 32 patterns).  Thread (pp = tid / 8, sb = tid % 8)
 // owns 8 output states of pattern pp: chunks of VEC = 16 / sizeof(T) consecutive states, interleaved over sb so that
@@ -20,11 +22,13 @@ constexpr int SP64 = 64;
 constexpr int GEN_TP = 32;        // patterns per tile
 constexpr int GEN_THREADS = 256;  // 32 patterns x 8 state-lanes
 
-template <typename T>
+template <typename T, int SP = SP64>
 struct Gen {
   static constexpr int VEC = 16 / sizeof(T);  // 4 (fp32) or 2 (fp64)
-  static constexpr int NCH = 8 / VEC;         // chunks per thread
-  static constexpr int TS = SP64 + VEC;       // padded tile row stride
+  static constexpr int NPT = SP / 8;          // states per thread (8 lanes share a pattern)
+  static constexpr int NCH = NPT / VEC;       // chunks per thread
+  static constexpr int TS = SP + VEC;         // padded tile row stride
+  static_assert(SP % 32 == 0 && NCH >= 1, "padded state count");
 };
 template <typename T>
 struct VecOf;
@@ -49,26 +53,26 @@ __device__ __forceinline__ int state_of(int sb, int i, int j) {
 }
 
 // A[x][s] <- transpose ? M[s][x] : M[x][s]    (M row-major [64][64] in global memory)
-template <typename T>
+template <typename T, int SP = SP64>
 __device__ __forceinline__ void fill_matrix(T* __restrict__ A, const T* __restrict__ M, bool transpose) {
-  for (int idx = threadIdx.x; idx < SP64 * SP64; idx += GEN_THREADS) {
+  for (int idx = threadIdx.x; idx < SP * SP; idx += GEN_THREADS) {
     const T v = M[idx];
-    const int r = idx >> 6, col = idx & 63;
-    if (transpose) A[col * SP64 + r] = v; else A[idx] = v;
+    const int r = idx / SP, col = idx % SP;
+    if (transpose) A[col * SP + r] = v; else A[idx] = v;
   }
 }
 
 // tile[pp][x] for patterns p0..p0+31 of one operand; rows beyond P are zero
-template <typename T>
+template <typename T, int SP = SP64>
 __device__ __forceinline__ void load_tile(T* __restrict__ tile, int kind, const void* ptr, int c, int p0, int P, int S) {
-  constexpr int VEC = Gen<T>::VEC, TS = Gen<T>::TS, CPR = SP64 / VEC;  // chunks per row
+  constexpr int VEC = Gen<T, SP>::VEC, TS = Gen<T, SP>::TS, CPR = SP / VEC;  // chunks per row
   using V = typename VecOf<T>::type;
   if (kind == KIND_NONE) {
     for (int idx = threadIdx.x; idx < GEN_TP * TS; idx += GEN_THREADS) tile[idx] = T(0);
   } else if (kind == KIND_STATES) {
     const uint8_t* st = static_cast<const uint8_t*>(ptr);
-    for (int idx = threadIdx.x; idx < GEN_TP * SP64; idx += GEN_THREADS) {
-      const int row = idx >> 6, x = idx & 63;
+    for (int idx = threadIdx.x; idx < GEN_TP * SP; idx += GEN_THREADS) {
+      const int row = idx / SP, x = idx % SP;
       T v = T(0);
       if (p0 + row < P) {
         const int z = st[p0 + row];
@@ -77,12 +81,12 @@ __device__ __forceinline__ void load_tile(T* __restrict__ tile, int kind, const 
       tile[row * TS + x] = v;
     }
   } else {
-    const T* base = static_cast<const T*>(ptr) + (kind == KIND_BCAST ? (size_t)0 : (size_t)c * P * SP64);
+    const T* base = static_cast<const T*>(ptr) + (kind == KIND_BCAST ? (size_t)0 : (size_t)c * P * SP);
     for (int idx = threadIdx.x; idx < GEN_TP * CPR; idx += GEN_THREADS) {
       const int row = idx / CPR, ch = idx % CPR;
       T tmp[VEC];
       if (p0 + row < P) {
-        unpack(*reinterpret_cast<const V*>(base + (size_t)(p0 + row) * SP64 + ch * VEC), tmp);
+        unpack(*reinterpret_cast<const V*>(base + (size_t)(p0 + row) * SP + ch * VEC), tmp);
       } else {
 #pragma unroll
         for (int j = 0; j < VEC; ++j) tmp[j] = T(0);
@@ -104,19 +108,19 @@ __device__ __forceinline__ int pending_exp(const void* mx, int p, int P, int C) 
 }
 
 // acc[i*VEC+j] = sum_x A[x][state_of(sb,i,j)] * vrow[x]
-template <typename T>
-__device__ __forceinline__ void mv64(const T* __restrict__ A, const T* __restrict__ vrow, int sb, T acc[8]) {
-  constexpr int VEC = Gen<T>::VEC, NCH = Gen<T>::NCH;
+template <typename T, int SP = SP64>
+__device__ __forceinline__ void mv64(const T* __restrict__ A, const T* __restrict__ vrow, int sb, T (&acc)[Gen<T, SP>::NPT]) {
+  constexpr int VEC = Gen<T, SP>::VEC, NCH = Gen<T, SP>::NCH;
   using V = typename VecOf<T>::type;
 #pragma unroll
-  for (int k = 0; k < 8; ++k) acc[k] = T(0);
+  for (int k = 0; k < Gen<T, SP>::NPT; ++k) acc[k] = T(0);
 #pragma unroll 4
-  for (int x = 0; x < SP64; ++x) {
+  for (int x = 0; x < SP; ++x) {
     const T v = vrow[x];
 #pragma unroll
     for (int i = 0; i < NCH; ++i) {
       T a[VEC];
-      unpack(*reinterpret_cast<const V*>(A + x * SP64 + (VEC * 8) * i + VEC * sb), a);
+      unpack(*reinterpret_cast<const V*>(A + x * SP + (VEC * 8) * i + VEC * sb), a);
 #pragma unroll
       for (int j = 0; j < VEC; ++j) acc[i * VEC + j] = fma(a[j], v, acc[i * VEC + j]);
     }
@@ -124,22 +128,22 @@ __device__ __forceinline__ void mv64(const T* __restrict__ A, const T* __restric
 }
 
 // acc = column z of the matrix (row z of A[x][s]); a missing state gives `missing` for real states, 0 for padding
-template <typename T>
-__device__ __forceinline__ void gather64(const T* __restrict__ A, int z, int S, T missing, int sb, T acc[8]) {
-  constexpr int VEC = Gen<T>::VEC, NCH = Gen<T>::NCH;
+template <typename T, int SP = SP64>
+__device__ __forceinline__ void gather64(const T* __restrict__ A, int z, int S, T missing, int sb, T (&acc)[Gen<T, SP>::NPT]) {
+  constexpr int VEC = Gen<T, SP>::VEC, NCH = Gen<T, SP>::NCH;
 #pragma unroll
   for (int i = 0; i < NCH; ++i)
 #pragma unroll
     for (int j = 0; j < VEC; ++j) {
       const int s = state_of<T>(sb, i, j);
-      acc[i * VEC + j] = z < S ? A[z * SP64 + s] : (s < S ? missing : T(0));
+      acc[i * VEC + j] = z < S ? A[z * SP + s] : (s < S ? missing : T(0));
     }
 }
 
-// store 8 owned states of pattern p to dst[p][.] (row stride SP64)
-template <typename T>
-__device__ __forceinline__ void store_states(T* __restrict__ dst_row, int sb, const T acc[8]) {
-  constexpr int VEC = Gen<T>::VEC, NCH = Gen<T>::NCH;
+// store the owned states of pattern p to dst[p][.] (row stride SP)
+template <typename T, int SP = SP64>
+__device__ __forceinline__ void store_states(T* __restrict__ dst_row, int sb, const T (&acc)[Gen<T, SP>::NPT]) {
+  constexpr int VEC = Gen<T, SP>::VEC, NCH = Gen<T, SP>::NCH;
   using V = typename VecOf<T>::type;
 #pragma unroll
   for (int i = 0; i < NCH; ++i)
@@ -161,30 +165,30 @@ __device__ __forceinline__ T lane8_sum(T v) {
   return v;
 }
 
-template <typename T>
+template <typename T, int SP = SP64>
 constexpr size_t post64_smem() {
-  return (2 * SP64 * SP64 + 2 * GEN_TP * Gen<T>::TS) * sizeof(T) + 2 * GEN_TP * sizeof(int);
+  return (2 * SP * SP + 2 * GEN_TP * Gen<T, SP>::TS) * sizeof(T) + 2 * GEN_TP * sizeof(int);
 }
-template <typename T>
+template <typename T, int SP = SP64>
 constexpr size_t pre64_smem() {
-  return (3 * SP64 * SP64 + 5 * GEN_TP * Gen<T>::TS) * sizeof(T) + 3 * GEN_TP * sizeof(int) +
+  return (3 * SP * SP + 5 * GEN_TP * Gen<T, SP>::TS) * sizeof(T) + 3 * GEN_TP * sizeof(int) +
          4 * GEN_TP * sizeof(double);
 }
-template <typename T>
+template <typename T, int SP = SP64>
 constexpr size_t deriv64_smem() {
-  return (SP64 * SP64 + 2 * GEN_TP * Gen<T>::TS) * sizeof(T) + 2 * GEN_TP * sizeof(double);
+  return (SP * SP + 2 * GEN_TP * Gen<T, SP>::TS) * sizeof(T) + 2 * GEN_TP * sizeof(double);
 }
 
 // ---------------------------------------------------------------------------------------------------------------
 // post-order update, one (tile, category, operation) per block (maxima for step 3)
 // ---------------------------------------------------------------------------------------------------------------
-template <typename T>
+template <typename T, int SP = SP64>
 __global__ void __launch_bounds__(GEN_THREADS) k_post64(const DevOp* __restrict__ ops, int P, int S, int C) {
-  constexpr int TS = Gen<T>::TS;
+  constexpr int TS = Gen<T, SP>::TS;
   extern __shared__ __align__(16) unsigned char smem_raw[];
   T* A0 = reinterpret_cast<T*>(smem_raw);
-  T* A1 = A0 + SP64 * SP64;
-  T* V0 = A1 + SP64 * SP64;
+  T* A1 = A0 + SP * SP;
+  T* V0 = A1 + SP * SP;
   T* V1 = V0 + GEN_TP * TS;
   int* sE = reinterpret_cast<int*>(V1 + GEN_TP * TS);
 
@@ -192,39 +196,39 @@ __global__ void __launch_bounds__(GEN_THREADS) k_post64(const DevOp* __restrict_
   const int c = blockIdx.y, p0 = blockIdx.x * GEN_TP;
   const int pp = threadIdx.x >> 3, sb = threadIdx.x & 7, p = p0 + pp;
 
-  fill_matrix<T>(A0, static_cast<const T*>(op.mat[0]) + (size_t)c * SP64 * SP64, true);
-  fill_matrix<T>(A1, static_cast<const T*>(op.mat[1]) + (size_t)c * SP64 * SP64, true);
-  if (op.kind[0] != KIND_STATES) load_tile<T>(V0, op.kind[0], op.child[0], c, p0, P, S);
-  if (op.kind[1] != KIND_STATES) load_tile<T>(V1, op.kind[1], op.child[1], c, p0, P, S);
+  fill_matrix<T, SP>(A0, static_cast<const T*>(op.mat[0]) + (size_t)c * SP * SP, true);
+  fill_matrix<T, SP>(A1, static_cast<const T*>(op.mat[1]) + (size_t)c * SP * SP, true);
+  if (op.kind[0] != KIND_STATES) load_tile<T, SP>(V0, op.kind[0], op.child[0], c, p0, P, S);
+  if (op.kind[1] != KIND_STATES) load_tile<T, SP>(V1, op.kind[1], op.child[1], c, p0, P, S);
   if (threadIdx.x < 2 * GEN_TP) {
     const int k = threadIdx.x / GEN_TP, r = threadIdx.x % GEN_TP;
     sE[threadIdx.x] = pending_exp<T>(op.cscale[k], p0 + r, P, C);
   }
   __syncthreads();
 
-  T a[8], b[8];
+  T a[Gen<T, SP>::NPT], b[Gen<T, SP>::NPT];
   if (op.kind[0] == KIND_STATES) {
     const int z = p < P ? static_cast<const uint8_t*>(op.child[0])[p] : 0;
-    gather64<T>(A0, z, S, T(1), sb, a);
+    gather64<T, SP>(A0, z, S, T(1), sb, a);
   } else {
-    mv64<T>(A0, V0 + pp * TS, sb, a);
+    mv64<T, SP>(A0, V0 + pp * TS, sb, a);
   }
   if (op.kind[1] == KIND_STATES) {
     const int z = p < P ? static_cast<const uint8_t*>(op.child[1])[p] : 0;
-    gather64<T>(A1, z, S, T(1), sb, b);
+    gather64<T, SP>(A1, z, S, T(1), sb, b);
   } else {
-    mv64<T>(A1, V1 + pp * TS, sb, b);
+    mv64<T, SP>(A1, V1 + pp * TS, sb, b);
   }
   const Pow2Pair<T> f0 = pow2_pair(-sE[pp], T(0)), f1 = pow2_pair(-sE[GEN_TP + pp], T(0));
   T mx = T(0);
 #pragma unroll
-  for (int k = 0; k < 8; ++k) {
+  for (int k = 0; k < Gen<T, SP>::NPT; ++k) {
     a[k] = ((a[k] * f0.f1) * f0.f2) * ((b[k] * f1.f1) * f1.f2);
     mx = fmax(mx, a[k]);
   }
   mx = lane8_max(mx);
   if (p < P) {
-    store_states<T>(static_cast<T*>(op.dest) + ((size_t)c * P + p) * SP64, sb, a);
+    store_states<T, SP>(static_cast<T*>(op.dest) + ((size_t)c * P + p) * SP, sb, a);
     if (sb == 0 && op.scale != nullptr) static_cast<T*>(op.scale)[(size_t)c * P + p] = mx;
   }
 }
@@ -233,19 +237,19 @@ __global__ void __launch_bounds__(GEN_THREADS) k_post64(const DevOp* __restrict_
 // pre-order update of both children of one parent + both branch derivatives
 // one (tile, item) per block, categories looped inside so that num_p and den_p are summed over c in the block
 // ---------------------------------------------------------------------------------------------------------------
-template <typename T>
+template <typename T, int SP = SP64>
 __global__ void __launch_bounds__(GEN_THREADS) k_pre64(const DevPreItem* __restrict__ items, int P, int S, int C,
                                                        const T* __restrict__ Qg, const double* __restrict__ catw,
                                                        const double* __restrict__ catr,
                                                        const double* __restrict__ weights,
                                                        double* __restrict__ grad_partial, int n_tiles,
                                                        double* __restrict__ site_out) {
-  constexpr int TS = Gen<T>::TS;
+  constexpr int TS = Gen<T, SP>::TS;
   extern __shared__ __align__(16) unsigned char smem_raw[];
   T* B0 = reinterpret_cast<T*>(smem_raw);
-  T* B1 = B0 + SP64 * SP64;
-  T* BQ = B1 + SP64 * SP64;
-  T* tQM = BQ + SP64 * SP64;
+  T* B1 = B0 + SP * SP;
+  T* BQ = B1 + SP * SP;
+  T* tQM = BQ + SP * SP;
   T* tX[2] = {tQM + GEN_TP * TS, tQM + 2 * GEN_TP * TS};
   T* tU[2] = {tQM + 3 * GEN_TP * TS, tQM + 4 * GEN_TP * TS};
   int* sE = reinterpret_cast<int*>(tQM + 5 * GEN_TP * TS);              // [3][32]: child0, child1, parent q
@@ -258,7 +262,7 @@ __global__ void __launch_bounds__(GEN_THREADS) k_pre64(const DevPreItem* __restr
   const bool want_grad = it.slot[0] >= 0 || it.slot[1] >= 0;
   T* B[2] = {B0, B1};
 
-  if (want_grad) fill_matrix<T>(BQ, Qg, true);
+  if (want_grad) fill_matrix<T, SP>(BQ, Qg, true);
   if (threadIdx.x < 3 * GEN_TP) {
     const int k = threadIdx.x / GEN_TP, r = threadIdx.x % GEN_TP;
     sE[threadIdx.x] = pending_exp<T>(k == 2 ? it.qm_scale : it.p_scale[k], p0 + r, P, C);
@@ -272,65 +276,65 @@ __global__ void __launch_bounds__(GEN_THREADS) k_pre64(const DevPreItem* __restr
 
   for (int c = 0; c < C; ++c) {
     __syncthreads();
-    fill_matrix<T>(B0, static_cast<const T*>(it.mat[0]) + (size_t)c * SP64 * SP64, true);
-    fill_matrix<T>(B1, static_cast<const T*>(it.mat[1]) + (size_t)c * SP64 * SP64, true);
-    load_tile<T>(tQM, KIND_PARTIALS, it.qm, c, p0, P, S);
-    load_tile<T>(tX[0], it.kind[0], it.p[0], c, p0, P, S);
-    load_tile<T>(tX[1], it.kind[1], it.p[1], c, p0, P, S);
+    fill_matrix<T, SP>(B0, static_cast<const T*>(it.mat[0]) + (size_t)c * SP * SP, true);
+    fill_matrix<T, SP>(B1, static_cast<const T*>(it.mat[1]) + (size_t)c * SP * SP, true);
+    load_tile<T, SP>(tQM, KIND_PARTIALS, it.qm, c, p0, P, S);
+    load_tile<T, SP>(tX[0], it.kind[0], it.p[0], c, p0, P, S);
+    load_tile<T, SP>(tX[1], it.kind[1], it.p[1], c, p0, P, S);
     __syncthreads();
 
-    T a[2][8], qx[2][8];
+    T a[2][Gen<T, SP>::NPT], qx[2][Gen<T, SP>::NPT];
 #pragma unroll
     for (int k = 0; k < 2; ++k) {
       if (it.kind[k] == KIND_STATES) {
-        gather64<T>(B[k], z[k], S, T(1), sb, a[k]);
-        if (want_grad) gather64<T>(BQ, z[k], S, T(0), sb, qx[k]);
+        gather64<T, SP>(B[k], z[k], S, T(1), sb, a[k]);
+        if (want_grad) gather64<T, SP>(BQ, z[k], S, T(0), sb, qx[k]);
       } else {
-        mv64<T>(B[k], tX[k] + pp * TS, sb, a[k]);
-        if (want_grad) mv64<T>(BQ, tX[k] + pp * TS, sb, qx[k]);
+        mv64<T, SP>(B[k], tX[k] + pp * TS, sb, a[k]);
+        if (want_grad) mv64<T, SP>(BQ, tX[k] + pp * TS, sb, qx[k]);
       }
       const Pow2Pair<T> f = pow2_pair(-sE[k * GEN_TP + pp], T(0));
 #pragma unroll
-      for (int i = 0; i < 8; ++i) a[k][i] = (a[k][i] * f.f1) * f.f2;
+      for (int i = 0; i < Gen<T, SP>::NPT; ++i) a[k][i] = (a[k][i] * f.f1) * f.f2;
     }
     {
       const Pow2Pair<T> f = pow2_pair(-sE[2 * GEN_TP + pp], T(0));
 #pragma unroll
-      for (int i = 0; i < Gen<T>::NCH; ++i)
+      for (int i = 0; i < Gen<T, SP>::NCH; ++i)
 #pragma unroll
-        for (int j = 0; j < Gen<T>::VEC; ++j) {
+        for (int j = 0; j < Gen<T, SP>::VEC; ++j) {
           const int s = state_of<T>(sb, i, j);
           const T qm = (tQM[pp * TS + s] * f.f1) * f.f2;
-          tU[0][pp * TS + s] = qm * a[1][i * Gen<T>::VEC + j];
-          tU[1][pp * TS + s] = qm * a[0][i * Gen<T>::VEC + j];
+          tU[0][pp * TS + s] = qm * a[1][i * Gen<T, SP>::VEC + j];
+          tU[1][pp * TS + s] = qm * a[0][i * Gen<T, SP>::VEC + j];
         }
     }
     __syncthreads();
-    fill_matrix<T>(B0, static_cast<const T*>(it.mat[0]) + (size_t)c * SP64 * SP64, false);
-    fill_matrix<T>(B1, static_cast<const T*>(it.mat[1]) + (size_t)c * SP64 * SP64, false);
+    fill_matrix<T, SP>(B0, static_cast<const T*>(it.mat[0]) + (size_t)c * SP * SP, false);
+    fill_matrix<T, SP>(B1, static_cast<const T*>(it.mat[1]) + (size_t)c * SP * SP, false);
     __syncthreads();
 
 #pragma unroll
     for (int k = 0; k < 2; ++k) {
-      T q[8];
-      mv64<T>(B[k], tU[k] + pp * TS, sb, q);
+      T q[Gen<T, SP>::NPT];
+      mv64<T, SP>(B[k], tU[k] + pp * TS, sb, q);
       T mx = T(0);
 #pragma unroll
-      for (int i = 0; i < 8; ++i) mx = fmax(mx, q[i]);
+      for (int i = 0; i < Gen<T, SP>::NPT; ++i) mx = fmax(mx, q[i]);
       mx = lane8_max(mx);
       if (it.q[k] != nullptr && p < P) {
-        store_states<T>(static_cast<T*>(it.q[k]) + ((size_t)c * P + p) * SP64, sb, q);
+        store_states<T, SP>(static_cast<T*>(it.q[k]) + ((size_t)c * P + p) * SP, sb, q);
         if (sb == 0) static_cast<T*>(it.q_scale[k])[(size_t)c * P + p] = mx;
       }
       if (it.slot[k] >= 0) {
         T n = T(0), d = T(0);
 #pragma unroll
-        for (int i = 0; i < Gen<T>::NCH; ++i)
+        for (int i = 0; i < Gen<T, SP>::NCH; ++i)
 #pragma unroll
-          for (int j = 0; j < Gen<T>::VEC; ++j) {
+          for (int j = 0; j < Gen<T, SP>::VEC; ++j) {
             const int s = state_of<T>(sb, i, j);
-            n = fma(q[i * Gen<T>::VEC + j], qx[k][i * Gen<T>::VEC + j], n);
-            d = fma(q[i * Gen<T>::VEC + j], tX[k][pp * TS + s], d);
+            n = fma(q[i * Gen<T, SP>::VEC + j], qx[k][i * Gen<T, SP>::VEC + j], n);
+            d = fma(q[i * Gen<T, SP>::VEC + j], tX[k][pp * TS + s], d);
           }
         n = lane8_sum(n);
         d = lane8_sum(d);
@@ -359,17 +363,17 @@ __global__ void __launch_bounds__(GEN_THREADS) k_pre64(const DevPreItem* __restr
 // ---------------------------------------------------------------------------------------------------------------
 // unfused branch derivatives from stored pre- and post-order partials
 // ---------------------------------------------------------------------------------------------------------------
-template <typename T>
+template <typename T, int SP = SP64>
 __global__ void __launch_bounds__(GEN_THREADS) k_deriv64(const DevBranch* __restrict__ br, int P, int S, int C,
                                                          const T* __restrict__ Qg, const double* __restrict__ catw,
                                                          const double* __restrict__ catr,
                                                          const double* __restrict__ weights,
                                                          double* __restrict__ grad_partial, int n_tiles,
                                                          double* __restrict__ site_out) {
-  constexpr int TS = Gen<T>::TS;
+  constexpr int TS = Gen<T, SP>::TS;
   extern __shared__ __align__(16) unsigned char smem_raw[];
   T* BQ = reinterpret_cast<T*>(smem_raw);
-  T* tQ = BQ + SP64 * SP64;
+  T* tQ = BQ + SP * SP;
   T* tX = tQ + GEN_TP * TS;
   double* sNum = reinterpret_cast<double*>(tX + GEN_TP * TS);
   double* sDen = sNum + GEN_TP;
@@ -377,22 +381,22 @@ __global__ void __launch_bounds__(GEN_THREADS) k_deriv64(const DevBranch* __rest
   const DevBranch b = br[blockIdx.y];
   const int p0 = blockIdx.x * GEN_TP;
   const int pp = threadIdx.x >> 3, sb = threadIdx.x & 7;
-  fill_matrix<T>(BQ, Qg, true);
+  fill_matrix<T, SP>(BQ, Qg, true);
   if (threadIdx.x < 2 * GEN_TP) sNum[threadIdx.x] = 0.0;
   for (int c = 0; c < C; ++c) {
     __syncthreads();
-    load_tile<T>(tQ, KIND_PARTIALS, b.q, c, p0, P, S);
-    load_tile<T>(tX, b.kind, b.p, c, p0, P, S);
+    load_tile<T, SP>(tQ, KIND_PARTIALS, b.q, c, p0, P, S);
+    load_tile<T, SP>(tX, b.kind, b.p, c, p0, P, S);
     __syncthreads();
-    T qx[8];
-    mv64<T>(BQ, tX + pp * TS, sb, qx);
+    T qx[Gen<T, SP>::NPT];
+    mv64<T, SP>(BQ, tX + pp * TS, sb, qx);
     T n = T(0), d = T(0);
 #pragma unroll
-    for (int i = 0; i < Gen<T>::NCH; ++i)
+    for (int i = 0; i < Gen<T, SP>::NCH; ++i)
 #pragma unroll
-      for (int j = 0; j < Gen<T>::VEC; ++j) {
+      for (int j = 0; j < Gen<T, SP>::VEC; ++j) {
         const int s = state_of<T>(sb, i, j);
-        n = fma(tQ[pp * TS + s], qx[i * Gen<T>::VEC + j], n);
+        n = fma(tQ[pp * TS + s], qx[i * Gen<T, SP>::VEC + j], n);
         d = fma(tQ[pp * TS + s], tX[pp * TS + s], d);
       }
     n = lane8_sum(n);

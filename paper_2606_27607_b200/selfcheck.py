@@ -43,6 +43,7 @@ def run(quick=False):
     cases = []
     wl4 = workloads.config(1, n_tips=12, n_patterns=n_nuc)
     wl61 = workloads.config(2, n_tips=8, n_patterns=n_cod)
+    wl20 = workloads.config(5, n_tips=8, n_patterns=n_cod)
     mixed = np.arange(wl4.tree.n_tips) % 3 == 0  # every third tip as partials, the others compact
     for prec, pname in ((plk.FP64, "fp64"), (plk.FP32, "fp32")):
         for name, flags in NUC_ARMS:
@@ -54,6 +55,9 @@ def run(quick=False):
             cases.append((f"codon-{pname}-{name}", wl61, prec, flags, False, False))
         cases.append((f"codon-{pname}-tensor-tip-partials", wl61, prec, plk.FLAG_TENSOR_CORES, True, False))
         cases.append((f"codon-{pname}-unfused", wl61, prec, 0, False, True))
+        cases.append((f"amino-{pname}", wl20, prec, 0, False, False))
+        cases.append((f"amino-{pname}-tip-partials", wl20, prec, 0, True, False))
+        cases.append((f"amino-{pname}-unfused", wl20, prec, 0, False, True))
     base = {}
     worst = 0.0
     total = 0
