@@ -12,7 +12,7 @@ Rules (task statement, section 3):
   * it shares no code with paper_2606_27607_b200/ (the CUDA path) and neither imports the other;
   * no expected value stored anywhere comes from the CUDA path.
 
-Pins: every function in models.py / likelihood.py / encode.py is pinned; the
+Pins: every function in models.py / likelihood.py / caching.py / encode.py is pinned; the
 fp32 / tensor-core GPU modes have no pin of their own -- they are compared with this fp64 oracle at 1e-4.
 """
-from . import encode, likelihood, models  # noqa: F401
+from . import caching, encode, likelihood, models  # noqa: F401
