@@ -224,6 +224,28 @@ PLK_API int plk_pre_order_gradient_device(plk_instance* inst, int eigen, int roo
                                           const plk_pre_op* ops, int count, double* d_out_gradient,
                                           double* d_out_site);
 
+/* S8a steps 1-6 in ONE call (the unit of work of an HMC step): transition matrices for the `matrix_count` listed
+ * branches, post-order partials for `ops`, the root log-likelihood over `scale_idx`, and the fused pre-order + derivative
+ * pass for `pre_ops` -- exactly plk_update_transition_matrices_device + plk_update_partials +
+ * plk_root_log_likelihoods_device + plk_pre_order_gradient_device with the same arguments, same kernels, same results.
+ * d_out: DEVICE fp64 [1 + pre_count] = [logL, derivative of the branch above pre_ops[0]'s node, ...].  Small problems
+ * are bound by launch latency, so the library caches the whole launch sequence of a call signature (all index arrays,
+ * the two device pointers, the model and the slot bindings) as a CUDA graph: the first use of a signature runs eagerly,
+ * the second is captured, every later one is a single graph launch.  Capture needs a non-default stream (a stream
+ * created by the caller, e.g. torch.cuda.Stream); on the legacy default stream every use runs eagerly.  At most 8
+ * signatures are cached per instance (then all are dropped).  Never synchronises, no value check. */
+PLK_API int plk_evaluate_device(plk_instance* inst, int eigen, const int32_t* matrix_idx, const double* d_branch_lengths,
+                                int matrix_count, const plk_op* ops, int op_count, int root_buffer,
+                                const int32_t* scale_idx, int scale_count, int root_pre_buffer, const plk_pre_op* pre_ops,
+                                int pre_count, double* d_out);
+/* The same with HOST branch lengths [matrix_count] (each finite and >= 0 else _OUT_OF_RANGE) and HOST results:
+ * out_logl [1], out_gradient [pre_count].  One upload, one graph launch, one download, one synchronisation.
+ * _FLOATING_POINT (outputs still written) if a value is not finite. */
+PLK_API int plk_evaluate(plk_instance* inst, int eigen, const int32_t* matrix_idx, const double* branch_lengths,
+                         int matrix_count, const plk_op* ops, int op_count, int root_buffer, const int32_t* scale_idx,
+                         int scale_count, int root_pre_buffer, const plk_pre_op* pre_ops, int pre_count, double* out_logl,
+                         double* out_gradient);
+
 /* S8f-1 / P:29.  Approximate gradient of logL with respect to every element of the rate matrix: the gradient
  * "w.r.t. elements of the rate matrix" evaluated with "a first-order approximation of the derivative of the matrix
  * exponential", d exp(Q tau) / d Q_ij ~= tau exp(Q tau) E_ij, which reduces the sandwich of branch b to an outer product

@@ -168,5 +168,20 @@ class Evaluator:
         self.step_root()
         self.step_pre_gradient()
 
+    def step_evaluate(self):
+        """The same evaluation as step_device() through plk_evaluate_device: ONE library call, replayed from a cached
+        CUDA graph from its third use (needs a non-default stream; otherwise it runs eagerly)."""
+        self.inst.evaluate_device(0, self.matrix_idx, self.d_t, self.ops, self.tree.root, self.scale_idx, self.tree.root,
+                                  self.pre_ops, self.d_out)
+
+    def evaluate(self, branch_lengths: Optional[np.ndarray] = None):
+        """(logL, gradient per node) through plk_evaluate: host branch lengths in, host results out."""
+        t = self.tree.branch_length if branch_lengths is None else branch_lengths
+        logl, g = self.inst.evaluate(0, self.matrix_idx, np.asarray(t)[self.matrix_idx], self.ops, self.tree.root,
+                                     self.scale_idx, self.tree.root, self.pre_ops)
+        grad = np.zeros(self.tree.n_nodes)
+        grad[self.branch_nodes] = g
+        return logl, grad
+
     def close(self):
         self.inst.destroy()

@@ -29,6 +29,8 @@ namespace {
 
 constexpr size_t ALIGN = 1024;
 constexpr size_t RING_BYTES = 8u << 20;  // parameter staging ring (pinned host + device mirror)
+constexpr size_t PLAN_BYTES = 4u << 20;  // descriptor blocks of the cached evaluation graphs (plk_evaluate*)
+constexpr int PLAN_MAX = 8;              // cached evaluation graphs per instance
 inline size_t round_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 constexpr int NUC_MAX_WALK_WARPS = 16384;  // walk-shape grid cap (256 SMs x 64 warps); sizes the partial-sum rows
 inline int nuc_lanes_per_pattern(int C) { return C % 4 == 0 ? 4 : (C % 2 == 0 ? 2 : 1); }  // NucMap<C>::LP
@@ -43,7 +45,7 @@ struct Layout {
   int n_tiles, max_grad;
   size_t off_post, off_compact, off_pre, off_pre_mx, off_matrix, off_eigen, off_scale, off_weights, off_pi,
       off_rates, off_catw, off_site, off_block_partial, off_grad_partial, off_grad_out, off_logl, off_site_deriv,
-      off_stage, off_ring, off_matrix_t, off_matrix_d, off_matrix_dt, off_cat_scratch, off_cross_partial, off_cross_out, total;
+      off_stage, off_ring, off_plan, off_eval_t, off_eval_out, off_matrix_t, off_matrix_d, off_matrix_dt, off_cat_scratch, off_cross_partial, off_cross_out, total;
   size_t stage_bytes;
 };
 
@@ -107,6 +109,9 @@ bool compute_layout(const plk_config& c, Layout& L) {
   L.stage_bytes = round_up((size_t)L.C * L.P * L.S * 8, ALIGN);
   L.off_stage = take(L.stage_bytes);
   L.off_ring = take(RING_BYTES);
+  L.off_plan = take(PLAN_BYTES);
+  L.off_eval_t = take((size_t)c.matrix_buffer_count * 8);        // plk_evaluate: branch lengths, [logL, gradient]
+  L.off_eval_out = take((size_t)(1 + c.partials_buffer_count) * 8);
   // fp32 tensor-core instances (tcgen05 pre-order kernels, plk_tc5_pre*.cuh): per matrix buffer M^T, D = M Q and D^T,
   // and the per-category num / den scratch of the class-specialised kernels ([slot][num, den][C][P] floats)
   const bool tc5 = L.SP == 64 && c.precision == PLK_FP32 && (c.flags & PLK_FLAG_TENSOR_CORES) && !(c.flags & PLK_FLAG_NO_TCGEN05);
@@ -152,6 +157,20 @@ struct plk_instance {
   int nt_bps[2][2] = {{0, 0}, {0, 0}};  // resident CTAs per SM of the TMA kernels [post|pre][level|walk]
   int lean_bps[3] = {0, 0, 0};          // the same for k_pre4_lean<T, CLS> (T is fixed per instance)
   int grad_parts = 0;  // partial sums per gradient slot written by the LAST gradient launch (row stride L.n_tiles)
+  // cached evaluation graphs (plk_evaluate*): one per distinct call signature
+  struct EvalPlan {
+    uint64_t key = 0;
+    int uses = 0;              // the first use runs eagerly (it also binds slots and sets kernel attributes)
+    bool failed = false;       // capture was refused once (e.g. legacy default stream): stay eager
+    cudaGraphExec_t exec = nullptr;
+    int64_t launches = 0;      // kernels in the graph
+  };
+  std::vector<EvalPlan> plans;
+  std::vector<char> plan_host;  // host image of the plan region (descriptors of the captured launches)
+  size_t plan_pos = 0;          // bump pointer inside the plan region
+  bool planning = false;        // ring_alloc serves from the plan region, copy_ring is deferred
+  uint64_t model_epoch = 0;     // bumped by every setter whose value is baked into launch parameters
+  uint64_t binding_epoch = 0;   // bumped when a buffer index is bound to a slot or changes kind
 
   template <typename X> X* at(size_t off) const { return reinterpret_cast<X*>(arena + off); }
   void* post_ptr(int idx) const {
@@ -188,6 +207,13 @@ namespace {
 // earlier asynchronous copies have left the pinned buffer.
 int ring_alloc(plk_instance* in, size_t bytes, char** h, char** d) {
   bytes = round_up(bytes, 256);
+  if (in->planning) {  // graph capture: descriptors live in the plan region for as long as the graph does
+    if (in->plan_pos + bytes > PLAN_BYTES) return PLK_ERR_OUT_OF_MEMORY;
+    *h = in->plan_host.data() + in->plan_pos;
+    *d = in->arena + in->L.off_plan + in->plan_pos;
+    in->plan_pos += bytes;
+    return PLK_SUCCESS;
+  }
   if (bytes > RING_BYTES) return PLK_ERR_OUT_OF_MEMORY;
   if (in->ring_pos + bytes > RING_BYTES) {
     CU(cudaStreamSynchronize(in->stream));
@@ -199,24 +225,28 @@ int ring_alloc(plk_instance* in, size_t bytes, char** h, char** d) {
   return PLK_SUCCESS;
 }
 int copy_ring(plk_instance* in, const char* h, char* d, size_t bytes) {
+  if (in->planning) return PLK_SUCCESS;  // uploaded in one piece after the capture (plk_evaluate_device)
   CU(cudaMemcpyAsync(d, h, bytes, cudaMemcpyHostToDevice, in->stream));
   return PLK_SUCCESS;
 }
 
 int bind_post_full(plk_instance* in, int idx, int kind) {
   if (in->post_slot[idx] >= 0 && in->post_kind[idx] != KIND_STATES) {
+    if (in->post_kind[idx] != kind) ++in->binding_epoch;
     in->post_kind[idx] = kind;
     return PLK_SUCCESS;
   }
   if (in->next_post_slot >= in->L.post_slots) return PLK_ERR_OUT_OF_MEMORY;
   in->post_slot[idx] = in->next_post_slot++;
   in->post_kind[idx] = kind;
+  ++in->binding_epoch;
   return PLK_SUCCESS;
 }
 int bind_pre(plk_instance* in, int idx) {
   if (in->pre_slot[idx] >= 0) return PLK_SUCCESS;
   if (in->next_pre_slot >= in->L.pre_slots) return PLK_ERR_OUT_OF_MEMORY;
   in->pre_slot[idx] = in->next_pre_slot++;
+  ++in->binding_epoch;
   return PLK_SUCCESS;
 }
 
@@ -767,6 +797,8 @@ int plk_create(const plk_config* cfg, void* d_arena, size_t arena_bytes, void* c
 int plk_destroy(plk_instance* in) {
   if (in == nullptr) return PLK_SUCCESS;
   cudaStreamSynchronize(in->stream);
+  for (auto& pl : in->plans)
+    if (pl.exec != nullptr) cudaGraphExecDestroy(pl.exec);
   if (in->h_ring) cudaFreeHost(in->h_ring);
   delete in;
   return PLK_SUCCESS;
@@ -798,6 +830,7 @@ int plk_set_tip_states(plk_instance* in, int tip, const int32_t* states) {
     if (in->next_compact_slot >= L.compact_slots) return PLK_ERR_OUT_OF_MEMORY;
     in->post_slot[tip] = in->next_compact_slot++;
     in->post_kind[tip] = KIND_STATES;
+    ++in->binding_epoch;
   }
   if ((size_t)L.P * 4 > L.stage_bytes) return PLK_ERR_OUT_OF_MEMORY;
   int32_t* stage = in->at<int32_t>(L.off_stage);
@@ -819,6 +852,7 @@ int plk_set_tip_states_u8(plk_instance* in, int tip, const uint8_t* states) {
     if (in->next_compact_slot >= L.compact_slots) return PLK_ERR_OUT_OF_MEMORY;
     in->post_slot[tip] = in->next_compact_slot++;
     in->post_kind[tip] = KIND_STATES;
+    ++in->binding_epoch;
   }
   CU(cudaMemcpyAsync(in->post_ptr(tip), states, (size_t)L.P, cudaMemcpyHostToDevice, in->stream));
   in->post_written[tip] = 1;
@@ -939,6 +973,7 @@ int plk_set_eigen_decomposition(plk_instance* in, int eigen, const double* U, co
   if (rc) return rc;
   in->eigen_written[eigen] = 1;
   in->q_written[eigen] = 1;
+  ++in->model_epoch;
   return PLK_SUCCESS;
 }
 
@@ -960,6 +995,7 @@ int plk_set_rate_matrix(plk_instance* in, int eigen, const double* Q) {
   int rc = fetch_q4(in, eigen);
   if (rc) return rc;
   in->q_written[eigen] = 1;
+  ++in->model_epoch;
   return PLK_SUCCESS;
 }
 
@@ -1596,6 +1632,168 @@ int plk_branch_derivatives(plk_instance* in, int eigen, const int32_t* post_idx,
                                             in->at<double>(L.off_grad_out));
   CHECK_LAUNCH(in);
   return finish_gradient(in, count, out_gradient, out_site, d_site);
+}
+
+// ---- steps 1-6 in one call, replayed from a cached CUDA graph ---------------------------------------------------------
+// Small problems (configs[0], the low end of configs[4]) are bound by launch latency, not by the GPU: an evaluation is
+// 10-20 dependent launches plus their descriptor uploads (SURVEY section 7 hard part 7).  plk_evaluate_device runs the
+// four steps through the very same code as the separate calls, but from its third use with an unchanged signature it
+// replays them as ONE cudaGraphLaunch: the first use runs eagerly (it binds slots and sets kernel attributes), the
+// second use is run once more under stream capture with the launch descriptors placed in a region of the arena that
+// belongs to the graph (uploaded once, after the capture), and every later use is the instantiated graph.
+
+namespace {
+
+uint64_t fnv1a(uint64_t h, const void* data, size_t bytes) {
+  const unsigned char* p = static_cast<const unsigned char*>(data);
+  for (size_t i = 0; i < bytes; ++i) h = (h ^ p[i]) * 1099511628211ull;
+  return h;
+}
+
+struct EvalArgs {
+  int eigen;
+  const int32_t* matrix_idx;
+  const double* d_t;
+  int matrix_count;
+  const plk_op* ops;
+  int op_count;
+  int root;
+  const int32_t* scale_idx;
+  int scale_count;
+  int root_pre;
+  const plk_pre_op* pre_ops;
+  int pre_count;
+  double* d_out;
+};
+
+int evaluate_steps(plk_instance* in, const EvalArgs& a) {
+  int rc = update_matrices_impl(in, a.eigen, a.matrix_idx, nullptr, a.d_t, a.matrix_count);
+  if (rc) return rc;
+  rc = plk_update_partials(in, a.ops, a.op_count);
+  if (rc) return rc;
+  rc = root_impl(in, a.root, a.scale_idx, a.scale_count, a.d_out, nullptr);
+  if (rc) return rc;
+  return pre_impl(in, a.eigen, a.root_pre, a.pre_ops, a.pre_count, true, a.d_out + 1, nullptr);
+}
+
+void drop_plans(plk_instance* in) {
+  cudaStreamSynchronize(in->stream);  // a graph still in flight reads its descriptor block
+  for (auto& pl : in->plans)
+    if (pl.exec != nullptr) cudaGraphExecDestroy(pl.exec);
+  in->plans.clear();
+  in->plan_pos = 0;
+}
+
+int evaluate_impl(plk_instance* in, const EvalArgs& a) {
+  if (a.matrix_count < 0 || a.op_count < 0 || a.scale_count < 0 || a.pre_count < 0) return PLK_ERR_OUT_OF_RANGE;
+  if ((a.matrix_count > 0 && (a.matrix_idx == nullptr || a.d_t == nullptr)) || (a.op_count > 0 && a.ops == nullptr) ||
+      (a.scale_count > 0 && a.scale_idx == nullptr) || (a.pre_count > 0 && a.pre_ops == nullptr) || a.d_out == nullptr)
+    return PLK_ERR_OUT_OF_RANGE;
+  uint64_t key = 1469598103934665603ull;
+  const int head[8] = {a.eigen, a.matrix_count, a.op_count, a.root, a.scale_count, a.root_pre, a.pre_count,
+                       in->root_pre_filled == a.root_pre ? 1 : 0};
+  key = fnv1a(key, head, sizeof(head));
+  key = fnv1a(key, a.matrix_idx, (size_t)a.matrix_count * 4);
+  key = fnv1a(key, a.ops, (size_t)a.op_count * sizeof(plk_op));
+  key = fnv1a(key, a.scale_idx, (size_t)a.scale_count * 4);
+  key = fnv1a(key, a.pre_ops, (size_t)a.pre_count * sizeof(plk_pre_op));
+  const uint64_t tail[4] = {(uint64_t)(uintptr_t)a.d_t, (uint64_t)(uintptr_t)a.d_out, in->model_epoch, in->binding_epoch};
+  key = fnv1a(key, tail, sizeof(tail));
+  plk_instance::EvalPlan* pl = nullptr;
+  for (auto& q : in->plans)
+    if (q.key == key) pl = &q;
+  if (pl != nullptr && pl->exec != nullptr) {  // replay
+    CU(cudaGraphLaunch(pl->exec, in->stream));
+    in->launches += pl->launches;
+    ++pl->uses;
+    return PLK_SUCCESS;
+  }
+  if (pl == nullptr) {  // first use: eager
+    if ((int)in->plans.size() >= PLAN_MAX) drop_plans(in);
+    in->plans.emplace_back();
+    in->plans.back().key = key;
+    in->plans.back().uses = 1;
+    return evaluate_steps(in, a);
+  }
+  ++pl->uses;
+  if (pl->failed) return evaluate_steps(in, a);
+  // second use: the same steps under stream capture, descriptors in the plan region
+  if (in->plan_host.empty()) in->plan_host.assign(PLAN_BYTES, 0);
+  const size_t plan_from = in->plan_pos;
+  const int64_t launches_before = in->launches;
+  if (cudaStreamBeginCapture(in->stream, cudaStreamCaptureModeRelaxed) != cudaSuccess) {
+    cudaGetLastError();  // e.g. the legacy default stream cannot be captured
+    pl->failed = true;
+    return evaluate_steps(in, a);
+  }
+  in->planning = true;
+  const int rc = evaluate_steps(in, a);
+  in->planning = false;
+  cudaGraph_t graph = nullptr;
+  const cudaError_t ce = cudaStreamEndCapture(in->stream, &graph);
+  const int64_t captured = in->launches - launches_before;
+  in->launches = launches_before;
+  cudaGraphExec_t exec = nullptr;
+  if (rc == PLK_SUCCESS && ce == cudaSuccess && graph != nullptr &&
+      cudaGraphInstantiate(&exec, graph, 0) == cudaSuccess) {
+    cudaGraphDestroy(graph);
+    // the descriptor block, once; stream order puts it before the first replay
+    if (in->plan_pos > plan_from)
+      CU(cudaMemcpyAsync(in->arena + in->L.off_plan + plan_from, in->plan_host.data() + plan_from, in->plan_pos - plan_from,
+                         cudaMemcpyHostToDevice, in->stream));
+    pl->exec = exec;
+    pl->launches = captured;
+    CU(cudaGraphLaunch(exec, in->stream));
+    in->launches += captured;
+    return PLK_SUCCESS;
+  }
+  if (graph != nullptr) cudaGraphDestroy(graph);
+  cudaGetLastError();
+  in->plan_pos = plan_from;
+  pl->failed = true;
+  if (rc != PLK_SUCCESS && rc != PLK_ERR_OUT_OF_MEMORY) return rc;  // a genuine argument error
+  return evaluate_steps(in, a);
+}
+
+}  // namespace
+
+int plk_evaluate_device(plk_instance* in, int eigen, const int32_t* matrix_idx, const double* d_branch_lengths,
+                        int matrix_count, const plk_op* ops, int op_count, int root_buffer, const int32_t* scale_idx,
+                        int scale_count, int root_pre_buffer, const plk_pre_op* pre_ops, int pre_count, double* d_out) {
+  if (in == nullptr) return PLK_ERR_OUT_OF_RANGE;
+  const EvalArgs a{eigen, matrix_idx, d_branch_lengths, matrix_count, ops, op_count, root_buffer, scale_idx, scale_count,
+                   root_pre_buffer, pre_ops, pre_count, d_out};
+  return evaluate_impl(in, a);
+}
+
+int plk_evaluate(plk_instance* in, int eigen, const int32_t* matrix_idx, const double* branch_lengths, int matrix_count,
+                 const plk_op* ops, int op_count, int root_buffer, const int32_t* scale_idx, int scale_count,
+                 int root_pre_buffer, const plk_pre_op* pre_ops, int pre_count, double* out_logl, double* out_gradient) {
+  if (in == nullptr || out_logl == nullptr || (pre_count > 0 && out_gradient == nullptr)) return PLK_ERR_OUT_OF_RANGE;
+  if (matrix_count < 0 || matrix_count > in->cfg.matrix_buffer_count || pre_count < 0 || pre_count > in->L.max_grad)
+    return PLK_ERR_OUT_OF_RANGE;
+  if (matrix_count > 0 && branch_lengths == nullptr) return PLK_ERR_OUT_OF_RANGE;
+  for (int i = 0; i < matrix_count; ++i)
+    if (!(branch_lengths[i] >= 0.0 && std::isfinite(branch_lengths[i]))) return PLK_ERR_OUT_OF_RANGE;
+  const Layout& L = in->L;
+  double* d_t = in->at<double>(L.off_eval_t);
+  double* d_out = in->at<double>(L.off_eval_out);
+  if (matrix_count > 0)
+    CU(cudaMemcpyAsync(d_t, branch_lengths, (size_t)matrix_count * 8, cudaMemcpyHostToDevice, in->stream));
+  const EvalArgs a{eigen, matrix_idx, d_t, matrix_count, ops, op_count, root_buffer, scale_idx, scale_count,
+                   root_pre_buffer, pre_ops, pre_count, d_out};
+  int rc = evaluate_impl(in, a);
+  if (rc) return rc;
+  std::vector<double> tmp(1 + (size_t)pre_count);
+  rc = download(in, tmp.data(), d_out, tmp.size());
+  if (rc) return rc;
+  *out_logl = tmp[0];
+  bool finite = std::isfinite(tmp[0]);
+  for (int i = 0; i < pre_count; ++i) {
+    out_gradient[i] = tmp[1 + i];
+    finite = finite && std::isfinite(tmp[1 + i]);
+  }
+  return finite ? PLK_SUCCESS : PLK_ERR_FLOATING_POINT;
 }
 
 // ---- 8(f)-1: approximate gradient with respect to the rate-matrix elements --------------------------------------------

@@ -73,6 +73,8 @@ _SIGNATURES = {
     "plk_branch_derivatives": (_I, [_P, _I, _P, _P, _I, _P, _P]),
     "plk_pre_order_gradient": (_I, [_P, _I, _I, _P, _I, _P, _P]),
     "plk_pre_order_gradient_device": (_I, [_P, _I, _I, _P, _I, _P, _P]),
+    "plk_evaluate_device": (_I, [_P, _I, _P, _P, _I, _P, _I, _I, _P, _I, _I, _P, _I, _P]),
+    "plk_evaluate": (_I, [_P, _I, _P, _P, _I, _P, _I, _I, _P, _I, _I, _P, _I, _P, _P]),
     "plk_rate_matrix_gradient": (_I, [_P, _P, _P, _P, _I, _P]),
     "plk_chain_rule_rate_matrix": (_I, [_P, _P, _I, _I, _P]),
     "plk_get_partials": (_I, [_P, _I, _I, _P]),
@@ -342,6 +344,30 @@ class Instance:
         self._call("plk_pre_order_gradient_device", eigen, root_pre_buffer, _ptr(ops), len(ops),
                    C.c_void_p(d_out_gradient.data_ptr()),
                    None if d_out_site is None else C.c_void_p(d_out_site.data_ptr()))
+
+    def evaluate_device(self, eigen, matrix_idx, d_branch_lengths, ops, root_buffer, scale_idx, root_pre_buffer, pre_ops,
+                        d_out):
+        """plk_evaluate_device: steps 1-6 in one call (cached CUDA graph); d_out = [logL, gradient] on the device."""
+        m, sc = _i32(matrix_idx), _i32(scale_idx)
+        ops = np.ascontiguousarray(ops, dtype=OP_DTYPE)
+        pre = np.ascontiguousarray(pre_ops, dtype=PRE_OP_DTYPE)
+        self._call("plk_evaluate_device", eigen, _ptr(m), C.c_void_p(d_branch_lengths.data_ptr()), m.size, _ptr(ops),
+                   len(ops), root_buffer, _ptr(sc), sc.size, root_pre_buffer, _ptr(pre), len(pre),
+                   C.c_void_p(d_out.data_ptr()))
+
+    def evaluate(self, eigen, matrix_idx, branch_lengths, ops, root_buffer, scale_idx, root_pre_buffer, pre_ops,
+                 allow_nonfinite=False):
+        """plk_evaluate: the same with host branch lengths in, (logL, gradient[len(pre_ops)]) out."""
+        m, sc = _i32(matrix_idx), _i32(scale_idx)
+        t = _f64(branch_lengths, m.size)
+        ops = np.ascontiguousarray(ops, dtype=OP_DTYPE)
+        pre = np.ascontiguousarray(pre_ops, dtype=PRE_OP_DTYPE)
+        logl = np.zeros(1)
+        grad = np.zeros(len(pre))
+        self._call("plk_evaluate", eigen, _ptr(m), _ptr(t), m.size, _ptr(ops), len(ops), root_buffer, _ptr(sc), sc.size,
+                   root_pre_buffer, _ptr(pre), len(pre), _ptr(logl), _ptr(grad),
+                   allow=(ERR_FLOATING_POINT,) if allow_nonfinite else ())
+        return float(logl[0]), grad
 
     def rate_matrix_gradient(self, post_idx, pre_idx, branch_lengths):
         a, b = _i32(post_idx), _i32(pre_idx)
