@@ -71,6 +71,13 @@ enum {                                                /* plk_config.flags (bit s
   PLK_FLAG_NO_PDL = 128,       /* 4-state gradient pass: plain stream-ordered launches instead of programmatic
                                   dependent launches (the item classes of one dependency level are independent of
                                   each other and otherwise overlap one another's tail; comparison arm)       */
+  PLK_FLAG_CACHE_RATE_PRODUCTS = 256, /* P:101 caching variant: reserve a second slot per full partials slot for
+                                  Q p_k.  plk_update_partials then also stores Q p_dest of every operation (Q of eigen
+                                  buffer 0; plk_cache_rate_products for any other buffer / eigen), and
+                                  plk_branch_derivatives evaluates the sandwich from the cached products            */
+  PLK_FLAG_ON_THE_FLY_MATRICES = 512, /* P:101 caching variant: reserve the ready flags of
+                                  plk_update_partials_on_the_fly (partials_buffer_count * P words); padded state counts
+                                  only (S > 4)                                                                      */
   PLK_FLAG_SITE_DERIVATIVES = 4 /* reserve partials_buffer_count * P doubles so that the gradient calls can
                                   return per-pattern derivatives (out_site != NULL); without it such a
                                   request returns PLK_ERR_UNSUPPORTED                                   */
@@ -191,6 +198,26 @@ PLK_API int plk_update_transition_matrices_device(plk_instance* inst, int eigen,
  * a dest_scale (_OUT_OF_RANGE).  Never synchronises. */
 PLK_API int plk_update_partials(plk_instance* inst, const plk_op* ops, int count);
 
+/* S8f-3 / P:101 ("for phylogeographic problems that typically have a large state-space size but only a single site
+ * pattern ... it is more efficient to form the transition probability matrix on-the-fly while calculating the likelihood
+ * ... through Felsenstein's pruning algorithm").  The same update as plk_update_partials -- same buffers, same deferred
+ * rescaling, results interchangeable -- but no transition matrix is read, formed or stored: for the branch above child k
+ * of ops[i], of length branch_lengths[2 i + k] (HOST, finite and >= 0), exp(Q r_c t) is applied to the child's partial as
+ * U (exp(lambda r_c t) o (U^-1 x)) from eigen buffer `eigen` (4 S^2 flops per edge, pattern and category; fp64 arithmetic
+ * in both precisions).  The child*_matrix fields of the operations are ignored.  The WHOLE list runs in ONE launch
+ * (dataflow over ready flags; independent subtrees run concurrently), in the order given.  Needs
+ * PLK_FLAG_ON_THE_FLY_MATRICES (else _UNSUPPORTED) and count <= partials_buffer_count.  Never synchronises. */
+PLK_API int plk_update_partials_on_the_fly(plk_instance* inst, int eigen, const plk_op* ops, int count,
+                                           const double* branch_lengths);
+
+/* S8f-3 / P:101 ("the product of the infinitesimal rate matrix and the post-order partial likelihood vector at each node
+ * could be cached directly").  Stores Qp_k[c,p,.] = Q p_k[c,p,.] (Q of eigen buffer `eigen`) for the listed post-order
+ * buffers; compact tips need none.  Needs PLK_FLAG_CACHE_RATE_PRODUCTS (else _UNSUPPORTED).  With that flag
+ * plk_update_partials calls it for the dests of its operations (eigen buffer 0) and plk_branch_derivatives reads
+ * num_p = sum_c w_c r_c q . Qp instead of applying Q; a listed buffer whose product was never cached, or whose partials
+ * were overwritten since, gives _UNINITIALIZED there.  Never synchronises. */
+PLK_API int plk_cache_rate_products(plk_instance* inst, int eigen, const int32_t* post_idx, int count);
+
 /* S8a step 4.  log l_p = log( sum_c w_c sum_s pi_s p_root[c,p,s] ) + sum over the listed scale buffers of their
  * log factor; logL = sum_p omega_p log l_p.  out_sum: HOST [1]; out_site: HOST [P] or NULL.
  * Returns _FLOATING_POINT (outputs still written) if logL is NaN or infinite. */
@@ -261,7 +288,8 @@ PLK_API int plk_rate_matrix_gradient(plk_instance* inst, const int32_t* post_idx
 /* ---- read-back (tests) -------------------------------------------------------------------------------------- */
 
 /* Partials [C][P][S] of a post-order (pre = 0) or pre-order (pre = 1) buffer; compact tips are expanded to
- * one-hot / all-ones rows. */
+ * one-hot / all-ones rows.  pre = 2: the cached rate product Q p_k of post-order buffer `buffer`
+ * (PLK_FLAG_CACHE_RATE_PRODUCTS; _UNINITIALIZED if it is not current, _UNSUPPORTED for a compact tip). */
 PLK_API int plk_get_partials(plk_instance* inst, int buffer, int pre, double* out);
 /* Natural-log scale factors [P] of one scale buffer (the stored power-of-two exponent times ln 2). */
 PLK_API int plk_get_scale_factors(plk_instance* inst, int scale, double* out);

@@ -87,6 +87,8 @@ class Evaluator:
                 part[np.nonzero(known)[0], st[known]] = 1.0
                 part[~known, :] = 1.0
                 inst.set_tip_partials(k, part)
+                if inst.cfg.flags & plk.FLAG_CACHE_RATE_PRODUCTS:  # Q p_k cached next to the partials
+                    inst.cache_rate_products(0, [k])
             else:
                 inst.set_tip_states(k, wl.tip_states[k].astype(np.int32))
 
@@ -103,6 +105,14 @@ class Evaluator:
             self.inst.update_transition_matrices(0, self.matrix_idx, np.asarray(t)[self.matrix_idx])
         self.inst.update_partials(self.ops)
         return self.inst.root_log_likelihoods(self.tree.root, self.scale_idx, want_site, allow_nonfinite)
+
+    def log_likelihood_on_the_fly(self, branch_lengths: Optional[np.ndarray] = None, want_site=True):
+        """The same through plk_update_partials_on_the_fly: no transition matrix is formed; needs
+        FLAG_ON_THE_FLY_MATRICES."""
+        t = np.asarray(self.tree.branch_length if branch_lengths is None else branch_lengths, dtype=np.float64)
+        bl = np.stack([t[self.ops["child1"]], t[self.ops["child2"]]], axis=1)
+        self.inst.update_partials_on_the_fly(0, self.ops, bl)
+        return self.inst.root_log_likelihoods(self.tree.root, self.scale_idx, want_site)
 
     def gradient(self, want_site=False):
         """After log_likelihood(): d logL / d t_k for every node k (0 at the root), fused pre-order + derivative."""

@@ -15,6 +15,7 @@
 #include "plk_nuc_tma.cuh"
 #include "plk_nuc_lean.cuh"
 #include "plk_cross.cuh"
+#include "plk_cache.cuh"
 #include "plk_schedule.h"
 #ifdef PLK_WITH_TENSOR
 #include "plk_tc.cuh"
@@ -45,7 +46,7 @@ struct Layout {
   int n_tiles, max_grad;
   size_t off_post, off_compact, off_pre, off_pre_mx, off_matrix, off_eigen, off_scale, off_weights, off_pi,
       off_rates, off_catw, off_site, off_block_partial, off_grad_partial, off_grad_out, off_logl, off_site_deriv,
-      off_stage, off_ring, off_plan, off_eval_t, off_eval_out, off_matrix_t, off_matrix_d, off_matrix_dt, off_cat_scratch, off_cross_partial, off_cross_out, total;
+      off_stage, off_ring, off_plan, off_eval_t, off_eval_out, off_qp, off_otf_ready, off_otf_sync, off_matrix_t, off_matrix_d, off_matrix_dt, off_cat_scratch, off_cross_partial, off_cross_out, total;
   size_t stage_bytes;
 };
 
@@ -112,6 +113,11 @@ bool compute_layout(const plk_config& c, Layout& L) {
   L.off_plan = take(PLAN_BYTES);
   L.off_eval_t = take((size_t)c.matrix_buffer_count * 8);        // plk_evaluate: branch lengths, [logL, gradient]
   L.off_eval_out = take((size_t)(1 + c.partials_buffer_count) * 8);
+  // caching variants of P:101 (plk_cache.cuh): Q p_k next to every full partials slot; ready flags of the one-launch
+  // on-the-fly post-order pass (one per operation and pattern) and its ticket counters
+  L.off_qp = take((c.flags & PLK_FLAG_CACHE_RATE_PRODUCTS) ? (size_t)L.post_slots * L.W : 0);
+  L.off_otf_ready = take((c.flags & PLK_FLAG_ON_THE_FLY_MATRICES) ? (size_t)c.partials_buffer_count * L.P * 4 : 0);
+  L.off_otf_sync = take(64);
   // fp32 tensor-core instances (tcgen05 pre-order kernels, plk_tc5_pre*.cuh): per matrix buffer M^T, D = M Q and D^T,
   // and the per-category num / den scratch of the class-specialised kernels ([slot][num, den][C][P] floats)
   const bool tc5 = L.SP == 64 && c.precision == PLK_FP32 && (c.flags & PLK_FLAG_TENSOR_CORES) && !(c.flags & PLK_FLAG_NO_TCGEN05);
@@ -142,6 +148,8 @@ struct plk_instance {
   // buffer tables (host bookkeeping only)
   std::vector<int> post_slot, post_kind, post_pending_scale;
   std::vector<char> post_written;
+  std::vector<char> qp_valid;   // PLK_FLAG_CACHE_RATE_PRODUCTS: Q p_k of this post-order buffer is current
+  unsigned int otf_epoch = 0;   // value of the ready flags of the current on-the-fly launch
   std::vector<int> pre_slot;
   std::vector<char> pre_written, pre_has_mx;
   std::vector<char> matrix_written, scale_written, eigen_written, q_written;
@@ -177,6 +185,7 @@ struct plk_instance {
     if (post_kind[idx] == KIND_STATES) return arena + L.off_compact + (size_t)post_slot[idx] * L.compact_bytes;
     return arena + L.off_post + (size_t)post_slot[idx] * L.W;
   }
+  void* qp_ptr(int idx) const { return arena + L.off_qp + (size_t)post_slot[idx] * L.W; }
   void* pre_ptr(int idx) const { return arena + L.off_pre + (size_t)pre_slot[idx] * L.W; }
   void* pre_mx_ptr(int idx) const { return arena + L.off_pre_mx + (size_t)pre_slot[idx] * L.mx_bytes; }
   void* matrix_ptr(int idx) const { return arena + L.off_matrix + (size_t)idx * L.matrix_bytes; }
@@ -720,6 +729,62 @@ int operand_of(const plk_instance* in, int idx, const void** ptr, int* kind, con
   return PLK_SUCCESS;
 }
 
+
+// P:101 variant (a): Qp_k = Q p_k for the listed post-order buffers (full or single-category partials; compact tips
+// need none), stored in the slot that shadows the buffer's partials slot.
+int cache_rate_products_impl(plk_instance* in, int eigen, const int32_t* post_idx, int count) {
+  const Layout& L = in->L;
+  if (!(in->cfg.flags & PLK_FLAG_CACHE_RATE_PRODUCTS)) return PLK_ERR_UNSUPPORTED;
+  if (count < 0 || (count > 0 && post_idx == nullptr)) return PLK_ERR_OUT_OF_RANGE;
+  if (eigen < 0 || eigen >= in->cfg.eigen_buffer_count) return PLK_ERR_OUT_OF_RANGE;
+  if (!in->q_written[eigen]) return PLK_ERR_UNINITIALIZED;
+  std::vector<DevQpItem> items;
+  for (int i = 0; i < count; ++i) {
+    const void* ptr;
+    const void* pending;
+    int kind;
+    int rc = operand_of(in, post_idx[i], &ptr, &kind, &pending);
+    if (rc) return rc;
+    in->qp_valid[post_idx[i]] = 1;
+    if (kind == KIND_STATES) continue;  // Q e_z is a column of Q: nothing to cache
+    items.push_back(DevQpItem{ptr, in->qp_ptr(post_idx[i]), kind, 0});
+  }
+  const int n = (int)items.size();
+  if (n == 0) return PLK_SUCCESS;
+  char *h, *d;
+  int rc = ring_alloc(in, (size_t)n * sizeof(DevQpItem), &h, &d);
+  if (rc) return rc;
+  std::memcpy(h, items.data(), (size_t)n * sizeof(DevQpItem));
+  rc = copy_ring(in, h, d, (size_t)n * sizeof(DevQpItem));
+  if (rc) return rc;
+  const DevQpItem* di = reinterpret_cast<const DevQpItem*>(d);
+  for (int first = 0; first < n; first += 32768) {
+    const int m = n - first < 32768 ? n - first : 32768;
+    rc = by_precision(in, [&](auto tag) -> int {
+      using T = decltype(tag);
+      const T* Q = static_cast<const T*>(in->eig_QT(eigen));
+      if (L.SP == 4) {
+        dim3 grid(blocks_for((size_t)L.C * L.P, 256), m);
+        k_rate_products4<T><<<grid, 256, 0, in->stream>>>(di + first, L.P, L.C, Q);
+      } else if (L.SP == 32) {
+        int r2 = opt_in_smem(k_rate_products64<T, 32>, rate_products64_smem<T, 32>());
+        if (r2) return r2;
+        dim3 grid(L.n_tiles, L.C, m);
+        k_rate_products64<T, 32><<<grid, GEN_THREADS, rate_products64_smem<T, 32>(), in->stream>>>(di + first, L.P, L.S, L.C, Q);
+      } else {
+        int r2 = opt_in_smem(k_rate_products64<T>, rate_products64_smem<T>());
+        if (r2) return r2;
+        dim3 grid(L.n_tiles, L.C, m);
+        k_rate_products64<T><<<grid, GEN_THREADS, rate_products64_smem<T>(), in->stream>>>(di + first, L.P, L.S, L.C, Q);
+      }
+      return PLK_SUCCESS;
+    });
+    if (rc) return rc;
+    CHECK_LAUNCH(in);
+  }
+  return PLK_SUCCESS;
+}
+
 }  // namespace
 
 // =================================================================================================================
@@ -742,8 +807,10 @@ int plk_create(const plk_config* cfg, void* d_arena, size_t arena_bytes, void* c
     return PLK_ERR_OUT_OF_RANGE;
   }
   if (cfg->flags & ~(PLK_FLAG_TENSOR_CORES | PLK_FLAG_NO_LEVEL_BATCH | PLK_FLAG_SITE_DERIVATIVES | PLK_FLAG_LEVEL_BATCH_ONLY |
-                     PLK_FLAG_PATTERN_WALK_ONLY | PLK_FLAG_NO_TMA | PLK_FLAG_NO_TCGEN05 | PLK_FLAG_NO_PDL))
+                     PLK_FLAG_PATTERN_WALK_ONLY | PLK_FLAG_NO_TMA | PLK_FLAG_NO_TCGEN05 | PLK_FLAG_NO_PDL |
+                     PLK_FLAG_CACHE_RATE_PRODUCTS | PLK_FLAG_ON_THE_FLY_MATRICES))
     return PLK_ERR_UNSUPPORTED;
+  if ((cfg->flags & PLK_FLAG_ON_THE_FLY_MATRICES) && L.SP == 4) return PLK_ERR_UNSUPPORTED;  // large state spaces only
   if ((cfg->flags & PLK_FLAG_LEVEL_BATCH_ONLY) && (cfg->flags & PLK_FLAG_PATTERN_WALK_ONLY)) return PLK_ERR_UNSUPPORTED;
 #ifndef PLK_WITH_TENSOR
   if ((cfg->flags & PLK_FLAG_TENSOR_CORES) && L.SP == 64) return PLK_ERR_UNSUPPORTED;
@@ -770,6 +837,7 @@ int plk_create(const plk_config* cfg, void* d_arena, size_t arena_bytes, void* c
   in->post_kind.assign(cfg->partials_buffer_count, KIND_PARTIALS);
   in->post_pending_scale.assign(cfg->partials_buffer_count, -1);
   in->post_written.assign(cfg->partials_buffer_count, 0);
+  in->qp_valid.assign(cfg->partials_buffer_count, 0);
   in->pre_slot.assign(cfg->preorder_buffer_count, -1);
   in->pre_written.assign(cfg->preorder_buffer_count, 0);
   in->pre_has_mx.assign(cfg->preorder_buffer_count, 0);
@@ -868,6 +936,7 @@ int plk_set_tip_partials(plk_instance* in, int tip, const double* partials) {
   if (rc) return rc;
   rc = upload_rows(in, partials, in->post_ptr(tip), (size_t)in->L.P);
   if (rc) return rc;
+  in->qp_valid[tip] = 0;
   in->post_written[tip] = 1;
   in->post_pending_scale[tip] = -1;
   return PLK_SUCCESS;
@@ -881,6 +950,7 @@ int plk_set_partials(plk_instance* in, int buffer, const double* partials) {
   if (rc) return rc;
   rc = upload_rows(in, partials, in->post_ptr(buffer), (size_t)in->L.C * in->L.P);
   if (rc) return rc;
+  in->qp_valid[buffer] = 0;
   in->post_written[buffer] = 1;
   in->post_pending_scale[buffer] = -1;
   return PLK_SUCCESS;
@@ -1170,8 +1240,17 @@ int plk_update_partials(plk_instance* in, const plk_op* ops, int count) {
       }
     }
   }
+  if (cfg.flags & PLK_FLAG_CACHE_RATE_PRODUCTS) {  // cache Q p_k while the traversal has p_k at hand
+    std::vector<int32_t> dests(count);
+    for (int i = 0; i < count; ++i) {
+      dests[i] = ops[i].dest;
+      in->qp_valid[ops[i].dest] = 0;
+    }
+    if (in->q_written[0]) return cache_rate_products_impl(in, 0, dests.data(), count);
+  }
   return PLK_SUCCESS;
 }
+
 
 // ---- step 4: root ---------------------------------------------------------------------------------------------------
 
@@ -1589,6 +1668,157 @@ int plk_pre_order_gradient(plk_instance* in, int eigen, int root_pre, const plk_
   return finish_gradient(in, count, out_gradient, out_site, d_site);
 }
 
+// P:101 variant (a), gradient side: the sandwich from the cached Q p_k (k_deriv*_cached) -- no matrix is applied.
+static int branch_derivatives_cached(plk_instance* in, int eigen, const int32_t* post_idx, const int32_t* pre_idx,
+                                     int count, double* out_gradient, double* out_site) {
+  const Layout& L = in->L;
+  const plk_config& cfg = in->cfg;
+  char *h, *d;
+  int rc = ring_alloc(in, (size_t)count * sizeof(DevBranchQp), &h, &d);
+  if (rc) return rc;
+  DevBranchQp* hb = reinterpret_cast<DevBranchQp*>(h);
+  for (int i = 0; i < count; ++i) {
+    if (pre_idx[i] < 0 || pre_idx[i] >= cfg.preorder_buffer_count) return PLK_ERR_OUT_OF_RANGE;
+    if (in->pre_slot[pre_idx[i]] < 0 || !in->pre_written[pre_idx[i]]) return PLK_ERR_UNINITIALIZED;
+    const void* pending;
+    rc = operand_of(in, post_idx[i], &hb[i].p, &hb[i].kind, &pending);
+    if (rc) return rc;
+    if (hb[i].kind != KIND_STATES && !in->qp_valid[post_idx[i]]) return PLK_ERR_UNINITIALIZED;  // plk_cache_rate_products first
+    hb[i].qp = hb[i].kind == KIND_STATES ? nullptr : in->qp_ptr(post_idx[i]);
+    hb[i].q = in->pre_ptr(pre_idx[i]);
+    hb[i].slot = i;
+  }
+  rc = copy_ring(in, h, d, (size_t)count * sizeof(DevBranchQp));
+  if (rc) return rc;
+  double* d_site = out_site != nullptr ? in->at<double>(L.off_site_deriv) : nullptr;
+  const DevBranchQp* db = reinterpret_cast<const DevBranchQp*>(d);
+  const double* cw = in->at<double>(L.off_catw);
+  const double* cr = in->at<double>(L.off_rates);
+  const double* wt = in->at<double>(L.off_weights);
+  double* gp = in->at<double>(L.off_grad_partial);
+  for (int first = 0; first < count; first += 32768) {
+    const int m = count - first < 32768 ? count - first : 32768;
+    rc = by_precision(in, [&](auto tag) -> int {
+      using T = decltype(tag);
+      const T* Q = static_cast<const T*>(in->eig_QT(eigen));
+      if (L.SP == 4) {
+        dim3 grid(blocks_for(L.P, NUC_THREADS), m);
+        switch (L.C) {
+#define CASE(CC) case CC: k_deriv4_cached<T, CC><<<grid, NUC_THREADS, 0, in->stream>>>(db + first, L.P, Q, cw, cr, wt, gp, L.n_tiles, d_site); break;
+          CASE(1) CASE(2) CASE(3) CASE(4) CASE(5) CASE(6) CASE(7) CASE(8)
+#undef CASE
+          default: return PLK_ERR_UNSUPPORTED;
+        }
+        in->grad_parts = (int)grid.x;
+      } else {
+        dim3 grid(L.n_tiles, m);
+        if (L.SP == 32)
+          k_deriv64_cached<T, 32><<<grid, GEN_THREADS, 0, in->stream>>>(db + first, L.P, L.S, L.C, Q, cw, cr, wt, gp, L.n_tiles, d_site);
+        else
+          k_deriv64_cached<T, 64><<<grid, GEN_THREADS, 0, in->stream>>>(db + first, L.P, L.S, L.C, Q, cw, cr, wt, gp, L.n_tiles, d_site);
+        in->grad_parts = L.n_tiles;
+      }
+      return PLK_SUCCESS;
+    });
+    if (rc) return rc;
+    CHECK_LAUNCH(in);
+  }
+  k_sum_rows<<<count, 128, 0, in->stream>>>(gp, nullptr, in->grad_parts, L.n_tiles, in->at<double>(L.off_grad_out));
+  CHECK_LAUNCH(in);
+  return finish_gradient(in, count, out_gradient, out_site, d_site);
+}
+
+int plk_cache_rate_products(plk_instance* in, int eigen, const int32_t* post_idx, int count) {
+  if (in == nullptr) return PLK_ERR_OUT_OF_RANGE;
+  return cache_rate_products_impl(in, eigen, post_idx, count);
+}
+
+// P:101 variant (b): the whole post-order list in one launch, transition matrices applied on the fly (k_post_otf).
+int plk_update_partials_on_the_fly(plk_instance* in, int eigen, const plk_op* ops, int count, const double* branch_lengths) {
+  if (in == nullptr || count < 0) return PLK_ERR_OUT_OF_RANGE;
+  const plk_config& cfg = in->cfg;
+  const Layout& L = in->L;
+  if (!(cfg.flags & PLK_FLAG_ON_THE_FLY_MATRICES)) return PLK_ERR_UNSUPPORTED;
+  if (count == 0) return PLK_SUCCESS;
+  if (ops == nullptr || branch_lengths == nullptr || count > cfg.partials_buffer_count) return PLK_ERR_OUT_OF_RANGE;
+  if (eigen < 0 || eigen >= cfg.eigen_buffer_count) return PLK_ERR_OUT_OF_RANGE;
+  if (!in->eigen_written[eigen] || !in->have_rates) return PLK_ERR_UNINITIALIZED;
+  std::vector<int> level;
+  const int n_levels = schedule_post(ops, count, level);
+  if (n_levels < 0) return n_levels;
+  std::vector<int> producer(cfg.partials_buffer_count, -1);
+  int fresh = 0;
+  for (int i = 0; i < count; ++i) {
+    const plk_op& o = ops[i];
+    if (o.dest >= cfg.partials_buffer_count || o.child1 >= cfg.partials_buffer_count || o.child2 >= cfg.partials_buffer_count ||
+        o.dest_scale >= cfg.scale_buffer_count || o.dest_scale < -1)
+      return PLK_ERR_OUT_OF_RANGE;
+    if (in->post_slot[o.dest] >= 0 && in->post_kind[o.dest] == KIND_STATES) return PLK_ERR_OUT_OF_RANGE;
+    for (int k = 0; k < 2; ++k) {
+      const double t = branch_lengths[2 * i + k];
+      if (!(t >= 0.0 && std::isfinite(t))) return PLK_ERR_OUT_OF_RANGE;
+      const int ch = k == 0 ? o.child1 : o.child2;
+      if (!(in->post_written[ch] || producer[ch] >= 0)) return PLK_ERR_UNINITIALIZED;
+    }
+    if (in->post_slot[o.dest] < 0 && producer[o.dest] < 0) ++fresh;
+    producer[o.dest] = i;
+  }
+  if (in->next_post_slot + fresh > L.post_slots) return PLK_ERR_OUT_OF_MEMORY;
+  char *h, *d;
+  int rc = ring_alloc(in, (size_t)count * sizeof(DevOtfOp), &h, &d);
+  if (rc) return rc;
+  DevOtfOp* ho = reinterpret_cast<DevOtfOp*>(h);
+  std::fill(producer.begin(), producer.end(), -1);
+  for (int i = 0; i < count; ++i) {  // list order: every dependency has a lower index
+    const plk_op& o = ops[i];
+    rc = bind_post_full(in, o.dest, KIND_PARTIALS);
+    if (rc) return rc;
+    DevOtfOp& x = ho[i];
+    x.dest = in->post_ptr(o.dest);
+    x.scale = o.dest_scale >= 0 ? in->scale_ptr(o.dest_scale) : nullptr;
+    const int ch[2] = {o.child1, o.child2};
+    for (int k = 0; k < 2; ++k) {
+      rc = operand_of(in, ch[k], &x.child[k], &x.kind[k], &x.cscale[k]);
+      if (rc) return rc;
+      x.t[k] = branch_lengths[2 * i + k];
+      x.dep[k] = producer[ch[k]];
+    }
+    producer[o.dest] = i;
+    in->post_written[o.dest] = 1;
+    in->qp_valid[o.dest] = 0;
+    in->post_pending_scale[o.dest] = o.dest_scale;
+    if (o.dest_scale >= 0) in->scale_written[o.dest_scale] = 1;
+  }
+  rc = copy_ring(in, h, d, (size_t)count * sizeof(DevOtfOp));
+  if (rc) return rc;
+  if (++in->otf_epoch == 0) {  // wrapped: clear the flags so that an old value cannot match
+    CU(cudaMemsetAsync(in->arena + L.off_otf_ready, 0, (size_t)cfg.partials_buffer_count * L.P * 4, in->stream));
+    in->otf_epoch = 1;
+  }
+  const long long total = (long long)count * L.P;
+  rc = by_precision(in, [&](auto tag) -> int {
+    using T = decltype(tag);
+    auto go = [&](auto kernel, size_t smem) -> int {
+      int r2 = opt_in_smem(kernel, smem);
+      if (r2) return r2;
+      int bps = 0;
+      CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&bps, kernel, OTF_THREADS, smem));
+      if (bps < 1) return PLK_ERR_CUDA;
+      long long g = (long long)in->sm_count * bps;
+      if (g > total) g = total;
+      kernel<<<(unsigned)g, OTF_THREADS, smem, in->stream>>>(
+          reinterpret_cast<const DevOtfOp*>(d), count, L.P, L.S, L.C, in->eig_U(eigen), in->eig_Uinv(eigen),
+          in->eig_lam(eigen), in->at<double>(L.off_rates), in->at<OtfSync>(L.off_otf_sync),
+          in->at<unsigned int>(L.off_otf_ready), in->otf_epoch);
+      return PLK_SUCCESS;
+    };
+    return L.SP == 32 ? go(k_post_otf<T, 32>, otf_smem<32>()) : go(k_post_otf<T, 64>, otf_smem<64>());
+  });
+  if (rc) return rc;
+  CHECK_LAUNCH(in);
+  return PLK_SUCCESS;
+}
+
 int plk_branch_derivatives(plk_instance* in, int eigen, const int32_t* post_idx, const int32_t* pre_idx, int count,
                            double* out_gradient, double* out_site) {
   if (in == nullptr || count < 0) return PLK_ERR_OUT_OF_RANGE;
@@ -1602,6 +1832,8 @@ int plk_branch_derivatives(plk_instance* in, int eigen, const int32_t* post_idx,
   if (!in->q_written[eigen]) return PLK_ERR_UNINITIALIZED;
   int rc = check_model_ready(in, true);
   if (rc) return rc;
+  if (cfg.flags & PLK_FLAG_CACHE_RATE_PRODUCTS)
+    return branch_derivatives_cached(in, eigen, post_idx, pre_idx, count, out_gradient, out_site);
   char *h, *d;
   rc = ring_alloc(in, (size_t)count * sizeof(DevBranch), &h, &d);
   if (rc) return rc;
@@ -1903,7 +2135,15 @@ int plk_get_partials(plk_instance* in, int buffer, int pre, double* out) {
   double* stage = in->at<double>(L.off_stage);
   const void* src;
   int kind = KIND_PARTIALS;
-  if (pre) {
+  if (pre == 2) {  // the cached rate product Q p_k of a post-order buffer (PLK_FLAG_CACHE_RATE_PRODUCTS)
+    if (!(in->cfg.flags & PLK_FLAG_CACHE_RATE_PRODUCTS)) return PLK_ERR_UNSUPPORTED;
+    const void* pending;
+    int rc = operand_of(in, buffer, &src, &kind, &pending);
+    if (rc) return rc;
+    if (kind == KIND_STATES) return PLK_ERR_UNSUPPORTED;
+    if (!in->qp_valid[buffer]) return PLK_ERR_UNINITIALIZED;
+    src = in->qp_ptr(buffer);
+  } else if (pre) {
     if (buffer < 0 || buffer >= in->cfg.preorder_buffer_count) return PLK_ERR_OUT_OF_RANGE;
     if (in->pre_slot[buffer] < 0 || !in->pre_written[buffer]) return PLK_ERR_UNINITIALIZED;
     src = in->pre_ptr(buffer);

@@ -24,6 +24,7 @@ FLAG_TENSOR_CORES, FLAG_NO_LEVEL_BATCH, FLAG_SITE_DERIVATIVES = 1, 2, 4
 FLAG_LEVEL_BATCH_ONLY, FLAG_PATTERN_WALK_ONLY, FLAG_NO_TMA = 8, 16, 32
 FLAG_NO_TCGEN05 = 64
 FLAG_NO_PDL = 128
+FLAG_CACHE_RATE_PRODUCTS, FLAG_ON_THE_FLY_MATRICES = 256, 512
 NUCLEOTIDE, CODON = 0, 1
 
 
@@ -67,6 +68,8 @@ _SIGNATURES = {
     "plk_update_transition_matrices": (_I, [_P, _I, _P, _P, _I]),
     "plk_update_transition_matrices_device": (_I, [_P, _I, _P, _P, _I]),
     "plk_update_partials": (_I, [_P, _P, _I]),
+    "plk_update_partials_on_the_fly": (_I, [_P, _I, _P, _I, _P]),
+    "plk_cache_rate_products": (_I, [_P, _I, _P, _I]),
     "plk_root_log_likelihoods": (_I, [_P, _I, _P, _I, _P, _P]),
     "plk_root_log_likelihoods_device": (_I, [_P, _I, _P, _I, _P, _P]),
     "plk_update_pre_partials": (_I, [_P, _I, _P, _I]),
@@ -345,6 +348,16 @@ class Instance:
                    C.c_void_p(d_out_gradient.data_ptr()),
                    None if d_out_site is None else C.c_void_p(d_out_site.data_ptr()))
 
+    def update_partials_on_the_fly(self, eigen, ops, branch_lengths):
+        """plk_update_partials_on_the_fly: branch_lengths [count][2] = lengths of the branches above child1 / child2."""
+        ops = np.ascontiguousarray(ops, dtype=OP_DTYPE)
+        t = _f64(branch_lengths, 2 * len(ops))
+        self._call("plk_update_partials_on_the_fly", eigen, _ptr(ops), len(ops), _ptr(t))
+
+    def cache_rate_products(self, eigen, post_idx):
+        a = _i32(post_idx)
+        self._call("plk_cache_rate_products", eigen, _ptr(a), a.size)
+
     def evaluate_device(self, eigen, matrix_idx, d_branch_lengths, ops, root_buffer, scale_idx, root_pre_buffer, pre_ops,
                         d_out):
         """plk_evaluate_device: steps 1-6 in one call (cached CUDA graph); d_out = [logL, gradient] on the device."""
@@ -378,8 +391,9 @@ class Instance:
 
     # -- read-back
     def get_partials(self, buffer, pre=False):
+        """pre: False / 0 post-order, True / 1 pre-order, 2 the cached rate product Q p_k of a post-order buffer."""
         out = np.zeros((self.Cc, self.P, self.S))
-        self._call("plk_get_partials", buffer, 1 if pre else 0, _ptr(out))
+        self._call("plk_get_partials", buffer, int(pre), _ptr(out))
         return out
 
     def get_scale_factors(self, scale):
