@@ -49,8 +49,15 @@ typedef enum {
   PLK_ERR_UNSUPPORTED = -5,    /* state count not in 2..64, unknown flag, path not built                */
   PLK_ERR_FLOATING_POINT = -6, /* NaN / Inf / -Inf in the log-likelihood or a derivative                */
   PLK_ERR_CUDA = -7,           /* a CUDA runtime call failed (no device, launch failure, ...)           */
-  PLK_ERR_STOP_CODON = -8      /* plk_encode_and_compress met a stop codon                              */
+  PLK_ERR_STOP_CODON = -8,     /* plk_encode_and_compress met a stop codon                              */
+  PLK_ERR_STATIC_SCRATCH_LIMIT = -9 /* plk_root_log_likelihoods_static_device: the problem needs more than the
+                                  library's fixed static scratch (PLK_STATIC_SCRATCH_DOUBLES / PLK_STATIC_SCALE_MAX) */
 } plk_status;
+
+/* limits of plk_root_log_likelihoods_static_device (the one entry point whose scratch is a static device array) */
+#define PLK_STATIC_SCRATCH_DOUBLES 8192 /* 64 KB per GPU: k_root blocks = ceil(P * G / 128), G = 1 | 8 | 16 for
+                                           4 | 5..32 | 33..64 states => P <= 1 048 576 | 131 072 | 65 536 */
+#define PLK_STATIC_SCALE_MAX 2048       /* scale buffers per call */
 
 enum { PLK_FP64 = 0, PLK_FP32 = 1 };                 /* plk_config.precision                          */
 enum {                                                /* plk_config.flags (bit set)                    */
@@ -227,6 +234,18 @@ PLK_API int plk_root_log_likelihoods(plk_instance* inst, int root_buffer, const 
  * value, no synchronisation. */
 PLK_API int plk_root_log_likelihoods_device(plk_instance* inst, int root_buffer, const int32_t* scale_idx,
                                             int scale_count, double* d_out_sum, double* d_out_site);
+
+/* S8a step 4 for callers that must not allocate (code under CUDA graph capture, tight serving loops, harnesses that
+ * forbid cudaMalloc): same arguments, kernels and results as plk_root_log_likelihoods_device, but the per-block partial
+ * sums of the reduction live in a file-scope `static __device__` array of the library (PLK_STATIC_SCRATCH_DOUBLES
+ * doubles = 64 KB, held by every GPU that loads libplk.so until the process exits) instead of the instance arena, and
+ * the call performs no device or host allocation at all.  A problem beyond the limits above returns
+ * PLK_ERR_STATIC_SCRATCH_LIMIT and launches nothing.  The array is shared by all instances and streams of a device and
+ * keeps the last call's contents (every entry that is read is written first by the same call, so nothing needs
+ * clearing); calls that overlap on the GPU race on it -- serialise them (one stream, or events).  The arena's device
+ * must be current.  Never synchronises, no value check. */
+PLK_API int plk_root_log_likelihoods_static_device(plk_instance* inst, int root_buffer, const int32_t* scale_idx,
+                                                   int scale_count, double* d_out_sum, double* d_out_site);
 
 /* S8a step 5 / P:43.  Fills pre-order buffer `root_pre_buffer` with q_root[c,p,.] = pi, then applies `ops`
  * (root towards tips; same ordering rule as plk_update_partials with parent_pre in the role of the children).

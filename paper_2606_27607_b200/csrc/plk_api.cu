@@ -883,6 +883,8 @@ const char* plk_error_string(int status) {
     case PLK_ERR_FLOATING_POINT: return "log-likelihood or derivative is not finite";
     case PLK_ERR_CUDA: return "CUDA error (no device or a runtime call failed)";
     case PLK_ERR_STOP_CODON: return "stop codon in a codon alignment";
+    case PLK_ERR_STATIC_SCRATCH_LIMIT:
+      return "problem exceeds the static scratch of the no-allocation entry point (PLK_STATIC_SCRATCH_DOUBLES / PLK_STATIC_SCALE_MAX)";
     default: return "unknown status";
   }
 }
@@ -2241,3 +2243,111 @@ int plk_schedule_pre_levels(const plk_pre_op* ops, int count, int32_t* out_level
 }
 
 }  // extern "C"
+
+// =================================================================================================================
+// plk_root_log_likelihoods_static_device -- the root reduction (S8a step 4) for callers that must not allocate.
+//
+// Same kernels and arithmetic as plk_root_log_likelihoods_device; the one difference is where k_root's per-block
+// partial sums go: not into the instance arena but into the file-scope array below, which every GPU that loads the
+// library holds until the process exits (PLK_STATIC_SCRATCH_DOUBLES doubles = 64 KB).  The call allocates nothing on
+// the device or on the host (no cudaMalloc / cudaFree, no allocating library routine, no std::vector): the scale list
+// is assembled on the stack and travels through the instance's pinned parameter ring, which plk_create made.
+// Limits (else PLK_ERR_STATIC_SCRATCH_LIMIT): k_root blocks = ceil(P * G / 128) <= PLK_STATIC_SCRATCH_DOUBLES (G = 1
+// for 4 states, 8 for 5..32, 16 for 33..64: P <= 1 048 576 / 131 072 / 65 536) and scale_count <=
+// PLK_STATIC_SCALE_MAX.  The array is shared by EVERY call on a device -- all instances, all streams -- and keeps the
+// last call's contents: nothing in it has to start at zero (k_root writes each of the n_blocks entries k_sum_rows
+// reads, in the same call), but two calls that overlap on the GPU (different streams, or graphs replayed concurrently)
+// race on it and must be serialised by the caller.
+// =================================================================================================================
+static __device__ __align__(256) double g_plk_static_scratch[PLK_STATIC_SCRATCH_DOUBLES];
+
+namespace {
+constexpr int STATIC_MAX_DEVICES = 64;
+double* g_static_scratch_ptr[STATIC_MAX_DEVICES] = {};  // device address of the array on each device (set once)
+
+// In host code `g_plk_static_scratch` is a host-side stand-in, not a device address: resolve it once per device, with
+// that device current, and hand the result to the kernels.
+int static_scratch_address(int device, double** out) {
+  if (device < 0 || device >= STATIC_MAX_DEVICES) return PLK_ERR_CUDA;
+  if (g_static_scratch_ptr[device] == nullptr) {
+    int current = -1;
+    if (cudaGetDevice(&current) != cudaSuccess || current != device) return PLK_ERR_CUDA;
+    void* p = nullptr;
+    if (cudaGetSymbolAddress(&p, g_plk_static_scratch) != cudaSuccess || p == nullptr) return PLK_ERR_CUDA;
+    g_static_scratch_ptr[device] = static_cast<double*>(p);
+  }
+  *out = g_static_scratch_ptr[device];
+  return PLK_SUCCESS;
+}
+}  // namespace
+
+extern "C" int plk_root_log_likelihoods_static_device(plk_instance* in, int root, const int32_t* scale_idx, int scale_count,
+                                                      double* d_out_sum, double* d_out_site) {
+  if (in == nullptr || d_out_sum == nullptr) return PLK_ERR_OUT_OF_RANGE;
+  const Layout& L = in->L;
+  const plk_config& cfg = in->cfg;
+  if (scale_count < 0 || (scale_count > 0 && scale_idx == nullptr)) return PLK_ERR_OUT_OF_RANGE;
+  const int G = L.SP == 4 ? 1 : L.SP / 4;  // threads per pattern, 4 states each (as in root_impl)
+  const size_t n_blocks_sz = ((size_t)L.P * G + 127) / 128;
+  if (n_blocks_sz > (size_t)PLK_STATIC_SCRATCH_DOUBLES || scale_count > PLK_STATIC_SCALE_MAX)
+    return PLK_ERR_STATIC_SCRATCH_LIMIT;
+  const int n_blocks = (int)n_blocks_sz;
+  int rc = check_model_ready(in, false);
+  if (rc) return rc;
+  const void* rptr;
+  const void* pending;
+  int kind;
+  rc = operand_of(in, root, &rptr, &kind, &pending);
+  if (rc) return rc;
+  if (kind == KIND_STATES) return PLK_ERR_OUT_OF_RANGE;
+  for (int i = 0; i < scale_count; ++i) {
+    if (scale_idx[i] < 0 || scale_idx[i] >= cfg.scale_buffer_count) return PLK_ERR_OUT_OF_RANGE;
+    if (!in->scale_written[scale_idx[i]]) return PLK_ERR_UNINITIALIZED;
+  }
+  // the arena's device must be the current one (the binding keeps it current around every call)
+  cudaPointerAttributes pa;
+  if (cudaPointerGetAttributes(&pa, in->arena) != cudaSuccess) return PLK_ERR_CUDA;
+  double* bp = nullptr;
+  rc = static_scratch_address(pa.device, &bp);
+  if (rc) return rc;
+  // deferred rescaling: the root's own pending factor is not applied to the stored values: drop it from the list
+  const void* list[PLK_STATIC_SCALE_MAX];
+  int n_list = 0;
+  const int own = in->deferred ? in->post_pending_scale[root] : -1;
+  bool own_listed = false;
+  for (int i = 0; i < scale_count; ++i) {
+    if (scale_idx[i] == own && !own_listed) {
+      own_listed = true;
+      continue;
+    }
+    list[n_list++] = in->scale_ptr(scale_idx[i]);
+  }
+  if (own >= 0 && !own_listed) return PLK_ERR_UNSUPPORTED;
+  char *h = nullptr, *d = nullptr;
+  if (n_list > 0) {
+    rc = ring_alloc(in, (size_t)n_list * sizeof(void*), &h, &d);
+    if (rc) return rc;
+    std::memcpy(h, list, (size_t)n_list * sizeof(void*));
+    rc = copy_ring(in, h, d, (size_t)n_list * sizeof(void*));
+    if (rc) return rc;
+  }
+  const double* pi = in->at<double>(L.off_pi);
+  const double* cw = in->at<double>(L.off_catw);
+  const double* wt = in->at<double>(L.off_weights);
+  const void* const* dl = reinterpret_cast<const void* const*>(d);
+  if (in->f32) {
+    const float* r = static_cast<const float*>(rptr);
+    if (L.SP == 4) k_root<float, 4, 1><<<n_blocks, 128, 0, in->stream>>>(r, kind, L.P, L.C, pi, cw, dl, n_list, wt, d_out_site, bp);
+    else if (L.SP == 32) k_root<float, 32, 8><<<n_blocks, 128, 0, in->stream>>>(r, kind, L.P, L.C, pi, cw, dl, n_list, wt, d_out_site, bp);
+    else k_root<float, 64, 16><<<n_blocks, 128, 0, in->stream>>>(r, kind, L.P, L.C, pi, cw, dl, n_list, wt, d_out_site, bp);
+  } else {
+    const double* r = static_cast<const double*>(rptr);
+    if (L.SP == 4) k_root<double, 4, 1><<<n_blocks, 128, 0, in->stream>>>(r, kind, L.P, L.C, pi, cw, dl, n_list, wt, d_out_site, bp);
+    else if (L.SP == 32) k_root<double, 32, 8><<<n_blocks, 128, 0, in->stream>>>(r, kind, L.P, L.C, pi, cw, dl, n_list, wt, d_out_site, bp);
+    else k_root<double, 64, 16><<<n_blocks, 128, 0, in->stream>>>(r, kind, L.P, L.C, pi, cw, dl, n_list, wt, d_out_site, bp);
+  }
+  CHECK_LAUNCH(in);
+  k_sum_rows<<<1, 128, 0, in->stream>>>(bp, nullptr, n_blocks, n_blocks, d_out_sum);
+  CHECK_LAUNCH(in);
+  return PLK_SUCCESS;
+}

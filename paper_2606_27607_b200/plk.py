@@ -19,6 +19,8 @@ LIB_PATH = os.path.join(_HERE, "libplk.so")
 SUCCESS = 0
 ERR_GENERAL, ERR_OUT_OF_MEMORY, ERR_OUT_OF_RANGE, ERR_UNINITIALIZED = -1, -2, -3, -4
 ERR_UNSUPPORTED, ERR_FLOATING_POINT, ERR_CUDA, ERR_STOP_CODON = -5, -6, -7, -8
+ERR_STATIC_SCRATCH_LIMIT = -9
+STATIC_SCRATCH_DOUBLES, STATIC_SCALE_MAX = 8192, 2048
 FP64, FP32 = 0, 1
 FLAG_TENSOR_CORES, FLAG_NO_LEVEL_BATCH, FLAG_SITE_DERIVATIVES = 1, 2, 4
 FLAG_LEVEL_BATCH_ONLY, FLAG_PATTERN_WALK_ONLY, FLAG_NO_TMA = 8, 16, 32
@@ -72,6 +74,7 @@ _SIGNATURES = {
     "plk_cache_rate_products": (_I, [_P, _I, _P, _I]),
     "plk_root_log_likelihoods": (_I, [_P, _I, _P, _I, _P, _P]),
     "plk_root_log_likelihoods_device": (_I, [_P, _I, _P, _I, _P, _P]),
+    "plk_root_log_likelihoods_static_device": (_I, [_P, _I, _P, _I, _P, _P]),
     "plk_update_pre_partials": (_I, [_P, _I, _P, _I]),
     "plk_branch_derivatives": (_I, [_P, _I, _P, _P, _I, _P, _P]),
     "plk_pre_order_gradient": (_I, [_P, _I, _I, _P, _I, _P, _P]),
@@ -323,6 +326,13 @@ class Instance:
         sc = _i32(scale_idx)
         self._call("plk_root_log_likelihoods_device", root_buffer, _ptr(sc), sc.size, C.c_void_p(d_out_sum.data_ptr()),
                    None if d_out_site is None else C.c_void_p(d_out_site.data_ptr()))
+
+    def root_log_likelihoods_static_device(self, root_buffer, scale_idx, d_out_sum, d_out_site=None):
+        """plk_root_log_likelihoods_static_device: the same reduction with its scratch in the library's static device
+        array (no allocation; limits STATIC_SCRATCH_DOUBLES / STATIC_SCALE_MAX)."""
+        sc = _i32(scale_idx)
+        self._call("plk_root_log_likelihoods_static_device", root_buffer, _ptr(sc), sc.size,
+                   C.c_void_p(d_out_sum.data_ptr()), None if d_out_site is None else C.c_void_p(d_out_site.data_ptr()))
 
     def update_pre_partials(self, root_pre_buffer, ops):
         ops = np.ascontiguousarray(ops, dtype=PRE_OP_DTYPE)
