@@ -340,10 +340,7 @@ __global__ void __launch_bounds__(NT_THREADS, 4) k_pre4_lean(const DevPreItem* _
 // tiles of 32 R patterns a warp takes per launch: a CTA lives long enough to amortise its table set-up (item
 // descriptor -> matrix pointers -> table entries: dependent global loads), and the loads of tile t + 1 are in flight
 // while tile t is computed
-#ifndef PLK_TIPS_TPW
-#define PLK_TIPS_TPW 1
-#endif
-constexpr int NL_TIPS_TPW = PLK_TIPS_TPW;
+constexpr int NL_TIPS_TPW = 1;  // (2 and 4 tiles per warp with prefetch measured slower: fewer, longer CTAs fill tails worse)
 
 template <typename T>
 struct NlTipsTile {  // what a lane reads for its R patterns of one tile
