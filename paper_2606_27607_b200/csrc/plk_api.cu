@@ -584,10 +584,11 @@ int launch_pre4_lean(plk_instance* in, int cls, const DevPreItem* d_items, int n
       if (in->cfg.flags & PLK_FLAG_NO_TMA) return launch_pre4_lean_c<T, 2>(in, d_items, n, Q, site, first_launch);
       const Layout& L = in->L;
       const bool pdl = !(in->cfg.flags & PLK_FLAG_NO_PDL);
+      constexpr int TPW = NlTipsTpw<T>::V;
       const int n_tp = (L.P + 32 * NlRows<T>::R - 1) / (32 * NlRows<T>::R);
       for (int first = 0; first < n; first += 32768) {
         const int m = n - first < 32768 ? n - first : 32768;
-        dim3 grid((n_tp + NT_CW * NL_TIPS_TPW - 1) / (NT_CW * NL_TIPS_TPW), m);
+        dim3 grid((n_tp + NT_CW * TPW - 1) / (NT_CW * TPW), m);
         CU(launch_chain(k_grad4_tips<T>, grid, dim3(NT_CW * 32), 0, in->stream, pdl, d_items + first, L.P,
                         (long long)L.off_matrix_d - (long long)L.off_matrix, nuc_model(in, site),
                         in->at<double>(L.off_grad_partial), L.n_tiles, ((first_launch && first == 0) || !pdl) ? 1 : 0));
@@ -995,12 +996,12 @@ static int rebuild_rate_matrix(plk_instance* in, int eigen) {
   std::memcpy(h, &qt, sizeof(void*));
   rc = copy_ring(in, h, d, sizeof(void*));
   if (rc) return rc;
-  const size_t smem = (size_t)(2 * L.S * L.S + L.S) * 8;
+  const size_t smem = transition_smem(L.S);
   rc = by_precision(in, [&](auto tag) -> int {
     using T = decltype(tag);
     int r2 = opt_in_smem(k_transition<T>, smem);
     if (r2) return r2;
-    k_transition<T><<<1, 256, smem, in->stream>>>(in->eig_U(eigen), in->eig_Uinv(eigen), in->eig_lam(eigen), nullptr,
+    k_transition<T><<<dim3(1, 1), 256, smem, in->stream>>>(in->eig_U(eigen), in->eig_Uinv(eigen), in->eig_lam(eigen), nullptr,
                                                  nullptr, reinterpret_cast<void* const*>(d), in->eig_Q64(eigen), L.S,
                                                  L.SP, 1, 1);
     return PLK_SUCCESS;
@@ -1119,12 +1120,12 @@ static int update_matrices_impl(plk_instance* in, int eigen, const int32_t* matr
   }
   rc = copy_ring(in, h, d, bytes);
   if (rc) return rc;
-  const size_t smem = (size_t)(2 * L.S * L.S + L.C * L.S) * 8;
+  const size_t smem = transition_smem(L.S);
   rc = by_precision(in, [&](auto tag) -> int {
     using T = decltype(tag);
     int r2 = opt_in_smem(k_transition<T>, smem);
     if (r2) return r2;
-    k_transition<T><<<count, 256, smem, in->stream>>>(in->eig_U(eigen), in->eig_Uinv(eigen), in->eig_lam(eigen),
+    k_transition<T><<<dim3(count, L.C), 256, smem, in->stream>>>(in->eig_U(eigen), in->eig_Uinv(eigen), in->eig_lam(eigen),
                                                      in->at<double>(L.off_rates), d_t,
                                                      reinterpret_cast<void* const*>(d), nullptr, L.S, L.SP, L.C, 0);
     return PLK_SUCCESS;
@@ -1481,23 +1482,46 @@ static int pre_impl(plk_instance* in, int eigen, int root_pre, const plk_pre_op*
       }
   }
   const int n_items = (int)items.size();
+  // Both-tips items (class 2) read q_parent and write no partials: nothing in the pass depends on them, so all of them
+  // run as ONE launch after the last level instead of one small launch per level (a level's few cherries do not fill
+  // the GPU: 9 launches of 66 MB at configs[1]).  They are placed in a pseudo-level behind the real ones.  Not done
+  // when the list overwrites a buffer that an earlier op reads as its parent (the deferred read would see the new
+  // contents).
+  int n_lv = n_levels;
+  if (lean) {
+    bool war = false;
+    std::vector<char> read_as_parent(cfg.preorder_buffer_count, 0);
+    for (int i = 0; i < count && !war; ++i) {
+      if (ops[i].dest_pre >= 0 && read_as_parent[ops[i].dest_pre]) war = true;
+      read_as_parent[ops[i].parent_pre] = 1;
+    }
+    if (!war) {
+      bool any = false;
+      for (HostItem& hi : items)
+        if (hi.cls == 2) {
+          hi.level = n_levels;
+          any = true;
+        }
+      if (any) n_lv = n_levels + 1;
+    }
+  }
   std::vector<int> slot_parts(count > 0 ? count : 0, 0);  // partial sums per gradient slot (0: nothing written)
   if (n_items > 0) {
-    std::vector<int> level_start(n_levels + 1, 0);
+    std::vector<int> level_start(n_lv + 1, 0);
     for (const HostItem& hi : items) ++level_start[hi.level + 1];
-    for (int l = 0; l < n_levels; ++l) level_start[l + 1] += level_start[l];
+    for (int l = 0; l < n_lv; ++l) level_start[l + 1] += level_start[l];
     std::vector<int> fill(level_start.begin(), level_start.end() - 1);
     char *h, *d;
     rc = ring_alloc(in, (size_t)n_items * sizeof(DevPreItem), &h, &d);
     if (rc) return rc;
     DevPreItem* hit = reinterpret_cast<DevPreItem*>(h);
     const bool walk = L.SP == 4 && nuc_use_walk(in, n_items, n_levels, want_grad);
-    std::vector<int> class_start((size_t)n_levels * 5, 0);  // per level: first item of class 0..3, end
+    std::vector<int> class_start((size_t)n_lv * 5, 0);  // per level: first item of class 0..3, end
     if (walk) {
       for (int i = 0; i < n_items; ++i) hit[i] = items[i].it;  // list order (plk_nuc.cuh "walk")
     } else {  // by level, and inside a level by class
       for (const HostItem& hi : items) ++class_start[(size_t)hi.level * 5 + hi.cls + 1];
-      for (int l = 0; l < n_levels; ++l) {
+      for (int l = 0; l < n_lv; ++l) {
         class_start[(size_t)l * 5] = level_start[l];
         for (int k = 0; k < 4; ++k) class_start[(size_t)l * 5 + k + 1] += class_start[(size_t)l * 5 + k];
       }
@@ -1541,7 +1565,7 @@ static int pre_impl(plk_instance* in, int eigen, int root_pre, const plk_pre_op*
       if (rc) return rc;
       mark_parts(0, n_items);
     }
-    if (!walk && L.SP == 4 && class_start[(size_t)(n_levels - 1) * 5 + 3] > 0) {
+    if (!walk && L.SP == 4 && class_start[(size_t)(n_lv - 1) * 5 + 3] > 0) {
       // some items run on the class-specialised kernels: their compact-tip children read D = M Q (one 4 x 4 product
       // per matrix and category, every matrix buffer; unwritten buffers give unused garbage)
       rc = by_precision(in, [&](auto tag) -> int {
@@ -1555,7 +1579,7 @@ static int pre_impl(plk_instance* in, int eigen, int root_pre, const plk_pre_op*
       });
       if (rc) return rc;
     }
-    for (int l = 0; l < (walk ? 0 : n_levels); ++l) {
+    for (int l = 0; l < (walk ? 0 : n_lv); ++l) {
       bool first_launch = true;  // of this level: see launch_pre4_lean_c
       for (int k = 0; k < 3; ++k) {  // specialised classes
         const int c0 = class_start[(size_t)l * 5 + k], m = class_start[(size_t)l * 5 + k + 1] - c0;

@@ -359,21 +359,27 @@ __global__ void __launch_bounds__(128) k_root(const T* __restrict__ root, int ki
       lik += catw[c] * acc;
     }
   }
+  // the scale buffers of a pattern are shared out over its G lanes (configs[3]: 255 buffers x 4 categories per pattern)
+  int esum = 0;
+  if (p < P) {
+    for (int k = g; k < n_scales; k += G) {
+      if (SP == 4) {
+        esum += static_cast<const int16_t*>(scales[k])[p];
+      } else {
+        const T* mxs = static_cast<const T*>(scales[k]);
+        T m = T(0);
+        for (int c = 0; c < C; ++c) m = fmax(m, mxs[(size_t)c * P + p]);
+        esum += exp_of(m);
+      }
+    }
+  }
 #pragma unroll
-  for (int o = G / 2; o > 0; o >>= 1) lik += __shfl_xor_sync(0xffffffffu, lik, o);
+  for (int o = G / 2; o > 0; o >>= 1) {
+    lik += __shfl_xor_sync(0xffffffffu, lik, o);
+    esum += __shfl_xor_sync(0xffffffffu, esum, o);
+  }
   if (p < P) {
     if (g == 0) {
-      long esum = 0;
-      for (int k = 0; k < n_scales; ++k) {
-        if (SP == 4) {
-          esum += static_cast<const int16_t*>(scales[k])[p];
-        } else {
-          const T* mxs = static_cast<const T*>(scales[k]);
-          T m = T(0);
-          for (int c = 0; c < C; ++c) m = fmax(m, mxs[(size_t)c * P + p]);
-          esum += exp_of(m);
-        }
-      }
       const double ll = log(lik) + 0.6931471805599453094 * (double)esum;
       if (site != nullptr) site[p] = ll;
       term = weights[p] * ll;

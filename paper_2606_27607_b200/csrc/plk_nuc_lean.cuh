@@ -340,7 +340,12 @@ __global__ void __launch_bounds__(NT_THREADS, 4) k_pre4_lean(const DevPreItem* _
 // tiles of 32 R patterns a warp takes per launch: a CTA lives long enough to amortise its table set-up (item
 // descriptor -> matrix pointers -> table entries: dependent global loads), and the loads of tile t + 1 are in flight
 // while tile t is computed
-constexpr int NL_TIPS_TPW = 1;  // (2 and 4 tiles per warp with prefetch measured slower: fewer, longer CTAs fill tails worse)
+// (all both-tips items of a pass run as ONE launch, plk_api.cu, so long CTAs leave no tail: fp64 141 us at 4 tiles per
+// warp against 175 at one; the fp32 body with two rows per lane runs out of registers at 4: 140 registers, 3 CTAs / SM)
+template <typename T>
+struct NlTipsTpw {
+  static constexpr int V = sizeof(T) == 8 ? 4 : 1;
+};
 
 template <typename T>
 struct NlTipsTile {  // what a lane reads for its R patterns of one tile
@@ -372,7 +377,7 @@ template <typename T>
 __global__ void __launch_bounds__(NT_CW * 32) k_grad4_tips(const DevPreItem* __restrict__ items, int P, long long dmat_delta,
                                                            NucModel md, double* __restrict__ grad_partial, int n_part,
                                                            int wait_first) {
-  constexpr int C = NL_C, R = NlRows<T>::R, TPW = NL_TIPS_TPW;
+  constexpr int C = NL_C, R = NlRows<T>::R, TPW = NlTipsTpw<T>::V;
   __shared__ __align__(16) T tabA[2][C][5][4];  // [child][category][state z (4 = missing)][x]: M_k[x][z]; missing: 1
   __shared__ __align__(16) T tabD[2][C][5][4];  // D_k[x][z]; missing: 0 (Q . 1 = 0)
   if (wait_first) pdl_wait();  // launch chain: see k_pre4_lean
