@@ -282,12 +282,54 @@ __global__ void __launch_bounds__(TC_THREADS, 1) k_post_tc(const DevOp* __restri
 
   const int n_tiles = (P + TP - 1) / TP;
   const long long total = (long long)n_ops * C * n_tiles;
-  const long long per = (total + gridDim.x - 1) / gridDim.x;
-  const long long i0 = (long long)blockIdx.x * per;
-  const long long i1 = i0 + per < total ? i0 + per : total;
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  // This CTA's contiguous run of work items i = (operation, category, tile), tile fastest.  Items differ in cost by an
+  // order of magnitude -- a child given as compact states is a column gather, a child with partials a 64^3 contraction
+  // -- so the runs are cut by COST (2 + 3 per contracted child; measured at configs[2] fp64: 3.7 / 8.8 / 14 us per item
+  // with 0 / 1 / 2 contracted children), not by count: with equal counts the SMs of a level were active 65 % of the
+  // launch (profiles/r02_codon_post_tc_fp64.txt).
+  __shared__ long long s_run[2];
+  if (warp == 0) {
+    const long long unit = (long long)C * n_tiles;
+    auto weight = [&](int o) -> long long {
+      if (o >= n_ops) return 0;
+      int n = 0;
+#pragma unroll
+      for (int k = 0; k < 2; ++k) n += (ops[o].kind[k] == KIND_PARTIALS || ops[o].kind[k] == KIND_BCAST) ? 1 : 0;
+      return 2 + 3 * n;
+    };
+    long long tot = 0;
+    for (int base = 0; base < n_ops; base += 32) {
+      long long w = weight(base + lane);
+#pragma unroll
+      for (int d = 16; d > 0; d >>= 1) w += __shfl_xor_sync(0xffffffffu, w, d);
+      tot += w;
+    }
+    tot *= unit;
+    const long long pos[2] = {tot / gridDim.x * blockIdx.x + tot % gridDim.x * blockIdx.x / gridDim.x,
+                              blockIdx.x + 1 == gridDim.x ? tot
+                                                          : tot / gridDim.x * (blockIdx.x + 1) + tot % gridDim.x * (blockIdx.x + 1) / gridDim.x};
+    if (lane < 2 && pos[lane] >= tot) s_run[lane] = total;
+    long long prefix = 0;
+    for (int base = 0; base < n_ops; base += 32) {
+      const long long w = weight(base + lane), mine = w * unit;
+      long long incl = mine;
+#pragma unroll
+      for (int d = 1; d < 32; d <<= 1) {
+        const long long v = __shfl_up_sync(0xffffffffu, incl, d);
+        if (lane >= d) incl += v;
+      }
+      const long long lo = prefix + incl - mine, hi = prefix + incl;
+#pragma unroll
+      for (int e = 0; e < 2; ++e)
+        if (w > 0 && lo <= pos[e] && pos[e] < hi) s_run[e] = (long long)(base + lane) * unit + (pos[e] - lo) / w;
+      prefix += __shfl_sync(0xffffffffu, incl, 31);
+    }
+  }
+  __syncthreads();
+  const long long i0 = s_run[0], i1 = s_run[1];
   if (i0 >= i1) return;
 
-  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int r = lane >> 2, c4 = lane & 3, m0 = warp * K::MT;
 
   auto issue = [&](long long i, int st) {
