@@ -213,8 +213,10 @@ def measure_device(wl, precision, flags, steps, warmup, peaks, sampler=None, dev
         ev = sh.local
         assert ev is not None, "empty shard: fewer pattern tiles than ranks"
     else:
-        ev = Evaluator(wl, precision=prec, flags=flags, device=device)
+        # a stream of its own: plk_evaluate* replays its cached CUDA graph only on a capturable (non-default) stream
+        ev = Evaluator(wl, precision=prec, flags=flags, device=device, stream=torch.cuda.Stream(device))
         ev.make_device_io()
+        torch.cuda.synchronize()  # set-up ran on torch's current stream; everything below on the instance's
     stream = ev.inst.stream
     d_site = torch.zeros(ev.wl.n_patterns, dtype=torch.float64, device=device) if keep_site else None
 
@@ -248,6 +250,22 @@ def measure_device(wl, precision, flags, steps, warmup, peaks, sampler=None, dev
     clocks = sampler.stop() if sampler is not None else None
     launches = ev.inst.kernel_launch_count() - l0
     total_ms = marks[0][0].elapsed_time(marks[-1][5])
+    # the same evaluation as ONE library call (plk_evaluate_device: eager, captured, then one CUDA-graph launch per use)
+    one_call = None
+    if sh is None:
+        for _ in range(4):
+            ev.step_evaluate()
+        torch.cuda.synchronize()
+        l1 = ev.inst.kernel_launch_count()
+        g0, g1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        g0.record(stream)
+        for _ in range(steps):
+            ev.step_evaluate()
+        g1.record(stream)
+        torch.cuda.synchronize()
+        one_call = {"ms_per_step": g0.elapsed_time(g1) / steps,
+                    "launches_per_step": (ev.inst.kernel_launch_count() - l1) / steps,
+                    "what": "plk_evaluate_device: steps 1-6 in one call, replayed from the cached CUDA graph"}
     phase = np.zeros(5)
     for s in range(steps):
         for i in range(5):
@@ -263,6 +281,7 @@ def measure_device(wl, precision, flags, steps, warmup, peaks, sampler=None, dev
         sys.path.insert(0, os.path.join(ROOT, "tests"))
         import oracle_runner as orc
 
+        ev.step_post()
         ev.inst.root_log_likelihoods_device(ev.tree.root, ev.scale_idx, ev.d_logl, d_site)
         torch.cuda.synchronize()
         site = {"client": (d_site.cpu().numpy(), logl, grad)}
@@ -295,14 +314,15 @@ def measure_device(wl, precision, flags, steps, warmup, peaks, sampler=None, dev
         "launches": int(launches), "logL": logl, "grad": grad, "site": site,
         "grad_norm": float(np.linalg.norm(grad)),
         "finite": bool(np.isfinite(logl) and np.all(np.isfinite(grad))),
-        "alg": alg, "clocks": clocks,
+        "alg": alg, "clocks": clocks, "one_call": one_call,
     }
     return res, ev
 
 
 def measure_e2e(ev, wl, steps, warmup):
-    """Same evaluation through the host-pointer C-ABI calls: every step uploads the tip states (pinned host memory)
-    and the branch lengths, and reads logL and the gradient back to the host."""
+    """Same evaluation through the host-pointer C-ABI calls a client makes per HMC step: every step uploads the tip
+    states (pinned host memory, one pitched copy: plk_set_all_tip_states_u8) and hands HOST branch lengths to
+    plk_evaluate, which returns logL and the gradient to the HOST (one upload, the cached graph, one download)."""
     import torch
 
     N, P = wl.tree.n_tips, wl.n_patterns
@@ -312,15 +332,10 @@ def measure_e2e(ev, wl, steps, warmup):
     t = np.ascontiguousarray(np.asarray(wl.tree.branch_length)[ev.matrix_idx])
 
     def one():
-        for k in range(N):
-            ev.inst.set_tip_states_u8(k, tips[k])
-        ev.inst.update_transition_matrices(0, ev.matrix_idx, t)
-        ev.inst.update_partials(ev.ops)
-        logl, _ = ev.inst.root_log_likelihoods(wl.tree.root, ev.scale_idx, want_site=False)
-        g, _ = ev.inst.pre_order_gradient(0, wl.tree.root, ev.pre_ops)
-        return logl, g
+        ev.inst.set_all_tip_states_u8(tips)
+        return ev.inst.evaluate(0, ev.matrix_idx, t, ev.ops, wl.tree.root, ev.scale_idx, wl.tree.root, ev.pre_ops)
 
-    for _ in range(max(1, min(warmup, 3))):
+    for _ in range(max(3, min(warmup, 5))):
         one()
     torch.cuda.synchronize()
     t0 = time.perf_counter()
@@ -547,6 +562,7 @@ def run_extras(peaks, steps, warmup, mm):
             "post_hbm_frac_of_8TBs": res["post_gbs"] / HBM_NOMINAL_GBS, "pre_hbm_frac_of_8TBs": res["pre_gbs"] / HBM_NOMINAL_GBS,
             "post_alg_tflops": res["post_tflops"], "pre_alg_tflops": res["pre_tflops"],
             "launches_per_step": res["launches"] / steps, "finite": res["finite"],
+            "one_call_ms_per_step": round(res["one_call"]["ms_per_step"], 4) if res["one_call"] else None,
         }
         if flags & 1 and mm is not None:
             codon.append(codon_roofline(name, wl, prec, "mma.sync" if (prec == "fp64" or flags & 64) else "tcgen05",
@@ -574,7 +590,8 @@ def run_sweep(peaks, steps, warmup):
                 "gradient_evals_per_s": res["gradient_evals_per_s"],
                 "post_hbm_frac": round(res["post_gbs"] / peaks["hbm_gbs"], 4),
                 "pre_hbm_frac": round(res["pre_gbs"] / peaks["hbm_gbs"], 4),
-                "launches_per_step": res["launches"] / steps, "finite": res["finite"]})
+                "launches_per_step": res["launches"] / steps, "finite": res["finite"],
+                "one_call_ms_per_step": round(res["one_call"]["ms_per_step"], 4)})
             del wl
     print(json.dumps({"sweep": "configs[4] HKY fp32", "unit": UNIT, "steps": steps, "points": points}))
 
@@ -649,6 +666,12 @@ def main():
     torch.cuda.synchronize()
     res, ev = measure_device(wl, args.precision, flags, args.steps, args.warmup, peaks, sampler, device=device,
                              keep_site=want_parity, shard=(rank, world, dist) if sharded_run else None)
+    # headline: the whole evaluation as the ONE call a client makes (plk_evaluate_device, graph replay); the per-phase
+    # times come from the pass above, in which the four steps are issued as separate calls with events between them
+    separate_ms = res["ms_per_step"]
+    if res["one_call"] is not None:
+        res["ms_per_step"] = res["one_call"]["ms_per_step"]
+        res["launches"] = int(round(res["one_call"]["launches_per_step"] * args.steps))
     ms = torch.tensor([res["ms_per_step"]], dtype=torch.float64, device=device)
     if dist is not None:
         dist.barrier()
@@ -719,8 +742,14 @@ def main():
         "clocks": res["clocks"],
         "e2e": {"value": updates_all / float(e2e_t[0]), "unit": UNIT, "h2d_bytes_per_step": h2d,
                 "d2h_bytes_per_step": d2h, "ms_per_step": float(e2e_t[0]) * 1e3,
-                "what": "tip states (pinned uint8, plk_set_tip_states_u8) + branch lengths uploaded, logL + gradient downloaded, every step"},
+                "what": "every step: tip states uploaded from pinned host memory (plk_set_all_tip_states_u8), host branch "
+                        "lengths in and host logL + gradient out through plk_evaluate"},
         "gpu_launches": res["launches"],
+        "timed_path": ("plk_evaluate_device (one call per evaluation, cached CUDA graph)" if res["one_call"] is not None
+                       else "four calls per evaluation"),
+        "separate_calls_ms_per_step": separate_ms,
+        "phase_ms_note": "phase_ms and the roofline come from a pass with the four steps issued as separate calls and "
+                         "CUDA events between them (separate_calls_ms_per_step); ms_per_step / value time the one-call path",
         "roofline": roofline,
     }
     if mm is not None:

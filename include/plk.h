@@ -165,6 +165,12 @@ PLK_API int plk_set_tip_states(plk_instance* inst, int tip, const int32_t* state
  * evaluation when its alignment changes (bench.py's end-to-end leg). */
 PLK_API int plk_set_tip_states_u8(plk_instance* inst, int tip, const uint8_t* states);
 
+/* Tips 0 .. count-1 at once: `states` is HOST memory [count][P] bytes (row t = tip t, values >= S: missing).  Tips
+ * that sit in consecutive compact slots -- all of them when they were first set in index order -- travel as ONE pitched
+ * asynchronous copy instead of `count` copies (configs[1]: 128 x 100 KB).  Same ownership exception and no
+ * synchronisation as plk_set_tip_states_u8.  _OUT_OF_RANGE if one of the tips was set as partials before. */
+PLK_API int plk_set_all_tip_states_u8(plk_instance* inst, const uint8_t* states, int count);
+
 /* Tip `tip` as partials [P][S], the same for every category (e.g. one-hot rows, all-ones rows for missing). */
 PLK_API int plk_set_tip_partials(plk_instance* inst, int tip, const double* partials);
 

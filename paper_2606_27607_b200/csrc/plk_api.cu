@@ -931,6 +931,51 @@ int plk_set_tip_states_u8(plk_instance* in, int tip, const uint8_t* states) {
   return PLK_SUCCESS;
 }
 
+int plk_set_all_tip_states_u8(plk_instance* in, const uint8_t* states, int count) {
+  if (in == nullptr || states == nullptr) return PLK_ERR_OUT_OF_RANGE;
+  if (count < 0 || count > in->cfg.tip_count) return PLK_ERR_OUT_OF_RANGE;
+  const Layout& L = in->L;
+  int fresh = 0;
+  for (int tip = 0; tip < count; ++tip) {
+    if (in->post_slot[tip] >= 0 && in->post_kind[tip] != KIND_STATES) return PLK_ERR_OUT_OF_RANGE;  // bound as partials
+    if (in->post_slot[tip] < 0) ++fresh;
+  }
+  if (in->next_compact_slot + fresh > L.compact_slots) return PLK_ERR_OUT_OF_MEMORY;
+  for (int tip = 0; tip < count; ++tip)
+    if (in->post_slot[tip] < 0) {
+      in->post_slot[tip] = in->next_compact_slot++;
+      in->post_kind[tip] = KIND_STATES;
+      ++in->binding_epoch;
+    }
+  // runs of tips that sit in consecutive compact slots travel as ONE pitched copy (usually a single run: all tips)
+  for (int first = 0; first < count;) {
+    int last = first;
+    while (last + 1 < count && in->post_slot[last + 1] == in->post_slot[last] + 1) ++last;
+    // a pitched host -> device copy runs at a third of the PCIe rate (one DMA descriptor per row: 0.75 ms for 12.8 MB);
+    // so: one LINEAR copy of as many rows as the staging area holds, then a device-side pitched copy into the slots
+    const size_t rows_per_chunk = L.compact_bytes == (size_t)L.P ? (size_t)(last - first + 1) : L.stage_bytes / (size_t)L.P;
+    if (rows_per_chunk == 0) return PLK_ERR_OUT_OF_MEMORY;
+    for (int r0 = first; r0 <= last; r0 += (int)rows_per_chunk) {
+      const size_t rows = (size_t)(last - r0 + 1) < rows_per_chunk ? (size_t)(last - r0 + 1) : rows_per_chunk;
+      const uint8_t* src = states + (size_t)r0 * L.P;
+      if (L.compact_bytes == (size_t)L.P) {
+        CU(cudaMemcpyAsync(in->post_ptr(r0), src, rows * L.P, cudaMemcpyHostToDevice, in->stream));
+      } else {
+        char* stage = in->arena + L.off_stage;
+        CU(cudaMemcpyAsync(stage, src, rows * L.P, cudaMemcpyHostToDevice, in->stream));
+        CU(cudaMemcpy2DAsync(in->post_ptr(r0), L.compact_bytes, stage, (size_t)L.P, (size_t)L.P, rows,
+                             cudaMemcpyDeviceToDevice, in->stream));
+      }
+    }
+    first = last + 1;
+  }
+  for (int tip = 0; tip < count; ++tip) {
+    in->post_written[tip] = 1;
+    in->post_pending_scale[tip] = -1;
+  }
+  return PLK_SUCCESS;
+}
+
 int plk_set_tip_partials(plk_instance* in, int tip, const double* partials) {
   if (in == nullptr || partials == nullptr) return PLK_ERR_OUT_OF_RANGE;
   if (tip < 0 || tip >= in->cfg.tip_count) return PLK_ERR_OUT_OF_RANGE;

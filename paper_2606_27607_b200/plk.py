@@ -58,6 +58,7 @@ _SIGNATURES = {
     "plk_error_string": (C.c_char_p, [_I]),
     "plk_set_tip_states": (_I, [_P, _I, _P]),
     "plk_set_tip_states_u8": (_I, [_P, _I, _P]),
+    "plk_set_all_tip_states_u8": (_I, [_P, _P, _I]),
     "plk_set_tip_partials": (_I, [_P, _I, _P]),
     "plk_set_partials": (_I, [_P, _I, _P]),
     "plk_set_pattern_weights": (_I, [_P, _P]),
@@ -268,6 +269,13 @@ class Instance:
         if s.size != self.P:
             raise ValueError("states must have pattern_count entries")
         self._call("plk_set_tip_states_u8", tip, _ptr(s))
+
+    def set_all_tip_states_u8(self, states):
+        """plk_set_all_tip_states_u8: `states` a contiguous uint8 array [n_tips][P] (pinned memory stays valid until the
+        next synchronising call); one pitched copy for tips in consecutive compact slots."""
+        if states.dtype != np.uint8 or not states.flags["C_CONTIGUOUS"] or states.ndim != 2 or states.shape[1] != self.P:
+            raise ValueError("states must be a C-contiguous uint8 array [n_tips][pattern_count]")
+        self._call("plk_set_all_tip_states_u8", _ptr(states), states.shape[0])
 
     def set_tip_partials(self, tip, partials):
         self._call("plk_set_tip_partials", tip, _ptr(_f64(partials, self.P * self.S)))

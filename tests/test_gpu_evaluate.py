@@ -133,3 +133,39 @@ def test_default_stream_runs_eagerly_and_errors_propagate():
                              ev.scale_idx, wl.tree.root, ev.pre_ops)
     finally:
         ev.close()
+
+
+@pytest.mark.parametrize("n_pat", [3001, 2048])  # staged pitched copy / one linear copy (P a multiple of the slot pitch)
+def test_set_all_tip_states_u8_matches_per_tip_upload(n_pat):
+    """plk_set_all_tip_states_u8: the whole alignment in one call.  Uploading the columns in reversed order must give
+    the reversed per-pattern log-likelihoods of the per-tip upload (patterns are independent), which the
+    other tests compare with the oracle."""
+    wl = workloads.config(1, n_tips=24, n_patterns=n_pat)
+    ref = orc.evaluate(wl, gradient=False)
+    ev = Evaluator(wl, precision=plk.FP64, eigen=orc.oracle_eigen(wl))
+    try:
+        logl, site = ev.log_likelihood()
+        pc.check_logl(site, logl, ref, plk.FP64)
+        rev = np.ascontiguousarray(np.minimum(wl.tip_states, 255).astype(np.uint8)[:, ::-1])
+        ev.inst.set_all_tip_states_u8(rev)
+        ev.inst.set_pattern_weights(wl.pattern_weights[::-1].copy())
+        logl2, site2 = ev.log_likelihood()
+        assert np.array_equal(site2, site[::-1])
+        assert abs(logl2 - logl) <= 1e-12 * abs(logl)
+        # a prefix of the tips only: the others keep their states
+        fwd = np.ascontiguousarray(np.minimum(wl.tip_states, 255).astype(np.uint8))
+        ev.inst.set_all_tip_states_u8(fwd[:10])
+        for k in range(10, wl.tree.n_tips):
+            ev.inst.set_tip_states_u8(k, fwd[k])
+        ev.inst.set_pattern_weights(wl.pattern_weights)
+        logl3, site3 = ev.log_likelihood()
+        assert np.array_equal(site3, site) and logl3 == logl
+    finally:
+        ev.close()
+    ev = Evaluator(wl, precision=plk.FP64, tips_as_partials=True)
+    try:
+        with pytest.raises(plk.PlkError) as e:  # tips bound as partials cannot become compact states
+            ev.inst.set_all_tip_states_u8(fwd)
+        assert e.value.status == plk.ERR_OUT_OF_RANGE
+    finally:
+        ev.close()
