@@ -178,7 +178,10 @@ __global__ void __launch_bounds__(NT_THREADS, 4) k_pre4_lean(const DevPreItem* _
   }
   // ---- consumers: lane = 8 g + pl takes category g of patterns warp * 8 + pl + 32 u, u < R
   const int g = lane >> 3, pl = lane & 7;
-  const double cw = md.catw[g], cwr = cw * md.catr[g];
+  // category sums and num / den in the working precision (fp32 instances: the double versions of the three products,
+  // five shuffles and the division were a tenth of the instructions of an issue-bound kernel; 1e-7 per pattern is far
+  // inside the fp32 tolerance); the weighted pattern sum stays fp64
+  const T cw = (T)md.catw[g], cwr = (T)(md.catw[g] * md.catr[g]);
   for (int j = 0; j < J; ++j) {
     const int s = j % NT_NS;
     unsigned char* stage = nt_smem + (size_t)s * St::BYTES;
@@ -303,16 +306,16 @@ __global__ void __launch_bounds__(NT_THREADS, 4) k_pre4_lean(const DevPreItem* _
         }
       }
       // ---- category sums: den on every lane, num_0 on the lanes of g = 0, num_1 on those of g = 1
-      double den = cw * (double)dd[u], m0 = cwr * (double)n0, m1 = cwr * (double)n1;
+      T den = cw * dd[u], m0 = cwr * n0, m1 = cwr * n1;
       den += __shfl_xor_sync(0xffffffffu, den, 16);
       m0 += __shfl_xor_sync(0xffffffffu, m0, 16);
       m1 += __shfl_xor_sync(0xffffffffu, m1, 16);
       den += __shfl_xor_sync(0xffffffffu, den, 8);
       const bool odd = g & 1;
-      const double got = __shfl_xor_sync(0xffffffffu, odd ? m0 : m1, 8);
-      const double num = (odd ? m1 : m0) + got;
+      const T got = __shfl_xor_sync(0xffffffffu, odd ? m0 : m1, 8);
+      const T num = (odd ? m1 : m0) + got;
       if (live[u] && g < 2) {
-        const double ratio = num / den;
+        const double ratio = (double)(num / den);
         if (md.site_out != nullptr) md.site_out[(size_t)it.slot[g] * P + p[u]] = ratio;
         contrib += reinterpret_cast<const double*>(stage + St::OFF_WTS)[r[u]] * ratio;
       }
@@ -380,6 +383,12 @@ __global__ void __launch_bounds__(NT_CW * 32) k_grad4_tips(const DevPreItem* __r
   constexpr int C = NL_C, R = NlRows<T>::R, TPW = NlTipsTpw<T>::V;
   __shared__ __align__(16) T tabA[2][C][5][4];  // [child][category][state z (4 = missing)][x]: M_k[x][z]; missing: 1
   __shared__ __align__(16) T tabD[2][C][5][4];  // D_k[x][z]; missing: 0 (Q . 1 = 0)
+  T scw[C], scwr[C];
+#pragma unroll
+  for (int c = 0; c < C; ++c) {
+    scw[c] = (T)md.catw[c];
+    scwr[c] = (T)(md.catw[c] * md.catr[c]);
+  }
   if (wait_first) pdl_wait();  // launch chain: see k_pre4_lean
   pdl_trigger();
   const DevPreItem& it = items[blockIdx.y];
@@ -414,7 +423,7 @@ __global__ void __launch_bounds__(NT_CW * 32) k_grad4_tips(const DevPreItem* __r
     double contrib[2] = {0.0, 0.0};
 #pragma unroll
     for (int u = 0; u < R; ++u) {
-      double den = 0.0, num0 = 0.0, num1 = 0.0;
+      T den = T(0), num0 = T(0), num1 = T(0);  // working precision, as in k_pre4_lean
 #pragma unroll
       for (int c = 0; c < C; ++c) {
         T a0[4], a1[4], d0[4], d1[4];
@@ -430,13 +439,12 @@ __global__ void __launch_bounds__(NT_CW * 32) k_grad4_tips(const DevPreItem* __r
           n0 = fma(u0, d0[x], n0);
           n1 = fma(u1, d1[x], n1);
         }
-        const double cw = md.catw[c], cwr = cw * md.catr[c];
-        den = fma(cw, (double)dd, den);
-        num0 = fma(cwr, (double)n0, num0);
-        num1 = fma(cwr, (double)n1, num1);
+        den = fma(scw[c], dd, den);
+        num0 = fma(scwr[c], n0, num0);
+        num1 = fma(scwr[c], n1, num1);
       }
       if (b.p[u] < P) {
-        const double w = md.weights[b.p[u]], r0 = num0 / den, r1 = num1 / den;
+        const double w = md.weights[b.p[u]], r0 = (double)(num0 / den), r1 = (double)(num1 / den);
         if (md.site_out != nullptr) {
           md.site_out[(size_t)slot0 * P + b.p[u]] = r0;
           md.site_out[(size_t)slot1 * P + b.p[u]] = r1;
