@@ -313,7 +313,11 @@ __global__ void __launch_bounds__(NUC_THREADS) k_post4_walk(const DevOp* __restr
     }
     const DevOp op = sOp[cur];
     int chunk = warp < total_warps ? warp : n_chunks;
-    if (sizeof(T) == 4) {  // two chunks per pass (see post4_cells)
+    if (sizeof(T) == 4) {  // three / two chunks per pass (see post4_cells)
+      for (; chunk + 2 * total_warps < n_chunks; chunk += 3 * total_warps) {
+        const int pp[3] = {chunk * Mp::PPW + pl, (chunk + total_warps) * Mp::PPW + pl, (chunk + 2 * total_warps) * Mp::PPW + pl};
+        post4_cells<T, C, 3>(op, sM[cur], P, pp, g);
+      }
       for (; chunk + total_warps < n_chunks; chunk += 2 * total_warps) {
         const int pp[2] = {chunk * Mp::PPW + pl, (chunk + total_warps) * Mp::PPW + pl};
         post4_cells<T, C, 2>(op, sM[cur], P, pp, g);

@@ -51,7 +51,8 @@ using pre::tmem_st_wait;
 using pre::umma_ta;
 
 constexpr int EPI_W = 8, PROD_W = 4, N_W = EPI_W + PROD_W + 1;
-constexpr int THREADS = N_W * 32;               // 416
+constexpr int META_W = N_W;                     // warp 13: per-row scalars of the next rounds (see the kernel)
+constexpr int THREADS = (N_W + 1) * 32;         // 448
 constexpr int STAGERS = (EPI_W + PROD_W) * 32;  // 384 threads stage the matrices of a segment
 constexpr uint32_t PLANE_A = 128 * 64 * 4;   // one plane (hi or lo) of a stacked [M_k; D_k] operand: 128 rows
 constexpr uint32_t OFF_MAT0 = 0, OFF_MAT1 = 2 * PLANE_A;        // [M_k; D_k] hi, lo  (class 1: raw tip tables at MAT1)
@@ -60,7 +61,8 @@ constexpr uint32_t OFF_XT = OFF_MT1 + 2 * M_PLANE;              // producers' tr
 constexpr uint32_t OFF_QS = OFF_XT + PROD_W * 2048;             // epilogue staging (q_m in, q_k out), 2 KB per warp
 constexpr uint32_t OFF_RED = OFF_QS + EPI_W * 2048;             // floats [2 parity][3][TP]: sub-1 partial sums
 constexpr uint32_t OFF_SMX = OFF_RED + 2 * 3 * TP * 4;          // floats [2 parity][2 child][TP]: sub-1 row maxima
-constexpr uint32_t OFF_ITEM = OFF_SMX + 2 * 2 * TP * 4;          // the segment's item descriptor (one L2 round trip per segment)
+constexpr uint32_t OFF_EXP = OFF_SMX + 2 * 2 * TP * 4;           // ints [2 parity][3][TP]: pending exponents of q_m, x_0, x_1 (class 1: tip state)
+constexpr uint32_t OFF_ITEM = OFF_EXP + 2 * 3 * TP * 4;          // the segment's item descriptor (one L2 round trip per segment)
 constexpr uint32_t OFF_BAR2 = OFF_ITEM + 128;
 constexpr uint32_t SMEM_USED2 = OFF_BAR2 + 256;
 static_assert(sizeof(DevPreItem) <= 128, "item descriptor slot");
@@ -76,7 +78,11 @@ enum { B_XFULL_A = 0,  // first tile of the round stored (producers)
        B_REGFREE,      // the second child's step A has run: its X region is free (commit)
        B_QREAD,        // the epilogue has read the round's q_k: the region they sat in is free
        B_QREAD1,       // class 1 only: rounds alternate between B_QREAD (even) and B_QREAD1 (odd), see the producers
-       B_AFULL0, B_AFULL1, B_UFULL0, B_UFULL1, B_QFULL, B_MATFULL, B_MATFREE, B_TMEM };
+       B_AFULL0, B_AFULL1, B_UFULL0, B_UFULL1, B_QFULL, B_MATFULL, B_MATFREE,
+       B_EXPFULL, B_EXPFULL1,  // the round's pending exponents are in shared memory (meta warp): even / odd rounds, so that
+                               // the writer may run two rounds ahead of the readers without wrapping a phase parity
+       B_EXPFREE, B_EXPFREE1,  // the epilogue has read them (even / odd rounds)
+       B_TMEM };
 constexpr uint32_t T_REG = 128, T_AB0 = 256, T_AB1 = 384;  // X region r at T_REG * r: hi 0..63, lo 64..127
 
 // byte deltas from a transition-matrix buffer to its derived copies (all inside the instance arena)
@@ -232,6 +238,10 @@ __global__ void __launch_bounds__(THREADS, 1)
     mbar_init(cx.barrier(B_QFULL), 1);
     mbar_init(cx.barrier(B_MATFULL), 1);
     mbar_init(cx.barrier(B_MATFREE), 1);
+    mbar_init(cx.barrier(B_EXPFULL), 1);
+    mbar_init(cx.barrier(B_EXPFULL1), 1);
+    mbar_init(cx.barrier(B_EXPFREE), EPI_W);
+    mbar_init(cx.barrier(B_EXPFREE1), EPI_W);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   if (warp == N_W - 1) {
@@ -314,6 +324,68 @@ __global__ void __launch_bounds__(THREADS, 1)
       if (CLS == 0) step_b(1, par, 1);
       umma_commit(cx.barrier(B_QFULL));
       if (ui + 1 == cx.n_rounds || tile == 0) umma_commit(cx.barrier(B_MATFREE));  // last round of its segment
+    }
+  } else if (warp == META_W) {
+    // ===== meta warp: pending per-pattern exponents (deferred rescaling) of q_m, child 0, child 1 -- class 1: the tip
+    // state of child 1 -- of every row of a round, up to two rounds ahead, handed to the epilogue through shared memory.
+    // (The epilogue warps used to load them themselves: twelve scattered DRAM loads per thread whose scoreboard every
+    // later wait of the warp inherited -- 4.5 k of the 24 k cycles of a round; on the producer warps they delayed the
+    // tile stores.  This warp has nothing else to wait for.)
+    int* sexp = reinterpret_cast<int*>(tc5v_smem_raw + (cx.smem - smem_u32(tc5v_smem_raw)) + OFF_EXP);
+    auto ldv = [](const float* m) {
+      float v;
+      asm volatile("ld.global.nc.f32 %0, [%1];" : "=f"(v) : "l"(m));
+      return v;
+    };
+    // the first four categories of src[.][pp] as independent loads (all of a round's loads are issued before the first
+    // of them is used); further categories, if any, in a tail loop
+    auto load4 = [&](const void* src, int pp) {
+      float4 v = make_float4(0.f, 0.f, 0.f, 0.f);
+      if (src != nullptr && pp < P) {
+        const float* m = static_cast<const float*>(src) + pp;
+        v.x = ldv(m);
+        if (C > 1) v.y = ldv(m + (size_t)P);
+        if (C > 2) v.z = ldv(m + 2 * (size_t)P);
+        if (C > 3) v.w = ldv(m + 3 * (size_t)P);
+      }
+      return v;
+    };
+    auto finish4 = [&](const float4 r4, const void* src, int pp) {
+      float v = fmaxf(fmaxf(r4.x, r4.y), fmaxf(r4.z, r4.w));
+      if (C > 4 && src != nullptr && pp < P)
+        for (int cc = 4; cc < C; ++cc) v = fmaxf(v, static_cast<const float*>(src)[(size_t)cc * P + pp]);
+      return exp_of(v);
+    };
+    Cur k = cx.first();
+    for (uint32_t ui = 0; ui < cx.n_rounds; ++ui, cx.advance(k)) {
+      const uint32_t par = ui & 1;
+      const DevPreItem& t = items[k.item];
+      const void* src[3] = {t.qm_scale, t.p_scale[0], CLS == 0 ? t.p_scale[1] : nullptr};
+      float4 raw[4][3];
+      int z[4];
+#pragma unroll
+      for (int j = 0; j < 4; ++j) {
+        const int pp = k.tile * TP + lane + 32 * j;
+#pragma unroll
+        for (int e = 0; e < (CLS == 0 ? 3 : 2); ++e) raw[j][e] = load4(src[e], pp);
+        z[j] = 64;
+        if (CLS == 1 && pp < P) asm volatile("ld.global.nc.u8 %0, [%1];" : "=r"(z[j]) : "l"(static_cast<const uint8_t*>(t.p[1]) + pp));
+      }
+      int ex[4][3];
+#pragma unroll
+      for (int j = 0; j < 4; ++j) {
+        const int pp = k.tile * TP + lane + 32 * j;
+        ex[j][0] = finish4(raw[j][0], src[0], pp);
+        ex[j][1] = finish4(raw[j][1], src[1], pp);
+        ex[j][2] = CLS == 0 ? finish4(raw[j][2], src[2], pp) : z[j];
+      }
+      if (ui > 1) mbar_wait(cx.barrier(par ? B_EXPFREE1 : B_EXPFREE), ((ui >> 1) + 1) & 1);  // round ui - 2 was read
+#pragma unroll
+      for (int j = 0; j < 4; ++j)
+#pragma unroll
+        for (int e = 0; e < 3; ++e) sexp[(par * 3 + e) * TP + lane + 32 * j] = ex[j][e];
+      __syncwarp();
+      if (lane == 0) mbar_arrive(cx.barrier(par ? B_EXPFULL1 : B_EXPFULL));
     }
   } else {
     const int st = (int)threadIdx.x;  // stager index 0..383 (warps 0..11)
@@ -465,49 +537,24 @@ __global__ void __launch_bounds__(THREADS, 1)
           qv[i] = (p0 + 32 * quarter + rr < P) ? ldg_nc(src + (size_t)rr * SP64 + 4 * j) : make_float4(0.f, 0.f, 0.f, 0.f);
         }
       };
-      // Pending per-pattern exponents (deferred rescaling) of q_m, child 0, child 1 and the tip state of this thread's
-      // row: the per-category maxima are fetched ONE ROUND AHEAD into registers (rq, rx0, rx1: float4 = categories 0..3)
-      // and reduced when the round starts, so their latency is off the critical path.
-      float4 rq = make_float4(0.f, 0.f, 0.f, 0.f), rx0 = rq, rx1 = rq;
-      int zraw = 64;
-      auto load4 = [&](const void* src, int pp) {
-        float4 v = make_float4(0.f, 0.f, 0.f, 0.f);
-        if (src != nullptr && pp < P) {
-          const float* m = static_cast<const float*>(src) + pp;
-          v.x = __ldg(m);
-          if (C > 1) v.y = __ldg(m + (size_t)P);
-          if (C > 2) v.z = __ldg(m + 2 * (size_t)P);
-          if (C > 3) v.w = __ldg(m + 3 * (size_t)P);
-        }
-        return v;
-      };
-      auto load_raw = [&](const DevPreItem& t, int pp) {
-        rq = load4(t.qm_scale, pp);
-        rx0 = load4(t.p_scale[0], pp);
-        if (CLS == 0) rx1 = load4(t.p_scale[1], pp);
-        if (CLS == 1) zraw = pp < P ? (int)__ldg(static_cast<const uint8_t*>(t.p[1]) + pp) : 64;
-      };
-      auto finish4 = [&](const float4 r4, const void* src, int pp) {
-        float v = fmaxf(fmaxf(r4.x, r4.y), fmaxf(r4.z, r4.w));
-        if (C > 4 && src != nullptr && pp < P)
-          for (int cc = 4; cc < C; ++cc) v = fmaxf(v, static_cast<const float*>(src)[(size_t)cc * P + pp]);
-        return exp_of(v);
-      };
+      const int* sexp = reinterpret_cast<const int*>(tc5v_smem_raw + (cx.smem - smem_u32(tc5v_smem_raw)) + OFF_EXP);
       Cur cur = cx.first();
       segment_start(cur);  // (the first round always opens a segment)
       load_qm(*sit, cur.c, cur.tile * TP, 0);
-      load_raw(*sit, cur.tile * TP + row);
       for (uint32_t ui = 0; ui < cx.n_rounds; ++ui) {
         const uint32_t par = ui & 1;
         if (ui > 0 && cur.tile == 0) segment_start(cur);
         const DevPreItem& it = *sit;
         const int c = cur.c, p0 = cur.tile * TP, p = p0 + row;
         const Cur nxt = cx.next(cur);
-        const Pow2Pair<float> fq = pow2_pair(-finish4(rq, it.qm_scale, p), 0.f);
-        const Pow2Pair<float> fx0 = pow2_pair(-finish4(rx0, it.p_scale[0], p), 0.f);
-        const Pow2Pair<float> fx1 = pow2_pair(-(CLS == 0 ? finish4(rx1, it.p_scale[1], p) : 0), 0.f);
-        const int z1 = zraw >= S ? 64 : zraw;  // class 1: compact state of the tip child (missing -> the summed row 64)
-        if (ui + 1 < cx.n_rounds) load_raw(item_of(nxt.item), nxt.tile * TP + row);
+        mbar_wait(cx.barrier(par ? B_EXPFULL1 : B_EXPFULL), (ui >> 1) & 1);  // this round's pending exponents (long since there)
+        const int e_q = sexp[(par * 3 + 0) * TP + row], e_x0 = sexp[(par * 3 + 1) * TP + row], e_2 = sexp[(par * 3 + 2) * TP + row];
+        const Pow2Pair<float> fq = pow2_pair(-e_q, 0.f);
+        const Pow2Pair<float> fx0 = pow2_pair(-e_x0, 0.f);
+        const Pow2Pair<float> fx1 = pow2_pair(-(CLS == 0 ? e_2 : 0), 0.f);
+        const int z1 = (CLS == 1 && e_2 < S) ? e_2 : 64;  // class 1: compact state of the tip child (missing -> the summed row 64)
+        __syncwarp();
+        if (lane == 0) mbar_arrive(cx.barrier(par ? B_EXPFREE1 : B_EXPFREE));
         // the usual case: every pending exponent fits ONE power-of-two factor (warp-uniform test)
         const bool one_factor = __all_sync(0xffffffffu, fq.f2 == 1.f && fx0.f2 == 1.f && fx1.f2 == 1.f);
         float dd = 0.f, n0 = 0.f, n1 = 0.f;
