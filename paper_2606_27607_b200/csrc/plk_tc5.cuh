@@ -149,16 +149,17 @@ __device__ __forceinline__ float4 ldg_nc(const float* p) {
                : "l"(p));
   return v;
 }
-__device__ __forceinline__ float tf32_rna(float x) {
-  uint32_t r;
-  asm("cvt.rna.tf32.f32 %0, %1;" : "=r"(r) : "f"(x));
-  return __uint_as_float(r);
-}
+// Split x = hi + lo for the three-product TF32 scheme with two plain ALU operations instead of two conversions and a
+// subtraction: hi = x with the 13 low mantissa bits cleared (a valid TF32 number whatever the tensor pipe does with low
+// bits), lo = x - hi exactly (<= 2^-10 |x|, 13 significant bits of which the pipe keeps 11: residual 2^-21 |x|, against
+// 2^-22 with round-to-nearest conversions -- both far inside the 1e-4 bar; the dropped lo.lo term is 2^-20).  The
+// conversion unit runs at a fraction of the ALU rate and every operand element and every U value went through it twice.
+__device__ __forceinline__ float tf32_hi(float x) { return __uint_as_float(__float_as_uint(x) & 0xffffe000u); }
 __device__ __forceinline__ void split4(const float4 v, float4& h, float4& l) {
-  h.x = tf32_rna(v.x); l.x = tf32_rna(v.x - h.x);
-  h.y = tf32_rna(v.y); l.y = tf32_rna(v.y - h.y);
-  h.z = tf32_rna(v.z); l.z = tf32_rna(v.z - h.z);
-  h.w = tf32_rna(v.w); l.w = tf32_rna(v.w - h.w);
+  h.x = tf32_hi(v.x); l.x = v.x - h.x;
+  h.y = tf32_hi(v.y); l.y = v.y - h.y;
+  h.z = tf32_hi(v.z); l.z = v.z - h.z;
+  h.w = tf32_hi(v.w); l.w = v.w - h.w;
 }
 __device__ __forceinline__ void sts128(uint32_t addr, const float4 v) {
   asm volatile("st.shared.v4.f32 [%0], {%1,%2,%3,%4};" ::"r"(addr), "f"(v.x), "f"(v.y), "f"(v.z), "f"(v.w) : "memory");

@@ -517,10 +517,10 @@ __global__ void __launch_bounds__(THREADS_PRE, 1)
             }
             const float u0 = qs * s1, u1 = qs * s0;
             dd = fmaf(u0, s0, dd);
-            u0h[j] = tf32_rna(u0);
-            u0l[j] = tf32_rna(u0 - u0h[j]);
-            u1h[j] = tf32_rna(u1);
-            u1l[j] = tf32_rna(u1 - u1h[j]);
+            u0h[j] = tf32_hi(u0);
+            u0l[j] = u0 - u0h[j];
+            u1h[j] = tf32_hi(u1);
+            u1l[j] = u1 - u1h[j];
           }
           tmem_st8(lane_tm + T_U0 + 8 * sub, u0h);
           tmem_st8(lane_tm + T_U0 + 64 + 8 * sub, u0l);

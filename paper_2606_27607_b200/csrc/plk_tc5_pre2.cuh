@@ -623,11 +623,11 @@ __global__ void __launch_bounds__(THREADS, 1)
               dd = fmaf(u0, s0, dd);
               n0 = fmaf(u0, t0, n0);
               n1 = fmaf(u1, t1, n1);
-              u0h[j] = tf32_rna(u0);
-              u0l[j] = tf32_rna(u0 - u0h[j]);
+              u0h[j] = tf32_hi(u0);
+              u0l[j] = u0 - u0h[j];
               if (CLS == 0) {
-                u1h[j] = tf32_rna(u1);
-                u1l[j] = tf32_rna(u1 - u1h[j]);
+                u1h[j] = tf32_hi(u1);
+                u1l[j] = u1 - u1h[j];
               }
             }
             tmem_st8(c0 + 8 * e, u0h);       // U_0 hi over a_0, lo over b_0
