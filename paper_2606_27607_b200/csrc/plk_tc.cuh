@@ -75,14 +75,11 @@ __device__ __forceinline__ void tc_mma(float (&d)[4], const uint32_t (&a)[4], co
       : "+f"(d[0]), "+f"(d[1]), "+f"(d[2]), "+f"(d[3])
       : "r"(a[0]), "r"(a[1]), "r"(a[2]), "r"(a[3]), "r"(b[0]), "r"(b[1]));
 }
-__device__ __forceinline__ uint32_t tc_tf32(float x) {
-  uint32_t r;
-  asm("cvt.rna.tf32.f32 %0, %1;" : "=r"(r) : "f"(x));
-  return r;
-}
+// x = hi + lo with hi = x, low 13 mantissa bits cleared, lo = x - hi exactly: two ALU operations instead of two
+// conversions and a subtraction (see tf32_hi in plk_tc5.cuh: the conversion unit is slow and was the bottleneck)
 __device__ __forceinline__ void tc_split(float x, uint32_t& hi, uint32_t& lo) {
-  hi = tc_tf32(x);
-  lo = tc_tf32(x - __uint_as_float(hi));
+  hi = __float_as_uint(x) & 0xffffe000u;
+  lo = __float_as_uint(x - __uint_as_float(hi));
 }
 
 // ---- staging ---------------------------------------------------------------------------------------------------
@@ -156,10 +153,10 @@ __device__ __forceinline__ void tc_split_matrix(float* sM) {
     const int r = idx >> 4, c4 = (idx & 15) * 4;
     float4 v = *reinterpret_cast<float4*>(sM + r * LD + c4);
     float4 h, l;
-    h.x = __uint_as_float(tc_tf32(v.x)); l.x = v.x - h.x;
-    h.y = __uint_as_float(tc_tf32(v.y)); l.y = v.y - h.y;
-    h.z = __uint_as_float(tc_tf32(v.z)); l.z = v.z - h.z;
-    h.w = __uint_as_float(tc_tf32(v.w)); l.w = v.w - h.w;
+    h.x = __uint_as_float(__float_as_uint(v.x) & 0xffffe000u); l.x = v.x - h.x;
+    h.y = __uint_as_float(__float_as_uint(v.y) & 0xffffe000u); l.y = v.y - h.y;
+    h.z = __uint_as_float(__float_as_uint(v.z) & 0xffffe000u); l.z = v.z - h.z;
+    h.w = __uint_as_float(__float_as_uint(v.w) & 0xffffe000u); l.w = v.w - h.w;
     *reinterpret_cast<float4*>(sM + r * LD + c4) = h;
     *reinterpret_cast<float4*>(sM + SP64 * LD + r * LD + c4) = l;
   }

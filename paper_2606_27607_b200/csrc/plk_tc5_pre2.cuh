@@ -94,26 +94,38 @@ struct MatDeltas {
 __global__ void __launch_bounds__(256) k_prep_matrices64(const float* __restrict__ mats, const float* __restrict__ Q,
                                                          float* __restrict__ out_d, float* __restrict__ out_t,
                                                          float* __restrict__ out_dt) {
-  __shared__ float sM[64][65];
-  __shared__ float sQ[64][65];
+  // operands widened ONCE on the way into shared memory (the product loop used to convert both operands of every
+  // FMA: half a million conversions per block on the slow conversion unit)
+  __shared__ double sM[64][64];                             // broadcast reads only: no padding needed
+  float(*sD)[65] = reinterpret_cast<float(*)[65]>(sM);     // D, written over M once every product is done
   const float* M = mats + (size_t)blockIdx.x * 4096;
   for (int i = threadIdx.x; i < 4096; i += 256) {
-    sM[i >> 6][i & 63] = M[i];
-    sQ[i >> 6][i & 63] = Q[i];
+    const float v = M[i];
+    sM[i >> 6][i & 63] = (double)v;
+    out_t[(size_t)blockIdx.x * 4096 + (i & 63) * 64 + (i >> 6)] = v;
   }
   __syncthreads();
-  for (int i = threadIdx.x; i < 4096; i += 256) {
-    const int r = i >> 6, col = i & 63;
-    double acc = 0.0;  // fp64 accumulation: the product is rounded once
-#pragma unroll 8
-    for (int k = 0; k < 64; ++k) acc = fma((double)sM[r][k], (double)sQ[k][col], acc);
-    out_d[(size_t)blockIdx.x * 4096 + i] = (float)acc;
-    out_t[(size_t)blockIdx.x * 4096 + col * 64 + r] = sM[r][col];
+  // thread (col = tid & 63, g = tid >> 6) forms D[r][col] for its 16 rows r = g + 4 i at once: one element of Q
+  // (converted once) serves 16 FMAs; the M operands are broadcast reads from shared memory; fp64 accumulation
+  const int col = threadIdx.x & 63, g = threadIdx.x >> 6;
+  double acc[16];
+#pragma unroll
+  for (int i = 0; i < 16; ++i) acc[i] = 0.0;
+#pragma unroll 4
+  for (int k = 0; k < 64; ++k) {
+    const double qk = (double)__ldg(Q + k * 64 + col);
+#pragma unroll
+    for (int i = 0; i < 16; ++i) acc[i] = fma(sM[g + 4 * i][k], qk, acc[i]);
   }
   __syncthreads();
-  for (int i = threadIdx.x; i < 4096; i += 256) sM[i >> 6][i & 63] = out_d[(size_t)blockIdx.x * 4096 + i];
+#pragma unroll
+  for (int i = 0; i < 16; ++i) {
+    const float d = (float)acc[i];
+    sD[g + 4 * i][col] = d;
+    out_d[(size_t)blockIdx.x * 4096 + (g + 4 * i) * 64 + col] = d;
+  }
   __syncthreads();
-  for (int i = threadIdx.x; i < 4096; i += 256) out_dt[(size_t)blockIdx.x * 4096 + i] = sM[i & 63][i >> 6];
+  for (int i = threadIdx.x; i < 4096; i += 256) out_dt[(size_t)blockIdx.x * 4096 + i] = sD[i & 63][i >> 6];
 }
 
 // (item, category, tile) of a round, advanced incrementally (no division in the round loops)
