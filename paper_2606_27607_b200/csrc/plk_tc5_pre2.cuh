@@ -722,16 +722,17 @@ __global__ void __launch_bounds__(THREADS, 1)
 
 // ---------------------------------------------------------------------------------------------------------------
 // both children compact tips: den_c = sum_s q_m[s] M_0[s][z0] M_1[s][z1], num_0 = sum_s q_m[s] M_1[s][z1] D_0[s][z0],
-// num_1 likewise.  One warp per pattern at a time: lanes hold 2 states each, q_m rows are read as whole 256-byte
-// lines, the table rows z are contiguous in shared memory; blockIdx.y = item, blockIdx.x = chunk of G_TP patterns.
+// num_1 likewise.  HALF A WARP per pattern: lane l of the half holds states 4 l .. 4 l + 3, so a pattern's q_m row is one
+// coalesced 256-byte request and the four table rows of its tip states are read as whole contiguous rows (128-bit
+// loads, no bank conflicts), followed by a 4-step shuffle reduction of the three sums.  (The first version gave a lane
+// a whole pattern: its 4 x 64 table values were gathered with scalar loads from rows that differ from lane to lane --
+// 4-way bank conflicts on top of 1 KB of shared-memory traffic per 256 B of q_m: 1.9 TB/s.)
+// blockIdx.x = chunk of G_TP patterns, blockIdx.y = item, blockIdx.z = category.
 // ---------------------------------------------------------------------------------------------------------------
 constexpr int G_THREADS = 256, G_TP = 1024;
-constexpr int G_LD = 65;  // table row stride (floats): lanes reading one column of different rows hit different banks
+constexpr int G_LD = 64;  // table row stride (floats): rows are read whole
 constexpr size_t G_SMEM = (size_t)4 * 65 * G_LD * 4;  // M_0^T, D_0^T, M_1^T, D_1^T with the summed row 64
 
-// grid: x = chunk of G_TP patterns, y = item, z = category (the per-category results go to the scratch anyway).
-// A lane owns a pattern: its q_m row is read as 16 float4 (whole lines over the 8 loads that share one), the four
-// table values of a state come from shared memory (row = tip state, padded stride), sums stay in registers.
 __global__ void __launch_bounds__(G_THREADS) k_grad64_tips(const DevPreItem* __restrict__ items, int P, int S, int C,
                                                            MatDeltas md, float* __restrict__ scratch) {
   extern __shared__ __align__(16) float g_tab[];  // [4][65][G_LD]
@@ -740,11 +741,10 @@ __global__ void __launch_bounds__(G_THREADS) k_grad64_tips(const DevPreItem* __r
   const int p_begin = blockIdx.x * G_TP, p_end = min(P, p_begin + G_TP);
   const size_t CP = (size_t)C * P;
   for (int i = threadIdx.x; i < 4 * 1024; i += G_THREADS) {
-    const int tb = i >> 10, e = i & 1023, z = e >> 4, ch = e & 15;
+    const int tb = i >> 10, e = i & 1023;  // e = 16 z + chunk: row z, four states
     const char* base = static_cast<const char*>(it.mat[tb >> 1]) + ((tb & 1) ? md.dt : md.t);
     const float4 v = ldg_nc(reinterpret_cast<const float*>(base) + (size_t)c * 4096 + 4 * e);
-    float* dst = g_tab + (tb * 65 + z) * G_LD + 4 * ch;
-    dst[0] = v.x; dst[1] = v.y; dst[2] = v.z; dst[3] = v.w;
+    *reinterpret_cast<float4*>(g_tab + tb * 65 * G_LD + 4 * e) = v;
   }
   __syncthreads();
   {
@@ -759,34 +759,60 @@ __global__ void __launch_bounds__(G_THREADS) k_grad64_tips(const DevPreItem* __r
   float* s1 = scratch + (size_t)it.slot[1] * 2 * CP + (size_t)c * P;
   const uint8_t* z0p = static_cast<const uint8_t*>(it.p[0]);
   const uint8_t* z1p = static_cast<const uint8_t*>(it.p[1]);
-#pragma unroll 1
-  for (int p = p_begin + threadIdx.x; p < p_end; p += G_THREADS) {
-    int z0 = z0p[p], z1 = z1p[p];
-    z0 = z0 >= S ? 64 : z0;
-    z1 = z1 >= S ? 64 : z1;
-    const float* a0 = g_tab + (0 * 65 + z0) * G_LD;
-    const float* b0 = g_tab + (1 * 65 + z0) * G_LD;
-    const float* a1 = g_tab + (2 * 65 + z1) * G_LD;
-    const float* b1 = g_tab + (3 * 65 + z1) * G_LD;
-    const float4* q4 = reinterpret_cast<const float4*>(qm + (size_t)p * SP64);
-    float dd = 0.f, n0 = 0.f, n1 = 0.f;
-#pragma unroll 4
-    for (int j = 0; j < 16; ++j) {
-      const float4 q = __ldg(q4 + j);
-      const float qv[4] = {q.x, q.y, q.z, q.w};
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, half = lane >> 4, l = lane & 15;
+  // a warp takes batches of 32 consecutive patterns: in step i its halves take patterns 2 i and 2 i + 1 of the batch;
+  // lane (half, l) keeps the sums of step l, so that after 16 steps the batch is stored with coalesced requests
+  for (int base = p_begin + 32 * warp; base < p_end; base += 32 * (G_THREADS / 32)) {
+    const int pz = base + lane;  // this lane's pattern for the coalesced state loads / result stores
+    int z0 = 64, z1 = 64;
+    if (pz < p_end) {
+      z0 = z0p[pz];
+      z1 = z1p[pz];
+      z0 = z0 >= S ? 64 : z0;
+      z1 = z1 >= S ? 64 : z1;
+    }
+    const int zz = z0 | (z1 << 8);
+    float vd[16], v0[16], v1[16];  // the three partial sums of the 16 steps (registers: the loops are unrolled)
 #pragma unroll
-      for (int e = 0; e < 4; ++e) {
-        const int s = 4 * j + e;
-        const float u0 = qv[e] * a1[s], u1 = qv[e] * a0[s];
-        dd = fmaf(u0, a0[s], dd);
-        n0 = fmaf(u0, b0[s], n0);
-        n1 = fmaf(u1, b1[s], n1);
+    for (int i = 0; i < 16; ++i) {
+      const int src = 2 * i + half, p = base + src;
+      const int y = __shfl_sync(0xffffffffu, zz, src), y0 = y & 255, y1 = y >> 8;
+      float4 q = make_float4(0.f, 0.f, 0.f, 0.f);
+      if (p < p_end) q = ldg_nc(qm + (size_t)p * SP64 + 4 * l);
+      const float4 a0 = *reinterpret_cast<const float4*>(g_tab + (0 * 65 + y0) * G_LD + 4 * l);
+      const float4 b0 = *reinterpret_cast<const float4*>(g_tab + (1 * 65 + y0) * G_LD + 4 * l);
+      const float4 a1 = *reinterpret_cast<const float4*>(g_tab + (2 * 65 + y1) * G_LD + 4 * l);
+      const float4 b1 = *reinterpret_cast<const float4*>(g_tab + (3 * 65 + y1) * G_LD + 4 * l);
+      const float u0x = q.x * a1.x, u0y = q.y * a1.y, u0z = q.z * a1.z, u0w = q.w * a1.w;
+      const float u1x = q.x * a0.x, u1y = q.y * a0.y, u1z = q.z * a0.z, u1w = q.w * a0.w;
+      vd[i] = fmaf(u0x, a0.x, fmaf(u0y, a0.y, fmaf(u0z, a0.z, u0w * a0.w)));
+      v0[i] = fmaf(u0x, b0.x, fmaf(u0y, b0.y, fmaf(u0z, b0.z, u0w * b0.w)));
+      v1[i] = fmaf(u1x, b1.x, fmaf(u1y, b1.y, fmaf(u1z, b1.z, u1w * b1.w)));
+    }
+    // sums over the 16 lanes of a half for all 16 steps at once: a reduce-scatter (8 + 4 + 2 + 1 exchanges per
+    // quantity instead of 16 x 4), after which lane l holds the complete sums of step l in element 0
+#pragma unroll
+    for (int w = 8; w >= 1; w >>= 1) {
+      const bool up = (l & w) != 0;
+#pragma unroll
+      for (int i = 0; i < w; ++i) {
+        const float gd = __shfl_xor_sync(0xffffffffu, up ? vd[i] : vd[i + w], w);
+        const float g0 = __shfl_xor_sync(0xffffffffu, up ? v0[i] : v0[i + w], w);
+        const float g1 = __shfl_xor_sync(0xffffffffu, up ? v1[i] : v1[i + w], w);
+        vd[i] = (up ? vd[i + w] : vd[i]) + gd;
+        v0[i] = (up ? v0[i + w] : v0[i]) + g0;
+        v1[i] = (up ? v1[i + w] : v1[i]) + g1;
       }
     }
-    s0[p] = n0;
-    s0[CP + p] = dd;
-    s1[p] = n1;
-    s1[CP + p] = dd;
+    const float kd = vd[0], k0 = v0[0], k1 = v1[0];
+    // lane (half, l) holds pattern base + 2 l + half
+    const int po = base + 2 * l + half;
+    if (po < p_end) {
+      s0[po] = k0;
+      s0[CP + po] = kd;
+      s1[po] = k1;
+      s1[CP + po] = kd;
+    }
   }
 }
 
