@@ -1640,7 +1640,7 @@ static int pre_impl(plk_instance* in, int eigen, int root_pre, const plk_pre_op*
           else if (k == 1)
             rc = tc5::pre2::launch_class<1>(in->stream, dit + c0, m, L.P, L.S, L.C, mdl, scr, in->sm_count, &in->launches);
           else
-            rc = tc5::pre2::launch_tips(in->stream, dit + c0, m, L.P, L.S, L.C, mdl, scr, &in->launches);
+            rc = tc5::pre2::launch_tips(in->stream, dit + c0, m, L.P, L.S, L.C, mdl, scr, in->sm_count, &in->launches);
           if (rc) return rc;
           for (int i = c0; i < c0 + m; ++i) {
             fin_slots.push_back(hit[i].slot[0]);

@@ -729,12 +729,12 @@ __global__ void __launch_bounds__(THREADS, 1)
 // 4-way bank conflicts on top of 1 KB of shared-memory traffic per 256 B of q_m: 1.9 TB/s.)
 // blockIdx.x = chunk of G_TP patterns, blockIdx.y = item, blockIdx.z = category.
 // ---------------------------------------------------------------------------------------------------------------
-constexpr int G_THREADS = 256, G_TP = 1024;
+constexpr int G_THREADS = 256;  // patterns per block: chosen by the launcher (tables are re-staged per block)
 constexpr int G_LD = 64;  // table row stride (floats): rows are read whole
 constexpr size_t G_SMEM = (size_t)4 * 65 * G_LD * 4;  // M_0^T, D_0^T, M_1^T, D_1^T with the summed row 64
 
 __global__ void __launch_bounds__(G_THREADS) k_grad64_tips(const DevPreItem* __restrict__ items, int P, int S, int C,
-                                                           MatDeltas md, float* __restrict__ scratch) {
+                                                           MatDeltas md, float* __restrict__ scratch, int G_TP) {
   extern __shared__ __align__(16) float g_tab[];  // [4][65][G_LD]
   const DevPreItem& it = items[blockIdx.y];
   const int c = blockIdx.z;
@@ -868,13 +868,16 @@ inline int launch_class(cudaStream_t stream, const DevPreItem* d_items, int n, i
 }
 
 inline int launch_tips(cudaStream_t stream, const DevPreItem* d_items, int n, int P, int S, int C, MatDeltas md,
-                       float* scratch, int64_t* launches) {
+                       float* scratch, int sm_count, int64_t* launches) {
   if (cudaFuncSetAttribute(k_grad64_tips, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)G_SMEM) != cudaSuccess)
     return PLK_ERR_CUDA;
+  // patterns per block: as many as still give every SM a few blocks (a block stages 66 KB of tables first)
+  int tp = 4096;
+  while (tp > 512 && (long long)((P + tp - 1) / tp) * n * C < 4LL * sm_count) tp >>= 1;
   for (int first = 0; first < n; first += 32768) {
     const int m = n - first < 32768 ? n - first : 32768;
-    dim3 grid((P + G_TP - 1) / G_TP, m, C);
-    k_grad64_tips<<<grid, G_THREADS, G_SMEM, stream>>>(d_items + first, P, S, C, md, scratch);
+    dim3 grid((P + tp - 1) / tp, m, C);
+    k_grad64_tips<<<grid, G_THREADS, G_SMEM, stream>>>(d_items + first, P, S, C, md, scratch, tp);
     if (cudaGetLastError() != cudaSuccess) return PLK_ERR_CUDA;
     ++*launches;
   }
