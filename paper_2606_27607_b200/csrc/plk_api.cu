@@ -1170,7 +1170,7 @@ static int update_matrices_impl(plk_instance* in, int eigen, const int32_t* matr
     using T = decltype(tag);
     int r2 = opt_in_smem(k_transition<T>, smem);
     if (r2) return r2;
-    k_transition<T><<<dim3(count, L.C), 256, smem, in->stream>>>(in->eig_U(eigen), in->eig_Uinv(eigen), in->eig_lam(eigen),
+    k_transition<T><<<dim3(count, L.C), L.S <= 8 ? 32 : 256, smem, in->stream>>>(in->eig_U(eigen), in->eig_Uinv(eigen), in->eig_lam(eigen),
                                                      in->at<double>(L.off_rates), d_t,
                                                      reinterpret_cast<void* const*>(d), nullptr, L.S, L.SP, L.C, 0);
     return PLK_SUCCESS;

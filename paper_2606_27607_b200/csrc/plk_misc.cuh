@@ -24,42 +24,55 @@ __global__ void __launch_bounds__(256) k_transition(const double* __restrict__ U
                                                     double* __restrict__ out64, int S, int SP, int C, int mode) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   const int NS = (S + 3) / 4, LD = 4 * NS;  // strips per row, padded row length of U^-1
-  double* sV = reinterpret_cast<double*>(smem_raw);  // [S][LD]  U^-1[k][j], zero padded (rows stay 32-byte aligned)
+  double* sV = reinterpret_cast<double*>(smem_raw);  // [S][LD]  U^-1[k][.], zero padded; within a row the columns are
+                                                     // stored as [strip js: cols 4js, 4js+1] x NS, then [cols 4js+2, 4js+3] x NS,
+                                                     // so that the lanes of a quarter warp read consecutive 16-byte chunks
   double* sW = sV + S * LD;                          // [S][S]   U[i][k] f[k]
   double* sF = sW + S * S;                           // [S]
   const int c = blockIdx.y;
   const double tb = mode == 0 ? t[blockIdx.x] : 0.0;
   for (int k = threadIdx.x; k < S; k += blockDim.x) sF[k] = mode == 0 ? exp(lam[k] * (rates[c] * tb)) : lam[k];
   for (int i = threadIdx.x; i < S * LD; i += blockDim.x) {
-    const int k = i / LD, j = i - k * LD;
-    sV[i] = j < S ? Uinv[k * S + j] : 0.0;
+    const int k = i / LD, j = i - k * LD;  // column j of row k -> strip j / 4, element j % 4
+    const int js = j >> 2, e = j & 3;
+    sV[k * LD + (e >> 1) * 2 * NS + 2 * js + (e & 1)] = j < S ? Uinv[k * S + j] : 0.0;
   }
   __syncthreads();
   for (int i = threadIdx.x; i < S * S; i += blockDim.x) sW[i] = U[i] * sF[i % S];
   __syncthreads();
   T* out = static_cast<T*>(mats[blockIdx.x]) + (size_t)c * SP * SP;
-  for (int idx = threadIdx.x; idx < S * NS; idx += blockDim.x) {
-    const int i = idx / NS, j0 = 4 * (idx - i * NS);
-    const double* w = sW + i * S;
-    const double* v = sV + j0;
-    double a0 = 0.0, a1 = 0.0, a2 = 0.0, a3 = 0.0;
+  const int NR = (S + 1) / 2;  // row pairs: a thread owns rows 2 ip, 2 ip + 1 x four columns (8 FMAs per two 32-byte loads)
+  for (int idx = threadIdx.x; idx < NR * NS; idx += blockDim.x) {
+    const int ip = idx / NS, js = idx - ip * NS, i0 = 2 * ip, i1 = i0 + 1 < S ? i0 + 1 : i0, j0 = 4 * js;
+    const double* w0 = sW + i0 * S;
+    const double* w1 = sW + i1 * S;
+    const double* v = sV + 2 * js;
+    double a[2][4] = {{0.0, 0.0, 0.0, 0.0}, {0.0, 0.0, 0.0, 0.0}};
 #pragma unroll 4
     for (int k = 0; k < S; ++k) {
-      const double wk = w[k];
+      const double x0 = w0[k], x1 = w1[k];
       const double2 v01 = *reinterpret_cast<const double2*>(v + k * LD);
-      const double2 v23 = *reinterpret_cast<const double2*>(v + k * LD + 2);
-      a0 = fma(wk, v01.x, a0);
-      a1 = fma(wk, v01.y, a1);
-      a2 = fma(wk, v23.x, a2);
-      a3 = fma(wk, v23.y, a3);
+      const double2 v23 = *reinterpret_cast<const double2*>(v + k * LD + 2 * NS);
+      a[0][0] = fma(x0, v01.x, a[0][0]);
+      a[0][1] = fma(x0, v01.y, a[0][1]);
+      a[0][2] = fma(x0, v23.x, a[0][2]);
+      a[0][3] = fma(x0, v23.y, a[0][3]);
+      a[1][0] = fma(x1, v01.x, a[1][0]);
+      a[1][1] = fma(x1, v01.y, a[1][1]);
+      a[1][2] = fma(x1, v23.x, a[1][2]);
+      a[1][3] = fma(x1, v23.y, a[1][3]);
     }
-    const double acc[4] = {a0, a1, a2, a3};
 #pragma unroll
-    for (int e = 0; e < 4; ++e)
-      if (j0 + e < S) {
-        out[(size_t)i * SP + j0 + e] = (T)acc[e];
-        if (out64 != nullptr) out64[(size_t)c * S * S + i * S + j0 + e] = acc[e];
-      }
+    for (int r = 0; r < 2; ++r) {
+      const int i = i0 + r;
+      if (i >= S) break;
+#pragma unroll
+      for (int e = 0; e < 4; ++e)
+        if (j0 + e < S) {
+          out[(size_t)i * SP + j0 + e] = (T)a[r][e];
+          if (out64 != nullptr) out64[(size_t)c * S * S + i * S + j0 + e] = a[r][e];
+        }
+    }
   }
 }
 
