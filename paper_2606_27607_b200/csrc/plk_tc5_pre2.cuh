@@ -35,9 +35,15 @@
 //     the first child's step A of round r + 1.  No tile store sits on the critical path.
 // TMEM (512 columns): region 0 = 0..127, region 1 = 128..255 (X_k hi | lo, later q_0 | q_1), [a_0|b_0] halves
 // 256..383, [a_1|b_1] halves 384..511.
-// Roles (13 warps): 0-7 epilogue (warp = quarter + 4 sub: TMEM lanes 32 quarter.., 16 of the 32 states of a half),
+// Roles (14 warps): 0-7 epilogue (warp = quarter + 4 sub: TMEM lanes 32 quarter.., 16 of the 32 states of a half),
 // 8-11 producers (warp w owns pattern rows 32 (w - 8)..; the next tile is always in registers and the ones after it
-// are prefetched into L2), 12 MMA issue + TMEM allocation.
+// are prefetched into L2), 12 MMA issue + TMEM allocation, 13 "meta": the per-row pending exponents (deferred
+// rescaling) and tip states of the next two rounds, handed to the epilogue through shared memory.
+// Round 2 measurements that shaped it (clock64 traces of one CTA, configs[3]): (i) the epilogue warps used to load
+// those per-row scalars themselves -- twelve scattered DRAM loads per thread whose scoreboard every later wait of the
+// warp inherited: 4.5 k of a round's 24 k cycles; (ii) the hi / lo split went through cvt.rna.tf32 twice per element
+// in producers and epilogue, and the conversion unit was the bottleneck of both: hi is now the value with its 13 low
+// mantissa bits masked off and lo one exact subtraction (tf32_hi, plk_tc5.cuh).  Together: 8.53 -> 6.50 ms per pass.
 #pragma once
 #include "plk_tc5_pre.cuh"
 
