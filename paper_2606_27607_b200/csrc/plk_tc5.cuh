@@ -39,7 +39,8 @@ namespace tc5 {
 
 constexpr int TP = 128;                    // patterns per tile = MMA M
 constexpr int EPI_WARPS = 8, PROD_WARPS = 8, N_WARPS = EPI_WARPS + PROD_WARPS + 1;
-constexpr int THREADS = N_WARPS * 32;      // 544
+constexpr int META_WARP = N_WARPS;         // warp 17: pending exponents of the next items' rows (see the kernel)
+constexpr int THREADS = (N_WARPS + 1) * 32;  // 576
 constexpr int PROD_THREADS = PROD_WARPS * 32;
 constexpr int GROUP_THREADS = PROD_THREADS / 2;  // one producer group per child
 constexpr int XCHUNKS = 16, MCHUNKS = 8;   // 16-byte chunks per producer thread: operand tile / matrix
@@ -50,13 +51,19 @@ constexpr uint32_t OFF_M = 4 * X_PLANE;    // [child][hi, lo]
 constexpr uint32_t OFF_STAGE = OFF_M + 4 * M_PLANE;
 constexpr uint32_t STAGE_WARP = 32 * 128;  // per epilogue warp: 32 rows x 32 columns, 16-byte chunks XOR-swizzled by row
 constexpr uint32_t OFF_MAX = OFF_STAGE + EPI_WARPS * STAGE_WARP;  // [2][TP] row maxima of the upper column half
-constexpr uint32_t OFF_BAR = OFF_MAX + 2 * TP * 4;
+constexpr uint32_t OFF_EXP = OFF_MAX + 2 * TP * 4;              // int16 [2 children][TP]: pending exponents of the next item
+constexpr uint32_t OFF_BAR = OFF_EXP + 2 * TP * 2;
 constexpr uint32_t SMEM_USED = OFF_BAR + 128;
 constexpr size_t SMEM_BYTES = SMEM_USED + 1024;  // + slack for the 1024-byte alignment the swizzle needs
+static_assert(SMEM_BYTES <= 232448, "shared memory budget (227 KB)");
 constexpr int PREFETCH_AHEAD = 2;          // items
 
 // barrier slots (8 bytes each) at OFF_BAR
-enum { B_FULL0 = 0, B_FULL1, B_EMPTY0, B_EMPTY1, B_MFULL, B_MEMPTY, B_TFULL0, B_TFULL1, B_TEMPTY0, B_TEMPTY1, B_TMEM_PTR };
+enum { B_FULL0 = 0, B_FULL1, B_EMPTY0, B_EMPTY1, B_MFULL, B_MEMPTY, B_TFULL0, B_TFULL1, B_TEMPTY0, B_TEMPTY1,
+       B_EXPFULL,  // the pending exponents of the next item are in shared memory (meta warp; one buffer: no room for two)
+       B_EXPFREE,  // the epilogue has read them
+       B_TMEM_PTR };
+static_assert((B_TMEM_PTR + 1) * 8 <= 128, "barrier slots");
 
 // instruction descriptor: D fp32 (bit 4), A and B TF32 (2 << 7, 2 << 10), both K-major, N = 64 (>> 3 at bit 17),
 // M = 128 (>> 4 at bit 24)
@@ -333,6 +340,8 @@ __global__ void __launch_bounds__(THREADS, 1) k_post_tc5(const DevOp* __restrict
     mbar_init(cx.barrier(B_TFULL1), 1);
     mbar_init(cx.barrier(B_TEMPTY0), EPI_WARPS);
     mbar_init(cx.barrier(B_TEMPTY1), EPI_WARPS);
+    mbar_init(cx.barrier(B_EXPFULL), 1);
+    mbar_init(cx.barrier(B_EXPFREE), EPI_WARPS);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   if (warp == N_WARPS - 1) {  // 256 TMEM columns: two accumulator sets of (D_0, D_1) = 2 x 64 columns each
@@ -349,42 +358,24 @@ __global__ void __launch_bounds__(THREADS, 1) k_post_tc5(const DevOp* __restrict
     // ===== epilogue: warp = 4 half + quarter takes patterns 32 quarter .. +31 (TMEM lanes) x states 32 half .. +31 =====
     const int quarter = warp & 3, half = warp >> 2;
     const uint32_t stage = cx.smem + OFF_STAGE + warp * STAGE_WARP;
-    // Pending maxima of both children (deferred rescaling) are fetched ONE ITEM AHEAD: the raw loads are issued before
-    // the current item is processed and reduced to exponents after it, so their latency is off the critical path.
-    float raw[2][4];
-    auto load_raw = [&](const Item& t) {
-      const DevOp& o = ops[t.op];
-      const int p = t.tile * TP + 32 * quarter + lane;
-#pragma unroll
-      for (int k = 0; k < 2; ++k) {
-        const float* m = static_cast<const float*>(o.cscale[k]);
-#pragma unroll
-        for (int c = 0; c < 4; ++c)
-          raw[k][c] = (m != nullptr && p < P && c < C) ? __ldg(m + (size_t)c * P + p) : 0.f;
-      }
-    };
-    auto finish_raw = [&](const Item& t, int k) {
-      float v = fmaxf(fmaxf(raw[k][0], raw[k][1]), fmaxf(raw[k][2], raw[k][3]));
-      if (C > 4) {
-        const float* m = static_cast<const float*>(ops[t.op].cscale[k]);
-        const int p = t.tile * TP + 32 * quarter + lane;
-        if (m != nullptr && p < P)
-          for (int c = 4; c < C; ++c) v = fmaxf(v, m[(size_t)c * P + p]);
-      }
-      return pow2_pair(-exp_of(v), 0.f);
-    };
-    load_raw(cx.first_item);
-    Pow2Pair<float> f0 = finish_raw(cx.first_item, 0), f1 = finish_raw(cx.first_item, 1);
+    // Pending exponents of both children (deferred rescaling) come from the meta warp through shared memory.  (The
+    // epilogue warps used to load the per-category maxima themselves, one item ahead: scattered DRAM loads whose
+    // scoreboard every later wait of the warp inherited -- see plk_tc5_pre2.cuh, where a cycle trace showed it.)
+    const short* sexp = reinterpret_cast<const short*>(tc5_smem_raw + (cx.smem - smem_u32(tc5_smem_raw)) + OFF_EXP);
     for (Item it = cx.first_item; cx.valid(it);) {
       const uint32_t n = it.n;
       const DevOp& o = ops[it.op];
       const int p0 = it.tile * TP, prow0 = p0 + 32 * quarter, p = prow0 + lane;
+      mbar_wait(cx.barrier(B_EXPFULL), n & 1);  // written while the previous item was processed
+      const Pow2Pair<float> f0 = pow2_pair(-(int)sexp[32 * quarter + lane], 0.f);
+      const Pow2Pair<float> f1 = pow2_pair(-(int)sexp[TP + 32 * quarter + lane], 0.f);
+      __syncwarp();
+      if (lane == 0) mbar_arrive(cx.barrier(B_EXPFREE));
       const bool one_factor = __all_sync(0xffffffffu, f0.f2 == 1.f && f1.f2 == 1.f);
       float* dest = static_cast<float*>(o.dest) + (size_t)it.c * P * SP64;
       float* scale = static_cast<float*>(o.scale);
       Item nx = it;
       cx.advance(nx);
-      if (cx.valid(nx)) load_raw(nx);
       const uint32_t a = n & 1;
       mbar_wait(cx.barrier(B_TFULL0 + a), (n >> 1) & 1);
       tc_fence_after();
@@ -436,10 +427,6 @@ __global__ void __launch_bounds__(THREADS, 1) k_post_tc5(const DevOp* __restrict
       if (half == 0 && p < P && scale != nullptr)
         scale[(size_t)it.c * P + p] = fmaxf(mx, lds32(cx.smem + OFF_MAX + (a * TP + 32 * quarter + lane) * 4));
       it = nx;
-      if (cx.valid(it)) {
-        f0 = finish_raw(it, 0);
-        f1 = finish_raw(it, 1);
-      }
     }
   } else if (warp < EPI_WARPS + PROD_WARPS) {
     // ===== producers: group g = child g =====
@@ -467,6 +454,56 @@ __global__ void __launch_bounds__(THREADS, 1) k_post_tc5(const DevOp* __restrict
       loaded = !cx.new_run(nx);
       if (loaded) prod_load(cx, nx, g, gt, r);
       it = nx;
+    }
+  } else if (warp == META_WARP) {
+    // ===== meta warp: exponent of max_c cscale[k][c][p] for the 128 rows of every item, one item ahead (its loads are
+    // in flight while it waits for the epilogue to have read the previous item's values) =====
+    short* sexp = reinterpret_cast<short*>(tc5_smem_raw + (cx.smem - smem_u32(tc5_smem_raw)) + OFF_EXP);
+    auto ldv = [](const float* m) {
+      float v;
+      asm volatile("ld.global.nc.f32 %0, [%1];" : "=f"(v) : "l"(m));
+      return v;
+    };
+    for (Item it = cx.first_item; cx.valid(it); cx.advance(it)) {
+      const uint32_t n = it.n;
+      const DevOp& o = ops[it.op];
+      const float* src[2] = {static_cast<const float*>(o.cscale[0]), static_cast<const float*>(o.cscale[1])};
+      float4 raw[4][2];  // all loads of the item are issued before the first one is used
+#pragma unroll
+      for (int j = 0; j < 4; ++j) {
+        const int p = it.tile * TP + lane + 32 * j;
+#pragma unroll
+        for (int k = 0; k < 2; ++k) {
+          float4 v = make_float4(0.f, 0.f, 0.f, 0.f);
+          if (src[k] != nullptr && p < P) {
+            const float* m = src[k] + p;
+            v.x = ldv(m);
+            if (C > 1) v.y = ldv(m + (size_t)P);
+            if (C > 2) v.z = ldv(m + 2 * (size_t)P);
+            if (C > 3) v.w = ldv(m + 3 * (size_t)P);
+          }
+          raw[j][k] = v;
+        }
+      }
+      int ex[4][2];
+#pragma unroll
+      for (int j = 0; j < 4; ++j) {
+        const int p = it.tile * TP + lane + 32 * j;
+#pragma unroll
+        for (int k = 0; k < 2; ++k) {
+          float v = fmaxf(fmaxf(raw[j][k].x, raw[j][k].y), fmaxf(raw[j][k].z, raw[j][k].w));
+          if (C > 4 && src[k] != nullptr && p < P)
+            for (int c = 4; c < C; ++c) v = fmaxf(v, src[k][(size_t)c * P + p]);
+          ex[j][k] = exp_of(v);
+        }
+      }
+      if (n > 0) mbar_wait(cx.barrier(B_EXPFREE), (n + 1) & 1);  // item n - 1 was read
+#pragma unroll
+      for (int j = 0; j < 4; ++j)
+#pragma unroll
+        for (int k = 0; k < 2; ++k) sexp[k * TP + lane + 32 * j] = (short)ex[j][k];
+      __syncwarp();
+      if (lane == 0) mbar_arrive(cx.barrier(B_EXPFULL));
     }
   } else {
     // ===== MMA issuer: the whole warp runs the loop, one elected lane executes each tcgen05.mma / commit =====
