@@ -170,7 +170,7 @@ __global__ void __launch_bounds__(NT_THREADS, 4) k_pre4_lean(const DevPreItem* _
         const int kind[3] = {KIND_PARTIALS, TIP0 ? KIND_STATES : KIND_PARTIALS, TIP1 ? KIND_STATES : KIND_PARTIALS};
         const void* mat[2] = {it->mat[0], it->mat[1]};
         nt_fill<T, C, 3, true, R>(nt_smem + (size_t)(j % NT_NS) * St::BYTES, &full[j % NT_NS], it, sizeof(DevPreItem),
-                                  ptr, kind, mat, md.weights, P, p0, n);
+                                  ptr, kind, mat, md.weights, P, p0, n, dmat_delta);
       }
     }
     if (!wait_first) pdl_wait();
@@ -204,14 +204,14 @@ __global__ void __launch_bounds__(NT_THREADS, 4) k_pre4_lean(const DevPreItem* _
     // num_k = u_k . qx_k and no q_k is formed (k_deriv_matrices4)
     T a0[R][4], a1[R][4], qx0[R][4], qx1[R][4];
     if (TIP0) {
-      const T* D0 = reinterpret_cast<const T*>(static_cast<const char*>(it.mat[0]) + dmat_delta) + g * 16;
+      const T* D0 = sOp + (size_t)C * TP * 4 + g * 16;  // staged in the child's unused operand segment (nt_fill)
 #pragma unroll
       for (int u = 0; u < R; ++u) {
         const int z = stage[St::OFF_ST + h.soff0 + r[u]];
 #pragma unroll
         for (int x = 0; x < 4; ++x) {
           a0[u][x] = z < 4 ? sM0[x * 4 + z] : T(1);
-          qx0[u][x] = z < 4 ? __ldg(D0 + x * 4 + z) : T(0);
+          qx0[u][x] = z < 4 ? D0[x * 4 + z] : T(0);
         }
       }
     } else {
@@ -222,14 +222,14 @@ __global__ void __launch_bounds__(NT_THREADS, 4) k_pre4_lean(const DevPreItem* _
       mvq4r<T, R>(Qc, x0, qx0);
     }
     if (TIP1) {
-      const T* D1 = reinterpret_cast<const T*>(static_cast<const char*>(it.mat[1]) + dmat_delta) + g * 16;
+      const T* D1 = sOp + (size_t)2 * C * TP * 4 + g * 16;
 #pragma unroll
       for (int u = 0; u < R; ++u) {
         const int z = stage[St::OFF_ST + (TP + 16) + h.soff1 + r[u]];
 #pragma unroll
         for (int x = 0; x < 4; ++x) {
           a1[u][x] = z < 4 ? sM1[x * 4 + z] : T(1);
-          qx1[u][x] = z < 4 ? __ldg(D1 + x * 4 + z) : T(0);
+          qx1[u][x] = z < 4 ? D1[x * 4 + z] : T(0);
         }
       }
     } else {

@@ -181,7 +181,9 @@ struct NtTiles {
 template <typename T, int C, int NOPS, bool WTS, int R = 1>
 __device__ __forceinline__ void nt_fill(unsigned char* stage, uint64_t* full, const void* desc, uint32_t desc_bytes,
                                         const void* const* ptr, const int* kind, const void* const* mat,
-                                        const double* weights, int P, int p0, int n) {
+                                        const double* weights, int P, int p0, int n, long long dmat_delta = 0) {
+  // dmat_delta != 0 (class-specialised gradient kernels): a child given as compact states leaves its operand segment of
+  // the stage unused; the derivative matrices D = M Q of its branch ([C][16], at mat + dmat_delta bytes) are copied there
   using St = NtStage<T, C, NOPS, WTS, R>;
   const uint32_t seg_bytes = (uint32_t)n * 4 * sizeof(T);
   const uint32_t mat_bytes = 16 * sizeof(T);
@@ -196,7 +198,7 @@ __device__ __forceinline__ void nt_fill(unsigned char* stage, uint64_t* full, co
   for (int o = 0; o < NOPS; ++o) {
     if (kind[o] == KIND_PARTIALS) bytes += C * seg_bytes;
     else if (kind[o] == KIND_BCAST) bytes += seg_bytes;
-    else if (kind[o] == KIND_STATES) bytes += ((uint32_t)(n + (p0 & 15)) + 15) & ~15u;
+    else if (kind[o] == KIND_STATES) bytes += (((uint32_t)(n + (p0 & 15)) + 15) & ~15u) + (dmat_delta != 0 ? C * mat_bytes : 0u);
   }
   if (kind[NOPS - 2] == KIND_STATES) h.soff0 = p0 & 15;
   if (kind[NOPS - 1] == KIND_STATES) h.soff1 = p0 & 15;
@@ -225,6 +227,8 @@ __device__ __forceinline__ void nt_fill(unsigned char* stage, uint64_t* full, co
       const int k = o - (NOPS - 2);
       bulk_g2s(stage + St::OFF_ST + k * (St::TP + 16), static_cast<const uint8_t*>(ptr[o]) + (p0 & ~15),
                ((uint32_t)(n + (p0 & 15)) + 15) & ~15u, full);
+      if (dmat_delta != 0)
+        bulk_g2s(dst, static_cast<const char*>(mat[k]) + dmat_delta, C * mat_bytes, full);
     }
   }
 }
