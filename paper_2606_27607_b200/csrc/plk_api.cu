@@ -630,10 +630,10 @@ template <typename T>
 int launch_post64(plk_instance* in, const DevOp* d_ops, int n_ops) {
   const Layout& L = in->L;
   if (L.SP == 32) {  // 5..32 states: the CUDA-core kernels instantiated for 32 padded states (plk_gen.cuh)
-    int rc = opt_in_smem(k_post64<T, 32>, post64_smem<T, 32>());
+    int rc = opt_in_smem(k_post64t<T, 32>, GenT<T, 32>::SMEM);
     if (rc) return rc;
-    dim3 grid(L.n_tiles, L.C, n_ops);
-    k_post64<T, 32><<<grid, GEN_THREADS, post64_smem<T, 32>(), in->stream>>>(d_ops, L.P, L.S, L.C);
+    dim3 grid((L.P + GenT<T, 32>::PT - 1) / GenT<T, 32>::PT, L.C, n_ops);
+    k_post64t<T, 32><<<grid, 128, GenT<T, 32>::SMEM, in->stream>>>(d_ops, L.P, L.S, L.C);
     CHECK_LAUNCH(in);
     return PLK_SUCCESS;
   }
@@ -644,10 +644,10 @@ int launch_post64(plk_instance* in, const DevOp* d_ops, int n_ops) {
     return tc_launch_post<T>(in->stream, d_ops, n_ops, L.P, L.S, L.C, in->sm_count, &in->launches);
   }
 #endif
-  int rc = opt_in_smem(k_post64<T>, post64_smem<T>());
+  int rc = opt_in_smem(k_post64t<T, 64>, GenT<T, 64>::SMEM);
   if (rc) return rc;
-  dim3 grid(L.n_tiles, L.C, n_ops);
-  k_post64<T><<<grid, GEN_THREADS, post64_smem<T>(), in->stream>>>(d_ops, L.P, L.S, L.C);
+  dim3 grid((L.P + GenT<T, 64>::PT - 1) / GenT<T, 64>::PT, L.C, n_ops);
+  k_post64t<T, 64><<<grid, 128, GenT<T, 64>::SMEM, in->stream>>>(d_ops, L.P, L.S, L.C);
   CHECK_LAUNCH(in);
   return PLK_SUCCESS;
 }

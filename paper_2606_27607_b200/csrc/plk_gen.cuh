@@ -234,6 +234,147 @@ __global__ void __launch_bounds__(GEN_THREADS) k_post64(const DevOp* __restrict_
 }
 
 // ---------------------------------------------------------------------------------------------------------------
+// post-order update, register-tiled (round 2; replaces k_post64 on the CUDA-core path).  k_post64 gives a thread 8 states
+// of ONE pattern, so every FMA needs its own shared-memory operand: 17 shared-memory wavefronts per 8 warp-FMAs, i.e.
+// the kernel is bound by shared memory at ~7 % of the fp64 FMA rate.  Here a thread owns 4 patterns x 8 states of a
+// tile of PT patterns (PT / 4 x SP / 8 = 128 threads): per contraction index x it reads 8 matrix values and 4 operand
+// values for 32 FMAs.  Layouts chosen so that no load conflicts: the matrix row A[x][.] (A[x][s] = M[s][x]) is stored in
+// 16-byte chunks interleaved as (chunk i of state group sg) -> position i * NSG + sg, so the lanes of a quarter warp
+// (distinct sg) read consecutive chunks; the operand tile is transposed to Vt[x][p] with an odd row stride, read as
+// broadcasts.  The two children go through the same buffers one after the other; a compact-tip child is a row gather.
+// Same arithmetic per output as k_post64 (sum over x in increasing order, deferred rescaling): results are identical.
+// ---------------------------------------------------------------------------------------------------------------
+template <typename T, int SP>
+struct GenT {
+  static constexpr int VEC = 16 / sizeof(T);       // elements per 16-byte chunk
+  static constexpr int NSG = SP / 8;               // state groups (8 states each)
+  static constexpr int PT = 128 * 4 / NSG;         // patterns per tile: 64 (SP = 64), 128 (SP = 32)
+  static constexpr int NCH = 8 / VEC;              // chunks per thread and matrix row
+  static constexpr int LDV = PT + 1;               // operand tile row stride (odd: conflict-free transposing stores)
+  static constexpr size_t SMEM = ((size_t)SP * SP + (size_t)SP * LDV) * sizeof(T) + 2 * PT * sizeof(int);
+};
+
+template <typename T, int SP = SP64>
+__global__ void __launch_bounds__(128) k_post64t(const DevOp* __restrict__ ops, int P, int S, int C) {
+  using G = GenT<T, SP>;
+  using V = typename VecOf<T>::type;
+  constexpr int VEC = G::VEC, NSG = G::NSG, PT = G::PT, NCH = G::NCH, LDV = G::LDV;
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  T* A = reinterpret_cast<T*>(smem_raw);  // [SP][SP], chunk-interleaved rows
+  T* Vt = A + SP * SP;                    // [SP][LDV]
+  int* sE = reinterpret_cast<int*>(Vt + SP * LDV);  // [2][PT] pending exponents of the children
+
+  const DevOp op = ops[blockIdx.z];
+  const int c = blockIdx.y, p0 = blockIdx.x * PT;
+  const int sg = threadIdx.x % NSG, pg = threadIdx.x / NSG;  // states 8 sg .., patterns p0 + 4 pg ..
+  for (int i = threadIdx.x; i < 2 * PT; i += 128) sE[i] = pending_exp<T>(op.cscale[i / PT], p0 + i % PT, P, C);
+
+  T acc[2][4][8];
+#pragma unroll
+  for (int k = 0; k < 2; ++k) {
+    __syncthreads();  // the previous child's buffers are no longer read
+    // matrix of child k: A[x][s] = M[s][x]; element (x, s) at A[x * SP + ((s % 8) / VEC * NSG + s / 8) * VEC + s % VEC]
+    // (filled in VEC x VEC blocks: 16-byte loads of VEC rows of M, 16-byte stores of VEC rows of A to consecutive
+    // chunk positions -- a scalar transposing copy would store at a stride of a whole row: 32-way bank conflicts)
+    const T* M = static_cast<const T*>(op.mat[k]) + (size_t)c * SP * SP;
+    constexpr int CPR = SP / VEC;
+    for (int idx = threadIdx.x; idx < CPR * CPR; idx += 128) {
+      const int pos = idx % CPR, xc = idx / CPR;     // chunk position inside the rows of A; chunk of x
+      const int cs = (pos % NSG) * NCH + pos / NSG;  // the chunk of states stored at that position
+      T blk[VEC][VEC];
+#pragma unroll
+      for (int j = 0; j < VEC; ++j) unpack(*reinterpret_cast<const V*>(M + (size_t)(cs * VEC + j) * SP + xc * VEC), blk[j]);
+#pragma unroll
+      for (int i = 0; i < VEC; ++i) {
+        T o[VEC];
+#pragma unroll
+        for (int j = 0; j < VEC; ++j) o[j] = blk[j][i];
+        *reinterpret_cast<V*>(A + (xc * VEC + i) * SP + pos * VEC) = pack(o, V());
+      }
+    }
+    const int kind = op.kind[k];
+    if (kind == KIND_PARTIALS || kind == KIND_BCAST) {  // operand tile, transposed: lane = pattern, loop over chunks
+      const T* base = static_cast<const T*>(op.child[k]) + (kind == KIND_BCAST ? (size_t)0 : (size_t)c * P * SP);
+      for (int idx = threadIdx.x; idx < PT * (SP / VEC); idx += 128) {
+        const int pp = idx % PT, ch = idx / PT;
+        T tmp[VEC];
+        if (p0 + pp < P) {
+          unpack(*reinterpret_cast<const V*>(base + (size_t)(p0 + pp) * SP + ch * VEC), tmp);
+        } else {
+#pragma unroll
+          for (int j = 0; j < VEC; ++j) tmp[j] = T(0);
+        }
+#pragma unroll
+        for (int j = 0; j < VEC; ++j) Vt[(ch * VEC + j) * LDV + pp] = tmp[j];
+      }
+    }
+    __syncthreads();
+    if (kind == KIND_STATES) {  // column z of M = row z of A; a missing state: 1 for real states
+#pragma unroll
+      for (int i = 0; i < 4; ++i) {
+        const int p = p0 + 4 * pg + i;
+        const int z = p < P ? static_cast<const uint8_t*>(op.child[k])[p] : S;
+#pragma unroll
+        for (int q = 0; q < NCH; ++q) {
+          T a[VEC];
+          unpack(*reinterpret_cast<const V*>(A + (z < S ? z : 0) * SP + (q * NSG + sg) * VEC), a);
+#pragma unroll
+          for (int j = 0; j < VEC; ++j) {
+            const int s = 8 * sg + q * VEC + j;
+            acc[k][i][q * VEC + j] = z < S ? a[j] : (s < S ? T(1) : T(0));
+          }
+        }
+      }
+    } else if (kind == KIND_NONE) {
+#pragma unroll
+      for (int i = 0; i < 4; ++i)
+#pragma unroll
+        for (int j = 0; j < 8; ++j) acc[k][i][j] = T(0);
+    } else {
+#pragma unroll
+      for (int i = 0; i < 4; ++i)
+#pragma unroll
+        for (int j = 0; j < 8; ++j) acc[k][i][j] = T(0);
+      const T* vrow = Vt + 4 * pg;
+      const T* arow = A + sg * VEC;
+#pragma unroll 2
+      for (int x = 0; x < SP; ++x) {
+        T a[8], v[4];
+#pragma unroll
+        for (int q = 0; q < NCH; ++q) unpack(*reinterpret_cast<const V*>(arow + x * SP + q * NSG * VEC), a + q * VEC);
+#pragma unroll
+        for (int i = 0; i < 4; ++i) v[i] = vrow[x * LDV + i];
+#pragma unroll
+        for (int i = 0; i < 4; ++i)
+#pragma unroll
+          for (int j = 0; j < 8; ++j) acc[k][i][j] = fma(a[j], v[i], acc[k][i][j]);
+      }
+    }
+  }
+  // product of the two children with their pending factors, per-pattern maximum, store
+#pragma unroll
+  for (int i = 0; i < 4; ++i) {
+    const int pl = 4 * pg + i, p = p0 + pl;
+    const Pow2Pair<T> f0 = pow2_pair(-sE[pl], T(0)), f1 = pow2_pair(-sE[PT + pl], T(0));
+    T mx = T(0);
+    T out[8];
+#pragma unroll
+    for (int j = 0; j < 8; ++j) {
+      out[j] = ((acc[0][i][j] * f0.f1) * f0.f2) * ((acc[1][i][j] * f1.f1) * f1.f2);
+      mx = fmax(mx, out[j]);
+    }
+#pragma unroll
+    for (int o = 1; o < NSG; o <<= 1) mx = fmax(mx, __shfl_xor_sync(0xffffffffu, mx, o));
+    if (p < P) {
+      T* drow = static_cast<T*>(op.dest) + ((size_t)c * P + p) * SP + 8 * sg;
+#pragma unroll
+      for (int q = 0; q < NCH; ++q) *reinterpret_cast<V*>(drow + q * VEC) = pack(out + q * VEC, V());
+      if (sg == 0 && op.scale != nullptr) static_cast<T*>(op.scale)[(size_t)c * P + p] = mx;
+    }
+  }
+}
+
+// ---------------------------------------------------------------------------------------------------------------
 // pre-order update of both children of one parent + both branch derivatives
 // one (tile, item) per block, categories looped inside so that num_p and den_p are summed over c in the block
 // ---------------------------------------------------------------------------------------------------------------
