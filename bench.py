@@ -700,7 +700,7 @@ def main():
     lean = nuc and wl.n_categories == 4 and args.staging == "tma" and args.shape != "walk"
     kname = {"post_order": ("k_post4_walk" if args.shape != "level" else "k_post4_tma") if nuc
              else (("k_post_tc5" if args.precision == "fp32" and args.codon_fp32 == "tcgen05" else "k_post_tc")
-                   if args.tensor else "k_post64"),
+                   if args.tensor else "k_post64t"),
              "pre_order_gradient": ("k_pre4_lean+k_grad4_tips" if lean else "k_pre4_tma/k_pre4/k_pre4_walk") if nuc
              else (("k_pre_tc5" if args.precision == "fp32" and args.codon_fp32 == "tcgen05" else "k_pre_tc")
                    if args.tensor else "k_pre64")}[dom]

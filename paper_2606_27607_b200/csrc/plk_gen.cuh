@@ -166,10 +166,6 @@ __device__ __forceinline__ T lane8_sum(T v) {
 }
 
 template <typename T, int SP = SP64>
-constexpr size_t post64_smem() {
-  return (2 * SP * SP + 2 * GEN_TP * Gen<T, SP>::TS) * sizeof(T) + 2 * GEN_TP * sizeof(int);
-}
-template <typename T, int SP = SP64>
 constexpr size_t pre64_smem() {
   return (3 * SP * SP + 5 * GEN_TP * Gen<T, SP>::TS) * sizeof(T) + 3 * GEN_TP * sizeof(int) +
          4 * GEN_TP * sizeof(double);
@@ -180,61 +176,7 @@ constexpr size_t deriv64_smem() {
 }
 
 // ---------------------------------------------------------------------------------------------------------------
-// post-order update, one (tile, category, operation) per block (maxima for step 3)
-// ---------------------------------------------------------------------------------------------------------------
-template <typename T, int SP = SP64>
-__global__ void __launch_bounds__(GEN_THREADS) k_post64(const DevOp* __restrict__ ops, int P, int S, int C) {
-  constexpr int TS = Gen<T, SP>::TS;
-  extern __shared__ __align__(16) unsigned char smem_raw[];
-  T* A0 = reinterpret_cast<T*>(smem_raw);
-  T* A1 = A0 + SP * SP;
-  T* V0 = A1 + SP * SP;
-  T* V1 = V0 + GEN_TP * TS;
-  int* sE = reinterpret_cast<int*>(V1 + GEN_TP * TS);
-
-  const DevOp op = ops[blockIdx.z];
-  const int c = blockIdx.y, p0 = blockIdx.x * GEN_TP;
-  const int pp = threadIdx.x >> 3, sb = threadIdx.x & 7, p = p0 + pp;
-
-  fill_matrix<T, SP>(A0, static_cast<const T*>(op.mat[0]) + (size_t)c * SP * SP, true);
-  fill_matrix<T, SP>(A1, static_cast<const T*>(op.mat[1]) + (size_t)c * SP * SP, true);
-  if (op.kind[0] != KIND_STATES) load_tile<T, SP>(V0, op.kind[0], op.child[0], c, p0, P, S);
-  if (op.kind[1] != KIND_STATES) load_tile<T, SP>(V1, op.kind[1], op.child[1], c, p0, P, S);
-  if (threadIdx.x < 2 * GEN_TP) {
-    const int k = threadIdx.x / GEN_TP, r = threadIdx.x % GEN_TP;
-    sE[threadIdx.x] = pending_exp<T>(op.cscale[k], p0 + r, P, C);
-  }
-  __syncthreads();
-
-  T a[Gen<T, SP>::NPT], b[Gen<T, SP>::NPT];
-  if (op.kind[0] == KIND_STATES) {
-    const int z = p < P ? static_cast<const uint8_t*>(op.child[0])[p] : 0;
-    gather64<T, SP>(A0, z, S, T(1), sb, a);
-  } else {
-    mv64<T, SP>(A0, V0 + pp * TS, sb, a);
-  }
-  if (op.kind[1] == KIND_STATES) {
-    const int z = p < P ? static_cast<const uint8_t*>(op.child[1])[p] : 0;
-    gather64<T, SP>(A1, z, S, T(1), sb, b);
-  } else {
-    mv64<T, SP>(A1, V1 + pp * TS, sb, b);
-  }
-  const Pow2Pair<T> f0 = pow2_pair(-sE[pp], T(0)), f1 = pow2_pair(-sE[GEN_TP + pp], T(0));
-  T mx = T(0);
-#pragma unroll
-  for (int k = 0; k < Gen<T, SP>::NPT; ++k) {
-    a[k] = ((a[k] * f0.f1) * f0.f2) * ((b[k] * f1.f1) * f1.f2);
-    mx = fmax(mx, a[k]);
-  }
-  mx = lane8_max(mx);
-  if (p < P) {
-    store_states<T, SP>(static_cast<T*>(op.dest) + ((size_t)c * P + p) * SP, sb, a);
-    if (sb == 0 && op.scale != nullptr) static_cast<T*>(op.scale)[(size_t)c * P + p] = mx;
-  }
-}
-
-// ---------------------------------------------------------------------------------------------------------------
-// post-order update, register-tiled (round 2; replaces k_post64 on the CUDA-core path).  k_post64 gives a thread 8 states
+// post-order update, register-tiled (round 2).  The first version (k_post64, removed) gave a thread 8 states
 // of ONE pattern, so every FMA needs its own shared-memory operand: 17 shared-memory wavefronts per 8 warp-FMAs, i.e.
 // the kernel is bound by shared memory at ~7 % of the fp64 FMA rate.  Here a thread owns 4 patterns x 8 states of a
 // tile of PT patterns (PT / 4 x SP / 8 = 128 threads): per contraction index x it reads 8 matrix values and 4 operand
@@ -242,7 +184,7 @@ __global__ void __launch_bounds__(GEN_THREADS) k_post64(const DevOp* __restrict_
 // 16-byte chunks interleaved as (chunk i of state group sg) -> position i * NSG + sg, so the lanes of a quarter warp
 // (distinct sg) read consecutive chunks; the operand tile is transposed to Vt[x][p] with an odd row stride, read as
 // broadcasts.  The two children go through the same buffers one after the other; a compact-tip child is a row gather.
-// Same arithmetic per output as k_post64 (sum over x in increasing order, deferred rescaling): results are identical.
+// Same arithmetic per output as before (sum over x in increasing order, deferred rescaling).
 // ---------------------------------------------------------------------------------------------------------------
 template <typename T, int SP>
 struct GenT {
