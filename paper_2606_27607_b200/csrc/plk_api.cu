@@ -952,7 +952,7 @@ int plk_set_all_tip_states_u8(plk_instance* in, const uint8_t* states, int count
     int last = first;
     while (last + 1 < count && in->post_slot[last + 1] == in->post_slot[last] + 1) ++last;
     // a pitched host -> device copy runs at a third of the PCIe rate (one DMA descriptor per row: 0.75 ms for 12.8 MB);
-    // so: one LINEAR copy of as many rows as the staging area holds, then a device-side pitched copy into the slots
+    // so: one LINEAR copy of as many rows as the staging area holds, then a kernel scatters the rows into the slots
     const size_t rows_per_chunk = L.compact_bytes == (size_t)L.P ? (size_t)(last - first + 1) : L.stage_bytes / (size_t)L.P;
     if (rows_per_chunk == 0) return PLK_ERR_OUT_OF_MEMORY;
     for (int r0 = first; r0 <= last; r0 += (int)rows_per_chunk) {
@@ -963,8 +963,9 @@ int plk_set_all_tip_states_u8(plk_instance* in, const uint8_t* states, int count
       } else {
         char* stage = in->arena + L.off_stage;
         CU(cudaMemcpyAsync(stage, src, rows * L.P, cudaMemcpyHostToDevice, in->stream));
-        CU(cudaMemcpy2DAsync(in->post_ptr(r0), L.compact_bytes, stage, (size_t)L.P, (size_t)L.P, rows,
-                             cudaMemcpyDeviceToDevice, in->stream));
+        k_scatter_rows<<<dim3(blocks_for(((size_t)L.P + 15) / 16, 256), (unsigned)rows), 256, 0, in->stream>>>(
+            reinterpret_cast<const uint8_t*>(stage), static_cast<uint8_t*>(in->post_ptr(r0)), (size_t)L.P, L.compact_bytes);
+        CHECK_LAUNCH(in);
       }
     }
     first = last + 1;

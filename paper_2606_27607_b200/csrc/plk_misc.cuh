@@ -114,6 +114,19 @@ __global__ void k_pack_states(const int32_t* __restrict__ src, uint8_t* __restri
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
   if (i < P) dst[i] = (uint8_t)((src[i] < 0 || src[i] >= S) ? S : src[i]);
 }
+// rows of `width` bytes from a dense block (row r at src + r * width) into pitched rows (dst + r * pitch); blockIdx.y = row.
+// (A pitched device-to-device cudaMemcpy2DAsync of 128 rows took 0.5 ms: the copy engine handles it row by row.)
+__global__ void k_scatter_rows(const uint8_t* __restrict__ src, uint8_t* __restrict__ dst, size_t width, size_t pitch) {
+  const uint8_t* s = src + (size_t)blockIdx.y * width;
+  uint8_t* d = dst + (size_t)blockIdx.y * pitch;
+  const size_t i = ((size_t)blockIdx.x * blockDim.x + threadIdx.x) * 16;
+  if (i >= width) return;
+  if (i + 16 <= width && ((reinterpret_cast<uintptr_t>(s + i) | reinterpret_cast<uintptr_t>(d + i)) & 15) == 0) {
+    *reinterpret_cast<uint4*>(d + i) = *reinterpret_cast<const uint4*>(s + i);
+  } else {
+    for (size_t j = i; j < width && j < i + 16; ++j) d[j] = s[j];
+  }
+}
 // expand compact states into fp64 partials [C][P][S] (plk_get_partials on a compact tip)
 __global__ void k_expand_states(const uint8_t* __restrict__ st, double* __restrict__ dst, int C, int P, int S) {
   const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
