@@ -169,3 +169,31 @@ def test_set_all_tip_states_u8_matches_per_tip_upload(n_pat):
         assert e.value.status == plk.ERR_OUT_OF_RANGE
     finally:
         ev.close()
+
+
+def test_more_signatures_than_cached_plans():
+    """The library caches at most 8 evaluation graphs per instance and then drops them all: twelve different call
+    signatures (the same evaluation with the branch list rotated), each used often enough to be captured and replayed,
+    must all give the same result as the first."""
+    import torch
+
+    wl = workloads.config(0, n_patterns=300)
+    ref = orc.evaluate(wl)
+    stream = torch.cuda.Stream()
+    with torch.cuda.stream(stream):
+        ev = Evaluator(wl, precision=plk.FP64, stream=stream, eigen=orc.oracle_eigen(wl))
+        try:
+            t = np.asarray(wl.tree.branch_length)
+            first = None
+            for rot in range(12):
+                idx = np.roll(ev.matrix_idx, rot)
+                for use in range(4):
+                    logl, g = ev.inst.evaluate(0, idx, t[idx], ev.ops, wl.tree.root, ev.scale_idx, wl.tree.root, ev.pre_ops)
+                    grad = np.zeros(wl.tree.n_nodes)
+                    grad[ev.branch_nodes] = g
+                    _check(logl, grad, ref, plk.FP64, wl.tree.root)
+                    if first is None:
+                        first = (logl, g.copy())
+                    assert logl == first[0] and np.array_equal(g, first[1])
+        finally:
+            ev.close()
