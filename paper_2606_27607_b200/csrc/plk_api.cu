@@ -585,7 +585,7 @@ int launch_pre4_lean(plk_instance* in, int cls, const DevPreItem* d_items, int n
       const Layout& L = in->L;
       const bool pdl = !(in->cfg.flags & PLK_FLAG_NO_PDL);
       constexpr int TPW = NlTipsTpw<T>::V;
-      const int n_tp = (L.P + 32 * NlRows<T>::R - 1) / (32 * NlRows<T>::R);
+      const int n_tp = (L.P + 32 * NlTipsRows<T>::R - 1) / (32 * NlTipsRows<T>::R);
       for (int first = 0; first < n; first += 32768) {
         const int m = n - first < 32768 ? n - first : 32768;
         dim3 grid((n_tp + NT_CW * TPW - 1) / (NT_CW * TPW), m);

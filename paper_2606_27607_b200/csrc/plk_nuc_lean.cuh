@@ -344,15 +344,21 @@ __global__ void __launch_bounds__(NT_THREADS, 4) k_pre4_lean(const DevPreItem* _
 // descriptor -> matrix pointers -> table entries: dependent global loads), and the loads of tile t + 1 are in flight
 // while tile t is computed
 // (all both-tips items of a pass run as ONE launch, plk_api.cu, so long CTAs leave no tail: fp64 141 us at 4 tiles per
-// warp against 175 at one; the fp32 body with two rows per lane runs out of registers at 4: 140 registers, 3 CTAs / SM)
+// warp against 175 at one; the fp32 body took two rows per lane at first and ran out of registers at 4 tiles per warp
+// (140 registers, 3 CTAs / SM); with ONE row per lane it needs 72 and takes 4 as well: configs[1] fp32 pre-order +
+// gradient 0.561 -> 0.542 ms; 8 tiles per warp: no further change)
 template <typename T>
 struct NlTipsTpw {
-  static constexpr int V = sizeof(T) == 8 ? 4 : 1;
+  static constexpr int V = 4;
+};
+template <typename T>
+struct NlTipsRows {  // pattern rows per lane of the both-tips kernel
+  static constexpr int R = 1;
 };
 
 template <typename T>
 struct NlTipsTile {  // what a lane reads for its R patterns of one tile
-  static constexpr int C = NL_C, R = NlRows<T>::R;
+  static constexpr int C = NL_C, R = NlTipsRows<T>::R;
   int p[R], z0[R], z1[R];
   T qm[R][C][4];
   __device__ __forceinline__ void load(int tile, int lane, int P, const T* __restrict__ qmp,
@@ -380,7 +386,7 @@ template <typename T>
 __global__ void __launch_bounds__(NT_CW * 32) k_grad4_tips(const DevPreItem* __restrict__ items, int P, long long dmat_delta,
                                                            NucModel md, double* __restrict__ grad_partial, int n_part,
                                                            int wait_first) {
-  constexpr int C = NL_C, R = NlRows<T>::R, TPW = NlTipsTpw<T>::V;
+  constexpr int C = NL_C, R = NlTipsRows<T>::R, TPW = NlTipsTpw<T>::V;
   __shared__ __align__(16) T tabA[2][C][5][4];  // [child][category][state z (4 = missing)][x]: M_k[x][z]; missing: 1
   __shared__ __align__(16) T tabD[2][C][5][4];  // D_k[x][z]; missing: 0 (Q . 1 = 0)
   T scw[C], scwr[C];
