@@ -15,6 +15,7 @@
 #include "plk_nuc_tma.cuh"
 #include "plk_nuc_lean.cuh"
 #include "plk_cross.cuh"
+#include "plk_cross_tc.cuh"
 #include "plk_cache.cuh"
 #include "plk_schedule.h"
 #ifdef PLK_WITH_TENSOR
@@ -129,7 +130,7 @@ bool compute_layout(const plk_config& c, Layout& L) {
   // rate-matrix gradient (plk_cross.cuh): per-block partial sums and the S x S result
   L.off_cross_partial = take(c.preorder_buffer_count > 0
                                  ? (L.SP == 4 ? (size_t)16 * ((L.P + CROSS4_THREADS - 1) / CROSS4_THREADS)
-                                              : (size_t)((L.P + CROSS64_TP - 1) / CROSS64_TP) * L.SP * L.SP) * 8
+                                              : (size_t)std::max((L.P + CROSS64_TP - 1) / CROSS64_TP, L.SP == 64 ? CROSS_TC_MAX_GRID : 0) * L.SP * L.SP) * 8
                                  : 0);
   L.off_cross_out = take((size_t)L.SP * L.SP * 8);
   L.total = o;
@@ -2157,12 +2158,28 @@ int plk_rate_matrix_gradient(plk_instance* in, const int32_t* post_idx, const in
     CHECK_LAUNCH(in);
   } else {
     const int n_blocks = (L.P + CROSS64_TP - 1) / CROSS64_TP;
+    int n_sum = n_blocks;  // partial sums to add up
     rc = by_precision(in, [&](auto tag) -> int {
       using T = decltype(tag);
       if (L.SP == 32) {
         int r3 = opt_in_smem(k_cross64<T, 32>, cross64_smem<T, 32>());
         if (r3) return r3;
         k_cross64<T, 32><<<n_blocks, CROSS64_THREADS, cross64_smem<T, 32>(), in->stream>>>(db, count, L.P, L.S, L.C, cw, cr, wt, part);
+        return PLK_SUCCESS;
+      }
+      if (cfg.flags & PLK_FLAG_TENSOR_CORES) {
+        // tensor cores (plk_cross_tc.cuh): units = pattern tiles x branch ranges, dealt round-robin to a fixed grid
+        const size_t smem = cross_tc_smem<T>(L.C);
+        if (smem + 1024 > 232448) return PLK_ERR_UNSUPPORTED;
+        int r4 = opt_in_smem(k_cross_tc<T>, smem);
+        if (r4) return r4;
+        const int per_sm = std::min(3, (int)(233472 / (smem + 1024)));
+        const int slots = std::min(CROSS_TC_MAX_GRID, in->sm_count * per_sm);
+        const int chunks = (L.P + CrossTc<T>::TP - 1) / CrossTc<T>::TP;
+        const int n_split = std::max(1, std::min(count, (8 * slots + chunks - 1) / chunks));
+        const long long units = (long long)chunks * n_split;
+        n_sum = (int)std::min<long long>(units, slots);
+        k_cross_tc<T><<<n_sum, CROSS_TC_THREADS, smem, in->stream>>>(db, count, n_split, (int)units, L.P, L.S, L.C, cw, cr, wt, part);
         return PLK_SUCCESS;
       }
       int r2 = opt_in_smem(k_cross64<T>, cross64_smem<T>());
@@ -2172,7 +2189,7 @@ int plk_rate_matrix_gradient(plk_instance* in, const int32_t* post_idx, const in
     });
     if (rc) return rc;
     CHECK_LAUNCH(in);
-    k_sum_blocks<<<(n_elem + 255) / 256, 256, 0, in->stream>>>(part, n_blocks, n_elem, d_out);
+    k_sum_blocks<<<(n_elem + 255) / 256, 256, 0, in->stream>>>(part, n_sum, n_elem, d_out);
     CHECK_LAUNCH(in);
   }
   std::vector<double> tmp(n_elem);

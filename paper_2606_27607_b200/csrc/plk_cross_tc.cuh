@@ -1,0 +1,248 @@
+// plk_cross_tc.cuh -- rate-matrix gradient at 61 states (padded to 64) on the tensor cores (PAPER.md:29,
+// :45-47, reading 14).  Same sum as k_cross64 (plk_cross.cuh):
+//     G[i][j] = sum_b t_b sum_p omega_p ( sum_c w_c r_c q_b[c,p,i] p_b[c,p,j] ) / ( sum_c w_c q_b[c,p]^T p_b[c,p] )
+// For one branch and category this is the contraction  G_c = (diag(s_c) Q_c)^T X_c  over the PATTERN axis: 64 x 64 x P.
+// The partials sit in HBM as [pattern][state], i.e. both operands have the contraction index as their slow index; the
+// mma.sync fragments take that directly from a shared-memory tile (a fragment's k index is the tile row), so nothing is
+// transposed.  fp64: DMMA m8n8k4, the accumulators ARE the fp64 sums.  fp32: split-TF32 m16n8k8 (three products,
+// plk_tc.cuh), fp32 accumulators over one branch (C x 32 patterns), widened into fp64 sums per branch.
+//   work unit = (tile of TP patterns, range of branches); units are dealt round-robin to a fixed grid, a CTA keeps its
+//   64 x 64 sums in registers over all its units and writes ONE partial (fixed order: bitwise repeatable).
+//   per (unit, branch): all C categories of q and p staged with cp.async (the quotient's denominator needs every
+//   category before the first product), den and the per-(category, pattern) factors s, then the products.
+//   4 warps, each a 32 x 32 block of G.  The m / n labels of a fragment are free, so a lane's rows / columns are chosen
+//   adjacent in memory: one 128-bit shared-memory load per operand row gives the values of all of the lane's fragments
+//   (fp32: rows i0 + 4g .. 4g+3 for both m-tiles; fp64: two loads of rows i0 + 2g, +1 and i0 + 16 + 2g, +1), and the
+//   row strides (72 floats / 68 doubles) make those loads conflict-free.
+#pragma once
+#include "plk_common.cuh"
+#include "plk_cross.cuh"
+#include "plk_tc.cuh"
+
+namespace plk {
+
+template <typename T>
+struct CrossTc;
+template <>
+struct CrossTc<float> {
+  static constexpr int TP = 32, LD = 72, KSTEP = 8;
+};
+template <>
+struct CrossTc<double> {
+  static constexpr int TP = 16, LD = 68, KSTEP = 4;
+};
+constexpr int CROSS_TC_THREADS = 128, CROSS_TC_MAX_GRID = 512;
+
+__device__ __forceinline__ void cross_tc_dmma(double& d0, double& d1, double a, double b) {
+  asm("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};" : "+d"(d0), "+d"(d1) : "d"(a), "d"(b));
+}
+
+template <typename T>
+inline size_t cross_tc_smem(int C) {
+  return (size_t)2 * C * CrossTc<T>::TP * CrossTc<T>::LD * sizeof(T) + (size_t)C * CrossTc<T>::TP * sizeof(T);
+}
+
+// rows p0 .. p0+TP-1 of one operand of one category -> tile[row][0..63] (row stride LD); rows beyond P are zero
+template <typename T>
+__device__ __forceinline__ void cross_tc_stage(T* __restrict__ tile, int kind, const void* ptr, int c, int p0, int P, int S) {
+  constexpr int TP = CrossTc<T>::TP, LD = CrossTc<T>::LD, VEC = 16 / (int)sizeof(T), CPR = SP64 / VEC;
+  if (kind == KIND_PARTIALS || kind == KIND_BCAST) {
+    const T* base = static_cast<const T*>(ptr) + (kind == KIND_BCAST ? (size_t)0 : (size_t)c * P * SP64);
+    for (int idx = threadIdx.x; idx < TP * CPR; idx += CROSS_TC_THREADS) {
+      const int row = idx / CPR, ch = idx % CPR;
+      T* dst = tile + row * LD + ch * VEC;
+      if (p0 + row < P) {
+        tc_cp_async16(dst, base + (size_t)(p0 + row) * SP64 + ch * VEC);
+      } else {
+#pragma unroll
+        for (int j = 0; j < VEC; ++j) dst[j] = T(0);
+      }
+    }
+  } else {
+    const uint8_t* st = static_cast<const uint8_t*>(ptr);
+    for (int idx = threadIdx.x; idx < TP * SP64; idx += CROSS_TC_THREADS) {
+      const int row = idx / SP64, x = idx % SP64;
+      T v = T(0);
+      if (kind == KIND_STATES && p0 + row < P) {
+        const int z = st[p0 + row];
+        v = (z >= S) ? (x < S ? T(1) : T(0)) : (x == z ? T(1) : T(0));
+      }
+      tile[row * LD + x] = v;
+    }
+  }
+}
+
+// partial[blockIdx.x][i * 64 + j]; padded rows / columns stay 0 (their operands are 0)
+template <typename T>
+__global__ void __launch_bounds__(CROSS_TC_THREADS, 3) k_cross_tc(const DevCrossBranch* __restrict__ br, int n_br, int n_split,
+                                                                  int n_units, int P, int S, int C,
+                                                                  const double* __restrict__ catw,
+                                                                  const double* __restrict__ catr,
+                                                                  const double* __restrict__ weights,
+                                                                  double* __restrict__ partial) {
+  using K = CrossTc<T>;
+  constexpr int TP = K::TP, LD = K::LD, VEC = 16 / (int)sizeof(T), CPR = SP64 / VEC;
+  using V = typename VecOf<T>::type;
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  T* sQ = reinterpret_cast<T*>(smem_raw);  // [C][TP][LD]
+  T* sX = sQ + (size_t)C * TP * LD;        // [C][TP][LD]
+  T* sScale = sX + (size_t)C * TP * LD;    // [C][TP]
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, g = lane >> 2, t = lane & 3;
+  const int i0 = (warp >> 1) * 32, j0 = (warp & 1) * 32;
+  const int pp = threadIdx.x >> 3, l8 = threadIdx.x & 7;  // den pass: 8 lanes per pattern, 16 patterns per sweep
+
+  double G[32];
+#pragma unroll
+  for (int e = 0; e < 32; ++e) G[e] = 0.0;
+
+  for (int u = blockIdx.x; u < n_units; u += gridDim.x) {
+    const int chunk = u / n_split, sp = u % n_split;
+    const int p0 = chunk * TP;
+    const int b_lo = (int)((long long)sp * n_br / n_split), b_hi = (int)((long long)(sp + 1) * n_br / n_split);
+    for (int b = b_lo; b < b_hi; ++b) {
+      const DevCrossBranch Br = br[b];
+      __syncthreads();  // the products of the previous branch have read the tiles
+      for (int c = 0; c < C; ++c) {
+        cross_tc_stage<T>(sQ + (size_t)c * TP * LD, KIND_PARTIALS, Br.q, c, p0, P, S);
+        cross_tc_stage<T>(sX + (size_t)c * TP * LD, Br.kind, Br.p, c, p0, P, S);
+      }
+      tc_cp_commit();
+      tc_cp_wait<0>();
+      __syncthreads();
+
+      // den_p = sum_c w_c q^T p (fp64 over categories), then s[c][p] = omega_p w_c r_c t_b / den_p
+#pragma unroll
+      for (int sweep = 0; sweep < TP / 16; ++sweep) {
+        const int row = sweep * 16 + pp, p = p0 + row;
+        double den = 0.0;
+        for (int c = 0; c < C; ++c) {
+          const T* q = sQ + ((size_t)c * TP + row) * LD;
+          const T* x = sX + ((size_t)c * TP + row) * LD;
+          T d = T(0);
+#pragma unroll
+          for (int k = 0; k < CPR / 8; ++k) {
+            T qa[VEC], xa[VEC];
+            unpack(*reinterpret_cast<const V*>(q + (l8 + 8 * k) * VEC), qa);
+            unpack(*reinterpret_cast<const V*>(x + (l8 + 8 * k) * VEC), xa);
+#pragma unroll
+            for (int j = 0; j < VEC; ++j) d = fma(qa[j], xa[j], d);
+          }
+          d = lane8_sum(d);
+          den = fma(catw[c], (double)d, den);
+        }
+        for (int c = l8; c < C; c += 8)
+          sScale[c * TP + row] = p < P ? (T)(weights[p] * catw[c] * catr[c] * Br.t / den) : T(0);
+      }
+      __syncthreads();
+
+      if constexpr (sizeof(T) == 4) {
+        float acc[2][4][4];
+#pragma unroll
+        for (int mt = 0; mt < 2; ++mt)
+#pragma unroll
+          for (int nt = 0; nt < 4; ++nt) acc[mt][nt][0] = acc[mt][nt][1] = acc[mt][nt][2] = acc[mt][nt][3] = 0.0f;
+        for (int c = 0; c < C; ++c) {
+          const float* q = sQ + (size_t)c * TP * LD + i0 + 4 * g;
+          const float* x = sX + (size_t)c * TP * LD + j0 + 4 * g;
+          const float* sc = sScale + c * TP;
+#pragma unroll
+          for (int ks = 0; ks < TP / 8; ++ks) {
+            const int r0 = ks * 8 + t, r1 = r0 + 4;
+            const float s0 = sc[r0], s1 = sc[r1];
+            const float4 qa = *reinterpret_cast<const float4*>(q + r0 * LD);
+            const float4 qb = *reinterpret_cast<const float4*>(q + r1 * LD);
+            const float4 xa = *reinterpret_cast<const float4*>(x + r0 * LD);
+            const float4 xb = *reinterpret_cast<const float4*>(x + r1 * LD);
+            // fragment row g <-> state i0 + 4g + 2 mt, row g + 8 <-> i0 + 4g + 2 mt + 1; column n = g of n-tile nt <->
+            // state j0 + 4g + nt
+            uint32_t ah[2][4], al[2][4], bh[4][2], bl[4][2];
+            tc_split(qa.x * s0, ah[0][0], al[0][0]);
+            tc_split(qa.y * s0, ah[0][1], al[0][1]);
+            tc_split(qb.x * s1, ah[0][2], al[0][2]);
+            tc_split(qb.y * s1, ah[0][3], al[0][3]);
+            tc_split(qa.z * s0, ah[1][0], al[1][0]);
+            tc_split(qa.w * s0, ah[1][1], al[1][1]);
+            tc_split(qb.z * s1, ah[1][2], al[1][2]);
+            tc_split(qb.w * s1, ah[1][3], al[1][3]);
+            tc_split(xa.x, bh[0][0], bl[0][0]);
+            tc_split(xb.x, bh[0][1], bl[0][1]);
+            tc_split(xa.y, bh[1][0], bl[1][0]);
+            tc_split(xb.y, bh[1][1], bl[1][1]);
+            tc_split(xa.z, bh[2][0], bl[2][0]);
+            tc_split(xb.z, bh[2][1], bl[2][1]);
+            tc_split(xa.w, bh[3][0], bl[3][0]);
+            tc_split(xb.w, bh[3][1], bl[3][1]);
+#pragma unroll
+            for (int mt = 0; mt < 2; ++mt)
+#pragma unroll
+              for (int nt = 0; nt < 4; ++nt) tc_mma(acc[mt][nt], al[mt], bh[nt]);
+#pragma unroll
+            for (int mt = 0; mt < 2; ++mt)
+#pragma unroll
+              for (int nt = 0; nt < 4; ++nt) tc_mma(acc[mt][nt], ah[mt], bl[nt]);
+#pragma unroll
+            for (int mt = 0; mt < 2; ++mt)
+#pragma unroll
+              for (int nt = 0; nt < 4; ++nt) tc_mma(acc[mt][nt], ah[mt], bh[nt]);
+          }
+        }
+#pragma unroll
+        for (int mt = 0; mt < 2; ++mt)
+#pragma unroll
+          for (int nt = 0; nt < 4; ++nt)
+#pragma unroll
+            for (int e = 0; e < 4; ++e) G[(mt * 4 + nt) * 4 + e] += (double)acc[mt][nt][e];
+      } else {
+        for (int c = 0; c < C; ++c) {
+          const double* q = sQ + (size_t)c * TP * LD + i0 + 2 * g;
+          const double* x = sX + (size_t)c * TP * LD + j0 + 2 * g;
+          const double* sc = sScale + c * TP;
+#pragma unroll
+          for (int ks = 0; ks < TP / 4; ++ks) {
+            const int r = ks * 4 + t;
+            const double s = sc[r];
+            const double2 qa = *reinterpret_cast<const double2*>(q + r * LD);
+            const double2 qb = *reinterpret_cast<const double2*>(q + r * LD + 16);
+            const double2 xa = *reinterpret_cast<const double2*>(x + r * LD);
+            const double2 xb = *reinterpret_cast<const double2*>(x + r * LD + 16);
+            // fragment row g of m-tile mt <-> state i0 + 16 (mt >> 1) + 2g + (mt & 1); the same for columns
+            const double a[4] = {qa.x * s, qa.y * s, qb.x * s, qb.y * s};
+            const double bb[4] = {xa.x, xa.y, xb.x, xb.y};
+#pragma unroll
+            for (int mt = 0; mt < 4; ++mt)
+#pragma unroll
+              for (int nt = 0; nt < 4; ++nt) cross_tc_dmma(G[(mt * 4 + nt) * 2], G[(mt * 4 + nt) * 2 + 1], a[mt], bb[nt]);
+          }
+        }
+      }
+    }
+  }
+
+  double* out = partial + (size_t)blockIdx.x * SP64 * SP64;
+  if constexpr (sizeof(T) == 4) {
+#pragma unroll
+    for (int mt = 0; mt < 2; ++mt)
+#pragma unroll
+      for (int nt = 0; nt < 4; ++nt)
+#pragma unroll
+        for (int e = 0; e < 4; ++e) {
+          // accumulator e: fragment row g (+8 for e >= 2), fragment column 2t + (e & 1)
+          const int i = i0 + 4 * g + 2 * mt + (e >> 1);
+          const int j = j0 + 4 * (2 * t + (e & 1)) + nt;
+          out[i * SP64 + j] = G[(mt * 4 + nt) * 4 + e];
+        }
+  } else {
+#pragma unroll
+    for (int mt = 0; mt < 4; ++mt)
+#pragma unroll
+      for (int nt = 0; nt < 4; ++nt)
+#pragma unroll
+        for (int e = 0; e < 2; ++e) {
+          const int i = i0 + 16 * (mt >> 1) + 2 * g + (mt & 1);
+          const int j = j0 + 16 * (nt >> 1) + 2 * (2 * t + e) + (nt & 1);
+          out[i * SP64 + j] = G[(mt * 4 + nt) * 2 + e];
+        }
+  }
+}
+
+}  // namespace plk

@@ -34,7 +34,12 @@ CASES = [pytest.param(0, None, 700, 4, plk.FP64, 0, id="hky8-fp64"),
          pytest.param(2, 12, 150, 4, plk.FP64, 0, id="gy94-fp64"),
          pytest.param(2, 12, 150, 4, plk.FP32, 0, id="gy94-fp32"),
          pytest.param(2, 12, 150, 4, plk.FP64, plk.FLAG_TENSOR_CORES, id="gy94-fp64-tensor-partials"),
-         pytest.param(2, 12, 33, 2, plk.FP32, plk.FLAG_TENSOR_CORES, id="gy94-fp32-tensor-partials")]
+         pytest.param(2, 12, 33, 2, plk.FP32, plk.FLAG_TENSOR_CORES, id="gy94-fp32-tensor-partials"),
+         # k_cross_tc: several pattern tiles with a ragged tail, more units than one wave would hold branch ranges for
+         pytest.param(2, 12, 1003, 4, plk.FP64, plk.FLAG_TENSOR_CORES, id="gy94-1003-fp64-tensor"),
+         pytest.param(2, 12, 1003, 4, plk.FP32, plk.FLAG_TENSOR_CORES, id="gy94-1003-fp32-tensor"),
+         pytest.param(2, 6, 4100, 3, plk.FP64, plk.FLAG_TENSOR_CORES, id="gy94-4100-3cat-fp64-tensor"),
+         pytest.param(2, 6, 4100, 3, plk.FP32, plk.FLAG_TENSOR_CORES, id="gy94-4100-3cat-fp32-tensor")]
 
 
 @pytest.mark.parametrize("cfg,n_tips,n_pat,n_cat,precision,flags", CASES)
