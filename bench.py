@@ -53,6 +53,8 @@ def parse_args():
     ap.add_argument("--sweep", action="store_true",
                     help="BASELINE configs[4]: HKY fp32, taxa {8,32,128,512} x patterns {1e2..5e5}; prints one JSON "
                          "line with the 20 points instead of the headline line")
+    ap.add_argument("--rate-matrix-gradient", action="store_true",
+                    help="also time plk_rate_matrix_gradient (SURVEY 8(f)-1) on the chosen workload")
     ap.add_argument("--no-extras", action="store_true", help="skip the other configs / precisions")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--shard-patterns", action="store_true",
@@ -319,6 +321,46 @@ def measure_device(wl, precision, flags, steps, warmup, peaks, sampler=None, dev
     return res, ev
 
 
+def measure_rate_matrix_gradient(wl, precision, flags, steps, peaks, device="cuda:0"):
+    """plk_rate_matrix_gradient over every branch, from the pre- and post-order
+    partials an evaluation leaves on the device (tips' pre-order partials stored).  Timed per call with CUDA events on
+    the instance's stream (the call ends with the 32 KB result read back).  Algorithmic bytes: q_k of every branch and
+    p_k of every internal node, read once; flops: 2 S^2 per (branch, pattern, category)."""
+    import torch
+
+    from paper_2606_27607_b200 import plk
+    from paper_2606_27607_b200.client import Evaluator
+
+    prec = plk.FP64 if precision == "fp64" else plk.FP32
+    ev = Evaluator(wl, precision=prec, flags=flags, device=device, store_tip_pre=True)
+    try:
+        ev.log_likelihood(want_site=False)
+        ev.gradient_unfused()
+        for _ in range(3):
+            G = ev.rate_matrix_gradient()
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        stream = torch.cuda.current_stream()
+        e0.record(stream)
+        for _ in range(steps):
+            G = ev.rate_matrix_gradient()
+        e1.record(stream)
+        torch.cuda.synchronize()
+        ms = e0.elapsed_time(e1) / steps
+    finally:
+        ev.close()
+    N, P, S, C = wl.tree.n_tips, wl.n_patterns, wl.n_states, wl.n_categories
+    w = 8 if precision == "fp64" else 4
+    sp = 4 if S == 4 else (32 if S <= 32 else 64)
+    n_br, n_int = 2 * N - 2, N - 2
+    nbytes = (n_br + n_int) * C * P * sp * w + N * P
+    flops = 2.0 * n_br * C * P * S * S
+    return {"ms": ms, "branches": n_br, "algorithmic_bytes": nbytes, "hbm_gbs": nbytes / ms / 1e6,
+            "frac_hbm": nbytes / ms / 1e6 / peaks["hbm_gbs"], "alg_tflops": flops / ms / 1e9,
+            "finite": bool(np.isfinite(G).all()),
+            "kernel": "k_cross4" if S == 4 else ("k_cross_tc" if (flags & 1 and sp == 64) else "k_cross64")}
+
+
 def measure_e2e(ev, wl, steps, warmup):
     """Same evaluation through the host-pointer C-ABI calls a client makes per HMC step: every step uploads the tip
     states (pinned host memory, one pitched copy: plk_set_all_tip_states_u8) and hands HOST branch lengths to
@@ -567,6 +609,11 @@ def run_extras(peaks, steps, warmup, mm):
         if flags & 1 and mm is not None:
             codon.append(codon_roofline(name, wl, prec, "mma.sync" if (prec == "fp64" or flags & 64) else "tcgen05",
                                         res, peaks, mm))
+        if name in ("cfg1_fp32", "cfg2_fp64_tensor", "cfg3_fp32_tensor"):
+            try:
+                out[name]["rate_matrix_gradient"] = measure_rate_matrix_gradient(wl, prec, flags, max(3, steps // 2), peaks)
+            except Exception as exc:
+                out[name]["rate_matrix_gradient"] = {"error": repr(exc)}
     return out, codon
 
 
@@ -754,6 +801,8 @@ def main():
     }
     if mm is not None:
         line["matmul_peaks"] = mm
+    if args.rate_matrix_gradient and not sharded_run:
+        line["rate_matrix_gradient"] = measure_rate_matrix_gradient(wl, args.precision, flags, args.steps, peaks, device)
     if not nuc and args.tensor and mm is not None:
         line["roofline_codon"] = [codon_roofline("headline", wl, args.precision,
                                                  "tcgen05" if (args.precision == "fp32" and args.codon_fp32 == "tcgen05")

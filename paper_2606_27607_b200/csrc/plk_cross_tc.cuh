@@ -39,35 +39,47 @@ __device__ __forceinline__ void cross_tc_dmma(double& d0, double& d1, double a, 
 
 template <typename T>
 inline size_t cross_tc_smem(int C) {
-  return (size_t)2 * C * CrossTc<T>::TP * CrossTc<T>::LD * sizeof(T) + (size_t)C * CrossTc<T>::TP * sizeof(T);
+  return (size_t)2 * C * CrossTc<T>::TP * CrossTc<T>::LD * sizeof(T) + (size_t)2 * C * 8 + (size_t)C * CrossTc<T>::TP * sizeof(T);
 }
 
-// rows p0 .. p0+TP-1 of one operand of one category -> tile[row][0..63] (row stride LD); rows beyond P are zero
+// rows p0 .. p0+TP-1 of one category of full partials (`base` = that category's [P][64] plane) -> tile[row][0..63]
+// (row stride LD); rows beyond P are zero.  A thread keeps its 16-byte column and takes every RPP-th row.
 template <typename T>
-__device__ __forceinline__ void cross_tc_stage(T* __restrict__ tile, int kind, const void* ptr, int c, int p0, int P, int S) {
+__device__ __forceinline__ void cross_tc_stage_partials(T* __restrict__ tile, const T* __restrict__ base, int p0, int P) {
   constexpr int TP = CrossTc<T>::TP, LD = CrossTc<T>::LD, VEC = 16 / (int)sizeof(T), CPR = SP64 / VEC;
-  if (kind == KIND_PARTIALS || kind == KIND_BCAST) {
-    const T* base = static_cast<const T*>(ptr) + (kind == KIND_BCAST ? (size_t)0 : (size_t)c * P * SP64);
-    for (int idx = threadIdx.x; idx < TP * CPR; idx += CROSS_TC_THREADS) {
-      const int row = idx / CPR, ch = idx % CPR;
-      T* dst = tile + row * LD + ch * VEC;
-      if (p0 + row < P) {
-        tc_cp_async16(dst, base + (size_t)(p0 + row) * SP64 + ch * VEC);
+  constexpr int RPP = CROSS_TC_THREADS / CPR, PASSES = TP / RPP;
+  const int ch = threadIdx.x % CPR, r0 = threadIdx.x / CPR;
+  const T* src = base + (size_t)(p0 + r0) * SP64 + ch * VEC;
+  T* dst = tile + r0 * LD + ch * VEC;
+  if (p0 + TP <= P) {
+#pragma unroll
+    for (int k = 0; k < PASSES; ++k) tc_cp_async16(dst + k * RPP * LD, src + (size_t)k * RPP * SP64);
+  } else {
+#pragma unroll
+    for (int k = 0; k < PASSES; ++k) {
+      if (p0 + r0 + k * RPP < P) {
+        tc_cp_async16(dst + k * RPP * LD, src + (size_t)k * RPP * SP64);
       } else {
 #pragma unroll
-        for (int j = 0; j < VEC; ++j) dst[j] = T(0);
+        for (int j = 0; j < VEC; ++j) dst[k * RPP * LD + j] = T(0);
       }
     }
-  } else {
-    const uint8_t* st = static_cast<const uint8_t*>(ptr);
-    for (int idx = threadIdx.x; idx < TP * SP64; idx += CROSS_TC_THREADS) {
-      const int row = idx / SP64, x = idx % SP64;
-      T v = T(0);
-      if (kind == KIND_STATES && p0 + row < P) {
-        const int z = st[p0 + row];
-        v = (z >= S) ? (x < S ? T(1) : T(0)) : (x == z ? T(1) : T(0));
-      }
-      tile[row * LD + x] = v;
+  }
+}
+// compact tip states (st == nullptr: an absent operand, zeros): indicator rows, the same for every category
+template <typename T>
+__device__ __forceinline__ void cross_tc_stage_states(T* __restrict__ tile, const uint8_t* __restrict__ st, int p0, int P, int S) {
+  constexpr int TP = CrossTc<T>::TP, LD = CrossTc<T>::LD, VEC = 16 / (int)sizeof(T), CPR = SP64 / VEC;
+  constexpr int RPP = CROSS_TC_THREADS / CPR, PASSES = TP / RPP;
+  const int ch = threadIdx.x % CPR, r0 = threadIdx.x / CPR;
+#pragma unroll
+  for (int k = 0; k < PASSES; ++k) {
+    const int row = r0 + k * RPP;
+    const int z = (st != nullptr && p0 + row < P) ? (int)st[p0 + row] : -1;
+#pragma unroll
+    for (int j = 0; j < VEC; ++j) {
+      const int x = ch * VEC + j;
+      tile[row * LD + x] = z < 0 ? T(0) : (z >= S ? (x < S ? T(1) : T(0)) : (x == z ? T(1) : T(0)));
     }
   }
 }
@@ -86,7 +98,12 @@ __global__ void __launch_bounds__(CROSS_TC_THREADS, 3) k_cross_tc(const DevCross
   extern __shared__ __align__(16) unsigned char smem_raw[];
   T* sQ = reinterpret_cast<T*>(smem_raw);  // [C][TP][LD]
   T* sX = sQ + (size_t)C * TP * LD;        // [C][TP][LD]
-  T* sScale = sX + (size_t)C * TP * LD;    // [C][TP]
+  double* sW = reinterpret_cast<double*>(sX + (size_t)C * TP * LD);  // w_c [C], then w_c r_c [C]
+  T* sScale = reinterpret_cast<T*>(sW + 2 * C);                        // [C][TP]
+  if (threadIdx.x < C) {
+    sW[threadIdx.x] = catw[threadIdx.x];
+    sW[C + threadIdx.x] = catw[threadIdx.x] * catr[threadIdx.x];
+  }
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, g = lane >> 2, t = lane & 3;
   const int i0 = (warp >> 1) * 32, j0 = (warp & 1) * 32;
   const int pp = threadIdx.x >> 3, l8 = threadIdx.x & 7;  // den pass: 8 lanes per pattern, 16 patterns per sweep
@@ -102,22 +119,33 @@ __global__ void __launch_bounds__(CROSS_TC_THREADS, 3) k_cross_tc(const DevCross
     for (int b = b_lo; b < b_hi; ++b) {
       const DevCrossBranch Br = br[b];
       __syncthreads();  // the products of the previous branch have read the tiles
+      // a tip's operand (compact states, single-category partials) is the same for every category: staged once
+      const bool per_cat = Br.kind == KIND_PARTIALS;
+      const size_t xstep = per_cat ? (size_t)TP * LD : 0;
       for (int c = 0; c < C; ++c) {
-        cross_tc_stage<T>(sQ + (size_t)c * TP * LD, KIND_PARTIALS, Br.q, c, p0, P, S);
-        cross_tc_stage<T>(sX + (size_t)c * TP * LD, Br.kind, Br.p, c, p0, P, S);
+        cross_tc_stage_partials<T>(sQ + (size_t)c * TP * LD, static_cast<const T*>(Br.q) + (size_t)c * P * SP64, p0, P);
+        if (per_cat) cross_tc_stage_partials<T>(sX + (size_t)c * TP * LD, static_cast<const T*>(Br.p) + (size_t)c * P * SP64, p0, P);
       }
+      if (Br.kind == KIND_BCAST) cross_tc_stage_partials<T>(sX, static_cast<const T*>(Br.p), p0, P);
+      else if (!per_cat) cross_tc_stage_states<T>(sX, Br.kind == KIND_STATES ? static_cast<const uint8_t*>(Br.p) : nullptr, p0, P, S);
       tc_cp_commit();
+      double wt_row[TP / 16];  // omega_p t_b of this thread's den rows, in flight while the tiles arrive
+#pragma unroll
+      for (int sweep = 0; sweep < TP / 16; ++sweep) {
+        const int p = p0 + sweep * 16 + pp;
+        wt_row[sweep] = p < P ? weights[p] * Br.t : 0.0;
+      }
       tc_cp_wait<0>();
       __syncthreads();
 
       // den_p = sum_c w_c q^T p (fp64 over categories), then s[c][p] = omega_p w_c r_c t_b / den_p
 #pragma unroll
       for (int sweep = 0; sweep < TP / 16; ++sweep) {
-        const int row = sweep * 16 + pp, p = p0 + row;
+        const int row = sweep * 16 + pp;
         double den = 0.0;
         for (int c = 0; c < C; ++c) {
           const T* q = sQ + ((size_t)c * TP + row) * LD;
-          const T* x = sX + ((size_t)c * TP + row) * LD;
+          const T* x = sX + c * xstep + (size_t)row * LD;
           T d = T(0);
 #pragma unroll
           for (int k = 0; k < CPR / 8; ++k) {
@@ -128,10 +156,10 @@ __global__ void __launch_bounds__(CROSS_TC_THREADS, 3) k_cross_tc(const DevCross
             for (int j = 0; j < VEC; ++j) d = fma(qa[j], xa[j], d);
           }
           d = lane8_sum(d);
-          den = fma(catw[c], (double)d, den);
+          den = fma(sW[c], (double)d, den);
         }
-        for (int c = l8; c < C; c += 8)
-          sScale[c * TP + row] = p < P ? (T)(weights[p] * catw[c] * catr[c] * Br.t / den) : T(0);
+        const double f = wt_row[sweep] != 0.0 ? wt_row[sweep] / den : 0.0;  // rows beyond P (den = 0) and weight 0: factor 0
+        for (int c = l8; c < C; c += 8) sScale[c * TP + row] = (T)(sW[C + c] * f);
       }
       __syncthreads();
 
@@ -143,7 +171,7 @@ __global__ void __launch_bounds__(CROSS_TC_THREADS, 3) k_cross_tc(const DevCross
           for (int nt = 0; nt < 4; ++nt) acc[mt][nt][0] = acc[mt][nt][1] = acc[mt][nt][2] = acc[mt][nt][3] = 0.0f;
         for (int c = 0; c < C; ++c) {
           const float* q = sQ + (size_t)c * TP * LD + i0 + 4 * g;
-          const float* x = sX + (size_t)c * TP * LD + j0 + 4 * g;
+          const float* x = sX + c * xstep + j0 + 4 * g;
           const float* sc = sScale + c * TP;
 #pragma unroll
           for (int ks = 0; ks < TP / 8; ++ks) {
@@ -195,7 +223,7 @@ __global__ void __launch_bounds__(CROSS_TC_THREADS, 3) k_cross_tc(const DevCross
       } else {
         for (int c = 0; c < C; ++c) {
           const double* q = sQ + (size_t)c * TP * LD + i0 + 2 * g;
-          const double* x = sX + (size_t)c * TP * LD + j0 + 2 * g;
+          const double* x = sX + c * xstep + j0 + 2 * g;
           const double* sc = sScale + c * TP;
 #pragma unroll
           for (int ks = 0; ks < TP / 4; ++ks) {
