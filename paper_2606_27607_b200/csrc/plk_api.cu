@@ -2171,7 +2171,8 @@ int plk_rate_matrix_gradient(plk_instance* in, const int32_t* post_idx, const in
         // tensor cores (plk_cross_tc.cuh): units = pattern tiles x branch ranges, dealt round-robin to a fixed grid
         const size_t smem = cross_tc_smem<T>(L.C);
         if (smem + 1024 > 232448) return PLK_ERR_UNSUPPORTED;
-        int r4 = opt_in_smem(k_cross_tc<T>, smem);
+        auto kern = L.C == 4 ? k_cross_tc<T, 4> : k_cross_tc<T, 0>;
+        int r4 = opt_in_smem(kern, smem);
         if (r4) return r4;
         const int per_sm = std::min(3, (int)(233472 / (smem + 1024)));
         const int slots = std::min(CROSS_TC_MAX_GRID, in->sm_count * per_sm);
@@ -2179,7 +2180,7 @@ int plk_rate_matrix_gradient(plk_instance* in, const int32_t* post_idx, const in
         const int n_split = std::max(1, std::min(count, (8 * slots + chunks - 1) / chunks));
         const long long units = (long long)chunks * n_split;
         n_sum = (int)std::min<long long>(units, slots);
-        k_cross_tc<T><<<n_sum, CROSS_TC_THREADS, smem, in->stream>>>(db, count, n_split, (int)units, L.P, L.S, L.C, cw, cr, wt, part);
+        kern<<<n_sum, CROSS_TC_THREADS, smem, in->stream>>>(db, count, n_split, (int)units, L.P, L.S, L.C, cw, cr, wt, part);
         return PLK_SUCCESS;
       }
       int r2 = opt_in_smem(k_cross64<T>, cross64_smem<T>());

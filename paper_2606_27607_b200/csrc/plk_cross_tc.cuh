@@ -5,7 +5,9 @@
 // The partials sit in HBM as [pattern][state], i.e. both operands have the contraction index as their slow index; the
 // mma.sync fragments take that directly from a shared-memory tile (a fragment's k index is the tile row), so nothing is
 // transposed.  fp64: DMMA m8n8k4, the accumulators ARE the fp64 sums.  fp32: split-TF32 m16n8k8 (three products,
-// plk_tc.cuh), fp32 accumulators over one branch (C x 32 patterns), widened into fp64 sums per branch.
+// plk_tc.cuh), fp32 accumulators over one branch (C x 32 patterns), widened into fp64 sums per branch.  In fp32 a
+// compact tip (the other half of the branches) is never staged: its indicator rows are formed from the state in
+// registers, exact in TF32, so its low-part product is skipped.
 //   work unit = (tile of TP patterns, range of branches); units are dealt round-robin to a fixed grid, a CTA keeps its
 //   64 x 64 sums in registers over all its units and writes ONE partial (fixed order: bitwise repeatable).
 //   per (unit, branch): all C categories of q and p staged with cp.async (the quotient's denominator needs every
@@ -39,7 +41,8 @@ __device__ __forceinline__ void cross_tc_dmma(double& d0, double& d1, double a, 
 
 template <typename T>
 inline size_t cross_tc_smem(int C) {
-  return (size_t)2 * C * CrossTc<T>::TP * CrossTc<T>::LD * sizeof(T) + (size_t)2 * C * 8 + (size_t)C * CrossTc<T>::TP * sizeof(T);
+  return (size_t)2 * C * CrossTc<T>::TP * CrossTc<T>::LD * sizeof(T) + (size_t)2 * C * sizeof(T) + (size_t)C * CrossTc<T>::TP * sizeof(T) +
+         (size_t)CrossTc<T>::TP * 4;
 }
 
 // rows p0 .. p0+TP-1 of one category of full partials (`base` = that category's [P][64] plane) -> tile[row][0..63]
@@ -84,8 +87,15 @@ __device__ __forceinline__ void cross_tc_stage_states(T* __restrict__ tile, cons
   }
 }
 
-// partial[blockIdx.x][i * 64 + j]; padded rows / columns stay 0 (their operands are 0)
+// indicator of a compact tip state z at state x (z < 0: a row beyond P, zeros; z >= S: missing, 1 for every real state)
 template <typename T>
+__device__ __forceinline__ T cross_tc_ind(int z, int x, int S) {
+  return z < 0 ? T(0) : (z >= S ? (x < S ? T(1) : T(0)) : (x == z ? T(1) : T(0)));
+}
+
+// partial[blockIdx.x][i * 64 + j]; padded rows / columns stay 0 (their operands are 0).  CC = the category count as a
+// compile-time constant (loops unrolled), 0 = the runtime value C.
+template <typename T, int CC>
 __global__ void __launch_bounds__(CROSS_TC_THREADS, 3) k_cross_tc(const DevCrossBranch* __restrict__ br, int n_br, int n_split,
                                                                   int n_units, int P, int S, int C,
                                                                   const double* __restrict__ catw,
@@ -93,20 +103,25 @@ __global__ void __launch_bounds__(CROSS_TC_THREADS, 3) k_cross_tc(const DevCross
                                                                   const double* __restrict__ weights,
                                                                   double* __restrict__ partial) {
   using K = CrossTc<T>;
-  constexpr int TP = K::TP, LD = K::LD, VEC = 16 / (int)sizeof(T), CPR = SP64 / VEC;
+  constexpr int TP = K::TP, LD = K::LD, VEC = 16 / (int)sizeof(T), CPR = SP64 / VEC, NR = TP / 16;
+  // fp32: a compact tip is never staged, its indicator rows are formed in registers (exact in TF32: no low-part
+  // product); fp64: staged once for all categories (forming 64-bit indicators per k-step was slower than reading them)
+  constexpr bool REG_TIPS = sizeof(T) == 4;
   using V = typename VecOf<T>::type;
+  const int Cn = CC ? CC : C;
   extern __shared__ __align__(16) unsigned char smem_raw[];
   T* sQ = reinterpret_cast<T*>(smem_raw);  // [C][TP][LD]
-  T* sX = sQ + (size_t)C * TP * LD;        // [C][TP][LD]
-  double* sW = reinterpret_cast<double*>(sX + (size_t)C * TP * LD);  // w_c [C], then w_c r_c [C]
-  T* sScale = reinterpret_cast<T*>(sW + 2 * C);                        // [C][TP]
-  if (threadIdx.x < C) {
-    sW[threadIdx.x] = catw[threadIdx.x];
-    sW[C + threadIdx.x] = catw[threadIdx.x] * catr[threadIdx.x];
+  T* sX = sQ + (size_t)Cn * TP * LD;       // [C][TP][LD]
+  T* sW = sX + (size_t)Cn * TP * LD;       // w_c [C], then w_c r_c [C]
+  T* sScale = sW + 2 * Cn;                 // [C][TP]
+  int* sZ = reinterpret_cast<int*>(sScale + Cn * TP);  // [TP] compact tip states of the item (-1 beyond P)
+  if (threadIdx.x < Cn) {
+    sW[threadIdx.x] = (T)catw[threadIdx.x];
+    sW[Cn + threadIdx.x] = (T)(catw[threadIdx.x] * catr[threadIdx.x]);
   }
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, g = lane >> 2, t = lane & 3;
   const int i0 = (warp >> 1) * 32, j0 = (warp & 1) * 32;
-  const int pp = threadIdx.x >> 3, l8 = threadIdx.x & 7;  // den pass: 8 lanes per pattern, 16 patterns per sweep
+  const int pp = threadIdx.x >> 3, l8 = threadIdx.x & 7;  // den pass: 8 lanes per pattern, rows pp (+ 16)
 
   double G[32];
 #pragma unroll
@@ -119,47 +134,69 @@ __global__ void __launch_bounds__(CROSS_TC_THREADS, 3) k_cross_tc(const DevCross
     for (int b = b_lo; b < b_hi; ++b) {
       const DevCrossBranch Br = br[b];
       __syncthreads();  // the products of the previous branch have read the tiles
-      // a tip's operand (compact states, single-category partials) is the same for every category: staged once
+      // a tip's operand is the same for every category: staged once, or (REG_TIPS) not at all
       const bool per_cat = Br.kind == KIND_PARTIALS;
+      const bool tip_states = Br.kind == KIND_STATES || Br.kind == KIND_NONE;
+      const bool states = REG_TIPS && tip_states;
       const size_t xstep = per_cat ? (size_t)TP * LD : 0;
-      for (int c = 0; c < C; ++c) {
+      if (states && threadIdx.x < TP)
+        sZ[threadIdx.x] = (Br.kind == KIND_STATES && p0 + threadIdx.x < P) ? (int)static_cast<const uint8_t*>(Br.p)[p0 + threadIdx.x] : -1;
+#pragma unroll
+      for (int c = 0; c < Cn; ++c) {
         cross_tc_stage_partials<T>(sQ + (size_t)c * TP * LD, static_cast<const T*>(Br.q) + (size_t)c * P * SP64, p0, P);
         if (per_cat) cross_tc_stage_partials<T>(sX + (size_t)c * TP * LD, static_cast<const T*>(Br.p) + (size_t)c * P * SP64, p0, P);
       }
       if (Br.kind == KIND_BCAST) cross_tc_stage_partials<T>(sX, static_cast<const T*>(Br.p), p0, P);
-      else if (!per_cat) cross_tc_stage_states<T>(sX, Br.kind == KIND_STATES ? static_cast<const uint8_t*>(Br.p) : nullptr, p0, P, S);
+      if (!REG_TIPS && tip_states)
+        cross_tc_stage_states<T>(sX, Br.kind == KIND_STATES ? static_cast<const uint8_t*>(Br.p) : nullptr, p0, P, S);
       tc_cp_commit();
-      double wt_row[TP / 16];  // omega_p t_b of this thread's den rows, in flight while the tiles arrive
+      T wt_row[NR];  // omega_p t_b of this thread's den rows, in flight while the tiles arrive
 #pragma unroll
-      for (int sweep = 0; sweep < TP / 16; ++sweep) {
-        const int p = p0 + sweep * 16 + pp;
-        wt_row[sweep] = p < P ? weights[p] * Br.t : 0.0;
+      for (int rr = 0; rr < NR; ++rr) {
+        const int p = p0 + rr * 16 + pp;
+        wt_row[rr] = p < P ? (T)(weights[p] * Br.t) : T(0);
       }
       tc_cp_wait<0>();
       __syncthreads();
 
-      // den_p = sum_c w_c q^T p (fp64 over categories), then s[c][p] = omega_p w_c r_c t_b / den_p
+      // den_p = sum_c w_c q^T p, then s[c][p] = omega_p w_c r_c t_b / den_p   (working precision: the quotient's
+      // error is that of the products it scales)
+      {
+        T dsum[NR];
 #pragma unroll
-      for (int sweep = 0; sweep < TP / 16; ++sweep) {
-        const int row = sweep * 16 + pp;
-        double den = 0.0;
-        for (int c = 0; c < C; ++c) {
-          const T* q = sQ + ((size_t)c * TP + row) * LD;
-          const T* x = sX + c * xstep + (size_t)row * LD;
-          T d = T(0);
+        for (int rr = 0; rr < NR; ++rr) {
+          const int row = rr * 16 + pp;
+          const int z = states ? sZ[row] : 0;
+          T ds = T(0);
 #pragma unroll
-          for (int k = 0; k < CPR / 8; ++k) {
-            T qa[VEC], xa[VEC];
-            unpack(*reinterpret_cast<const V*>(q + (l8 + 8 * k) * VEC), qa);
-            unpack(*reinterpret_cast<const V*>(x + (l8 + 8 * k) * VEC), xa);
+          for (int c = 0; c < Cn; ++c) {
+            const T* q = sQ + ((size_t)c * TP + row) * LD;
+            const T* x = sX + c * xstep + (size_t)row * LD;
+            T d[2] = {T(0), T(0)};
 #pragma unroll
-            for (int j = 0; j < VEC; ++j) d = fma(qa[j], xa[j], d);
+            for (int k = 0; k < CPR / 8; ++k) {
+              T qa[VEC], xa[VEC];
+              unpack(*reinterpret_cast<const V*>(q + (l8 + 8 * k) * VEC), qa);
+              if (states) {
+#pragma unroll
+                for (int j = 0; j < VEC; ++j) xa[j] = cross_tc_ind<T>(z, (l8 + 8 * k) * VEC + j, S);
+              } else {
+                unpack(*reinterpret_cast<const V*>(x + (l8 + 8 * k) * VEC), xa);
+              }
+#pragma unroll
+              for (int j = 0; j < VEC; ++j) d[k & 1] = fma(qa[j], xa[j], d[k & 1]);
+            }
+            ds = fma(sW[c], d[0] + d[1], ds);
           }
-          d = lane8_sum(d);
-          den = fma(sW[c], (double)d, den);
+          dsum[rr] = ds;
         }
-        const double f = wt_row[sweep] != 0.0 ? wt_row[sweep] / den : 0.0;  // rows beyond P (den = 0) and weight 0: factor 0
-        for (int c = l8; c < C; c += 8) sScale[c * TP + row] = (T)(sW[C + c] * f);
+#pragma unroll
+        for (int rr = 0; rr < NR; ++rr) dsum[rr] = lane8_sum(dsum[rr]);
+#pragma unroll
+        for (int rr = 0; rr < NR; ++rr) {
+          const T f = wt_row[rr] != T(0) ? wt_row[rr] / dsum[rr] : T(0);  // rows beyond P (den = 0), weight 0: factor 0
+          for (int c = l8; c < Cn; c += 8) sScale[c * TP + rr * 16 + pp] = sW[Cn + c] * f;
+        }
       }
       __syncthreads();
 
@@ -169,7 +206,8 @@ __global__ void __launch_bounds__(CROSS_TC_THREADS, 3) k_cross_tc(const DevCross
         for (int mt = 0; mt < 2; ++mt)
 #pragma unroll
           for (int nt = 0; nt < 4; ++nt) acc[mt][nt][0] = acc[mt][nt][1] = acc[mt][nt][2] = acc[mt][nt][3] = 0.0f;
-        for (int c = 0; c < C; ++c) {
+#pragma unroll 1
+        for (int c = 0; c < Cn; ++c) {
           const float* q = sQ + (size_t)c * TP * LD + i0 + 4 * g;
           const float* x = sX + c * xstep + j0 + 4 * g;
           const float* sc = sScale + c * TP;
@@ -179,8 +217,6 @@ __global__ void __launch_bounds__(CROSS_TC_THREADS, 3) k_cross_tc(const DevCross
             const float s0 = sc[r0], s1 = sc[r1];
             const float4 qa = *reinterpret_cast<const float4*>(q + r0 * LD);
             const float4 qb = *reinterpret_cast<const float4*>(q + r1 * LD);
-            const float4 xa = *reinterpret_cast<const float4*>(x + r0 * LD);
-            const float4 xb = *reinterpret_cast<const float4*>(x + r1 * LD);
             // fragment row g <-> state i0 + 4g + 2 mt, row g + 8 <-> i0 + 4g + 2 mt + 1; column n = g of n-tile nt <->
             // state j0 + 4g + nt
             uint32_t ah[2][4], al[2][4], bh[4][2], bl[4][2];
@@ -192,22 +228,35 @@ __global__ void __launch_bounds__(CROSS_TC_THREADS, 3) k_cross_tc(const DevCross
             tc_split(qa.w * s0, ah[1][1], al[1][1]);
             tc_split(qb.z * s1, ah[1][2], al[1][2]);
             tc_split(qb.w * s1, ah[1][3], al[1][3]);
-            tc_split(xa.x, bh[0][0], bl[0][0]);
-            tc_split(xb.x, bh[0][1], bl[0][1]);
-            tc_split(xa.y, bh[1][0], bl[1][0]);
-            tc_split(xb.y, bh[1][1], bl[1][1]);
-            tc_split(xa.z, bh[2][0], bl[2][0]);
-            tc_split(xb.z, bh[2][1], bl[2][1]);
-            tc_split(xa.w, bh[3][0], bl[3][0]);
-            tc_split(xb.w, bh[3][1], bl[3][1]);
+            if (states) {  // indicator rows: exact in TF32, no low part
+              const int z0 = sZ[r0], z1 = sZ[r1];
+#pragma unroll
+              for (int nt = 0; nt < 4; ++nt) {
+                bh[nt][0] = __float_as_uint(cross_tc_ind<float>(z0, j0 + 4 * g + nt, S));
+                bh[nt][1] = __float_as_uint(cross_tc_ind<float>(z1, j0 + 4 * g + nt, S));
+              }
+            } else {
+              const float4 xa = *reinterpret_cast<const float4*>(x + r0 * LD);
+              const float4 xb = *reinterpret_cast<const float4*>(x + r1 * LD);
+              tc_split(xa.x, bh[0][0], bl[0][0]);
+              tc_split(xb.x, bh[0][1], bl[0][1]);
+              tc_split(xa.y, bh[1][0], bl[1][0]);
+              tc_split(xb.y, bh[1][1], bl[1][1]);
+              tc_split(xa.z, bh[2][0], bl[2][0]);
+              tc_split(xb.z, bh[2][1], bl[2][1]);
+              tc_split(xa.w, bh[3][0], bl[3][0]);
+              tc_split(xb.w, bh[3][1], bl[3][1]);
+            }
 #pragma unroll
             for (int mt = 0; mt < 2; ++mt)
 #pragma unroll
               for (int nt = 0; nt < 4; ++nt) tc_mma(acc[mt][nt], al[mt], bh[nt]);
+            if (!states) {
 #pragma unroll
-            for (int mt = 0; mt < 2; ++mt)
+              for (int mt = 0; mt < 2; ++mt)
 #pragma unroll
-              for (int nt = 0; nt < 4; ++nt) tc_mma(acc[mt][nt], ah[mt], bl[nt]);
+                for (int nt = 0; nt < 4; ++nt) tc_mma(acc[mt][nt], ah[mt], bl[nt]);
+            }
 #pragma unroll
             for (int mt = 0; mt < 2; ++mt)
 #pragma unroll
@@ -221,7 +270,7 @@ __global__ void __launch_bounds__(CROSS_TC_THREADS, 3) k_cross_tc(const DevCross
 #pragma unroll
             for (int e = 0; e < 4; ++e) G[(mt * 4 + nt) * 4 + e] += (double)acc[mt][nt][e];
       } else {
-        for (int c = 0; c < C; ++c) {
+        for (int c = 0; c < Cn; ++c) {
           const double* q = sQ + (size_t)c * TP * LD + i0 + 2 * g;
           const double* x = sX + c * xstep + j0 + 2 * g;
           const double* sc = sScale + c * TP;
@@ -231,11 +280,18 @@ __global__ void __launch_bounds__(CROSS_TC_THREADS, 3) k_cross_tc(const DevCross
             const double s = sc[r];
             const double2 qa = *reinterpret_cast<const double2*>(q + r * LD);
             const double2 qb = *reinterpret_cast<const double2*>(q + r * LD + 16);
-            const double2 xa = *reinterpret_cast<const double2*>(x + r * LD);
-            const double2 xb = *reinterpret_cast<const double2*>(x + r * LD + 16);
             // fragment row g of m-tile mt <-> state i0 + 16 (mt >> 1) + 2g + (mt & 1); the same for columns
             const double a[4] = {qa.x * s, qa.y * s, qb.x * s, qb.y * s};
-            const double bb[4] = {xa.x, xa.y, xb.x, xb.y};
+            double bb[4];
+            if (states) {
+              const int z = sZ[r];
+#pragma unroll
+              for (int nt = 0; nt < 4; ++nt) bb[nt] = cross_tc_ind<double>(z, j0 + 16 * (nt >> 1) + 2 * g + (nt & 1), S);
+            } else {
+              const double2 xa = *reinterpret_cast<const double2*>(x + r * LD);
+              const double2 xb = *reinterpret_cast<const double2*>(x + r * LD + 16);
+              bb[0] = xa.x; bb[1] = xa.y; bb[2] = xb.x; bb[3] = xb.y;
+            }
 #pragma unroll
             for (int mt = 0; mt < 4; ++mt)
 #pragma unroll
