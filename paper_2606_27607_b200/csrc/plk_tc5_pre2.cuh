@@ -79,8 +79,8 @@ static_assert(2 * TAB_BYTES <= 2 * PLANE_A, "tip tables fit the [M_1; D_1] slot"
 static_assert(SMEM_BYTES2 <= 232448, "shared memory budget");
 
 // every barrier completes exactly once per round (MATFULL / MATFREE: once per segment)
-enum { B_XFULL_A = 0,  // first tile of the round stored (producers)
-       B_XFULL_B,      // second tile stored (class 0)
+enum { B_XFULL_A = 0,  // first tile of the round stored (producers); class 1: even rounds
+       B_XFULL_B,      // second tile stored (class 0); class 1: the tile of odd rounds
        B_REGFREE,      // the second child's step A has run: its X region is free (commit)
        B_QREAD,        // the epilogue has read the round's q_k: the region they sat in is free
        B_QREAD1,       // class 1 only: rounds alternate between B_QREAD (even) and B_QREAD1 (odd), see the producers
@@ -313,7 +313,13 @@ __global__ void __launch_bounds__(THREADS, 1)
         ++seg;
       }
       if (++tile == cx.n_tiles) tile = 0;
-      mbar_wait(cx.barrier(B_XFULL_A), par);
+      // Class 1 has no wait that ties a producer warp to the CURRENT round (its next store only needs the q_0 of two
+      // rounds ago to have been read), so a fast warp may be one round ahead of a slow one: with a single barrier its
+      // arrival for round ui + 1 would complete the phase of round ui without the slow warp's rows (seen as rare
+      // last-bits differences between repeated evaluations, a few rows of one quarter of a tile).  Even and odd rounds
+      // therefore arrive on two barriers, as for QREAD / QREAD1.
+      if (CLS == 0) mbar_wait(cx.barrier(B_XFULL_A), par);
+      else mbar_wait(cx.barrier(par ? B_XFULL_B : B_XFULL_A), (ui >> 1) & 1);
       tc_fence_after();
       if (CLS == 0) {
         const int f = (int)par;  // first child = region index
@@ -520,7 +526,7 @@ __global__ void __launch_bounds__(THREADS, 1)
         }
         tc_fence_after();
         store_tile(T_REG * par);
-        if (lane == 0) mbar_arrive(cx.barrier(B_XFULL_A));
+        if (lane == 0) mbar_arrive(cx.barrier((CLS == 1 && par) ? B_XFULL_B : B_XFULL_A));  // class 1: see the MMA warp
         if (ld.ui < cx.n_rounds) load_tile(ld);
         tile_next(ld);
         prefetch_tile(pf);

@@ -7,7 +7,7 @@ every output is compared: all site log-likelihoods element by element, logL, eve
 of SURVEY 8(c) row 18) and all per-pattern derivatives.  The one exception is the largest sweep point of configs[4]
 (512 taxa x 500 000 patterns, 49 GB of partials, minutes of oracle time): there 60 seeded patterns out of every
 block of 10 000 (3 000 in all) are compared one by one and the rest is covered by properties that hold at any size.
-No assertion below compares the library with itself except the bitwise repeatability check."""
+No assertion below compares the library with itself except the bitwise repeatability checks."""
 import numpy as np
 import pytest
 
@@ -69,6 +69,30 @@ def test_full_size_all_patterns(cfg, n_tips, n_patterns, precision, flags):
     assert abs(grad[a] - grad[b]) <= pc.tol_of(precision) * max(ref["cond"][a], ref["cond"][b])
     # repeatability (fixed-order reductions, no atomics): the only library-vs-library comparison in this file
     assert logl2 == logl and np.array_equal(grad2, grad)
+
+
+@pytest.mark.parametrize("precision,flags", [pytest.param(plk.FP32, plk.FLAG_TENSOR_CORES, id="cfg3-fp32-tcgen05"),
+                                             pytest.param(plk.FP64, plk.FLAG_TENSOR_CORES, id="cfg3-fp64-dmma")])
+def test_repeated_evaluations_are_bitwise_equal(precision, flags):
+    """Forty evaluations of configs[3] in a row: logL, every branch gradient and every per-pattern derivative bitwise
+    equal to the first.  The warp-specialised kernels hand tiles between warps through phase-counted barriers; a
+    protocol error shows up as rare last-bits differences in a few rows of a tile (round 2: the class-1 producers of
+    k_pre_tc5v could complete another round's phase -- 9 % of the evaluations at this size differed), which a single
+    repeat does not catch reliably.  Library against itself: repeatability only, parity is the test above."""
+    wl = workloads.config(3)
+    ev = Evaluator(wl, precision=precision, flags=flags | plk.FLAG_SITE_DERIVATIVES)
+    try:
+        logl0, _ = ev.log_likelihood(want_site=False)
+        g0, s0 = ev.gradient(want_site=True)
+        for it in range(40):
+            if it % 4 == 0:
+                logl, _ = ev.log_likelihood(want_site=False)
+                assert logl == logl0
+            g, s = ev.gradient(want_site=True)
+            assert np.array_equal(g, g0), f"evaluation {it}: gradient differs at nodes {np.nonzero(g != g0)[0][:8]}"
+            assert np.array_equal(s, s0), f"evaluation {it}: per-pattern derivatives differ at {np.argwhere(s != s0)[:8]}"
+    finally:
+        ev.close()
 
 
 def test_largest_sweep_point_sampled():
