@@ -71,15 +71,19 @@ def test_full_size_all_patterns(cfg, n_tips, n_patterns, precision, flags):
     assert logl2 == logl and np.array_equal(grad2, grad)
 
 
-@pytest.mark.parametrize("precision,flags", [pytest.param(plk.FP32, plk.FLAG_TENSOR_CORES, id="cfg3-fp32-tcgen05"),
-                                             pytest.param(plk.FP64, plk.FLAG_TENSOR_CORES, id="cfg3-fp64-dmma")])
-def test_repeated_evaluations_are_bitwise_equal(precision, flags):
-    """Forty evaluations of configs[3] in a row: logL, every branch gradient and every per-pattern derivative bitwise
+@pytest.mark.parametrize("cfg,precision,flags", [pytest.param(3, plk.FP32, plk.FLAG_TENSOR_CORES, id="cfg3-fp32-tcgen05"),
+                                                 pytest.param(3, plk.FP64, plk.FLAG_TENSOR_CORES, id="cfg3-fp64-dmma"),
+                                                 pytest.param(3, plk.FP32, plk.FLAG_TENSOR_CORES | plk.FLAG_NO_TCGEN05,
+                                                              id="cfg3-fp32-mma-sync"),
+                                                 pytest.param(1, plk.FP64, 0, id="cfg1-fp64"),
+                                                 pytest.param(1, plk.FP32, 0, id="cfg1-fp32")])
+def test_repeated_evaluations_are_bitwise_equal(cfg, precision, flags):
+    """Forty evaluations of a full-size config in a row: logL, every branch gradient and every per-pattern derivative bitwise
     equal to the first.  The warp-specialised kernels hand tiles between warps through phase-counted barriers; a
     protocol error shows up as rare last-bits differences in a few rows of a tile (round 2: the class-1 producers of
     k_pre_tc5v could complete another round's phase -- 9 % of the evaluations at this size differed), which a single
     repeat does not catch reliably.  Library against itself: repeatability only, parity is the test above."""
-    wl = workloads.config(3)
+    wl = workloads.config(cfg)
     ev = Evaluator(wl, precision=precision, flags=flags | plk.FLAG_SITE_DERIVATIVES)
     try:
         logl0, _ = ev.log_likelihood(want_site=False)
