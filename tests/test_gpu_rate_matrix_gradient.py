@@ -42,6 +42,24 @@ CASES = [pytest.param(0, None, 700, 4, plk.FP64, 0, id="hky8-fp64"),
          pytest.param(2, 6, 4100, 3, plk.FP32, plk.FLAG_TENSOR_CORES, id="gy94-4100-3cat-fp32-tensor")]
 
 
+@pytest.mark.parametrize("precision", [plk.FP64, plk.FP32])
+def test_tensor_kernel_with_tips_given_as_partials(precision):
+    """k_cross_tc with single-category tip partials (the operand kind staged once for all categories) instead of
+    compact states: same oracle, same bars."""
+    wl = workloads.config(2, n_tips=10, n_patterns=530, n_categories=4)
+    ev = Evaluator(wl, precision=precision, flags=plk.FLAG_TENSOR_CORES, store_tip_pre=True, tips_as_partials=True,
+                   eigen=orc.oracle_eigen(wl))
+    try:
+        ev.log_likelihood()
+        ev.gradient_unfused()
+        G = ev.rate_matrix_gradient()
+    finally:
+        ev.close()
+    G_ref, scale, _ = _oracle_G(wl)
+    err = np.max(np.abs(G - G_ref) / scale)
+    assert err <= (1e-10 if precision == plk.FP64 else 1e-4), f"rate-matrix gradient err / scale = {err:.3e}"
+
+
 @pytest.mark.parametrize("cfg,n_tips,n_pat,n_cat,precision,flags", CASES)
 def test_rate_matrix_gradient_matches_oracle(cfg, n_tips, n_pat, n_cat, precision, flags):
     wl = workloads.config(cfg, n_tips=n_tips, n_patterns=n_pat, n_categories=n_cat) if cfg else workloads.config(0, n_patterns=n_pat)
