@@ -129,7 +129,7 @@ bool compute_layout(const plk_config& c, Layout& L) {
   L.off_cat_scratch = take((tc5 && c.preorder_buffer_count > 0) ? (size_t)L.max_grad * 2 * L.C * L.P * 4 : 0);
   // rate-matrix gradient (plk_cross.cuh): per-block partial sums and the S x S result
   L.off_cross_partial = take(c.preorder_buffer_count > 0
-                                 ? (L.SP == 4 ? (size_t)16 * ((L.P + CROSS4_THREADS - 1) / CROSS4_THREADS)
+                                 ? (L.SP == 4 ? (size_t)16 * CROSS4_SPLITS * ((L.P + CROSS4_THREADS - 1) / CROSS4_THREADS)
                                               : (size_t)std::max((L.P + CROSS64_TP - 1) / CROSS64_TP, L.SP == 64 ? CROSS_TC_MAX_GRID : 0) * L.SP * L.SP) * 8
                                  : 0);
   L.off_cross_out = take((size_t)L.SP * L.SP * 8);
@@ -2141,11 +2141,17 @@ int plk_rate_matrix_gradient(plk_instance* in, const int32_t* post_idx, const in
   const double* wt = in->at<double>(L.off_weights);
   double* part = in->at<double>(L.off_cross_partial);
   if (L.SP == 4) {
-    const int n_blocks = (L.P + CROSS4_THREADS - 1) / CROSS4_THREADS;
+    const int n_pblocks = (L.P + CROSS4_THREADS - 1) / CROSS4_THREADS;
+    // branch ranges: enough blocks for ~64 warps per SM, at most CROSS4_SPLITS (the layout's bound) and one branch each
+    int splits = 1;
+    while (splits < CROSS4_SPLITS && splits * 2 <= count && (long long)n_pblocks * splits * (CROSS4_THREADS / 32) < 64LL * in->sm_count)
+      splits *= 2;
+    const int n_blocks = n_pblocks * splits;
+    const dim3 grid4(n_pblocks, splits);
     rc = by_precision(in, [&](auto tag) -> int {
       using T = decltype(tag);
       switch (L.C) {
-#define CASE(CC) case CC: k_cross4<T, CC><<<n_blocks, CROSS4_THREADS, 0, in->stream>>>(db, count, L.P, cw, cr, wt, part, n_blocks); break;
+#define CASE(CC) case CC: k_cross4<T, CC><<<grid4, CROSS4_THREADS, 0, in->stream>>>(db, count, L.P, cw, cr, wt, part, n_blocks); break;
         CASE(1) CASE(2) CASE(3) CASE(4) CASE(5) CASE(6) CASE(7) CASE(8)
 #undef CASE
         default: return PLK_ERR_UNSUPPORTED;

@@ -25,9 +25,11 @@ struct DevCrossBranch {
   int32_t pad;
 };
 
-constexpr int CROSS4_THREADS = 128;
+constexpr int CROSS4_THREADS = 128, CROSS4_SPLITS = 8;
 
-// grid.x = pattern blocks; every block walks ALL branches for its patterns.  partial[e][block], e = 4 i + j.
+// grid.x = pattern blocks, grid.y = branch ranges (a thread's walk over the branches is one dependent chain of loads:
+// with one range the 782 blocks of configs[1] gave an SM 21 warps and the kernel ran at a third of the HBM rate).
+// partial[e][blockIdx.y * gridDim.x + blockIdx.x], e = 4 i + j; n_blocks = gridDim.x * gridDim.y.
 template <typename T, int C>
 __global__ void __launch_bounds__(CROSS4_THREADS) k_cross4(const DevCrossBranch* __restrict__ br, int n_br, int P,
                                                            const double* __restrict__ catw, const double* __restrict__ catr,
@@ -40,35 +42,38 @@ __global__ void __launch_bounds__(CROSS4_THREADS) k_cross4(const DevCrossBranch*
   for (int e = 0; e < 16; ++e) g[e] = 0.0;
   if (p < P) {
     const double wp = weights[p];
-    for (int b = 0; b < n_br; ++b) {
+    const int b_lo = (int)((long long)blockIdx.y * n_br / gridDim.y), b_hi = (int)((long long)(blockIdx.y + 1) * n_br / gridDim.y);
+    for (int b = b_lo; b < b_hi; ++b) {
       const DevCrossBranch B = br[b];
-      double num[16], den = 0.0;
+      // category sums in the working precision, widened once per branch (16 fp64 FMAs and conversions per category
+      // made the fp32 instantiation as slow as fp64)
+      T num[16], den = T(0);
 #pragma unroll
-      for (int e = 0; e < 16; ++e) num[e] = 0.0;
+      for (int e = 0; e < 16; ++e) num[e] = T(0);
 #pragma unroll
       for (int c = 0; c < C; ++c) {
         T q[4], x[4];
         ld4(static_cast<const T*>(B.q) + ((size_t)c * P + p) * 4, q);
         operand4<T>(B.kind, B.p, c, p, P, x);
-        const double cw = catw[c], cwr = cw * catr[c];
+        const T cw = (T)catw[c], cwr = (T)(catw[c] * catr[c]);
         T d = T(0);
 #pragma unroll
         for (int i = 0; i < 4; ++i) {
           d += q[i] * x[i];
 #pragma unroll
-          for (int j = 0; j < 4; ++j) num[4 * i + j] = fma(cwr, (double)(q[i] * x[j]), num[4 * i + j]);
+          for (int j = 0; j < 4; ++j) num[4 * i + j] = fma(cwr, q[i] * x[j], num[4 * i + j]);
         }
-        den = fma(cw, (double)d, den);
+        den = fma(cw, d, den);
       }
-      const double s = wp * B.t / den;
+      const double s = wp * B.t / (double)den;
 #pragma unroll
-      for (int e = 0; e < 16; ++e) g[e] = fma(s, num[e], g[e]);
+      for (int e = 0; e < 16; ++e) g[e] = fma(s, (double)num[e], g[e]);
     }
   }
 #pragma unroll
   for (int e = 0; e < 16; ++e) {
     const double s = block_sum(g[e], red);
-    if (threadIdx.x == 0) partial[(size_t)e * n_blocks + blockIdx.x] = s;
+    if (threadIdx.x == 0) partial[(size_t)e * n_blocks + blockIdx.y * gridDim.x + blockIdx.x] = s;
   }
 }
 
