@@ -306,7 +306,9 @@ PLK_API int plk_evaluate(plk_instance* inst, int eigen, const int32_t* matrix_id
  *   out_G[a][b] = sum_i t_i sum_p omega_p ( sum_c w_c r_c q[c,p,a] p[c,p,b] ) / ( sum_c w_c q[c,p]^T p[c,p] )
  * out_G: HOST [S][S] row-major (diagonal included).  branch_lengths: HOST [count], finite and >= 0.  Needs the
  * pre-order partials of every listed node (plk_update_pre_partials, or plk_pre_order_gradient with dest_pre >= 0).
- * Exact in every direction dQ that commutes with Q (an overall rate).  _FLOATING_POINT if an element is not finite. */
+ * Exact in every direction dQ that commutes with Q (an overall rate).  _FLOATING_POINT if an element is not finite.
+ * With PLK_FLAG_TENSOR_CORES and 33..64 states the pattern contraction runs on the tensor cores (fp64: DMMA, fp32:
+ * split TF32; pattern sums in fp64 in a fixed order in every case: bitwise repeatable). */
 PLK_API int plk_rate_matrix_gradient(plk_instance* inst, const int32_t* post_idx, const int32_t* pre_idx,
                                      const double* branch_lengths, int count, double* out_G);
 
