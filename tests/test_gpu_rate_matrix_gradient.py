@@ -42,6 +42,36 @@ CASES = [pytest.param(0, None, 700, 4, plk.FP64, 0, id="hky8-fp64"),
          pytest.param(2, 6, 4100, 3, plk.FP32, plk.FLAG_TENSOR_CORES, id="gy94-4100-3cat-fp32-tensor")]
 
 
+_full = {}
+
+
+@pytest.mark.parametrize("cfg,precision,flags", [pytest.param(2, plk.FP64, plk.FLAG_TENSOR_CORES, id="cfg2-fp64-tensor"),
+                                                 pytest.param(2, plk.FP32, plk.FLAG_TENSOR_CORES, id="cfg2-fp32-tensor"),
+                                                 pytest.param(2, plk.FP64, 0, id="cfg2-fp64-cuda"),
+                                                 pytest.param(1, plk.FP64, 0, id="cfg1-fp64"),
+                                                 pytest.param(1, plk.FP32, 0, id="cfg1-fp32")])
+def test_full_size_configs(cfg, precision, flags):
+    """BASELINE configs[1] / configs[2] at full size, in the launch configuration bench.py --rate-matrix-gradient times
+    (k_cross_tc: several waves of units, branch ranges; k_cross4: branch ranges in blockIdx.y), every element of G
+    against the oracle on all patterns."""
+    if cfg not in _full:
+        _full.clear()
+        wl = workloads.config(cfg)
+        _full[cfg] = (wl,) + _oracle_G(wl)
+    wl, G_ref, scale, Q = _full[cfg]
+    ev = Evaluator(wl, precision=precision, flags=flags, store_tip_pre=True, eigen=orc.oracle_eigen(wl))
+    try:
+        ev.log_likelihood(want_site=False)
+        ev.gradient_unfused()
+        G = ev.rate_matrix_gradient()
+        G2 = ev.rate_matrix_gradient()
+    finally:
+        ev.close()
+    err = np.max(np.abs(G - G_ref) / scale)
+    assert err <= (1e-10 if precision == plk.FP64 else 1e-4), f"rate-matrix gradient err / scale = {err:.3e}"
+    assert np.array_equal(G, G2)
+
+
 @pytest.mark.parametrize("precision", [plk.FP64, plk.FP32])
 def test_tensor_kernel_with_tips_given_as_partials(precision):
     """k_cross_tc with single-category tip partials (the operand kind staged once for all categories) instead of
