@@ -22,8 +22,9 @@ def _oracle_G(wl, t=None):
                                       wl.cat_weights, tips, wl.pattern_weights)
     # conditioning scale: |G| with the absolute value of every pattern's term = the cross products of all-positive
     # partials weighted the same way; an upper bound that needs no second code path: sum_p omega_p |...| >= |G_ij|
-    Gabs = lk.rate_matrix_cross_products(orc.children_list(wl.tree), wl.tree.root, np.asarray(t), Q, pi, wl.rates,
-                                         wl.cat_weights, tips, np.abs(wl.pattern_weights))
+    Gabs = G if np.all(wl.pattern_weights >= 0) else lk.rate_matrix_cross_products(
+        orc.children_list(wl.tree), wl.tree.root, np.asarray(t), Q, pi, wl.rates, wl.cat_weights, tips,
+        np.abs(wl.pattern_weights))
     return G, np.maximum(np.abs(Gabs), np.max(np.abs(Gabs)) * 1e-3), Q
 
 
@@ -49,9 +50,10 @@ _full = {}
                                                  pytest.param(2, plk.FP32, plk.FLAG_TENSOR_CORES, id="cfg2-fp32-tensor"),
                                                  pytest.param(2, plk.FP64, 0, id="cfg2-fp64-cuda"),
                                                  pytest.param(1, plk.FP64, 0, id="cfg1-fp64"),
-                                                 pytest.param(1, plk.FP32, 0, id="cfg1-fp32")])
+                                                 pytest.param(1, plk.FP32, 0, id="cfg1-fp32"),
+                                                 pytest.param(3, plk.FP32, plk.FLAG_TENSOR_CORES, id="cfg3-fp32-tensor")])
 def test_full_size_configs(cfg, precision, flags):
-    """BASELINE configs[1] / configs[2] at full size, in the launch configuration bench.py --rate-matrix-gradient times
+    """BASELINE configs[1] / configs[2] / configs[3] (oracle: ~70 s on one core) at full size, in the launch configuration bench.py --rate-matrix-gradient times
     (k_cross_tc: several waves of units, branch ranges; k_cross4: branch ranges in blockIdx.y), every element of G
     against the oracle on all patterns."""
     if cfg not in _full:
