@@ -801,8 +801,11 @@ def main():
     }
     if mm is not None:
         line["matmul_peaks"] = mm
-    if args.rate_matrix_gradient and not sharded_run:
-        line["rate_matrix_gradient"] = measure_rate_matrix_gradient(wl, args.precision, flags, args.steps, peaks, device)
+    if (args.rate_matrix_gradient or not args.no_extras) and not sharded_run and world == 1:
+        try:
+            line["rate_matrix_gradient"] = measure_rate_matrix_gradient(wl, args.precision, flags, args.steps, peaks, device)
+        except Exception as exc:  # report, never hide
+            line["rate_matrix_gradient"] = {"error": repr(exc)}
     if not nuc and args.tensor and mm is not None:
         line["roofline_codon"] = [codon_roofline("headline", wl, args.precision,
                                                  "tcgen05" if (args.precision == "fp32" and args.codon_fp32 == "tcgen05")
