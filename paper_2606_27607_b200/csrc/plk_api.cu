@@ -1342,9 +1342,11 @@ static int root_impl(plk_instance* in, int root, const int32_t* scale_idx, int s
     rc = copy_ring(in, h, d, list.size() * sizeof(void*));
     if (rc) return rc;
   }
-  double* bp = in->at<double>(L.off_block_partial);
   const int G = L.SP == 4 ? 1 : L.SP / 4;  // threads per pattern, 4 states each
   const int n_blocks = (int)blocks_for((size_t)L.P * G, 128);
+  // one block (a few patterns: the latency-bound end of configs[4], single-pattern large-S problems): its partial sum IS
+  // the result, written straight to the output -- one launch less per evaluation
+  double* bp = n_blocks == 1 ? d_sum : in->at<double>(L.off_block_partial);
   by_precision(in, [&](auto tag) -> int {
     using T = decltype(tag);
     const T* r = static_cast<const T*>(rptr);
@@ -1366,8 +1368,10 @@ static int root_impl(plk_instance* in, int root, const int32_t* scale_idx, int s
     return PLK_SUCCESS;
   });
   CHECK_LAUNCH(in);
-  k_sum_rows<<<1, 128, 0, in->stream>>>(bp, nullptr, n_blocks, n_blocks, d_sum);
-  CHECK_LAUNCH(in);
+  if (n_blocks > 1) {
+    k_sum_rows<<<1, 128, 0, in->stream>>>(bp, nullptr, n_blocks, n_blocks, d_sum);
+    CHECK_LAUNCH(in);
+  }
   return PLK_SUCCESS;
 }
 

@@ -112,7 +112,9 @@ def test_on_the_fly_post_order_matches_oracle(cfg, n_tips, n_pat, n_cat, precisi
     try:
         n0 = ev.inst.kernel_launch_count()
         logl, site = ev.log_likelihood_on_the_fly()
-        assert ev.inst.kernel_launch_count() - n0 == 3  # ONE post-order launch + the root reduction (2)
+        # ONE post-order launch + the root reduction (site kernel + sum kernel; one kernel when its grid is one block)
+        root_blocks = -(-wl.n_patterns * (1 if wl.n_states == 4 else (8 if wl.n_states <= 32 else 16)) // 128)
+        assert ev.inst.kernel_launch_count() - n0 == (2 if root_blocks == 1 else 3)
         pc.check_logl(site, logl, ref, precision)
         assert np.max(np.abs(site - site_fly) / np.abs(site_fly)) <= tol
         # repeatable bit for bit (fixed arithmetic order per ticket, whatever CTA takes it)
